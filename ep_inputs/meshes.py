@@ -1,0 +1,185 @@
+"""Seeded synthetic tetrahedral meshes shaped like the paper's workloads.
+
+Everything here is input generation only: lattice points, the Kuhn/Freudenthal split of a cube into six
+tetrahedra (reading A12: only the counts 20,160 / 315,000 / 2,520,000 = 6 x cubes are printed),
+carving of ellipsoidal shells out of the lattice, fibre fields by the paper's transmural rule
+(alpha = alpha_endo*d + alpha_epi*(1-d), +-60 degrees) and cell-type bands.
+No finite-volume or cell-model arithmetic lives here; both the oracle tests and the CUDA path consume these arrays.
+"""
+from __future__ import annotations
+
+import itertools
+from dataclasses import dataclass, field
+
+import numpy as np
+
+from .prng import uniform
+
+# The six Kuhn simplices of the unit cube: one per permutation of the axes; all share the (0,0,0)-(1,1,1) diagonal.
+_KUHN_PERMS = list(itertools.permutations((0, 1, 2)))
+
+
+@dataclass
+class TetMesh:
+    xyz: np.ndarray            # [n_nodes,3] float64, mm
+    tets: np.ndarray           # [n_tets,4] int32, 0-based
+    fibre: np.ndarray | None = None        # [n_tets,3] float64 (unit) or None = isotropic
+    cell_type: np.ndarray | None = None    # [n_tets] uint8: 0 endo, 1 mid, 2 epi
+    sigma_scale: np.ndarray | None = None  # [n_tets] float64 or None
+    meta: dict = field(default_factory=dict)
+
+    @property
+    def n_nodes(self) -> int:
+        return int(self.xyz.shape[0])
+
+    @property
+    def n_tets(self) -> int:
+        return int(self.tets.shape[0])
+
+    def centroids(self) -> np.ndarray:
+        return self.xyz[self.tets].mean(axis=1)
+
+
+def _kuhn_tets_of_cubes(ci, cj, ck, nx, ny, nz) -> np.ndarray:
+    """Tets (node ids in the full (nx+1)(ny+1)(nz+1) lattice, x fastest) of the listed cubes. [6*M,4] int64."""
+    sx, sy, sz = 1, nx + 1, (nx + 1) * (ny + 1)
+    strides = np.array([sx, sy, sz], dtype=np.int64)
+    base = ci.astype(np.int64) * sx + cj.astype(np.int64) * sy + ck.astype(np.int64) * sz
+    out = np.empty((base.shape[0], 6, 4), dtype=np.int64)
+    for t, p in enumerate(_KUHN_PERMS):
+        out[:, t, 0] = base
+        out[:, t, 1] = base + strides[p[0]]
+        out[:, t, 2] = base + strides[p[0]] + strides[p[1]]
+        out[:, t, 3] = base + sx + sy + sz
+    return out.reshape(-1, 4)
+
+
+def lattice_nodes(nx, ny, nz, h, origin=(0.0, 0.0, 0.0)) -> np.ndarray:
+    k, j, i = np.meshgrid(np.arange(nz + 1), np.arange(ny + 1), np.arange(nx + 1), indexing="ij")
+    xyz = np.stack([i.ravel(), j.ravel(), k.ravel()], axis=1).astype(np.float64) * h
+    return xyz + np.asarray(origin, dtype=np.float64)
+
+
+def kuhn_slab(nx: int, ny: int, nz: int, h: float) -> TetMesh:
+    """Box [0,nx*h]x[0,ny*h]x[0,nz*h] cut into nx*ny*nz cubes of edge h, six Kuhn tets each."""
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    tets = _kuhn_tets_of_cubes(i.ravel(), j.ravel(), k.ravel(), nx, ny, nz)
+    xyz = lattice_nodes(nx, ny, nz, h)
+    return TetMesh(xyz=xyz, tets=tets.astype(np.int32), meta={"kind": "kuhn_slab", "dims": (nx, ny, nz), "h": h})
+
+
+def jitter_interior(mesh: TetMesh, amplitude: float, seed: int) -> None:
+    """Move interior lattice nodes by U(-amplitude, amplitude) per axis (reading G3); boundary nodes stay put."""
+    nx, ny, nz = mesh.meta["dims"]
+    h = mesh.meta["h"]
+    ijk = np.rint(mesh.xyz / h).astype(np.int64)
+    interior = ((ijk[:, 0] > 0) & (ijk[:, 0] < nx) & (ijk[:, 1] > 0) & (ijk[:, 1] < ny)
+                & (ijk[:, 2] > 0) & (ijk[:, 2] < nz))
+    n = mesh.n_nodes
+    ctr = np.arange(n, dtype=np.uint64)
+    for ax in range(3):
+        d = uniform(seed, ctr * np.uint64(3) + np.uint64(ax), -amplitude, amplitude)
+        mesh.xyz[:, ax] += np.where(interior, d, 0.0)
+    mesh.meta["jitter"] = amplitude
+
+
+def carve_lattice(inside, lo, hi, h: float) -> TetMesh:
+    """Keep the cubes of an h-lattice over the box [lo,hi] whose centre satisfies inside(xyz)->bool; Kuhn-split
+    them; renumber the nodes that are used. Conforming by construction (same split in every cube)."""
+    lo = np.asarray(lo, dtype=np.float64)
+    hi = np.asarray(hi, dtype=np.float64)
+    dims = np.maximum(1, np.ceil((hi - lo) / h - 1e-9).astype(np.int64))
+    nx, ny, nz = (int(d) for d in dims)
+    keep_i, keep_j, keep_k = [], [], []
+    jj, ii = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    for k in range(nz):  # slab by slab keeps the temporary arrays small for the 20M-cell config
+        c = np.stack([lo[0] + (ii.ravel() + 0.5) * h, lo[1] + (jj.ravel() + 0.5) * h,
+                      np.full(ii.size, lo[2] + (k + 0.5) * h)], axis=1)
+        m = inside(c)
+        keep_i.append(ii.ravel()[m])
+        keep_j.append(jj.ravel()[m])
+        keep_k.append(np.full(int(m.sum()), k, dtype=np.int64))
+    ci, cj, ck = np.concatenate(keep_i), np.concatenate(keep_j), np.concatenate(keep_k)
+    tets_full = _kuhn_tets_of_cubes(ci, cj, ck, nx, ny, nz)
+    used, inv = np.unique(tets_full.ravel(), return_inverse=True)
+    tets = inv.reshape(-1, 4).astype(np.int32)
+    sy, sz = nx + 1, (nx + 1) * (ny + 1)
+    xyz = np.stack([used % sy, (used // sy) % (ny + 1), used // sz], axis=1).astype(np.float64) * h + lo
+    return TetMesh(xyz=xyz, tets=tets, meta={"kind": "carved", "h": h, "dims": (nx, ny, nz), "n_cubes": int(ci.size)})
+
+
+# ----------------------------------------------------------------------------------------------------------
+# ellipsoidal shells
+
+
+def shell_depth(p: np.ndarray, centre, inner, outer, iters: int = 60) -> np.ndarray:
+    """Transmural coordinate d in [0,1] (0 = inner/endocardial surface, 1 = outer/epicardial): the t for which p
+    lies on the ellipsoid with semi-axes inner + t*(outer-inner). Bisection; values outside the wall are clipped."""
+    q = p - np.asarray(centre, dtype=np.float64)
+    a0 = np.asarray(inner, dtype=np.float64)
+    da = np.asarray(outer, dtype=np.float64) - a0
+    lo = np.full(q.shape[0], -0.5)
+    hi = np.full(q.shape[0], 1.5)
+    for _ in range(iters):
+        mid = 0.5 * (lo + hi)
+        ax = a0[None, :] + mid[:, None] * da[None, :]
+        g = ((q / ax) ** 2).sum(axis=1) - 1.0  # >0: p is outside the level-mid ellipsoid => true t is larger
+        lo = np.where(g > 0, mid, lo)
+        hi = np.where(g > 0, hi, mid)
+    return np.clip(0.5 * (lo + hi), 0.0, 1.0)
+
+
+def ellipsoid_frame(p: np.ndarray, centre, axes):
+    """Unit (normal, circumferential, longitudinal) directions of the ellipsoid family through p; the long axis is z."""
+    q = p - np.asarray(centre, dtype=np.float64)
+    n = q / (np.asarray(axes, dtype=np.float64) ** 2)[None, :]
+    n /= np.maximum(np.linalg.norm(n, axis=1, keepdims=True), 1e-300)
+    zhat = np.array([0.0, 0.0, 1.0])
+    circ = np.cross(zhat[None, :], n)
+    nc = np.linalg.norm(circ, axis=1)
+    bad = nc < 1e-9
+    circ[bad] = np.array([1.0, 0.0, 0.0])  # poles: fall back to x-hat
+    circ /= np.where(bad, 1.0, nc)[:, None]
+    lon = np.cross(n, circ)
+    lon /= np.maximum(np.linalg.norm(lon, axis=1, keepdims=True), 1e-300)
+    return n, circ, lon
+
+
+def helical_fibres(p, centre, inner, outer, alpha_endo_deg=60.0, alpha_epi_deg=-60.0):
+    """alpha = alpha_endo*(1-d) + alpha_epi*d with d=0 at the endocardium (labels as in SURVEY 8(d) C3);
+    f = cos(alpha) e_circ + sin(alpha) e_long. Returns (fibre [n,3], d [n])."""
+    d = shell_depth(p, centre, inner, outer)
+    mid_axes = 0.5 * (np.asarray(inner, dtype=np.float64) + np.asarray(outer, dtype=np.float64))
+    _, circ, lon = ellipsoid_frame(p, centre, mid_axes)
+    alpha = np.deg2rad(alpha_endo_deg * (1.0 - d) + alpha_epi_deg * d)
+    f = np.cos(alpha)[:, None] * circ + np.sin(alpha)[:, None] * lon
+    f /= np.linalg.norm(f, axis=1, keepdims=True)
+    return f, d
+
+
+def thirds(d: np.ndarray) -> np.ndarray:
+    """endo / mid / epi bands by thirds of the transmural coordinate (0 endo, 1 mid, 2 epi)."""
+    return np.minimum(2, np.floor(d * 3.0)).astype(np.uint8)
+
+
+def in_ellipsoid(p, centre, axes) -> np.ndarray:
+    q = (p - np.asarray(centre, dtype=np.float64)) / np.asarray(axes, dtype=np.float64)
+    return (q * q).sum(axis=1) <= 1.0
+
+
+def validate(mesh: TetMesh) -> dict:
+    """Harness-side sanity checks: positive volumes after orientation is ignored, every face
+    shared by at most two cells. Returns counts; raises on failure."""
+    x = mesh.xyz[mesh.tets]
+    vol = np.abs(np.einsum("ij,ij->i", np.cross(x[:, 1] - x[:, 0], x[:, 2] - x[:, 0]), x[:, 3] - x[:, 0])) / 6.0
+    if not (vol > 0).all():
+        raise ValueError("degenerate tetrahedron")
+    t = mesh.tets.astype(np.int64)
+    faces = np.concatenate([np.sort(np.delete(t, j, axis=1), axis=1) for j in range(4)], axis=0)
+    nn = np.int64(mesh.n_nodes)
+    key = (faces[:, 0] * nn + faces[:, 1]) * nn + faces[:, 2]
+    _, cnt = np.unique(key, return_counts=True)
+    if cnt.max() > 2:
+        raise ValueError("face shared by more than two cells")
+    return {"n_faces": int(cnt.size), "n_boundary_faces": int((cnt == 1).sum()), "min_vol": float(vol.min()),
+            "mean_vol": float(vol.mean())}
