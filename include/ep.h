@@ -1,0 +1,122 @@
+/* ep.h -- C-ABI of libep: the explicit monodomain + ten Tusscher-Panfilov 2006 time step of
+ * arXiv 2112.12854 (section 3.2) on a tetrahedral cell-centred finite-volume mesh, one B200 (sm_100a), fp64.
+ *
+ * Citations are PAPER.md:<line> (section / equation).  Readings of silent or ambiguous points (A1..A18, B1..B9) are
+ * listed in DESIGN.md section 3.
+ *
+ * Conventions
+ *   - every function returns EP_OK (0) or a negative error code and never throws across the ABI;
+ *     ep_last_error() returns a thread-local, NUL-terminated message for the last failing call of this thread;
+ *   - all pointer arguments are HOST pointers unless the comment says "device"; inputs are copied before the call
+ *     returns (the caller may free them), outputs are written into caller-owned buffers;
+ *   - cells and nodes keep the CALLER's numbering at the ABI: the space-filling-curve permutation used on the device
+ *     is invisible except through ep_device_vm();
+ *   - one handle is used by one thread at a time; there is no global state besides the error string;
+ *   - there is no CPU fallback: without a CUDA device ep_mesh_create() fails with EP_ERR_CUDA.
+ *     (ep_host_stencil() runs the one-time host preprocessor only and needs no device; it exists so that the
+ *     host logic can be tested on a machine without a GPU.)
+ *   - units: lengths mm, conductivities mS/cm, chi 1/cm, Cm uF/cm^2, potentials mV, time ms, stimulus uA/cm^2
+ *     (PAPER.md:113 gives the same physics in mm units: chi = 140 1/mm, Cm = 0.01 uF/mm^2; reading A14).
+ */
+#ifndef EP_H_
+#define EP_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ep_sim ep_sim; /* opaque; owns all host and device memory it allocates */
+
+enum { EP_OK = 0, EP_ERR_ARG = -1, EP_ERR_MESH = -2, EP_ERR_STATE = -3, EP_ERR_CUDA = -4, EP_ERR_NOMEM = -5,
+       EP_ERR_NUMERIC = -6 };
+enum { EP_MODEL_TP06 = 0, EP_MODEL_CRN98 = 1 };
+enum { EP_MAX_STIM_SLOTS = 8 };
+
+/* Number of state variables of a cell model, Vm included (TP06 19, Courtemanche 21); <0 if unknown. */
+int ep_model_n_states(int model);
+
+/* Build the simulation object: validate the mesh, run the one-time preprocessor (geometry, face matching, node stars,
+ * the Fig. 8 a->e pipeline of PAPER.md:164-168 with the eq. (8) correction folded into per-cell gather coefficients,
+ * Morton reordering, ELL packing) and upload the tables.
+ *   xyz_mm       [n_nodes*3] node coordinates, mm
+ *   tets         [n_tets*4]  0-based node ids, any orientation
+ *   fibre        [n_tets*3]  per-cell fibre direction (normalised inside); NULL => isotropic sigma_l
+ *   sigma_scale  [n_tets]    per-cell multiplier of the conductivity tensor (PAPER.md:309 pathologies); NULL => 1
+ *   sigma_l/t    mS/cm, M_c = scale*[sigma_t I + (sigma_l - sigma_t) f f^T]  (eq. (2)-(3))
+ *   chi, Cm      surface-to-volume ratio 1/cm and membrane capacitance uF/cm^2
+ * Errors: EP_ERR_ARG (NULL/negative sizes, non-positive sigma/chi/Cm), EP_ERR_MESH (index out of range, zero volume,
+ * face shared by >2 cells, non-finite coordinate, zero fibre vector), EP_ERR_CUDA, EP_ERR_NOMEM.  *out is NULL on error. */
+int ep_mesh_create(ep_sim **out, int64_t n_nodes, const double *xyz_mm, int64_t n_tets, const int32_t *tets,
+                   const double *fibre, const double *sigma_scale, double sigma_l, double sigma_t, double chi,
+                   double Cm);
+
+/* Choose the cell model and set every cell to an initial state.
+ *   cell_type [n_tets] TP06: 0 endo, 1 mid, 2 epi (reading B5); NULL => 0
+ *   y0        [n_types*S] one state vector per cell type (n_types = 3 for TP06, 1 for CRN98); NULL => built-in rest state
+ * Resets the step counter, the activation times (to -1) and keeps the stimulus slots. */
+int ep_state_init(ep_sim *sim, int model, const uint8_t *cell_type, const double *y0);
+
+/* Stimulus of eq. (4): I_s = amplitude on the listed cells while t_start <= t < t_start+duration,
+ * with the window taken on integer step indices (reading A16).  amplitude in uA/cm^2; NEGATIVE depolarises (A15).
+ * slot in [0, EP_MAX_STIM_SLOTS); n_cells = 0 clears the slot.  Overlapping slots add. */
+int ep_stimulus_set(ep_sim *sim, int slot, int64_t n_cells, const int64_t *cell_ids, double amplitude_uA_cm2,
+                    double t_start_ms, double duration_ms);
+
+/* Advance n_steps explicit steps of size dt_ms (everything on the right-hand side at t^n; gates by
+ * Rush-Larsen, the rest by forward Euler; v by eq. (7)).  Asynchronous on the sim's stream; errors are sticky.
+ * EP_ERR_STATE: before ep_state_init, dt <= 0, or dt different from the previous call's after the first step. */
+int ep_step(ep_sim *sim, int64_t n_steps, double dt_ms);
+
+/* Wait for all queued work of this sim; returns the sticky error if any (EP_ERR_NUMERIC if a non-finite Vm was seen by
+ * ep_check_finite). */
+int ep_synchronize(ep_sim *sim);
+
+/* Read-back, caller's cell order; each synchronises. */
+int ep_read_vm(ep_sim *sim, double *out /*[n_tets]*/);
+int ep_read_state(ep_sim *sim, int var /*0..S-1, 0 = Vm*/, double *out /*[n_tets]*/);
+int ep_write_state(ep_sim *sim, int var, const double *in /*[n_tets]*/);
+/* First instant Vm exceeded 0 mV (reading A18: t=(n+1)dt of the step that crossed); -1 where never. */
+int ep_activation_times(ep_sim *sim, double *out /*[n_tets]*/);
+
+/* Diagnostics.  D = div(M grad v) in uA/cm^3 for a host cell field v [mV], through the device gather tables. */
+int ep_apply_diffusion(ep_sim *sim, const double *v /*[n_tets]*/, double *D /*[n_tets]*/);
+/* Largest explicit step of the diffusion part alone: 2 chi Cm / rho(A), rho by power iteration on the device. */
+int ep_stable_dt(ep_sim *sim, double *dt_max_ms);
+/* Sets *all_finite = 0 and the sticky error EP_ERR_NUMERIC if any Vm is NaN/Inf. Synchronises. */
+int ep_check_finite(ep_sim *sim, int *all_finite);
+
+/* Stream interop: cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL => the sim's own stream. */
+int ep_set_stream(ep_sim *sim, void *cuda_stream);
+/* Zero-copy DEVICE views, valid until the next ep_step/ep_state_init: *vm_dptr -> double[n_tets] current Vm in device
+ * (permuted) order, *perm_dptr -> int32[n_tets] with perm[device index] = caller's cell id.  Either may be NULL. */
+int ep_device_vm(ep_sim *sim, void **vm_dptr, void **perm_dptr);
+
+int64_t ep_n_cells(const ep_sim *sim);
+int64_t ep_n_nodes(const ep_sim *sim);
+int64_t ep_step_count(const ep_sim *sim);
+double ep_time(const ep_sim *sim); /* step_count * dt (reading A17) */
+/* Device bytes held by the sim, and the algorithmic HBM bytes one time step must move. */
+int64_t ep_device_bytes(const ep_sim *sim);
+int64_t ep_step_bytes(const ep_sim *sim);
+/* Kernel launches issued by this sim so far (bench.py's gpu_launches). */
+int64_t ep_launch_count(const ep_sim *sim);
+void ep_destroy(ep_sim *sim);
+const char *ep_last_error(void);
+
+/* Host-only preprocessor output for tests (no CUDA call is made).  Returns the factored stencil in the CALLER's
+ * numbering: for cell c,  dv_diff[c] = sum_{m<8} a[c*8+m] * v_node[node[c*8+m]] + sum_{j<4} b[c*4+j] * (v[nbr[c*4+j]] - v[c])
+ * in mV/ms (= D_c/(chi Cm)), where v_node[n] = sum_{k<node_deg[n]} w[node_ptr[n]+k] * v[node_cell[node_ptr[n]+k]].
+ * Unused slots have coefficient 0 and a valid index.  Caller-allocated: node [n_tets*8] int32, a [n_tets*8],
+ * nbr [n_tets*4] int32, b [n_tets*4], node_ptr [n_nodes+1] int64, node_cell/w [n_tets*4]; perm [n_tets] int32 (device
+ * position -> caller cell id).  Any output pointer may be NULL. */
+int ep_host_stencil(int64_t n_nodes, const double *xyz_mm, int64_t n_tets, const int32_t *tets, const double *fibre,
+                    const double *sigma_scale, double sigma_l, double sigma_t, double chi, double Cm, int32_t *node,
+                    double *a, int32_t *nbr, double *b, int64_t *node_ptr, int32_t *node_cell, double *w,
+                    int32_t *perm);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EP_H_ */

@@ -1,0 +1,218 @@
+"""ctypes binding of libep.so: same names as include/ep.h, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+EP_MODEL_TP06, EP_MODEL_CRN98 = 0, 1
+_dp = C.POINTER(C.c_double)
+_i32p = C.POINTER(C.c_int32)
+_i64p = C.POINTER(C.c_int64)
+_u8p = C.POINTER(C.c_uint8)
+_vp = C.c_void_p
+
+# name -> (restype, argtypes); tests/test_abi.py checks this table against include/ep.h
+SIGNATURES = {
+    "ep_model_n_states": (C.c_int, [C.c_int]),
+    "ep_mesh_create": (C.c_int, [C.POINTER(_vp), C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double,
+                                 C.c_double, C.c_double]),
+    "ep_state_init": (C.c_int, [_vp, C.c_int, _u8p, _dp]),
+    "ep_stimulus_set": (C.c_int, [_vp, C.c_int, C.c_int64, _i64p, C.c_double, C.c_double, C.c_double]),
+    "ep_step": (C.c_int, [_vp, C.c_int64, C.c_double]),
+    "ep_synchronize": (C.c_int, [_vp]),
+    "ep_read_vm": (C.c_int, [_vp, _dp]),
+    "ep_read_state": (C.c_int, [_vp, C.c_int, _dp]),
+    "ep_write_state": (C.c_int, [_vp, C.c_int, _dp]),
+    "ep_activation_times": (C.c_int, [_vp, _dp]),
+    "ep_apply_diffusion": (C.c_int, [_vp, _dp, _dp]),
+    "ep_stable_dt": (C.c_int, [_vp, _dp]),
+    "ep_check_finite": (C.c_int, [_vp, C.POINTER(C.c_int)]),
+    "ep_set_stream": (C.c_int, [_vp, _vp]),
+    "ep_device_vm": (C.c_int, [_vp, C.POINTER(_vp), C.POINTER(_vp)]),
+    "ep_n_cells": (C.c_int64, [_vp]),
+    "ep_n_nodes": (C.c_int64, [_vp]),
+    "ep_step_count": (C.c_int64, [_vp]),
+    "ep_time": (C.c_double, [_vp]),
+    "ep_device_bytes": (C.c_int64, [_vp]),
+    "ep_step_bytes": (C.c_int64, [_vp]),
+    "ep_launch_count": (C.c_int64, [_vp]),
+    "ep_destroy": (None, [_vp]),
+    "ep_last_error": (C.c_char_p, []),
+    "ep_host_stencil": (C.c_int, [C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double, C.c_double,
+                                  C.c_double, _i32p, _dp, _i32p, _dp, _i64p, _i32p, _dp, _i32p]),
+}
+
+_lib = None
+
+
+class EpError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libep error {code}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Load (building if stale) libep.so.  Raises if it cannot be built or loaded: there is no fallback."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        L._path = path
+        _lib = L
+    return _lib
+
+
+def _chk(rc: int) -> None:
+    if rc != 0:
+        raise EpError(rc, lib().ep_last_error().decode())
+
+
+def _p(a, ct=C.c_double):
+    return a.ctypes.data_as(C.POINTER(ct)) if a is not None else None
+
+
+def model_n_states(model: int) -> int:
+    return int(lib().ep_model_n_states(model))
+
+
+def host_stencil(xyz, tets, fibre=None, sigma_scale=None, sigma_l=1.3, sigma_t=0.18, chi=1400.0, Cm=1.0):
+    """ep_host_stencil: the preprocessor's factored stencil in the caller's numbering (no GPU needed)."""
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+    tets = np.ascontiguousarray(tets, dtype=np.int32)
+    fibre = None if fibre is None else np.ascontiguousarray(fibre, dtype=np.float64)
+    sigma_scale = None if sigma_scale is None else np.ascontiguousarray(sigma_scale, dtype=np.float64)
+    nn, nc = xyz.shape[0], tets.shape[0]
+    out = dict(node=np.empty((nc, 8), np.int32), a=np.empty((nc, 8)), nbr=np.empty((nc, 4), np.int32),
+               b=np.empty((nc, 4)), node_ptr=np.empty(nn + 1, np.int64), node_cell=np.empty(4 * nc, np.int32),
+               w=np.empty(4 * nc), perm=np.empty(nc, np.int32))
+    _chk(lib().ep_host_stencil(nn, _p(xyz), nc, _p(tets, C.c_int32), _p(fibre), _p(sigma_scale), sigma_l, sigma_t,
+                               chi, Cm, _p(out["node"], C.c_int32), _p(out["a"]), _p(out["nbr"], C.c_int32),
+                               _p(out["b"]), _p(out["node_ptr"], C.c_int64), _p(out["node_cell"], C.c_int32),
+                               _p(out["w"]), _p(out["perm"], C.c_int32)))
+    return out
+
+
+class Sim:
+    """One simulation handle (ep_sim*).  Method names follow the C-ABI calls."""
+
+    def __init__(self, xyz, tets, fibre=None, sigma_scale=None, sigma_l=1.3, sigma_t=0.18, chi=1400.0, Cm=1.0):
+        xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+        tets = np.ascontiguousarray(tets, dtype=np.int32)
+        fibre = None if fibre is None else np.ascontiguousarray(fibre, dtype=np.float64)
+        sigma_scale = None if sigma_scale is None else np.ascontiguousarray(sigma_scale, dtype=np.float64)
+        self._h = _vp()
+        _chk(lib().ep_mesh_create(C.byref(self._h), xyz.shape[0], _p(xyz), tets.shape[0], _p(tets, C.c_int32),
+                                  _p(fibre), _p(sigma_scale), sigma_l, sigma_t, chi, Cm))
+        self.n_tets = int(lib().ep_n_cells(self._h))
+        self.n_nodes = int(lib().ep_n_nodes(self._h))
+        self.n_states = 0
+
+    @classmethod
+    def from_problem(cls, prob):
+        m = prob.mesh
+        s = cls(m.xyz, m.tets, m.fibre, m.sigma_scale, prob.sigma_l, prob.sigma_t, prob.chi, prob.Cm)
+        s.state_init(prob.model, m.cell_type)
+        for k, st in enumerate(prob.stimuli):
+            s.stimulus_set(k, st.cell_ids, st.amplitude, st.t_start, st.duration)
+        return s
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().ep_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def state_init(self, model=EP_MODEL_TP06, cell_type=None, y0=None):
+        ct = None if cell_type is None else np.ascontiguousarray(cell_type, dtype=np.uint8)
+        y0 = None if y0 is None else np.ascontiguousarray(y0, dtype=np.float64)
+        _chk(lib().ep_state_init(self._h, model, _p(ct, C.c_uint8), _p(y0)))
+        self.n_states = model_n_states(model)
+
+    def stimulus_set(self, slot, cell_ids, amplitude, t_start, duration):
+        ids = np.ascontiguousarray(cell_ids, dtype=np.int64)
+        _chk(lib().ep_stimulus_set(self._h, slot, ids.size, _p(ids, C.c_int64), amplitude, t_start, duration))
+
+    def step(self, n_steps, dt):
+        _chk(lib().ep_step(self._h, int(n_steps), float(dt)))
+
+    def synchronize(self):
+        _chk(lib().ep_synchronize(self._h))
+
+    def read_vm(self, out=None):
+        out = np.empty(self.n_tets) if out is None else out
+        _chk(lib().ep_read_vm(self._h, _p(out)))
+        return out
+
+    def read_state(self, var, out=None):
+        out = np.empty(self.n_tets) if out is None else out
+        _chk(lib().ep_read_state(self._h, int(var), _p(out)))
+        return out
+
+    def write_state(self, var, arr):
+        arr = np.ascontiguousarray(arr, dtype=np.float64)
+        assert arr.size == self.n_tets
+        _chk(lib().ep_write_state(self._h, int(var), _p(arr)))
+
+    def activation_times(self, out=None):
+        out = np.empty(self.n_tets) if out is None else out
+        _chk(lib().ep_activation_times(self._h, _p(out)))
+        return out
+
+    def apply_diffusion(self, v):
+        v = np.ascontiguousarray(v, dtype=np.float64)
+        out = np.empty(self.n_tets)
+        _chk(lib().ep_apply_diffusion(self._h, _p(v), _p(out)))
+        return out
+
+    def stable_dt(self):
+        d = C.c_double()
+        _chk(lib().ep_stable_dt(self._h, C.byref(d)))
+        return d.value
+
+    def check_finite(self):
+        f = C.c_int()
+        rc = lib().ep_check_finite(self._h, C.byref(f))
+        if rc not in (0, -6):
+            _chk(rc)
+        return bool(f.value)
+
+    def set_stream(self, cuda_stream: int | None):
+        _chk(lib().ep_set_stream(self._h, _vp(cuda_stream) if cuda_stream else None))
+
+    def device_vm(self):
+        vm, perm = _vp(), _vp()
+        _chk(lib().ep_device_vm(self._h, C.byref(vm), C.byref(perm)))
+        return vm.value, perm.value
+
+    @property
+    def step_count(self):
+        return int(lib().ep_step_count(self._h))
+
+    @property
+    def time(self):
+        return float(lib().ep_time(self._h))
+
+    @property
+    def device_bytes(self):
+        return int(lib().ep_device_bytes(self._h))
+
+    @property
+    def step_bytes(self):
+        return int(lib().ep_step_bytes(self._h))
+
+    @property
+    def launch_count(self):
+        return int(lib().ep_launch_count(self._h))

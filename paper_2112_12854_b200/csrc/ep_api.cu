@@ -1,0 +1,437 @@
+// ep_api.cu -- the C-ABI of include/ep.h: argument checks, host preprocessing, device memory, launches.
+// There is no CPU fallback: every compute entry point needs a CUDA device and fails with EP_ERR_CUDA otherwise.
+#include "../../include/ep.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "ep_host.h"
+#include "ep_kernels.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string& msg) {
+    g_err = msg;
+    return code;
+}
+
+struct StimSlot {
+    bool set = false;
+    double amp = 0.0, t0 = 0.0, dur = 0.0;
+    int64_t n_cells = 0;
+};
+
+}  // namespace
+
+struct ep_sim {
+    int64_t nc = 0, nn = 0, nc_pad = 0;
+    double chi = 0.0, Cm = 0.0;
+    // host copies kept for the life of the sim
+    std::vector<int32_t> perm_c, inv_c;
+    std::vector<uint8_t> smask_host;   // device order
+    StimSlot stim[EP_MAX_STIM_SLOTS];
+    int64_t star_entries = 0;
+    // device
+    epk::DeviceMesh dm;
+    int32_t *d_cidx = nullptr, *d_nidx = nullptr, *d_perm = nullptr, *d_inv = nullptr;
+    double *d_ccoef = nullptr, *d_nw = nullptr;
+    int64_t* d_slice_ptr = nullptr;
+    double *d_vm[2] = {nullptr, nullptr}, *d_y = nullptr, *d_vn = nullptr, *d_tact = nullptr, *d_tmp = nullptr,
+           *d_tmp2 = nullptr, *d_red = nullptr;
+    uint8_t *d_ctype = nullptr, *d_smask = nullptr, *d_tmp8 = nullptr;
+    int cur = 0;   // d_vm[cur] holds Vm at the current time level
+    cudaStream_t own_stream = nullptr, stream = nullptr;
+    int model = -1, S = 0;
+    int64_t step = 0;
+    double dt = 0.0;
+    int sticky = EP_OK;
+    int64_t dev_bytes = 0, launches = 0;
+};
+
+namespace {
+
+#define EP_CUDA(sim, call)                                                                        \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess) {                                                                  \
+            if (sim) (sim)->sticky = EP_ERR_CUDA;                                                 \
+            return fail(e_ == cudaErrorMemoryAllocation ? EP_ERR_NOMEM : EP_ERR_CUDA,             \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                      \
+        }                                                                                         \
+    } while (0)
+
+template <class T>
+int dev_alloc(ep_sim* s, T** p, int64_t count) {
+    const size_t bytes = (size_t)(count > 0 ? count : 1) * sizeof(T);
+    EP_CUDA(s, cudaMalloc((void**)p, bytes));
+    s->dev_bytes += (int64_t)bytes;
+    return EP_OK;
+}
+
+template <class T>
+int upload(ep_sim* s, T** p, const std::vector<T>& h) {
+    int rc = dev_alloc(s, p, (int64_t)h.size());
+    if (rc) return rc;
+    if (!h.empty()) EP_CUDA(s, cudaMemcpy(*p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return EP_OK;
+}
+
+int64_t step_index(double t, double dt) { return (int64_t)std::ceil(t / dt - 1e-9); }   // reading A16
+
+void free_all(ep_sim* s) {
+    void* ptrs[] = {s->d_cidx, s->d_nidx, s->d_perm, s->d_inv, s->d_ccoef, s->d_nw, s->d_slice_ptr, s->d_vm[0],
+                    s->d_vm[1], s->d_y, s->d_vn, s->d_tact, s->d_tmp, s->d_tmp2, s->d_red, s->d_ctype, s->d_smask,
+                    s->d_tmp8};
+    for (void* p : ptrs) if (p) cudaFree(p);
+    if (s->own_stream) cudaStreamDestroy(s->own_stream);
+}
+
+int check_sim(ep_sim* s) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    if (s->sticky != EP_OK) return fail(s->sticky, "sim is in a sticky error state: " + g_err);
+    return EP_OK;
+}
+
+// device (permuted) array -> host array in the caller's order
+int read_back(ep_sim* s, const double* d_src, double* out) {
+    epk::launch_gather_f64(s->nc, d_src, s->d_inv, s->d_tmp, s->stream);
+    s->launches++;
+    EP_CUDA(s, cudaMemcpyAsync(out, s->d_tmp, sizeof(double) * s->nc, cudaMemcpyDeviceToHost, s->stream));
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    return EP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ep_last_error(void) { return g_err.c_str(); }
+
+int ep_model_n_states(int model) { return epk::model_n_states(model); }
+
+int ep_host_stencil(int64_t n_nodes, const double* xyz, int64_t n_tets, const int32_t* tets, const double* fibre,
+                    const double* sigma_scale, double sigma_l, double sigma_t, double chi, double Cm, int32_t* node,
+                    double* a, int32_t* nbr, double* b, int64_t* node_ptr, int32_t* node_cell, double* w,
+                    int32_t* perm) {
+    try {
+        ep::Stencil st;
+        std::string err;
+        int rc = ep::build_stencil(n_nodes, xyz, n_tets, tets, fibre, sigma_scale, sigma_l, sigma_t, chi, Cm, st, err);
+        if (rc) return fail(rc, err);
+        if (node) std::memcpy(node, st.node.data(), sizeof(int32_t) * st.node.size());
+        if (a) std::memcpy(a, st.a.data(), sizeof(double) * st.a.size());
+        if (nbr) std::memcpy(nbr, st.nbr.data(), sizeof(int32_t) * st.nbr.size());
+        if (b) std::memcpy(b, st.b.data(), sizeof(double) * st.b.size());
+        if (node_ptr) std::memcpy(node_ptr, st.node_ptr.data(), sizeof(int64_t) * st.node_ptr.size());
+        if (node_cell) std::memcpy(node_cell, st.node_cell.data(), sizeof(int32_t) * st.node_cell.size());
+        if (w) std::memcpy(w, st.w.data(), sizeof(double) * st.w.size());
+        if (perm) {
+            ep::Packed pk;
+            rc = ep::pack(st, xyz, pk, err);
+            if (rc) return fail(rc, err);
+            std::memcpy(perm, pk.perm_c.data(), sizeof(int32_t) * pk.perm_c.size());
+        }
+        return EP_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(EP_ERR_NOMEM, "host allocation failed");
+    } catch (...) {
+        return fail(EP_ERR_ARG, "unexpected exception in preprocessor");
+    }
+}
+
+int ep_mesh_create(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_tets, const int32_t* tets,
+                   const double* fibre, const double* sigma_scale, double sigma_l, double sigma_t, double chi,
+                   double Cm) {
+    if (!out) return fail(EP_ERR_ARG, "out is NULL");
+    *out = nullptr;
+    ep_sim* s = nullptr;
+    try {
+        int ndev = 0;
+        if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+            cudaGetLastError();
+            return fail(EP_ERR_CUDA, "no CUDA device: libep has no CPU fallback");
+        }
+        ep::Stencil st;
+        ep::Packed pk;
+        std::string err;
+        int rc = ep::build_stencil(n_nodes, xyz, n_tets, tets, fibre, sigma_scale, sigma_l, sigma_t, chi, Cm, st, err);
+        if (rc) return fail(rc, err);
+        rc = ep::pack(st, xyz, pk, err);
+        if (rc) return fail(rc, err);
+        s = new ep_sim();
+        s->nc = pk.nc; s->nn = pk.nn; s->nc_pad = pk.nc_pad; s->chi = chi; s->Cm = Cm;
+        s->star_entries = pk.star_entries;
+        s->perm_c = pk.perm_c; s->inv_c = pk.inv_c;
+        s->smask_host.assign(s->nc_pad, 0);
+        auto bail = [&](int code) { free_all(s); delete s; return code; };
+        if (cudaStreamCreateWithFlags(&s->own_stream, cudaStreamNonBlocking) != cudaSuccess)
+            return bail(fail(EP_ERR_CUDA, "cudaStreamCreate failed"));
+        s->stream = s->own_stream;
+        if ((rc = upload(s, &s->d_cidx, pk.cidx)) || (rc = upload(s, &s->d_ccoef, pk.ccoef)) ||
+            (rc = upload(s, &s->d_slice_ptr, pk.slice_ptr)) || (rc = upload(s, &s->d_nidx, pk.nidx)) ||
+            (rc = upload(s, &s->d_nw, pk.nw)) || (rc = upload(s, &s->d_perm, pk.perm_c)) ||
+            (rc = upload(s, &s->d_inv, pk.inv_c)))
+            return bail(rc);
+        if ((rc = dev_alloc(s, &s->d_vm[0], s->nc_pad)) || (rc = dev_alloc(s, &s->d_vm[1], s->nc_pad)) ||
+            (rc = dev_alloc(s, &s->d_vn, s->nn)) || (rc = dev_alloc(s, &s->d_tact, s->nc_pad)) ||
+            (rc = dev_alloc(s, &s->d_tmp, s->nc_pad)) || (rc = dev_alloc(s, &s->d_tmp2, s->nc_pad)) ||
+            (rc = dev_alloc(s, &s->d_red, 1024 + 8)) || (rc = dev_alloc(s, &s->d_ctype, s->nc_pad)) ||
+            (rc = dev_alloc(s, &s->d_smask, s->nc_pad)) || (rc = dev_alloc(s, &s->d_tmp8, s->nc_pad)))
+            return bail(rc);
+        cudaMemset(s->d_vm[0], 0, sizeof(double) * s->nc_pad);
+        cudaMemset(s->d_vm[1], 0, sizeof(double) * s->nc_pad);
+        cudaMemset(s->d_ctype, 0, s->nc_pad);
+        cudaMemset(s->d_smask, 0, s->nc_pad);
+        s->dm.nc = s->nc; s->dm.nn = s->nn; s->dm.nc_pad = s->nc_pad; s->dm.n_slices = pk.n_slices;
+        s->dm.cidx = s->d_cidx; s->dm.ccoef = s->d_ccoef; s->dm.slice_ptr = s->d_slice_ptr;
+        s->dm.nidx = s->d_nidx; s->dm.nw = s->d_nw;
+        if (cudaDeviceSynchronize() != cudaSuccess) return bail(fail(EP_ERR_CUDA, "upload failed"));
+        *out = s;
+        return EP_OK;
+    } catch (const std::bad_alloc&) {
+        if (s) { free_all(s); delete s; }
+        return fail(EP_ERR_NOMEM, "host allocation failed");
+    } catch (...) {
+        if (s) { free_all(s); delete s; }
+        return fail(EP_ERR_ARG, "unexpected exception");
+    }
+}
+
+void ep_destroy(ep_sim* s) {
+    if (!s) return;
+    cudaStreamSynchronize(s->stream);
+    free_all(s);
+    delete s;
+}
+
+int ep_set_stream(ep_sim* s, void* cuda_stream) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    cudaStreamSynchronize(s->stream);
+    s->stream = cuda_stream ? (cudaStream_t)cuda_stream : s->own_stream;
+    return EP_OK;
+}
+
+int ep_state_init(ep_sim* s, int model, const uint8_t* cell_type, const double* y0) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    const int S = epk::model_n_states(model);
+    if (S < 0) return fail(EP_ERR_ARG, "unknown cell model");
+    const int n_types = (model == EP_MODEL_TP06) ? 3 : 1;
+    try {
+        if (cell_type) {
+            std::vector<uint8_t> ct(s->nc_pad, 0);
+            for (int64_t i = 0; i < s->nc; ++i) {
+                const uint8_t t = cell_type[s->perm_c[i]];
+                if (t >= n_types) return fail(EP_ERR_ARG, "cell_type out of range for this model");
+                ct[i] = t;
+            }
+            EP_CUDA(s, cudaMemcpy(s->d_ctype, ct.data(), s->nc_pad, cudaMemcpyHostToDevice));
+        } else {
+            EP_CUDA(s, cudaMemset(s->d_ctype, 0, s->nc_pad));
+        }
+    } catch (const std::bad_alloc&) {
+        return fail(EP_ERR_NOMEM, "host allocation failed");
+    }
+    if (s->S != S) {
+        if (s->d_y) { cudaFree(s->d_y); s->dev_bytes -= (int64_t)sizeof(double) * s->S * s->nc_pad; s->d_y = nullptr; }
+        int rc = dev_alloc(s, &s->d_y, (int64_t)S * s->nc_pad);
+        if (rc) return rc;
+    }
+    double* d_y0 = nullptr;
+    if (y0) {
+        for (int k = 0; k < n_types * S; ++k)
+            if (!std::isfinite(y0[k])) return fail(EP_ERR_ARG, "non-finite initial state");
+        EP_CUDA(s, cudaMalloc((void**)&d_y0, sizeof(double) * n_types * S));
+        EP_CUDA(s, cudaMemcpy(d_y0, y0, sizeof(double) * n_types * S, cudaMemcpyHostToDevice));
+    }
+    s->model = model; s->S = S; s->step = 0; s->dt = 0.0; s->cur = 0; s->sticky = EP_OK;
+    epk::launch_state_fill(model, s->nc, s->nc_pad, s->d_ctype, d_y0, s->d_y, s->d_vm[0], s->d_tact, s->stream);
+    s->launches++;
+    EP_CUDA(s, cudaMemcpyAsync(s->d_vm[1], s->d_vm[0], sizeof(double) * s->nc_pad, cudaMemcpyDeviceToDevice, s->stream));
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    if (d_y0) cudaFree(d_y0);
+    return EP_OK;
+}
+
+int ep_stimulus_set(ep_sim* s, int slot, int64_t n_cells, const int64_t* cell_ids, double amp, double t0, double dur) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    if (slot < 0 || slot >= EP_MAX_STIM_SLOTS) return fail(EP_ERR_ARG, "stimulus slot out of range");
+    if (n_cells < 0 || (n_cells > 0 && !cell_ids)) return fail(EP_ERR_ARG, "bad stimulus cell list");
+    if (!std::isfinite(amp) || !std::isfinite(t0) || !std::isfinite(dur) || dur < 0.0)
+        return fail(EP_ERR_ARG, "bad stimulus amplitude or window");
+    for (int64_t k = 0; k < n_cells; ++k)
+        if (cell_ids[k] < 0 || cell_ids[k] >= s->nc) return fail(EP_ERR_ARG, "stimulus cell id out of range");
+    const uint8_t bit = (uint8_t)(1u << slot);
+    for (int64_t i = 0; i < s->nc; ++i) s->smask_host[i] &= (uint8_t)~bit;
+    for (int64_t k = 0; k < n_cells; ++k) s->smask_host[s->inv_c[cell_ids[k]]] |= bit;
+    s->stim[slot].set = n_cells > 0;
+    s->stim[slot].amp = amp; s->stim[slot].t0 = t0; s->stim[slot].dur = dur; s->stim[slot].n_cells = n_cells;
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    EP_CUDA(s, cudaMemcpy(s->d_smask, s->smask_host.data(), s->nc_pad, cudaMemcpyHostToDevice));
+    return EP_OK;
+}
+
+int ep_step(ep_sim* s, int64_t n_steps, double dt) {
+    int rc = check_sim(s);
+    if (rc) return rc;
+    if (s->model < 0) return fail(EP_ERR_STATE, "ep_step before ep_state_init");
+    if (!(dt > 0.0) || !std::isfinite(dt)) return fail(EP_ERR_STATE, "dt must be positive");
+    if (n_steps < 0) return fail(EP_ERR_ARG, "n_steps must be non-negative");
+    if (s->step > 0 && dt != s->dt) return fail(EP_ERR_STATE, "dt may not change after the first step");
+    s->dt = dt;
+    int64_t n_on[EP_MAX_STIM_SLOTS], n_off[EP_MAX_STIM_SLOTS];
+    for (int k = 0; k < EP_MAX_STIM_SLOTS; ++k) {
+        n_on[k] = n_off[k] = 0;
+        if (!s->stim[k].set) continue;
+        n_on[k] = step_index(s->stim[k].t0, dt);
+        n_off[k] = step_index(s->stim[k].t0 + s->stim[k].dur, dt);
+    }
+    for (int64_t it = 0; it < n_steps; ++it) {
+        const int64_t n = s->step;
+        epk::StepArgs a;
+        a.vm_cur = s->d_vm[s->cur]; a.vm_next = s->d_vm[s->cur ^ 1];
+        a.y = s->d_y; a.vn = s->d_vn; a.ctype = s->d_ctype; a.smask = s->d_smask; a.tact = s->d_tact;
+        a.dt = dt; a.t_next = (double)(n + 1) * dt;   // reading A17: time from the integer counter
+        for (int k = 0; k < EP_MAX_STIM_SLOTS; ++k)
+            a.istim[k] = (s->stim[k].set && n_on[k] <= n && n < n_off[k]) ? s->stim[k].amp / s->Cm : 0.0;
+        epk::launch_node_gather(s->dm, a.vm_cur, s->d_vn, s->stream);
+        epk::launch_cell_step(s->dm, s->model, a, s->stream);
+        s->launches += 2;
+        s->cur ^= 1;
+        s->step = n + 1;
+    }
+    EP_CUDA(s, cudaGetLastError());
+    return EP_OK;
+}
+
+int ep_synchronize(ep_sim* s) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    if (s->sticky != EP_OK) return fail(s->sticky, "sticky error");
+    return EP_OK;
+}
+
+int ep_read_vm(ep_sim* s, double* out) { return ep_read_state(s, 0, out); }
+
+int ep_read_state(ep_sim* s, int var, double* out) {
+    if (!s || !out) return fail(EP_ERR_ARG, "null argument");
+    if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
+    if (var < 0 || var >= s->S) return fail(EP_ERR_ARG, "state variable index out of range");
+    const double* src = (var == 0) ? s->d_vm[s->cur] : s->d_y + (int64_t)var * s->nc_pad;
+    return read_back(s, src, out);
+}
+
+int ep_write_state(ep_sim* s, int var, const double* in) {
+    if (!s || !in) return fail(EP_ERR_ARG, "null argument");
+    if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
+    if (var < 0 || var >= s->S) return fail(EP_ERR_ARG, "state variable index out of range");
+    double* dst = (var == 0) ? s->d_vm[s->cur] : s->d_y + (int64_t)var * s->nc_pad;
+    EP_CUDA(s, cudaMemcpyAsync(s->d_tmp, in, sizeof(double) * s->nc, cudaMemcpyHostToDevice, s->stream));
+    epk::launch_gather_f64(s->nc, s->d_tmp, s->d_perm, dst, s->stream);
+    s->launches++;
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    return EP_OK;
+}
+
+int ep_activation_times(ep_sim* s, double* out) {
+    if (!s || !out) return fail(EP_ERR_ARG, "null argument");
+    if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
+    return read_back(s, s->d_tact, out);
+}
+
+int ep_apply_diffusion(ep_sim* s, const double* v, double* D) {
+    if (!s || !v || !D) return fail(EP_ERR_ARG, "null argument");
+    EP_CUDA(s, cudaMemcpyAsync(s->d_tmp, v, sizeof(double) * s->nc, cudaMemcpyHostToDevice, s->stream));
+    epk::launch_gather_f64(s->nc, s->d_tmp, s->d_perm, s->d_tmp2, s->stream);
+    epk::launch_node_gather(s->dm, s->d_tmp2, s->d_vn, s->stream);
+    epk::launch_diffusion_only(s->dm, s->d_tmp2, s->d_vn, s->d_tmp, s->stream);
+    epk::launch_gather_f64(s->nc, s->d_tmp, s->d_inv, s->d_tmp2, s->stream);
+    s->launches += 4;
+    EP_CUDA(s, cudaMemcpyAsync(D, s->d_tmp2, sizeof(double) * s->nc, cudaMemcpyDeviceToHost, s->stream));
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    const double k = s->chi * s->Cm;   // the tables hold D/(chi Cm)
+    for (int64_t c = 0; c < s->nc; ++c) D[c] *= k;
+    return EP_OK;
+}
+
+int ep_stable_dt(ep_sim* s, double* dt_max) {
+    if (!s || !dt_max) return fail(EP_ERR_ARG, "null argument");
+    // power iteration on B = A/(chi Cm) [1/ms]: x <- Bx/|Bx|, rho ~ |Bx|; start from a fixed pseudo-random vector
+    try {
+        std::vector<double> x0(s->nc);
+        uint64_t z = 0x9E3779B97F4A7C15ULL;
+        for (int64_t i = 0; i < s->nc; ++i) {
+            z ^= z << 13; z ^= z >> 7; z ^= z << 17;
+            x0[i] = (double)(z >> 11) * (1.0 / 9007199254740992.0) - 0.5;
+        }
+        EP_CUDA(s, cudaMemcpyAsync(s->d_tmp, x0.data(), sizeof(double) * s->nc, cudaMemcpyHostToDevice, s->stream));
+        EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    } catch (const std::bad_alloc&) {
+        return fail(EP_ERR_NOMEM, "host allocation failed");
+    }
+    double rho = 0.0;
+    const int iters = 300;
+    for (int it = 0; it < iters; ++it) {
+        epk::launch_norm2(s->nc, s->d_tmp, s->d_red, s->d_red + 1024, s->stream);
+        epk::launch_scale_by_inv_norm(s->nc, s->d_tmp, s->d_red + 1024, s->d_tmp2, s->stream);
+        epk::launch_node_gather(s->dm, s->d_tmp2, s->d_vn, s->stream);
+        epk::launch_diffusion_only(s->dm, s->d_tmp2, s->d_vn, s->d_tmp, s->stream);
+        s->launches += 5;
+    }
+    epk::launch_norm2(s->nc, s->d_tmp, s->d_red, s->d_red + 1024, s->stream);
+    s->launches += 2;
+    double n2 = 0.0;
+    EP_CUDA(s, cudaMemcpyAsync(&n2, s->d_red + 1024, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    rho = std::sqrt(n2);
+    if (!(rho > 0.0) || !std::isfinite(rho)) return fail(EP_ERR_NUMERIC, "power iteration failed");
+    *dt_max = 2.0 / rho;
+    return EP_OK;
+}
+
+int ep_check_finite(ep_sim* s, int* all_finite) {
+    if (!s || !all_finite) return fail(EP_ERR_ARG, "null argument");
+    if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
+    epk::launch_count_nonfinite(s->nc, s->d_vm[s->cur], s->d_red, s->d_red + 1024, s->stream);
+    s->launches += 2;
+    double bad = 0.0;
+    EP_CUDA(s, cudaMemcpyAsync(&bad, s->d_red + 1024, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    *all_finite = (bad == 0.0);
+    if (bad != 0.0) {
+        s->sticky = EP_ERR_NUMERIC;
+        return fail(EP_ERR_NUMERIC, "non-finite membrane potential (explicit step unstable? see ep_stable_dt)");
+    }
+    return EP_OK;
+}
+
+int ep_device_vm(ep_sim* s, void** vm, void** perm) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    if (vm) *vm = s->d_vm[s->cur];
+    if (perm) *perm = s->d_perm;
+    return EP_OK;
+}
+
+int64_t ep_n_cells(const ep_sim* s) { return s ? s->nc : 0; }
+int64_t ep_n_nodes(const ep_sim* s) { return s ? s->nn : 0; }
+int64_t ep_step_count(const ep_sim* s) { return s ? s->step : 0; }
+double ep_time(const ep_sim* s) { return s ? (double)s->step * s->dt : 0.0; }
+int64_t ep_device_bytes(const ep_sim* s) { return s ? s->dev_bytes : 0; }
+int64_t ep_launch_count(const ep_sim* s) { return s ? s->launches : 0; }
+
+int64_t ep_step_bytes(const ep_sim* s) {
+    if (!s) return 0;
+    const int64_t S = s->S > 0 ? s->S : 19;
+    // state read + write, cell tables (12 f64 + 12 i32), node table (f64 + i32 per star entry),
+    // node values written once and read once, cell type + stimulus mask.  Gathers are assumed cache hits.
+    return s->nc * (2 * 8 * S + 12 * 12 + 2) + s->star_entries * 12 + s->nn * 16;
+}
+
+}  // extern "C"

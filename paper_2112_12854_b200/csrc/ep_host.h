@@ -1,0 +1,52 @@
+// ep_host.h -- one-time host preprocessor of libep.  Plain C++, no CUDA.
+//
+// Turns (nodes, tets, fibres, sigma) into the factored, atomic-free gather form of the paper's finite-volume
+// diffusion operator (Fig. 8 a->e, eq. (7)-(8)):
+//
+//     v_n        = sum_{k in star(n)} w_nk v_k                       (cell -> node)
+//     dv_diff[c] = sum_{m<8} a_cm v_n[node_cm] + sum_{j<4} b_cj (v[nbr_cj] - v[c])      [mV/ms] = D_c / (chi Cm)
+//
+// The algebra that collapses steps b->e into the 8 + 4 coefficients is derived in DESIGN.md section 5.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+namespace ep {
+
+struct Stencil {              // caller numbering
+    int64_t nn = 0, nc = 0;
+    std::vector<int32_t> node;     // [nc*8] node ids touched by cell c (own 4 first), unused slots = node[c*8]
+    std::vector<double> a;         // [nc*8]
+    std::vector<int32_t> nbr;      // [nc*4] face-neighbour cell (face j is opposite vertex j); boundary => c itself
+    std::vector<double> b;         // [nc*4] (0 on boundary faces: no-flux, reading A11)
+    std::vector<int64_t> node_ptr; // [nn+1]
+    std::vector<int32_t> node_cell;// [nc*4] star cells, ascending cell id
+    std::vector<double> w;         // [nc*4] inverse-distance weights, normalised per node
+    std::vector<double> centroid;  // [nc*3]
+};
+
+struct Packed {               // device numbering and device layout
+    int64_t nn = 0, nc = 0;
+    int64_t nc_pad = 0;            // nc rounded up to a multiple of 32 (column stride of the cell tables)
+    std::vector<int32_t> perm_c;   // [nc] device position -> caller cell id
+    std::vector<int32_t> inv_c;    // [nc] caller cell id -> device position
+    std::vector<int32_t> perm_n;   // [nn]
+    std::vector<int32_t> cidx;     // [12][nc_pad]: rows 0..7 device node ids, rows 8..11 device neighbour cells
+    std::vector<double> ccoef;     // [12][nc_pad]: rows 0..7 a, rows 8..11 b
+    // node table: sliced ELL, slices of 32 nodes, entries of slice s start at slice_ptr[s] (in elements) and are laid
+    // out [k][lane] with k < slice_w[s]
+    int64_t n_slices = 0;
+    std::vector<int64_t> slice_ptr;  // [n_slices+1]
+    std::vector<int32_t> nidx;       // device cell ids
+    std::vector<double> nw;
+    int64_t star_entries = 0;        // sum of node valences (= 4*nc), unpadded
+};
+
+// Returns 0 or a negative EP_ERR_* code; err receives a message.
+int build_stencil(int64_t nn, const double* xyz, int64_t nc, const int32_t* tets, const double* fibre,
+                  const double* scale, double sigma_l, double sigma_t, double chi, double Cm, Stencil& out,
+                  std::string& err);
+int pack(const Stencil& st, const double* xyz, Packed& out, std::string& err);
+
+}  // namespace ep

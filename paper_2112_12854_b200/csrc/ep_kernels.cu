@@ -1,0 +1,206 @@
+// ep_kernels.cu -- sm_100a kernels of the monodomain + TP06 step.  fp64 throughout.
+//
+// Layout: cells and nodes are in Morton order; every per-cell array is a column of length
+// nc_pad so that consecutive threads touch consecutive addresses (coalesced 8-byte loads/stores); the stencil is a
+// fixed-width gather (8 node + 4 neighbour coefficients per cell, sliced-ELL node table), so there are no atomics
+// and the result is deterministic.  Nothing here is a dense contraction: no tensor cores.
+#include "ep_kernels.cuh"
+#include "ep_tp06.cuh"
+
+namespace epk {
+
+namespace {
+
+constexpr int CELL_THREADS = 128;
+constexpr int NODE_THREADS = 256;
+
+// ---------------------------------------------------------------------------------------------------------
+// S1: cell -> node interpolation.  One warp per slice of 32 nodes; lane = node; the slice is stored [k][lane].
+__global__ void __launch_bounds__(NODE_THREADS) node_gather_kernel(int64_t nn, int64_t n_slices,
+                                                                    const int64_t* __restrict__ slice_ptr,
+                                                                    const int32_t* __restrict__ nidx,
+                                                                    const double* __restrict__ nw,
+                                                                    const double* __restrict__ vm,
+                                                                    double* __restrict__ vn) {
+    const int64_t slice = (int64_t)blockIdx.x * (NODE_THREADS / 32) + (threadIdx.x >> 5);
+    if (slice >= n_slices) return;
+    const int lane = threadIdx.x & 31;
+    const int64_t beg = slice_ptr[slice], end = slice_ptr[slice + 1];
+    double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
+    int64_t p = beg + lane;
+    for (; p + 96 < end; p += 128) {   // four independent gathers in flight
+        const int32_t i0 = nidx[p], i1 = nidx[p + 32], i2 = nidx[p + 64], i3 = nidx[p + 96];
+        const double w0 = nw[p], w1 = nw[p + 32], w2 = nw[p + 64], w3 = nw[p + 96];
+        acc0 = fma(w0, vm[i0], acc0);
+        acc1 = fma(w1, vm[i1], acc1);
+        acc2 = fma(w2, vm[i2], acc2);
+        acc3 = fma(w3, vm[i3], acc3);
+    }
+    for (; p < end; p += 32) acc0 = fma(nw[p], vm[nidx[p]], acc0);
+    const int64_t n = slice * 32 + lane;
+    if (n < nn) vn[n] = (acc0 + acc1) + (acc2 + acc3);
+}
+
+// S2+S3: the factored diffusion gather.  dv = sum_m a_m v_n[node_m] + sum_j b_j (v[nbr_j] - v_c)   [mV/ms]
+__device__ __forceinline__ double diffusion_gather(int64_t i, int64_t stride, const int32_t* __restrict__ cidx,
+                                                   const double* __restrict__ ccoef, const double* __restrict__ vm,
+                                                   const double* __restrict__ vn, double vc) {
+    int32_t id[12];
+    double cf[12];
+#pragma unroll
+    for (int m = 0; m < 12; ++m) {
+        id[m] = __ldg(cidx + m * stride + i);
+        cf[m] = __ldg(ccoef + m * stride + i);
+    }
+    double accn = 0.0, accc = 0.0;
+#pragma unroll
+    for (int m = 0; m < 8; ++m) accn = fma(cf[m], vn[id[m]], accn);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) accc = fma(cf[8 + j], vm[id[8 + j]] - vc, accc);
+    return accn + accc;
+}
+
+__global__ void __launch_bounds__(CELL_THREADS) diffusion_only_kernel(int64_t nc, int64_t stride,
+                                                                      const int32_t* __restrict__ cidx,
+                                                                      const double* __restrict__ ccoef,
+                                                                      const double* __restrict__ vm,
+                                                                      const double* __restrict__ vn,
+                                                                      double* __restrict__ out) {
+    const int64_t i = (int64_t)blockIdx.x * CELL_THREADS + threadIdx.x;
+    if (i >= nc) return;
+    out[i] = diffusion_gather(i, stride, cidx, ccoef, vm, vn, vm[i]);
+}
+
+// S2..S9 fused, TP06.  One thread per cell; state rows are read once and written once.
+__global__ void __launch_bounds__(CELL_THREADS) cell_step_tp06_kernel(int64_t nc, int64_t stride,
+                                                                      const int32_t* __restrict__ cidx,
+                                                                      const double* __restrict__ ccoef,
+                                                                      StepArgs a) {
+    const int64_t i = (int64_t)blockIdx.x * CELL_THREADS + threadIdx.x;
+    if (i >= nc) return;
+    double y[TP06_S];
+    y[0] = a.vm_cur[i];
+#pragma unroll
+    for (int k = 1; k < TP06_S; ++k) y[k] = a.y[k * stride + i];
+    const double v_old = y[0];
+    const double dv = diffusion_gather(i, stride, cidx, ccoef, a.vm_cur, a.vn, v_old);
+    // S4: stimulus, eq. (4) PAPER.md:130-132 (window already resolved on the host into istim[k])
+    const unsigned mask = a.smask[i];
+    double istim = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+        if (mask & (1u << k)) istim += a.istim[k];
+    tp06_step(y, a.ctype[i], a.dt, istim, dv);
+    a.vm_next[i] = y[0];
+#pragma unroll
+    for (int k = 1; k < TP06_S; ++k) a.y[k * stride + i] = y[k];
+    // S9: activation time = first upward crossing of 0 mV (reading A18)
+    if (v_old <= 0.0 && y[0] > 0.0) {
+        if (a.tact[i] < 0.0) a.tact[i] = a.t_next;
+    }
+}
+
+__global__ void state_fill_kernel(int S, int64_t nc, int64_t stride, const uint8_t* __restrict__ ctype,
+                                  const double* __restrict__ y0, double* __restrict__ y, double* __restrict__ vm,
+                                  double* __restrict__ tact) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= stride) return;
+    const int t = (i < nc) ? ctype[i] : 0;
+    for (int k = 0; k < S; ++k) {
+        const double val = y0 ? y0[t * S + k] : TP06_REST_STATE[k];
+        if (k == 0) vm[i] = val; else y[k * stride + i] = val;
+    }
+    tact[i] = -1.0;
+}
+
+__global__ void gather_f64_kernel(int64_t n, const double* __restrict__ src, const int32_t* __restrict__ idx,
+                                  double* __restrict__ dst) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = src[idx[i]];
+}
+__global__ void gather_u8_kernel(int64_t n, const uint8_t* __restrict__ src, const int32_t* __restrict__ idx,
+                                 uint8_t* __restrict__ dst) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = src[idx[i]];
+}
+
+// deterministic two-pass reductions: 1024 blocks x 256 threads, fixed tree
+template <int MODE>   // 0: sum of squares, 1: count of non-finite entries
+__global__ void __launch_bounds__(256) reduce_partial_kernel(int64_t n, const double* __restrict__ x,
+                                                              double* __restrict__ partial) {
+    __shared__ double sh[256];
+    double acc = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (int64_t)gridDim.x * 256) {
+        const double v = x[i];
+        acc += (MODE == 0) ? v * v : (isfinite(v) ? 0.0 : 1.0);
+    }
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+        if ((int)threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+__global__ void __launch_bounds__(1024) reduce_final_kernel(const double* __restrict__ partial, double* out) {
+    __shared__ double sh[1024];
+    sh[threadIdx.x] = partial[threadIdx.x];
+    __syncthreads();
+    for (int s = 512; s > 0; s >>= 1) {
+        if ((int)threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[0] = sh[0];
+}
+__global__ void scale_by_inv_norm_kernel(int64_t n, const double* __restrict__ x, const double* __restrict__ norm2,
+                                         double* __restrict__ out) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = x[i] / sqrt(norm2[0]);
+}
+
+inline unsigned blocks_for(int64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+}  // namespace
+
+int model_n_states(int model) { return model == 0 ? (int)TP06_S : -1; }
+
+void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaStream_t s) {
+    const unsigned grid = blocks_for(m.n_slices, NODE_THREADS / 32);
+    node_gather_kernel<<<grid, NODE_THREADS, 0, s>>>(m.nn, m.n_slices, m.slice_ptr, m.nidx, m.nw, vm, vn);
+}
+
+void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStream_t s) {
+    (void)model;
+    cell_step_tp06_kernel<<<blocks_for(m.nc, CELL_THREADS), CELL_THREADS, 0, s>>>(m.nc, m.nc_pad, m.cidx, m.ccoef, a);
+}
+
+void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* vn, double* out, cudaStream_t s) {
+    diffusion_only_kernel<<<blocks_for(m.nc, CELL_THREADS), CELL_THREADS, 0, s>>>(m.nc, m.nc_pad, m.cidx, m.ccoef, vm,
+                                                                                  vn, out);
+}
+
+void launch_state_fill(int model, int64_t nc, int64_t nc_pad, const uint8_t* ctype, const double* y0_dev, double* y,
+                       double* vm, double* tact, cudaStream_t s) {
+    state_fill_kernel<<<blocks_for(nc_pad, 256), 256, 0, s>>>(model_n_states(model), nc, nc_pad, ctype, y0_dev, y, vm,
+                                                              tact);
+}
+
+void launch_gather_f64(int64_t n, const double* src, const int32_t* idx, double* dst, cudaStream_t s) {
+    gather_f64_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, src, idx, dst);
+}
+void launch_gather_u8(int64_t n, const uint8_t* src, const int32_t* idx, uint8_t* dst, cudaStream_t s) {
+    gather_u8_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, src, idx, dst);
+}
+void launch_norm2(int64_t n, const double* x, double* partial, double* out, cudaStream_t s) {
+    reduce_partial_kernel<0><<<1024, 256, 0, s>>>(n, x, partial);
+    reduce_final_kernel<<<1, 1024, 0, s>>>(partial, out);
+}
+void launch_count_nonfinite(int64_t n, const double* x, double* partial, double* out, cudaStream_t s) {
+    reduce_partial_kernel<1><<<1024, 256, 0, s>>>(n, x, partial);
+    reduce_final_kernel<<<1, 1024, 0, s>>>(partial, out);
+}
+void launch_scale_by_inv_norm(int64_t n, const double* x, const double* norm2, double* out, cudaStream_t s) {
+    scale_by_inv_norm_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, x, norm2, out);
+}
+
+}  // namespace epk

@@ -1,0 +1,49 @@
+// ep_kernels.cuh -- launch interface between the C-ABI layer (ep_api.cu) and the sm_100a kernels (ep_kernels.cu).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace epk {
+
+struct DeviceMesh {
+    int64_t nc = 0, nn = 0, nc_pad = 0, n_slices = 0;
+    const int32_t* cidx = nullptr;      // [12][nc_pad]
+    const double* ccoef = nullptr;      // [12][nc_pad]
+    const int64_t* slice_ptr = nullptr; // [n_slices+1]
+    const int32_t* nidx = nullptr;
+    const double* nw = nullptr;
+};
+
+struct StepArgs {
+    const double* vm_cur;   // [nc_pad]
+    double* vm_next;        // [nc_pad]
+    double* y;              // [S][nc_pad]; row 0 unused (Vm lives in vm_cur/vm_next)
+    double* vn;             // [nn] node values scratch
+    const uint8_t* ctype;   // [nc_pad]
+    const uint8_t* smask;   // [nc_pad] bit k = cell belongs to stimulus slot k
+    double* tact;           // [nc_pad]
+    double dt;
+    double t_next;          // (n+1)*dt, recorded on an upward crossing of 0 mV
+    double istim[8];        // I_s/C_m of each slot at step n (0 when the slot's window is closed)
+};
+
+// S1 of SURVEY 8(a): v_n = sum_k w_nk v_k
+void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaStream_t s);
+// S2..S9 fused: diffusion gather + stimulus + cell model + RL/FE updates + Vm write + activation record
+void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStream_t s);
+// diagnostics: out[i] = D_c/(chi Cm) [mV/ms] from vm and vn
+void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* vn, double* out, cudaStream_t s);
+// fill y rows with one state vector per cell type; y0 is a DEVICE pointer [n_types*S]; NULL = built-in rest state
+void launch_state_fill(int model, int64_t nc, int64_t nc_pad, const uint8_t* ctype, const double* y0_dev, double* y,
+                       double* vm, double* tact, cudaStream_t s);
+// permutation helpers: dst[i] = src[idx[i]]
+void launch_gather_f64(int64_t n, const double* src, const int32_t* idx, double* dst, cudaStream_t s);
+void launch_gather_u8(int64_t n, const uint8_t* src, const int32_t* idx, uint8_t* dst, cudaStream_t s);
+// reductions for the power iteration and the finite check (deterministic two-pass)
+void launch_norm2(int64_t n, const double* x, double* partial /*[1024]*/, double* out /*[1]*/, cudaStream_t s);
+void launch_scale_by_inv_norm(int64_t n, const double* x, const double* norm2, double* out, cudaStream_t s);
+void launch_count_nonfinite(int64_t n, const double* x, double* partial, double* out, cudaStream_t s);
+
+int model_n_states(int model);
+
+}  // namespace epk
