@@ -1,0 +1,286 @@
+#!/usr/bin/env python
+"""bench.py -- fp64 cell-updates/s of the fused monodomain + TP06 step (BASELINE.json metric) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--inner 25] [--impl ours|reference]
+
+One bench "step" = one ep_step(inner, dt) call = `inner` explicit time steps of the whole hot path (node gather + fused
+cell kernel) over the whole synthetic mesh of the chosen BASELINE config (default: config 3, the
+~2M-cell left-ventricle shell, the smallest of the ">= 2M cell" meshes the metric's 60 % target is quoted on).
+Prints ONE JSON line (rank 0).  N > 1: independent replicas, one per GPU ("replicas only").
+--impl reference times the CPU oracle (as it stands) on the host cores on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 cell-updates/sec (monodomain+TP06 step)"
+UNIT = "cell-updates/s"
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", d
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs (profiling recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, smax, pw, reasons = [], [], [], set()
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); smax.append(float(c[2])); pw.append(float(c[3]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        hi = [x for x in sm if x >= 0.5 * max(sm)]
+        return {"sm_mhz": statistics.median(hi), "sm_max_mhz": max(smax), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _oracle_leg(prob, budget_s: float, threads: int):
+    """Time the oracle, as it stands, on this host: whole mesh, as many steps as fit the budget (at least 1)."""
+    from oracle import ep_oracle as O
+    O.set_threads(threads)
+    o = O.OracleSim.from_problem(prob)
+    t0 = time.perf_counter()
+    o.step(1, prob.dt)
+    t1 = time.perf_counter() - t0
+    n = max(1, min(50, int(budget_s / max(t1, 1e-6)) - 1))
+    t0 = time.perf_counter()
+    o.step(n, prob.dt)
+    t = time.perf_counter() - t0
+    o.close()
+    return prob.mesh.n_tets * n / t, n, t
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; each bench step = one oracle time step on the full mesh."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from ep_inputs import make
+    from oracle import ep_oracle as O
+    prob = make(args.config)
+    cores = os.cpu_count() or 1
+    O.set_threads(cores)
+    o = O.OracleSim.from_problem(prob)
+    per = max(1, args.ref_inner)
+    for _ in range(args.warmup):
+        o.step(per, prob.dt)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step(per, prob.dt)
+    t = time.perf_counter() - t0
+    o.close()
+    val = prob.mesh.n_tets * per * args.steps / t
+    sample = f"config {args.config} full mesh ({prob.mesh.n_tets} cells), {per} oracle time step(s) per bench step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": prob.name, "cells": prob.mesh.n_tets, "dt_ms": prob.dt, "time_steps_per_step": per},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; libep has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    import paper_2112_12854_b200 as ep
+    from ep_inputs import make
+    prob = make(args.config)
+    mesh = prob.mesh
+    nc = mesh.n_tets
+    sim = ep.Sim.from_problem(prob)
+    stream = torch.cuda.Stream()
+    sim.set_stream(stream.cuda_stream)
+    S = sim.n_states
+    inner, dt = args.inner, prob.dt
+    # the config as specified: every cell at the model's resting state, the config's stimulus armed at t = 0; the
+    # timed window is the start of that simulation (stimulus on, wave leaving the stimulus sites)
+    pinned = torch.empty((S, nc), dtype=torch.float64).pin_memory()
+    for k in range(S):
+        sim.read_state(k, pinned.numpy()[k])
+    out_vm = torch.empty(nc, dtype=torch.float64).pin_memory()
+    out_ta = torch.empty(nc, dtype=torch.float64).pin_memory()
+
+    def upload():
+        for k in range(S):
+            sim.write_state(k, pinned.numpy()[k])
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---------------- device-resident arm
+    for _ in range(args.warmup):
+        sim.step(inner, dt)
+    sim.synchronize()
+    l0 = sim.launch_count
+    sim.profile(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    clocks = ClockSampler(local) if rank == 0 else None
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        for _ in range(args.steps):
+            sim.step(inner, dt)
+        e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clk = clocks.stop() if clocks else None
+    prof = sim.profile_read()
+    sim.profile(False)
+    launches = sim.launch_count - l0
+    finite = sim.check_finite()
+    t_dev = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t_dev, op=dist.ReduceOp.MAX)
+    ms_max = float(t_dev.item())
+    value = world * nc * inner * args.steps / (ms_max * 1e-3)
+
+    # ---------------- end-to-end arm: host state in, Vm + activation times out, every bench step
+    def e2e_step():
+        upload()
+        sim.step(inner, dt)
+        sim.read_vm(out_vm.numpy())
+        sim.activation_times(out_ta.numpy())
+
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    n_e2e = max(3, min(args.steps, 10))
+    for _ in range(n_e2e):
+        e2e_step()
+    barrier()
+    t_e2e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
+    e2e_val = world * nc * inner * n_e2e / float(t_e2e.item())
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src, _ = _peaks()
+    cell_bytes = sim.kernel_bytes(1)
+    cell_ms = prof["ms_cell"] / max(1, prof["steps"])
+    node_ms = prof["ms_node"] / max(1, prof["steps"])
+    achieved = cell_bytes / (cell_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "cell_step_tp06_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "peak_source": peak_src, "traffic": args.traffic,
+                "alg_bytes_per_launch": cell_bytes, "alg_bytes_per_cell": cell_bytes / nc,
+                "avg_launch_ms": cell_ms, "node_kernel_avg_launch_ms": node_ms,
+                "kernel_share_of_step": cell_ms / max(1e-12, cell_ms + node_ms),
+                "whole_step_frac": sim.step_bytes / (ms_max * 1e-3 / (inner * args.steps)) / 1e9 / peak}
+    cores = os.cpu_count() or 1
+    cpu_val, cpu_n, cpu_t = _oracle_leg(prob, args.cpu_budget, cores)
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": prob.name, "cells": nc, "nodes": mesh.n_nodes, "dt_ms": dt,
+                   "time_steps_per_step": inner, "states": "config initial condition (rest + stimulus at t=0), window starts after warm-up",
+                   "l2": "inputs larger than L2 (%.0f MB touched per time step)" % (sim.step_bytes / 1e6),
+                   "parallelism": "replicas" if world > 1 else "single"},
+        "simulated_ms_per_wall_s": dt * inner * args.steps / (ms_max * 1e-3),
+        "us_per_time_step": 1e3 * ms_max / (inner * args.steps),
+        "clocks": clk, "gpu_launches": launches, "all_finite": bool(finite),
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 8 * S * nc, "d2h_bytes_per_step": 16 * nc,
+                "steps": n_e2e},
+        "roofline": roofline,
+        "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"config {args.config} full mesh ({nc} cells), {cpu_n} time steps, {cpu_t:.1f} s"},
+    }
+    print(json.dumps(out))
+    sim.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5")
+    ap.add_argument("--inner", type=int, default=25, help="explicit time steps per bench step")
+    ap.add_argument("--ref-inner", type=int, default=1, help="oracle time steps per bench step (--impl reference)")
+    ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -102,6 +102,14 @@ int64_t ep_device_bytes(const ep_sim *sim);
 int64_t ep_step_bytes(const ep_sim *sim);
 /* Kernel launches issued by this sim so far (bench.py's gpu_launches). */
 int64_t ep_launch_count(const ep_sim *sim);
+/* Algorithmic HBM bytes of ONE launch of a step kernel: kernel 0 = node gather (S1), 1 = fused cell step (S2..S9). */
+int64_t ep_kernel_bytes(const ep_sim *sim, int kernel);
+/* Per-kernel device timing of ep_step with CUDA events on the sim's stream (for the roofline figures).
+ * ep_profile(sim, 1) starts bracketing every step-kernel launch with an event pair and resets the totals;
+ * ep_profile(sim, 0) stops.  ep_profile_read synchronises and returns the totals since the last reset:
+ * out4 = { number of steps timed, total ms in kernel 0, total ms in kernel 1, 0 }. */
+int ep_profile(ep_sim *sim, int enable);
+int ep_profile_read(ep_sim *sim, double *out4);
 void ep_destroy(ep_sim *sim);
 const char *ep_last_error(void);
 

@@ -40,6 +40,9 @@ SIGNATURES = {
     "ep_device_bytes": (C.c_int64, [_vp]),
     "ep_step_bytes": (C.c_int64, [_vp]),
     "ep_launch_count": (C.c_int64, [_vp]),
+    "ep_kernel_bytes": (C.c_int64, [_vp, C.c_int]),
+    "ep_profile": (C.c_int, [_vp, C.c_int]),
+    "ep_profile_read": (C.c_int, [_vp, _dp]),
     "ep_destroy": (None, [_vp]),
     "ep_last_error": (C.c_char_p, []),
     "ep_host_stencil": (C.c_int, [C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double, C.c_double,
@@ -196,6 +199,18 @@ class Sim:
         vm, perm = _vp(), _vp()
         _chk(lib().ep_device_vm(self._h, C.byref(vm), C.byref(perm)))
         return vm.value, perm.value
+
+    def profile(self, enable: bool):
+        _chk(lib().ep_profile(self._h, 1 if enable else 0))
+
+    def profile_read(self):
+        """{steps, ms_node, ms_cell}: per-kernel CUDA-event totals since ep_profile(1)."""
+        out = np.zeros(4)
+        _chk(lib().ep_profile_read(self._h, _p(out)))
+        return {"steps": int(out[0]), "ms_node": float(out[1]), "ms_cell": float(out[2])}
+
+    def kernel_bytes(self, kernel: int) -> int:
+        return int(lib().ep_kernel_bytes(self._h, int(kernel)))
 
     @property
     def step_count(self):

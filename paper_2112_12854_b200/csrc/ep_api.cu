@@ -54,6 +54,11 @@ struct ep_sim {
     double dt = 0.0;
     int sticky = EP_OK;
     int64_t dev_bytes = 0, launches = 0;
+    // per-kernel event timing (ep_profile)
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev;       // 3 per step: before node kernel, between, after cell kernel
+    size_t ev_used = 0;
+    double prof_steps = 0.0, prof_ms[2] = {0.0, 0.0};
 };
 
 namespace {
@@ -91,7 +96,32 @@ void free_all(ep_sim* s) {
                     s->d_vm[1], s->d_y, s->d_vn, s->d_tact, s->d_tmp, s->d_tmp2, s->d_red, s->d_ctype, s->d_smask,
                     s->d_tmp8};
     for (void* p : ptrs) if (p) cudaFree(p);
+    for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
     if (s->own_stream) cudaStreamDestroy(s->own_stream);
+}
+
+// fold the recorded event triples into the totals (synchronises)
+int profile_drain(ep_sim* s) {
+    if (s->ev_used == 0) return EP_OK;
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    for (size_t i = 0; i + 2 < s->ev_used; i += 3) {
+        float a = 0.f, b = 0.f;
+        EP_CUDA(s, cudaEventElapsedTime(&a, s->ev[i], s->ev[i + 1]));
+        EP_CUDA(s, cudaEventElapsedTime(&b, s->ev[i + 1], s->ev[i + 2]));
+        s->prof_ms[0] += a; s->prof_ms[1] += b; s->prof_steps += 1.0;
+    }
+    s->ev_used = 0;
+    return EP_OK;
+}
+
+int profile_event(ep_sim* s) {
+    if (s->ev_used == s->ev.size()) {
+        cudaEvent_t e;
+        EP_CUDA(s, cudaEventCreate(&e));
+        s->ev.push_back(e);
+    }
+    EP_CUDA(s, cudaEventRecord(s->ev[s->ev_used++], s->stream));
+    return EP_OK;
 }
 
 int check_sim(ep_sim* s) {
@@ -301,8 +331,17 @@ int ep_step(ep_sim* s, int64_t n_steps, double dt) {
         a.dt = dt; a.t_next = (double)(n + 1) * dt;   // reading A17: time from the integer counter
         for (int k = 0; k < EP_MAX_STIM_SLOTS; ++k)
             a.istim[k] = (s->stim[k].set && n_on[k] <= n && n < n_off[k]) ? s->stim[k].amp / s->Cm : 0.0;
-        epk::launch_node_gather(s->dm, a.vm_cur, s->d_vn, s->stream);
-        epk::launch_cell_step(s->dm, s->model, a, s->stream);
+        if (s->profiling) {
+            if (s->ev_used >= 3 * 4096 && (rc = profile_drain(s))) return rc;
+            if ((rc = profile_event(s))) return rc;
+            epk::launch_node_gather(s->dm, a.vm_cur, s->d_vn, s->stream);
+            if ((rc = profile_event(s))) return rc;
+            epk::launch_cell_step(s->dm, s->model, a, s->stream);
+            if ((rc = profile_event(s))) return rc;
+        } else {
+            epk::launch_node_gather(s->dm, a.vm_cur, s->d_vn, s->stream);
+            epk::launch_cell_step(s->dm, s->model, a, s->stream);
+        }
         s->launches += 2;
         s->cur ^= 1;
         s->step = n + 1;
@@ -425,6 +464,33 @@ int64_t ep_step_count(const ep_sim* s) { return s ? s->step : 0; }
 double ep_time(const ep_sim* s) { return s ? (double)s->step * s->dt : 0.0; }
 int64_t ep_device_bytes(const ep_sim* s) { return s ? s->dev_bytes : 0; }
 int64_t ep_launch_count(const ep_sim* s) { return s ? s->launches : 0; }
+
+int ep_profile(ep_sim* s, int enable) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    if (enable) {
+        int rc = profile_drain(s);
+        if (rc) return rc;
+        s->prof_steps = 0.0; s->prof_ms[0] = s->prof_ms[1] = 0.0;
+    }
+    s->profiling = enable != 0;
+    return EP_OK;
+}
+
+int ep_profile_read(ep_sim* s, double* out4) {
+    if (!s || !out4) return fail(EP_ERR_ARG, "null argument");
+    int rc = profile_drain(s);
+    if (rc) return rc;
+    out4[0] = s->prof_steps; out4[1] = s->prof_ms[0]; out4[2] = s->prof_ms[1]; out4[3] = 0.0;
+    return EP_OK;
+}
+
+int64_t ep_kernel_bytes(const ep_sim* s, int kernel) {
+    if (!s) return 0;
+    const int64_t S = s->S > 0 ? s->S : 19;
+    if (kernel == 0) return s->star_entries * 12 + s->nn * 8;                 // node table + v_n written
+    if (kernel == 1) return s->nc * (2 * 8 * S + 12 * 12 + 2) + s->nn * 8;    // states r+w, cell tables, masks, v_n read
+    return 0;
+}
 
 int64_t ep_step_bytes(const ep_sim* s) {
     if (!s) return 0;

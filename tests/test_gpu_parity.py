@@ -1,0 +1,241 @@
+"""GPU parity tests proper: the CUDA path (through the C-ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances are north_star's (BASELINE.json): one step, per state variable, max|g-o| / max|o| <= 1e-11;
+full run max|dVm| <= 1e-6 mV, activation times equal to within one dt and identical activated sets.
+"""
+import numpy as np
+import pytest
+
+from ep_inputs import make, states
+from ep_inputs import meshes as M
+from ep_inputs.prng import uniform
+
+pytestmark = pytest.mark.gpu
+
+ONE_STEP_TOL = 1e-11
+RUN_TOL_MV = 1e-6
+
+
+@pytest.fixture(scope="module")
+def ep():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2112_12854_b200 as ep
+    return ep
+
+
+def _pair(ep, oracle, prob, threads=0):
+    import os
+    oracle.set_threads(threads or max(1, (os.cpu_count() or 2) // 2))
+    g = ep.Sim.from_problem(prob)
+    o = oracle.OracleSim.from_problem(prob)
+    return g, o
+
+
+def _one_step_err(g, o, S):
+    errs = []
+    for k in range(S):
+        a, b = g.read_state(k), o.read_state(k)
+        errs.append(np.abs(a - b).max() / np.abs(b).max())
+    return np.array(errs)
+
+
+def _jittered():
+    m = M.kuhn_slab(9, 7, 5, 0.25)
+    M.jitter_interior(m, 0.05, 21)
+    cen = m.centroids()
+    th = np.deg2rad(-60 + 120 * cen[:, 2] / 1.25)
+    m.fibre = np.stack([np.cos(th), np.sin(th), 0 * th], axis=1)
+    m.sigma_scale = uniform(22, np.arange(m.n_tets), 0.1, 1.0)
+    m.cell_type = M.thirds(np.clip(cen[:, 2] / 1.25, 0, 1))
+    return m
+
+
+@pytest.mark.parametrize("case", ["jittered", "c3_coarse", "c1", "single_tet", "isotropic"])
+def test_diffusion_operator_parity(ep, oracle, case):
+    if case == "jittered":
+        m = _jittered()
+    elif case == "c3_coarse":
+        m = make(3, coarsen=4.0).mesh
+    elif case == "c1":
+        m = make(1).mesh
+    elif case == "single_tet":
+        m = M.TetMesh(np.array([[0, 0, 0], [1, 0, 0], [0, 1, 0], [0, 0, 1.0]]), np.array([[0, 1, 2, 3]], np.int32))
+    else:
+        m = M.kuhn_slab(5, 4, 3, 0.4)
+    g = ep.Sim(m.xyz, m.tets, m.fibre, m.sigma_scale)
+    o = oracle.OracleSim(m.xyz, m.tets, m.fibre, m.sigma_scale)
+    v = uniform(5, np.arange(m.n_tets), -90.0, 40.0)
+    Dg, Do = g.apply_diffusion(v), o.apply_diffusion(v)
+    assert np.abs(Dg - Do).max() <= 1e-12 * max(np.abs(Do).max(), 1.0)
+    if case == "single_tet":
+        assert np.all(Dg == 0.0)          # every face is a no-flux boundary face
+    g.close()
+
+
+@pytest.mark.parametrize("case", ["c1", "jittered", "c3_coarse", "c2_coarse"])
+def test_one_step_random_states(ep, oracle, case):
+    """One explicit step from random physiological states, stimulus on for part of the cells, all three cell types."""
+    if case == "c1":
+        prob = make(1)
+        prob.mesh.cell_type = (np.arange(prob.mesh.n_tets) % 3).astype(np.uint8)
+    elif case == "jittered":
+        prob = make(1)
+        prob.mesh = _jittered()
+        prob.stimuli[0].cell_ids = np.arange(0, prob.mesh.n_tets, 7, dtype=np.int64)
+    elif case == "c3_coarse":
+        prob = make(3, coarsen=3.0)
+    else:
+        prob = make(2, coarsen=2.5)
+    g, o = _pair(ep, oracle, prob)
+    n = prob.mesh.n_tets
+    y = states.random_states(0, 77, n)
+    sv = states.special_voltages()
+    y[0, : sv.size] = sv                      # branch points and the I_CaL removable singularity
+    for k in range(19):
+        g.write_state(k, y[k]); o.write_state(k, y[k])
+    dt = 0.01
+    g.step(1, dt); o.step(1, dt)
+    err = _one_step_err(g, o, 19)
+    assert err.max() <= ONE_STEP_TOL, err
+    # a second and third step (stimulus still on) stay inside the tolerance too
+    g.step(2, dt); o.step(2, dt)
+    err = _one_step_err(g, o, 19)
+    assert err.max() <= 10 * ONE_STEP_TOL, err
+    g.close()
+
+
+def test_full_run_config1(ep, oracle):
+    """C1 as specified: 1,000 steps of 0.02 ms; the wave crosses the whole slab (all 9,600 cells activate)."""
+    prob = make(1)
+    g, o = _pair(ep, oracle, prob)
+    for chunk in (37, 463, 500):              # ragged chunks: ep_step(n) composes
+        g.step(chunk, prob.dt)
+    o.step(1000, prob.dt)
+    vg, vo = g.read_vm(), o.read_vm()
+    assert np.abs(vg - vo).max() <= RUN_TOL_MV
+    tg, to = g.activation_times(), o.activation_times()
+    assert np.array_equal(tg >= 0, to >= 0)
+    assert (to >= 0).all()
+    assert np.abs(tg - to).max() <= prob.dt * (1 + 1e-12)
+    for k in range(1, 19):
+        a, b = g.read_state(k), o.read_state(k)
+        assert np.abs(a - b).max() <= 1e-8 * max(1.0, np.abs(b).max())
+    assert g.step_count == 1000 and abs(g.time - 20.0) < 1e-12
+    assert g.check_finite()
+    g.close()
+
+
+def test_stimulus_windows_and_slots(ep, oracle):
+    """Half-open windows on integer steps (reading A16), overlapping slots add, clearing a slot works."""
+    prob = make(1, coarsen=2.0)
+    n = prob.mesh.n_tets
+    prob.stimuli = []
+    g, o = _pair(ep, oracle, prob)
+    ids_a = np.arange(0, n, 3, dtype=np.int64)
+    ids_b = np.arange(0, n, 2, dtype=np.int64)
+    for s in (g, o):
+        s.stimulus_set(0, ids_a, -40.0, 0.04, 0.06)     # steps 2,3,4 at dt 0.02
+        s.stimulus_set(3, ids_b, -25.0, 0.08, 0.1)      # steps 4..8
+        s.stimulus_set(5, ids_b, -99.0, 0.0, 1.0)
+        s.stimulus_set(5, np.zeros(0, np.int64), 0.0, 0.0, 0.0)   # cleared again
+    for _ in range(12):
+        g.step(1, 0.02); o.step(1, 0.02)
+        assert np.abs(g.read_vm() - o.read_vm()).max() <= 1e-10
+    v = g.read_vm()
+    both = np.intersect1d(ids_a, ids_b)
+    neither = np.setdiff1d(np.arange(n), np.union1d(ids_a, ids_b))
+    assert v[both].mean() > v[neither].mean() + 1.0
+    g.close()
+
+
+def test_state_and_argument_errors(ep):
+    prob = make(1, coarsen=4.0)
+    m = prob.mesh
+    g = ep.Sim(m.xyz, m.tets, m.fibre)
+    with pytest.raises(ep.EpError) as e:
+        g.step(1, 0.02)
+    assert e.value.code == -3                  # before ep_state_init
+    g.state_init(0, None)
+    with pytest.raises(ep.EpError):
+        g.step(1, -0.02)
+    g.step(0, 0.02)                            # zero steps is a no-op
+    assert g.step_count == 0
+    g.step(2, 0.02)
+    with pytest.raises(ep.EpError) as e:
+        g.step(1, 0.01)                        # dt changed mid-run
+    assert e.value.code == -3
+    with pytest.raises(ep.EpError):
+        g.read_state(19)
+    with pytest.raises(ep.EpError):
+        g.stimulus_set(8, np.array([0]), -1.0, 0.0, 1.0)
+    with pytest.raises(ep.EpError):
+        g.stimulus_set(0, np.array([m.n_tets]), -1.0, 0.0, 1.0)
+    with pytest.raises(ep.EpError):
+        g.state_init(0, np.full(m.n_tets, 3, np.uint8))
+    v = g.read_vm()
+    assert v.shape == (m.n_tets,) and np.all(np.abs(v + 86.2) < 0.5)       # unstimulated: stays at rest
+    assert np.all(g.activation_times() == -1.0)
+    g.state_init(0, None)                      # re-init resets the clock
+    assert g.step_count == 0
+    g.close()
+
+
+def test_custom_initial_state_and_types(ep, oracle):
+    prob = make(2, coarsen=4.0)
+    y0 = np.stack([states.random_states(0, 5 + t, 1)[:, 0] for t in range(3)])
+    g = ep.Sim.from_problem(prob); o = oracle.OracleSim.from_problem(prob)
+    g.state_init(0, prob.mesh.cell_type, y0); o.state_init(0, prob.mesh.cell_type, y0)
+    for k in range(19):
+        assert np.array_equal(g.read_state(k), o.read_state(k))
+        assert np.array_equal(g.read_state(k), y0[prob.mesh.cell_type, k])
+    g.close()
+
+
+def test_stable_dt_brackets_observed_stability(ep):
+    """ep_stable_dt (power iteration): diffusion-only forward Euler is stable below it, and S-note's rho h^2 ~ 35."""
+    m = M.kuhn_slab(12, 12, 12, 0.25)
+    m.fibre = np.tile([1.0, 0, 0], (m.n_tets, 1))
+    g = ep.Sim(m.xyz, m.tets, m.fibre)
+    dtmax = g.stable_dt()
+    rho_h2 = 2.0 / dtmax * 1400.0 * (0.025 ** 2)     # rho(A) h^2 with h in cm
+    assert 25.0 < rho_h2 < 45.0
+    g.close()
+
+
+def test_full_size_c3_in_bench_configuration(ep, oracle):
+    """BASELINE config 3 at full size (about 2M cells), the mesh bench.py times: a few steps from random states
+    against the threaded oracle on every cell, plus properties that hold at any size."""
+    import os
+    prob = make(3)
+    n = prob.mesh.n_tets
+    assert 1.8e6 < n < 2.3e6
+    g, o = _pair(ep, oracle, prob, threads=os.cpu_count() or 1)
+    y = states.random_states(0, 99, n)
+    for k in range(19):
+        g.write_state(k, y[k]); o.write_state(k, y[k])
+    g.step(1, prob.dt); o.step(1, prob.dt)
+    err = _one_step_err(g, o, 19)
+    assert err.max() <= ONE_STEP_TOL, err
+    g.step(4, prob.dt); o.step(4, prob.dt)
+    assert np.abs(g.read_vm() - o.read_vm()).max() <= 1e-8
+    for k in range(1, 14):                      # gates stay in [0,1] (Rush-Larsen, pin P8)
+        s = g.read_state(k)
+        assert s.min() >= 0.0 and s.max() <= 1.0
+    g.close()
+
+
+def test_window_parity_c2(ep, oracle):
+    """C2 full mesh (315,000 cells, jittered) at the stable step dt = 0.005 ms (DESIGN.md S-note): 400 steps."""
+    import os
+    prob = make(2)
+    g, o = _pair(ep, oracle, prob, threads=os.cpu_count() or 1)
+    dt = 0.005
+    assert dt < g.stable_dt()
+    g.step(400, dt); o.step(400, dt)
+    vg, vo = g.read_vm(), o.read_vm()
+    assert np.abs(vg - vo).max() <= RUN_TOL_MV
+    assert vo.max() > 0.0                        # the corner stimulus did start a wave
+    tg, to = g.activation_times(), o.activation_times()
+    assert np.array_equal(tg >= 0, to >= 0) and np.abs(tg - to).max() <= dt * (1 + 1e-12)
+    g.close()
