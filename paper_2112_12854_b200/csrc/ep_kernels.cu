@@ -76,6 +76,8 @@ __global__ void __launch_bounds__(CELL_THREADS) cell_step_tp06_kernel(int64_t nc
                                                                       const int32_t* __restrict__ cidx,
                                                                       const double* __restrict__ ccoef,
                                                                       StepArgs a) {
+    // per-thread columns of the transcendental batches (ep_math.cuh): slot s of thread t at xs[s][t]
+    __shared__ double xs[tp06::N_SLOTS][CELL_THREADS];
     const int64_t i = (int64_t)blockIdx.x * CELL_THREADS + threadIdx.x;
     if (i >= nc) return;
     double y[TP06_S];
@@ -90,7 +92,7 @@ __global__ void __launch_bounds__(CELL_THREADS) cell_step_tp06_kernel(int64_t nc
 #pragma unroll
     for (int k = 0; k < 8; ++k)
         if (mask & (1u << k)) istim += a.istim[k];
-    tp06_step(y, a.ctype[i], a.dt, istim, dv);
+    tp06_step<CELL_THREADS>(y, a.ctype[i], a.dt, istim, dv, &xs[0][threadIdx.x]);
     a.vm_next[i] = y[0];
 #pragma unroll
     for (int k = 1; k < TP06_S; ++k) a.y[k * stride + i] = y[k];

@@ -1,113 +1,113 @@
 // ep_math.cuh -- fp64 device math for the cell-model kernels (sm_100a).
 //
-// The B200 fp64 pipe (64 lanes/SM) is the co-limiting resource of the fused step, so the
-// transcendental and division sequences are written out here with exactly the work the cell model needs:
-//   - ep_rcp / ep_div: MUFU.RCP64H seed + two Newton steps, no special-case slow path (arguments are finite, normal
-//     and far from the ends of the exponent range in every call site);
-//   - ep_exp: Cody-Waite reduction + degree-13 polynomial, argument clamped to [-700, 700] (no overflow, underflow
-//     or NaN handling: call sites pass finite arguments);
-//   - ep_log: frexp by bit manipulation + atanh series in s = (m-1)/(m+1).
-// Accuracy of each is <= 2 ulp over the ranges used (tests/test_gpu_math.py measures it against numpy on the GPU box),
-// four orders of magnitude inside the 1e-11 one-step parity tolerance.
+// The B200 fp64 pipe (64 lanes/SM, one warp instruction per 2 cycles per SM sub-partition) and the issue slots are the
+// co-limiting resources of the fused step.  The ncu capture of the first version
+// (profiles/r1a_*.md) showed three things this file is built around:
+//   * 64-bit literals cost two extra issue slots each (UMOV pairs) unless they come from the constant bank through
+//     LDCU.128 into uniform registers  ->  polynomial coefficients live in __constant__ arrays;
+//   * 60 inlined exponentials made the kernel 86 KB of SASS, far beyond the 32 KB instruction cache (top stall:
+//     no_instruction)  ->  exponentials and logarithms are evaluated in BATCHES: a thread writes its arguments into
+//     its own column of a shared-memory slot array and one rolled loop (two arguments per trip for ILP) replaces
+//     them by their exponentials; the loop body exists once in the kernel and its constants stay in uniform registers;
+//   * IEEE division is ~10 fp64 instructions plus a slow-path call  ->  ep_rcp: MUFU.RCP64H seed + one third-order
+//     step (3 DFMA), arguments are finite, normal and far from the ends of the exponent range at every call site.
+// Accuracy: exp and log <= 1 ulp-ish (polynomial error 2e-17), rcp <= 1 ulp, a*rcp(b) <= 2 ulp; measured on the
+// GPU by tests/test_gpu_math.py.  No lookup tables (north_star: "precomputed-free exp paths").
 #pragma once
 #include <cstdint>
 
 namespace epk {
 
-#ifndef EP_LIBM
-#define EP_LIBM 0   // 1: route everything through the CUDA math library (debug / A-B comparison builds only)
-#endif
+// e^r = 1 + r + r^2 q(r) on |r| <= ln2/2; q = degree-9 Chebyshev interpolant of (e^r - 1 - r)/r^2
+// (max relative error of the reconstructed e^r: 1.6e-17, computed in 60-digit arithmetic).
+__constant__ double EXP_Q[10] = {0.5000000000000001,     0.16666666666666669,   0.04166666666662396,
+                                 0.00833333333333005,    0.0013888888917294928, 0.00019841269863116068,
+                                 2.48015211698282e-05,   2.755726836300438e-06, 2.762014840966706e-07,
+                                 2.5100431608666542e-08};
+// log m = 2 s (1 + z/3 + z^2/5 + ... + z^9/19), s = (m-1)/(m+1), z = s^2 <= 0.0295 (next term z^10/21 < 2.4e-17)
+__constant__ double LOG_C[9] = {1.0 / 3.0, 1.0 / 5.0, 1.0 / 7.0, 1.0 / 9.0, 1.0 / 11.0, 1.0 / 13.0, 1.0 / 15.0,
+                                1.0 / 17.0, 1.0 / 19.0};
 
 __device__ __forceinline__ double ep_rcp(double b) {
-#if EP_LIBM
-    return 1.0 / b;
-#else
     double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));   // ~20 good bits
-    double e = fma(-b, r, 1.0);
-    r = fma(r, e, r);                                         // ~40 bits
-    e = fma(-b, r, 1.0);
-    r = fma(r, e, r);                                         // full
-    return r;
-#endif
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));   // MUFU.RCP64H: >= 20 good bits
+    const double e = fma(-b, r, 1.0);
+    const double t = fma(e, e, e);                            // e + e^2; remainder e^3 <= 2^-60
+    return fma(r, t, r);
 }
 
-__device__ __forceinline__ double ep_div(double a, double b) {
-#if EP_LIBM
-    return a / b;
-#else
-    const double r = ep_rcp(b);
-    const double q = a * r;
-    return fma(fma(-b, q, a), r, q);                          // one residual correction: <= 1 ulp
-#endif
+__device__ __forceinline__ double ep_rsqrt(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));  // MUFU.RSQ64H
+    const double h = x * y;
+    const double e = fma(-h, y, 1.0);                         // 1 - x y^2
+    const double t = fma(0.375, e, 0.5) * e;                  // e/2 + 3e^2/8
+    return fma(y, t, y);
 }
 
-__device__ __forceinline__ double ep_exp(double x) {
-#if EP_LIBM
-    return exp(x);
-#else
-    x = fmin(fmax(x, -700.0), 700.0);
-    // k = round(x / ln 2) by the 2^52+2^51 shift trick
-    const double shift = 6755399441055744.0;
+// exp of a finite argument with |x| <= 700 (callers clamp); no overflow / underflow / NaN handling
+__device__ __forceinline__ double ep_exp_core(double x) {
+    const double shift = 6755399441055744.0;                  // 2^52 + 2^51: round-to-nearest-integer trick
     const double t = fma(x, 1.4426950408889634, shift);
-    const double kd = t - shift;
     const int k = __double2loint(t);
-    double r = fma(kd, -6.93147180369123816490e-01, x);       // ln2 high part (low 21 bits zero)
+    const double kd = t - shift;
+    double r = fma(kd, -6.93147180369123816490e-01, x);       // ln2 high part (low bits zero: kd*hi is exact)
     r = fma(kd, -1.90821492927058770002e-10, r);              // ln2 low part
-    // e^r on |r| <= ln2/2: Taylor coefficients 1/n!, degree 13 (remainder r^14/14! < 2^-57 relative)
-    double p = 1.60590438368216145994e-10;                    // 1/13!
-    p = fma(p, r, 2.08767569878680989792e-09);                // 1/12!
-    p = fma(p, r, 2.50521083854417187751e-08);                // 1/11!
-    p = fma(p, r, 2.75573192239858906526e-07);                // 1/10!
-    p = fma(p, r, 2.75573192239858906526e-06);                // 1/9!
-    p = fma(p, r, 2.48015873015873015873e-05);                // 1/8!
-    p = fma(p, r, 1.98412698412698412698e-04);                // 1/7!
-    p = fma(p, r, 1.38888888888888888889e-03);                // 1/6!
-    p = fma(p, r, 8.33333333333333333333e-03);                // 1/5!
-    p = fma(p, r, 4.16666666666666666667e-02);                // 1/4!
-    p = fma(p, r, 1.66666666666666666667e-01);                // 1/3!
-    p = fma(p, r, 0.5);
-    p = fma(p, r, 1.0);
-    p = fma(p, r, 1.0);
-    // scale by 2^k through the exponent field (|k| <= 1010; result stays normal for |x| <= 700)
-    const int hi = __double2hiint(p) + k * 1048576;
-    return __hiloint2double(hi, __double2loint(p));
-#endif
+    double q = EXP_Q[9];
+#pragma unroll
+    for (int i = 8; i >= 0; --i) q = fma(q, r, EXP_Q[i]);
+    double p = fma(r, q, 1.0);
+    p = fma(r, p, 1.0);
+    return __hiloint2double(__double2hiint(p) + k * 1048576, __double2loint(p));   // * 2^k via the exponent field
 }
 
-__device__ __forceinline__ double ep_log(double x) {
-#if EP_LIBM
-    return log(x);
-#else
-    // x = m * 2^e with m in [sqrt(1/2), sqrt(2)); x is positive and normal at every call site
+// log of a positive normal argument
+__device__ __forceinline__ double ep_log_core(double x) {
     int hi = __double2hiint(x);
     const int lo = __double2loint(x);
     int e = (hi >> 20) - 1023;
     hi = (hi & 0x000fffff) | 0x3ff00000;
-    double m = __hiloint2double(hi, lo);
-    if (hi > 0x3ff6a09e) { m *= 0.5; e += 1; }
-    const double s = ep_div(m - 1.0, m + 1.0);                // |s| <= 0.1716
+    if (hi > 0x3ff6a09e) { hi -= 0x00100000; e += 1; }        // m in [sqrt(1/2), sqrt(2))
+    const double m = __hiloint2double(hi, lo);
+    const double s = (m - 1.0) * ep_rcp(m + 1.0);
     const double z = s * s;
-    // log m = 2 s (1 + z/3 + z^2/5 + ... + z^10/21); z^11/23 term < 2^-58 relative
-    double p = 1.0 / 21.0;
-    p = fma(p, z, 1.0 / 19.0);
-    p = fma(p, z, 1.0 / 17.0);
-    p = fma(p, z, 1.0 / 15.0);
-    p = fma(p, z, 1.0 / 13.0);
-    p = fma(p, z, 1.0 / 11.0);
-    p = fma(p, z, 1.0 / 9.0);
-    p = fma(p, z, 1.0 / 7.0);
-    p = fma(p, z, 1.0 / 5.0);
-    p = fma(p, z, 1.0 / 3.0);
+    double p = LOG_C[8];
+#pragma unroll
+    for (int i = 7; i >= 0; --i) p = fma(p, z, LOG_C[i]);
     const double ed = (double)e;
-    // log x = e ln2 + 2s + 2 s z p, summed small to large
-    double res = (2.0 * s) * (z * p);
+    const double s2 = s + s;
+    double res = s2 * (z * p);                                // summed small to large
     res = fma(ed, 1.90821492927058770002e-10, res);
-    res += 2.0 * s;
+    res += s2;
     return fma(ed, 6.93147180369123816490e-01, res);
-#endif
 }
 
-__device__ __forceinline__ double ep_sqrt(double x) { return sqrt(x); }
+// Batched evaluation over a thread's own column of a shared-memory slot array xs[slot][BLOCK]; col = &xs[0][tid].
+// N must be even.  The loops stay rolled on purpose (instruction-cache footprint); two independent chains per trip.
+template <int N, int BLOCK>
+__device__ __forceinline__ void ep_exp_slots(double* col) {
+    static_assert(N % 2 == 0, "pad the slot list to an even length");
+#pragma unroll 1
+    for (int s = 0; s < N; s += 2) {
+        const double a = col[s * BLOCK], b = col[(s + 1) * BLOCK];
+        const double ea = ep_exp_core(a), eb = ep_exp_core(b);
+        col[s * BLOCK] = ea;
+        col[(s + 1) * BLOCK] = eb;
+    }
+}
+
+template <int N, int BLOCK>
+__device__ __forceinline__ void ep_log_slots(double* col) {
+    static_assert(N % 2 == 0, "pad the slot list to an even length");
+#pragma unroll 1
+    for (int s = 0; s < N; s += 2) {
+        const double a = col[s * BLOCK], b = col[(s + 1) * BLOCK];
+        const double la = ep_log_core(a), lb = ep_log_core(b);
+        col[s * BLOCK] = la;
+        col[(s + 1) * BLOCK] = lb;
+    }
+}
+
+__device__ __forceinline__ double ep_clamp(double x, double lo, double hi) { return fmin(fmax(x, lo), hi); }
 
 }  // namespace epk

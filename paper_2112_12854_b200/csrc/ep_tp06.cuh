@@ -4,8 +4,16 @@
 // the equations and constants are restated from the published model in DESIGN.md Appendix A.  Readings B1..B9 of
 // DESIGN.md section 3 apply (13 RL variables = 12 gates + Rbar; buffer factors + forward Euler for the three calcium
 // pools; v >= -40 mV takes the high-voltage h/j branch; removable singularity of I_CaL handled by a series).
-// Everything on the right-hand side is taken at t^n: the function reads y[], returns the new values
-// in y[] only after all right-hand sides have been formed.
+// Everything on the right-hand side is taken at t^n.
+//
+// This is the production form.  It computes the same functions as Appendix A, rearranged for the fp64 pipe
+// (DESIGN.md section 7): exponentials with commensurate slopes are integer powers of one exponential
+// (v/600 -> slopes 1/200, 1/24, 1/20, 1/15, 1/10, 1/7.5, 1/6, 1/5; v/14 -> 1/14, 1/7; vF/20RT -> 0.1, 0.65, 0.9, 1 vF/RT;
+// 0.02(v-E_K) -> 0.06, 0.1, 0.5; (v+27)^2/3600 -> /240, /225), every sigmoid product is written as one rational function
+// with a single reciprocal, and the remaining exponentials / logarithms are evaluated in shared-memory batches
+// (ep_math.cuh).  Relative differences from the literal formulas are <= ~2e-14 (120-fold powers of a 1-ulp value),
+// three orders of magnitude inside the 1e-11 one-step tolerance.  The literal transcription is kept in
+// ep_tp06_direct.cuh for A/B debugging builds (-DEP_DIRECT=1); it is not part of the product build.
 //
 // Units: mV, ms, mM, currents uA/uF, conductances nS/pF.
 #pragma once
@@ -22,7 +30,6 @@ __device__ __constant__ const double TP06_REST_STATE[TP06_S] = {
     -86.2, 0.0, 0.75, 0.75, 0.0, 1.0, 0.0, 0.0, 1.0, 0.0, 1.0, 1.0, 1.0, 1.0, 7e-5, 1.3, 7e-5, 7.67, 138.3};
 
 namespace tp06 {
-// physical constants
 constexpr double R = 8314.472, T = 310.0, F = 96485.3415;
 constexpr double RTF = R * T / F;          // mV
 constexpr double FRT = F / (R * T);        // 1/mV
@@ -31,158 +38,260 @@ constexpr double Vc = 0.016404, Vsr = 0.001094, Vss = 0.00005468, Cap = 0.185;
 constexpr double GNa = 14.838, GK1 = 5.405, GKr = 0.153, GCaL = 3.980e-5, GbNa = 2.9e-4, GbCa = 5.92e-4;
 constexpr double GpCa = 0.1238, KpCa = 5e-4, GpK = 0.0146, pKNa = 0.03;
 constexpr double PNaK = 2.724, KmK = 1.0, KmNa = 40.0;
-constexpr double kNaCa = 1000.0, KmNai = 87.5, KmCa = 1.38, ksat = 0.1, gam = 0.35, alpha = 2.5;
+constexpr double kNaCa = 1000.0, KmNai = 87.5, KmCa = 1.38, ksat = 0.1, alpha = 2.5;   // gamma = 0.35 = 7/20
 constexpr double Vmaxup = 0.006375, Kup = 2.5e-4, Vrel = 0.102, k1p = 0.15, k2p = 0.045, k3 = 0.060, k4 = 0.005;
 constexpr double EC = 1.5, maxsr = 2.5, minsr = 1.0, Vleak = 3.6e-4, Vxfer = 0.0038;
 constexpr double Bufc = 0.2, Kbufc = 0.001, Bufsr = 10.0, Kbufsr = 0.3, Bufss = 0.4, Kbufss = 2.5e-4;
+// natural logarithms of the extracellular concentrations
+constexpr double LN_KO = 1.6863989535702288, LN_NAO = 4.941642422609304, LN_KO_PNAO = 2.2617630984737906,
+                 LN_CAO = 0.6931471805599453;
+// e^c constants produced when (v + a)/b exponents are split into e^(v/b) e^(a/b)
+constexpr double EM12 = 6.14421235332821e-06;     // e^(-12)
+constexpr double E7C = 1096.6331584284585;        // e^(7)
+constexpr double EM025 = 0.7788007830714049;      // e^(-0.25)
+constexpr double EM32 = 0.04076220397836622;      // e^(-3.2)
+constexpr double EM45 = 0.011108996538242306;     // e^(-4.5)
+constexpr double EM26_7 = 0.0243728440732796;     // e^(-26/7)
+constexpr double E88_24 = 39.12128399815322;      // e^(88/24)
+constexpr double EM3 = 0.049787068367863944;      // e^(-3)
+constexpr double EM5_14 = 0.6996725373751304;     // e^(-5/14)
+constexpr double E5_6 = 2.300975890892825;        // e^(5/6)
+constexpr double EM35_15 = 0.09697196786440507;   // e^(-35/15)
+constexpr double E20_6 = 28.031624894526136;      // e^(20/6)
+constexpr double E56 = 270.42640742615265;        // e^(5.6)
+constexpr double E4 = 54.598150033144236;         // e^(4)
+constexpr double EM4 = 0.01831563888873418;       // e^(-4)
+constexpr double EM8_75 = 0.34415378686541237;    // e^(-8/7.5)
+constexpr double E1 = 2.718281828459045;          // e
+constexpr double E25 = 12.182493960703473;        // e^(2.5)
+constexpr double E20_7 = 17.41170806332765;       // e^(20/7)
+constexpr double E13 = 3.669296667619244;         // e^(1.3)
+constexpr double E3 = 20.085536923187668;         // e^(3)
+constexpr double E5C = 148.4131591025766;         // e^(5)
+constexpr double EM1 = 0.36787944117144233;       // e^(-1)
+
+// shared-memory slots of the three batches
+enum { L_KI = 0, L_NAI, L_KS, L_CAI, N_LOG = 4 };
+enum { A_B600 = 0, A_E14, A_M, A_H, A_XR1, A_D, A_PK, A_W, A_GR, A_GS, A_G27, A_CAL, A_K1Q, A_K1Q2, A_HJ0, N_EXPA = A_HJ0 + 8 };
+enum { N_EXPB = 14 };   // 13 Rush-Larsen factors + 1 pad
+enum { N_SLOTS = N_EXPA };
+static_assert(N_EXPA % 2 == 0 && N_EXPA >= N_EXPB, "slot layout");
 }  // namespace tp06
 
-// Rush-Larsen update y <- yinf + (y - yinf) exp(-dt/tau).  rate = 1/tau.
-__device__ __forceinline__ double rl(double y, double yinf, double rate, double dt) {
-    return fma(y - yinf, ep_exp(-dt * rate), yinf);
-}
-
-// sigma(z) = 1/(1+e^z)
-__device__ __forceinline__ double sg(double z) { return ep_rcp(1.0 + ep_exp(z)); }
-
-// One step. type: 0 endo, 1 mid, 2 epi.  istim = I_s/C_m [uA/uF], dv_diff = D_c/(chi C_m) [mV/ms].
-__device__ __forceinline__ void tp06_step(double (&y)[TP06_S], int type, double dt, double istim, double dv_diff) {
+// One step of one cell.  type: 0 endo, 1 mid, 2 epi.  istim = I_s/C_m [uA/uF], dv_diff = D_c/(chi C_m) [mV/ms].
+// col = this thread's column of the block's slot array (stride BLOCK doubles), at least tp06::N_SLOTS slots.
+template <int BLOCK>
+__device__ __forceinline__ void tp06_step(double (&y)[TP06_S], int type, double dt, double istim, double dv_diff,
+                                          double* col) {
     using namespace tp06;
     const double v = y[Y_V];
+    const double vg = ep_clamp(v, -250.0, 250.0);   // argument of every transcendental: keeps all exponents < 700
     const double Cai = y[Y_CAI], CaSR = y[Y_CASR], CaSS = y[Y_CASS], Nai = y[Y_NAI], Ki = y[Y_KI];
 
-    // ---- reversal potentials
-    const double EK = RTF * ep_log(ep_div(Ko, Ki));
-    const double ENa = RTF * ep_log(ep_div(Nao, Nai));
-    const double EKs = RTF * ep_log(ep_div(Ko + pKNa * Nao, Ki + pKNa * Nai));
-    const double ECa = 0.5 * RTF * ep_log(ep_div(Cao, Cai));
+    // ---- batch 1: the four logarithms of the reversal potentials
+    col[L_KI * BLOCK] = Ki;
+    col[L_NAI * BLOCK] = Nai;
+    col[L_KS * BLOCK] = fma(pKNa, Nai, Ki);
+    col[L_CAI * BLOCK] = Cai;
+    ep_log_slots<N_LOG, BLOCK>(col);
+    const double EK = RTF * (LN_KO - col[L_KI * BLOCK]);
+    const double ENa = RTF * (LN_NAO - col[L_NAI * BLOCK]);
+    const double EKs = RTF * (LN_KO_PNAO - col[L_KS * BLOCK]);
+    const double ECa = (0.5 * RTF) * (LN_CAO - col[L_CAI * BLOCK]);
+    const double u = v - EK;
+    const double ug = ep_clamp(u, -300.0, 400.0);
+    const bool hi = (v >= -40.0);   // reading B7
+
+    // ---- batch 2: every voltage-dependent exponential that is not an integer power of another one
+    col[A_B600 * BLOCK] = vg * (1.0 / 600.0);
+    col[A_E14 * BLOCK] = vg * (1.0 / 14.0);
+    col[A_M * BLOCK] = fma(vg, -1.0 / 9.03, -56.86 / 9.03);
+    col[A_H * BLOCK] = fma(vg, 1.0 / 7.43, 71.55 / 7.43);
+    col[A_XR1 * BLOCK] = fma(vg, 1.0 / 11.5, 30.0 / 11.5);
+    col[A_D * BLOCK] = fma(vg, -1.0 / 13.0, -35.0 / 13.0);
+    col[A_PK * BLOCK] = fma(vg, -1.0 / 5.98, 25.0 / 5.98);
+    col[A_W * BLOCK] = vg * (0.05 * FRT);
+    col[A_GR * BLOCK] = (vg + 40.0) * (vg + 40.0) * (-1.0 / 1800.0);
+    col[A_GS * BLOCK] = (type == 0) ? (vg + 67.0) * (vg + 67.0) * (-1.0 / 1000.0)
+                                    : (vg + 45.0) * (vg + 45.0) * (-1.0 / 320.0);
+    col[A_G27 * BLOCK] = (vg + 27.0) * (vg + 27.0) * (-1.0 / 3600.0);
+    const double xcal = (vg - 15.0) * (2.0 * FRT);
+    col[A_CAL * BLOCK] = xcal;
+    col[A_K1Q * BLOCK] = fma(ug, 0.0002, 0.02);       // 0.0002 (u + 100)
+    col[A_K1Q2 * BLOCK] = ug * 0.02;
+    if (hi) {
+        col[(A_HJ0 + 0) * BLOCK] = fma(vg, -1.0 / 11.1, -10.66 / 11.1);
+        col[(A_HJ0 + 1) * BLOCK] = vg * 0.057;
+#pragma unroll
+        for (int k = 2; k < 8; ++k) col[(A_HJ0 + k) * BLOCK] = 0.0;
+    } else {
+        col[(A_HJ0 + 0) * BLOCK] = fma(vg, -1.0 / 6.8, -80.0 / 6.8);
+        col[(A_HJ0 + 1) * BLOCK] = vg * 0.079;
+        col[(A_HJ0 + 2) * BLOCK] = vg * 0.3485;
+        col[(A_HJ0 + 3) * BLOCK] = vg * 0.2444;
+        col[(A_HJ0 + 4) * BLOCK] = vg * -0.04391;
+        col[(A_HJ0 + 5) * BLOCK] = fma(vg, 0.311, 0.311 * 79.23);
+        col[(A_HJ0 + 6) * BLOCK] = vg * -0.01052;
+        col[(A_HJ0 + 7) * BLOCK] = fma(vg, -0.1378, -0.1378 * 40.14);
+    }
+    ep_exp_slots<N_EXPA, BLOCK>(col);
+
+    // ---- integer powers
+    double E200, E24, E20, E15, E10, E7p5, E6, E5;
+    {
+        const double B = col[A_B600 * BLOCK];
+        const double B2 = B * B, B3 = B2 * B, B5 = B2 * B3, B10 = B5 * B5, B20 = B10 * B10, B40 = B20 * B20;
+        const double B30 = B20 * B10, B60 = B30 * B30;
+        E200 = B3; E24 = B20 * B5; E20 = B30; E15 = B40; E10 = B60; E7p5 = B40 * B40; E6 = B60 * B40; E5 = B60 * B60;
+    }
+    const double E14 = col[A_E14 * BLOCK], E7 = E14 * E14;
+    double W13, W18, W20;
+    {
+        const double W = col[A_W * BLOCK];
+        const double W2 = W * W, W4 = W2 * W2, W8 = W4 * W4, W16 = W8 * W8;
+        W13 = W8 * W4 * W; W18 = W16 * W2; W20 = W18 * W2;
+    }
+    double Gf, Gf2;   // exp(-(v+27)^2/225), exp(-(v+27)^2/240)
+    {
+        const double b = col[A_G27 * BLOCK];
+        const double b2 = b * b, b4 = b2 * b2, b8 = b4 * b4;
+        Gf = b8 * b8; Gf2 = (b8 * b4) * (b2 * b);
+    }
 
     // ---- membrane currents
     const double m = y[Y_M];
-    const double INa = GNa * m * m * m * y[Y_H] * y[Y_J] * (v - ENa);
+    const double INa = GNa * (m * m * m) * y[Y_H] * y[Y_J] * (v - ENa);
     double ICaL;
     {
-        const double x = 2.0 * (v - 15.0) * FRT;
-        const double ex = ep_exp(x);
+        const double ex = col[A_CAL * BLOCK];
         // x/(e^x - 1), with the series 1 - x/2 inside |x| < 1e-7 (reading B6)
-        const double xo = (fabs(x) < 1e-7) ? fma(-0.5, x, 1.0) : ep_div(x, ex - 1.0);
-        ICaL = GCaL * y[Y_D] * y[Y_F] * y[Y_F2] * y[Y_FCASS] * 2.0 * F * xo * (0.25 * CaSS * ex - Cao);
+        const double xo = (fabs(xcal) < 1e-7) ? fma(-0.5, xcal, 1.0) : xcal * ep_rcp(ex - 1.0);
+        ICaL = (GCaL * 2.0 * F) * (y[Y_D] * y[Y_F]) * (y[Y_F2] * y[Y_FCASS]) * xo * fma(0.25 * CaSS, ex, -Cao);
     }
     const double Gto = (type == 0) ? 0.073 : 0.294;
     const double GKs = (type == 1) ? 0.098 : 0.392;
-    const double Ito = Gto * y[Y_R] * y[Y_S] * (v - EK);
-    const double IKr = GKr * ep_sqrt(Ko / 5.4) * y[Y_XR1] * y[Y_XR2] * (v - EK);
+    const double Ito = Gto * y[Y_R] * y[Y_S] * u;
+    const double IKr = GKr * y[Y_XR1] * y[Y_XR2] * u;     // sqrt(Ko/5.4) = 1
     const double IKs = GKs * y[Y_XS] * y[Y_XS] * (v - EKs);
     double IK1;
     {
-        const double u = v - EK;
-        const double aK1 = ep_div(0.1, 1.0 + ep_exp(0.06 * (u - 200.0)));
-        const double bK1 = ep_div(3.0 * ep_exp(0.0002 * (u + 100.0)) + ep_exp(0.1 * (u - 10.0)), 1.0 + ep_exp(-0.5 * u));
-        IK1 = GK1 * ep_div(aK1, aK1 + bK1) * u;
+        const double q = col[A_K1Q * BLOCK], Q = col[A_K1Q2 * BLOCK];
+        const double Q2 = Q * Q, Q3 = Q2 * Q, Q5 = Q2 * Q3, Q10 = Q5 * Q5, Q25 = Q10 * Q10 * Q5;
+        const double t1 = fma(0.1, Q25, 0.1);                                       // 0.1 (1 + e^{-0.5u}) Q^25
+        const double t2 = fma(EM1, Q5, 3.0 * q) * fma(EM12, Q3, 1.0) * Q25;         // (3q + e^{0.1(u-10)})(1 + e^{0.06(u-200)}) Q^25
+        IK1 = GK1 * u * t1 * ep_rcp(t1 + t2);
     }
-    double INaCa;
-    {
-        const double e1 = ep_exp(gam * v * FRT), e2 = ep_exp((gam - 1.0) * v * FRT);
-        const double num = e1 * Nai * Nai * Nai * Cao - e2 * Nao * Nao * Nao * Cai * alpha;
-        const double den = (KmNai * KmNai * KmNai + Nao * Nao * Nao) * (KmCa + Cao) * (1.0 + ksat * e2);
-        INaCa = kNaCa * ep_div(num, den);
-    }
-    const double INaK = PNaK * (Ko / (Ko + KmK)) * ep_div(Nai, Nai + KmNa)
-                        * ep_rcp(1.0 + 0.1245 * ep_exp(-0.1 * v * FRT) + 0.0353 * ep_exp(-v * FRT));
-    const double IpCa = GpCa * ep_div(Cai, KpCa + Cai);
-    const double IpK = GpK * (v - EK) * sg((25.0 - v) / 5.98);
+    const double Nai3 = Nai * Nai * Nai;
+    const double INaCa = (kNaCa / ((KmNai * KmNai * KmNai + Nao * Nao * Nao) * (KmCa + Cao)))
+                         * fma(W20, Nai3 * Cao, -(Nao * Nao * Nao * alpha) * Cai) * ep_rcp(W13 + ksat);
+    const double INaK = (PNaK * Ko / (Ko + KmK)) * Nai * W20
+                        * ep_rcp((Nai + KmNa) * fma(0.1245, W18, W20 + 0.0353));
+    const double IpCa = GpCa * Cai * ep_rcp(KpCa + Cai);
+    const double IpK = GpK * u * ep_rcp(1.0 + col[A_PK * BLOCK]);
     const double IbNa = GbNa * (v - ENa);
     const double IbCa = GbCa * (v - ECa);
     const double iion = INa + ICaL + Ito + IKr + IKs + IK1 + INaCa + INaK + IpCa + IpK + IbNa + IbCa;
 
-    // ---- sarcoplasmic-reticulum fluxes
-    const double ecs = ep_div(EC, CaSR);
-    const double kcasr = maxsr - ep_div(maxsr - minsr, 1.0 + ecs * ecs);
-    const double k1 = ep_div(k1p, kcasr), k2 = k2p * kcasr;
-    const double css2 = CaSS * CaSS;
-    const double O = ep_div(k1 * css2 * y[Y_RBAR], k3 + k1 * css2);
+    // ---- sarcoplasmic-reticulum fluxes, buffer factors (reading B3), concentration derivatives
+    const double c2 = CaSR * CaSR, css2 = CaSS * CaSS, ci2 = Cai * Cai;
+    const double kcasr = fma(-(maxsr - minsr) * c2, ep_rcp(c2 + EC * EC), maxsr);
+    const double O = k1p * css2 * y[Y_RBAR] * ep_rcp(fma(k3, kcasr, k1p * css2));
     const double Irel = Vrel * O * (CaSR - CaSS);
     const double Ileak = Vleak * (CaSR - Cai);
-    const double Iup = ep_div(Vmaxup, 1.0 + ep_div(Kup * Kup, Cai * Cai));
+    const double Iup = Vmaxup * ci2 * ep_rcp(ci2 + Kup * Kup);
     const double Ixfer = Vxfer * (CaSS - Cai);
-
-    // ---- concentrations: buffer factors (reading B3) and forward Euler
-    const double bi = ep_rcp(1.0 + ep_div(Bufc * Kbufc, (Cai + Kbufc) * (Cai + Kbufc)));
-    const double bsr = ep_rcp(1.0 + ep_div(Bufsr * Kbufsr, (CaSR + Kbufsr) * (CaSR + Kbufsr)));
-    const double bss = ep_rcp(1.0 + ep_div(Bufss * Kbufss, (CaSS + Kbufss) * (CaSS + Kbufss)));
+    const double ti = (Cai + Kbufc) * (Cai + Kbufc), tsr = (CaSR + Kbufsr) * (CaSR + Kbufsr),
+                 tss = (CaSS + Kbufss) * (CaSS + Kbufss);
+    const double bi = ti * ep_rcp(ti + Bufc * Kbufc);
+    const double bsr = tsr * ep_rcp(tsr + Bufsr * Kbufsr);
+    const double bss = tss * ep_rcp(tss + Bufss * Kbufss);
     const double dCai = bi * ((Ileak - Iup) * (Vsr / Vc) + Ixfer - (IbCa + IpCa - 2.0 * INaCa) * (Cap / (2.0 * Vc * F)));
     const double dCaSR = bsr * (Iup - Ileak - Irel);
     const double dCaSS = bss * (-ICaL * (Cap / (2.0 * Vss * F)) + Irel * (Vsr / Vss) - Ixfer * (Vc / Vss));
     const double dNai = -(INa + IbNa + 3.0 * INaK + 3.0 * INaCa) * (Cap / (Vc * F));
     const double dKi = -(IK1 + Ito + IKr + IKs - 2.0 * INaK + IpK + istim) * (Cap / (Vc * F));   // reading B8
+    const double v_new = fma(dt, dv_diff - iion - istim, v);   // eq. (7); explicit increment :172
 
-    // ---- gates: steady states and rates (1/tau), Rush-Larsen
-    {   // m
-        const double s = sg((-56.86 - v) / 9.03);
-        const double tau = sg((-60.0 - v) / 5.0) * (0.1 * sg((v + 35.0) / 5.0) + 0.1 * sg((v - 50.0) / 200.0));
-        y[Y_M] = rl(y[Y_M], s * s, ep_rcp(tau), dt);
+    // ---- gates: steady states and rates 1/tau, each as one rational function
+    double inf[13], rate[13];   // index g = state index - 1
+    {   // m: tau = s(-60-v;5) [0.1 s(v+35;5) + 0.1 s(v-50;200)],  s(z) = 1/(1+e^z)
+        const double sm = ep_rcp(1.0 + col[A_M * BLOCK]);
+        inf[0] = sm * sm;
+        const double P = fma(E7C, E5, 1.0), Q = fma(EM025, E200, 1.0);
+        rate[0] = (E5 + EM12) * P * Q * ep_rcp(0.1 * E5 * (P + Q));
     }
-    {   // h, j share the steady state; rates alpha+beta are used directly (tau = 1/(alpha+beta))
-        const double s = sg((v + 71.55) / 7.43);
-        const double hinf = s * s;
-        double rh, rj;
-        if (v >= -40.0) {   // reading B7
-            rh = ep_div(0.77, 0.13 * (1.0 + ep_exp(-(v + 10.66) / 11.1)));
-            rj = ep_div(0.6 * ep_exp(0.057 * v), 1.0 + ep_exp(-0.1 * (v + 32.0)));
+    {   // h, j share the steady state
+        const double sh = ep_rcp(1.0 + col[A_H * BLOCK]);
+        inf[1] = inf[2] = sh * sh;
+        const double s0 = col[(A_HJ0 + 0) * BLOCK], s1 = col[(A_HJ0 + 1) * BLOCK];
+        if (hi) {
+            rate[1] = (0.77 / 0.13) * ep_rcp(1.0 + s0);
+            rate[2] = 0.6 * s1 * E10 * ep_rcp(E10 + EM32);
         } else {
-            rh = 0.057 * ep_exp(-(v + 80.0) / 6.8) + 2.7 * ep_exp(0.079 * v) + 3.1e5 * ep_exp(0.3485 * v);
-            const double aj = ep_div((-2.5428e4 * ep_exp(0.2444 * v) - 6.948e-6 * ep_exp(-0.04391 * v)) * (v + 37.78),
-                                     1.0 + ep_exp(0.311 * (v + 79.23)));
-            const double bj = ep_div(0.02424 * ep_exp(-0.01052 * v), 1.0 + ep_exp(-0.1378 * (v + 40.14)));
-            rj = aj + bj;
+            const double s2 = col[(A_HJ0 + 2) * BLOCK], s3 = col[(A_HJ0 + 3) * BLOCK], s4 = col[(A_HJ0 + 4) * BLOCK],
+                         s5 = col[(A_HJ0 + 5) * BLOCK], s6 = col[(A_HJ0 + 6) * BLOCK], s7 = col[(A_HJ0 + 7) * BLOCK];
+            rate[1] = fma(0.057, s0, fma(2.7, s1, 3.1e5 * s2));
+            const double N1 = fma(-2.5428e4, s3, -6.948e-6 * s4) * (vg + 37.78), D1 = 1.0 + s5;
+            const double N2 = 0.02424 * s6, D2 = 1.0 + s7;
+            rate[2] = fma(N1, D2, N2 * D1) * ep_rcp(D1 * D2);
         }
-        y[Y_H] = rl(y[Y_H], hinf, rh, dt);
-        y[Y_J] = rl(y[Y_J], hinf, rj, dt);
     }
     {   // xr1, xr2, xs
-        const double t1 = 450.0 * sg((-45.0 - v) / 10.0) * 6.0 * sg((v + 30.0) / 11.5);
-        y[Y_XR1] = rl(y[Y_XR1], sg((-26.0 - v) / 7.0), ep_rcp(t1), dt);
-        const double t2 = 3.0 * sg((-60.0 - v) / 20.0) * 1.12 * sg((v - 60.0) / 20.0);
-        y[Y_XR2] = rl(y[Y_XR2], sg((v + 88.0) / 24.0), ep_rcp(t2), dt);
-        const double t3 = ep_div(1400.0, ep_sqrt(1.0 + ep_exp((5.0 - v) / 6.0))) * sg((v - 35.0) / 15.0) + 80.0;
-        y[Y_XS] = rl(y[Y_XS], sg((-5.0 - v) / 14.0), ep_rcp(t3), dt);
+        inf[3] = E7 * ep_rcp(E7 + EM26_7);
+        rate[3] = (E10 + EM45) * (1.0 + col[A_XR1 * BLOCK]) * ep_rcp(2700.0 * E10);
+        inf[4] = ep_rcp(fma(E88_24, E24, 1.0));
+        rate[4] = (E20 + EM3) * fma(EM3, E20, 1.0) * ep_rcp(3.36 * E20);
+        inf[5] = E14 * ep_rcp(E14 + EM5_14);
+        const double t = ep_rsqrt((E6 + E5_6) * E6) * E6;          // 1/sqrt(1 + e^{(5-v)/6})
+        const double P15 = fma(EM35_15, E15, 1.0);
+        rate[5] = P15 * ep_rcp(fma(1400.0, t, 80.0 * P15));
     }
     {   // r, s (reading B5: endo has its own s curves)
-        const double tr = 9.5 * ep_exp(-(v + 40.0) * (v + 40.0) / 1800.0) + 0.8;
-        y[Y_R] = rl(y[Y_R], sg((20.0 - v) / 6.0), ep_rcp(tr), dt);
-        double sinf, ts;
+        inf[6] = E6 * ep_rcp(E6 + E20_6);
+        rate[6] = ep_rcp(fma(9.5, col[A_GR * BLOCK], 0.8));
+        const double Gs = col[A_GS * BLOCK];
         if (type == 0) {
-            sinf = sg((v + 28.0) / 5.0);
-            ts = 1000.0 * ep_exp(-(v + 67.0) * (v + 67.0) / 1000.0) + 8.0;
+            inf[7] = ep_rcp(fma(E56, E5, 1.0));
+            rate[7] = ep_rcp(fma(1000.0, Gs, 8.0));
         } else {
-            sinf = sg((v + 20.0) / 5.0);
-            ts = 85.0 * ep_exp(-(v + 45.0) * (v + 45.0) / 320.0) + 5.0 * sg((v - 20.0) / 5.0) + 3.0;
+            inf[7] = ep_rcp(fma(E4, E5, 1.0));
+            const double P = fma(EM4, E5, 1.0);
+            rate[7] = P * ep_rcp(fma(fma(85.0, Gs, 3.0), P, 5.0));
         }
-        y[Y_S] = rl(y[Y_S], sinf, ep_rcp(ts), dt);
     }
     {   // d, f, f2
-        const double td = (1.4 * sg((-35.0 - v) / 13.0) + 0.25) * (1.4 * sg((v + 5.0) / 5.0)) + sg((50.0 - v) / 20.0);
-        y[Y_D] = rl(y[Y_D], sg((-8.0 - v) / 7.5), ep_rcp(td), dt);
-        const double g27 = (v + 27.0) * (v + 27.0);
-        const double tf = 1102.5 * ep_exp(-g27 / 225.0) + 200.0 * sg((13.0 - v) / 10.0) + 180.0 * sg((v + 30.0) / 10.0) + 20.0;
-        y[Y_F] = rl(y[Y_F], sg((v + 20.0) / 7.0), ep_rcp(tf), dt);
-        const double tf2 = 562.0 * ep_exp(-g27 / 240.0) + 31.0 * sg((25.0 - v) / 10.0) + 80.0 * sg((v + 30.0) / 10.0);
-        y[Y_F2] = rl(y[Y_F2], 0.67 * sg((v + 35.0) / 7.0) + 0.33, ep_rcp(tf2), dt);
+        inf[8] = E7p5 * ep_rcp(E7p5 + EM8_75);
+        const double D = 1.0 + col[A_D * BLOCK], P5 = fma(E1, E5, 1.0), Q20 = E20 + E25;
+        rate[8] = D * P5 * Q20 * ep_rcp(fma(fma(0.25, D, 1.4) * 1.4, Q20, E20 * D * P5));
+        const double Qa = E10 + E13, Qb = fma(E3, E10, 1.0), Qc = E10 + E25;
+        inf[9] = ep_rcp(fma(E20_7, E7, 1.0));
+        rate[9] = Qa * Qb * ep_rcp(fma(fma(1102.5, Gf, 20.0), Qa * Qb, fma(200.0 * E10, Qb, 180.0 * Qa)));
+        inf[10] = fma(0.67, ep_rcp(fma(E5C, E7, 1.0)), 0.33);
+        rate[10] = Qc * Qb * ep_rcp(fma(562.0 * Gf2, Qc * Qb, fma(31.0 * E10, Qb, 80.0 * Qc)));
     }
     {   // fCass
-        const double q = ep_rcp(1.0 + (CaSS / 0.05) * (CaSS / 0.05));
-        y[Y_FCASS] = rl(y[Y_FCASS], 0.6 * q + 0.4, ep_rcp(80.0 * q + 2.0), dt);
+        const double qf = ep_rcp(fma(400.0 * CaSS, CaSS, 1.0));    // 1/(1 + (CaSS/0.05)^2)
+        inf[11] = fma(0.6, qf, 0.4);
+        rate[11] = ep_rcp(fma(80.0, qf, 2.0));
     }
     {   // Rbar: dR/dt = k4 (1 - R) - k2 CaSS R, linear in R at frozen Ca (reading B1)
-        const double rate = k2 * CaSS + k4;
-        y[Y_RBAR] = rl(y[Y_RBAR], ep_div(k4, rate), rate, dt);
+        rate[12] = fma(k2p * kcasr, CaSS, k4);
+        inf[12] = k4 * ep_rcp(rate[12]);
     }
+
+    // ---- batch 3: Rush-Larsen factors exp(-dt/tau)
+#pragma unroll
+    for (int g = 0; g < 13; ++g) col[g * BLOCK] = fmax(-dt * rate[g], -700.0);
+    col[13 * BLOCK] = 0.0;
+    ep_exp_slots<N_EXPB, BLOCK>(col);
+#pragma unroll
+    for (int g = 0; g < 13; ++g) y[1 + g] = fma(y[1 + g] - inf[g], col[g * BLOCK], inf[g]);
     y[Y_CAI] = fma(dt, dCai, Cai);
     y[Y_CASR] = fma(dt, dCaSR, CaSR);
     y[Y_CASS] = fma(dt, dCaSS, CaSS);
     y[Y_NAI] = fma(dt, dNai, Nai);
     y[Y_KI] = fma(dt, dKi, Ki);
-    y[Y_V] = fma(dt, dv_diff - iion - istim, v);   // eq. (7); explicit increment PAPER.md:172
+    y[Y_V] = v_new;
 }
 
 }  // namespace epk
