@@ -62,7 +62,7 @@ def lib():
     """Load (building if stale) libep.so.  Raises if it cannot be built or loaded: there is no fallback."""
     global _lib
     if _lib is None:
-        path = _build.build()
+        path = os.environ.get("EP_LIB_OVERRIDE") or _build.build()   # override: A/B builds of the same ABI
         L = C.CDLL(path)
         for name, (res, args) in SIGNATURES.items():
             fn = getattr(L, name)

@@ -37,7 +37,7 @@ def _stale() -> bool:
 def build(force: bool = False, libm: bool = False, verbose: bool = False) -> str:
     if not (force or _stale()):
         return LIB
-    cmd = [_nvcc(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+    cmd = [_nvcc(), "-O3", "-std=c++20", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
            "-Xcompiler", "-fPIC,-O2", "-shared", "-cudart", "static"]
     if verbose:
         cmd += ["-Xptxas", "-v"]

@@ -72,7 +72,10 @@ __global__ void __launch_bounds__(CELL_THREADS) diffusion_only_kernel(int64_t nc
 }
 
 // S2..S9 fused, TP06.  One thread per cell; state rows are read once and written once.
-__global__ void __launch_bounds__(CELL_THREADS) cell_step_tp06_kernel(int64_t nc, int64_t stride,
+#ifndef EP_CELL_MIN_BLOCKS
+#define EP_CELL_MIN_BLOCKS 4
+#endif
+__global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_tp06_kernel(int64_t nc, int64_t stride,
                                                                       const int32_t* __restrict__ cidx,
                                                                       const double* __restrict__ ccoef,
                                                                       StepArgs a) {
@@ -80,11 +83,7 @@ __global__ void __launch_bounds__(CELL_THREADS) cell_step_tp06_kernel(int64_t nc
     __shared__ double xs[tp06::N_SLOTS][CELL_THREADS];
     const int64_t i = (int64_t)blockIdx.x * CELL_THREADS + threadIdx.x;
     if (i >= nc) return;
-    double y[TP06_S];
-    y[0] = a.vm_cur[i];
-#pragma unroll
-    for (int k = 1; k < TP06_S; ++k) y[k] = a.y[k * stride + i];
-    const double v_old = y[0];
+    const double v_old = a.vm_cur[i];
     const double dv = diffusion_gather(i, stride, cidx, ccoef, a.vm_cur, a.vn, v_old);
     // S4: stimulus, eq. (4) PAPER.md:130-132 (window already resolved on the host into istim[k])
     const unsigned mask = a.smask[i];
@@ -92,12 +91,11 @@ __global__ void __launch_bounds__(CELL_THREADS) cell_step_tp06_kernel(int64_t nc
 #pragma unroll
     for (int k = 0; k < 8; ++k)
         if (mask & (1u << k)) istim += a.istim[k];
-    tp06_step<CELL_THREADS>(y, a.ctype[i], a.dt, istim, dv, &xs[0][threadIdx.x]);
-    a.vm_next[i] = y[0];
-#pragma unroll
-    for (int k = 1; k < TP06_S; ++k) a.y[k * stride + i] = y[k];
+    const double v_new = tp06_step<CELL_THREADS>(v_old, a.y + i, stride, a.ctype[i], a.dt, istim, dv,
+                                                 &xs[0][threadIdx.x]);
+    a.vm_next[i] = v_new;
     // S9: activation time = first upward crossing of 0 mV (reading A18)
-    if (v_old <= 0.0 && y[0] > 0.0) {
+    if (v_old <= 0.0 && v_new > 0.0) {
         if (a.tact[i] < 0.0) a.tact[i] = a.t_next;
     }
 }

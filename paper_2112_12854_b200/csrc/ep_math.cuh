@@ -82,17 +82,49 @@ __device__ __forceinline__ double ep_log_core(double x) {
     return fma(ed, 6.93147180369123816490e-01, res);
 }
 
+// W exponentials at once, written stage by stage so that the W dependency chains are interleaved in issue order
+// (the fp64 pipe needs several independent chains per warp to stay busy).  Same arithmetic as ep_exp_core.
+template <int W>
+__device__ __forceinline__ void ep_exp_wide(double (&x)[W]) {
+    const double shift = 6755399441055744.0;
+    double t[W], r[W], q[W];
+    int k[W];
+#pragma unroll
+    for (int j = 0; j < W; ++j) t[j] = fma(x[j], 1.4426950408889634, shift);
+#pragma unroll
+    for (int j = 0; j < W; ++j) { k[j] = __double2loint(t[j]); t[j] -= shift; }
+#pragma unroll
+    for (int j = 0; j < W; ++j) r[j] = fma(t[j], -6.93147180369123816490e-01, x[j]);
+#pragma unroll
+    for (int j = 0; j < W; ++j) r[j] = fma(t[j], -1.90821492927058770002e-10, r[j]);
+#pragma unroll
+    for (int j = 0; j < W; ++j) q[j] = fma(EXP_Q[9], r[j], EXP_Q[8]);
+#pragma unroll
+    for (int i = 7; i >= 0; --i) {
+#pragma unroll
+        for (int j = 0; j < W; ++j) q[j] = fma(q[j], r[j], EXP_Q[i]);
+    }
+#pragma unroll
+    for (int j = 0; j < W; ++j) q[j] = fma(r[j], q[j], 1.0);
+#pragma unroll
+    for (int j = 0; j < W; ++j) q[j] = fma(r[j], q[j], 1.0);
+#pragma unroll
+    for (int j = 0; j < W; ++j) x[j] = __hiloint2double(__double2hiint(q[j]) + k[j] * 1048576, __double2loint(q[j]));
+}
+
 // Batched evaluation over a thread's own column of a shared-memory slot array xs[slot][BLOCK]; col = &xs[0][tid].
-// N must be even.  The loops stay rolled on purpose (instruction-cache footprint); two independent chains per trip.
-template <int N, int BLOCK>
+// N must be a multiple of W.  The loops stay rolled on purpose (instruction-cache footprint).
+template <int N, int BLOCK, int W>
 __device__ __forceinline__ void ep_exp_slots(double* col) {
-    static_assert(N % 2 == 0, "pad the slot list to an even length");
+    static_assert(N % W == 0, "pad the slot list to a multiple of W");
 #pragma unroll 1
-    for (int s = 0; s < N; s += 2) {
-        const double a = col[s * BLOCK], b = col[(s + 1) * BLOCK];
-        const double ea = ep_exp_core(a), eb = ep_exp_core(b);
-        col[s * BLOCK] = ea;
-        col[(s + 1) * BLOCK] = eb;
+    for (int s = 0; s < N; s += W) {
+        double x[W];
+#pragma unroll
+        for (int j = 0; j < W; ++j) x[j] = col[(s + j) * BLOCK];
+        ep_exp_wide<W>(x);
+#pragma unroll
+        for (int j = 0; j < W; ++j) col[(s + j) * BLOCK] = x[j];
     }
 }
 

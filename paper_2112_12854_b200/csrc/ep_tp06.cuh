@@ -19,6 +19,13 @@
 #pragma once
 #include "ep_math.cuh"
 
+// A 64-bit literal costs two issue slots (UMOV pair) each time it is used; a double non-type template argument (C++20)
+// instantiates one __constant__ word per distinct value, which ptxas reads with LDC.64 / LDCU.128 instead.
+// Values whose low 32 mantissa bits are zero (1.0, 0.25, 1400.0 ...) stay literals: they are free DFMA immediates.
+template <double V>
+__device__ __constant__ double EPK_CONST = V;
+#define CK(x) (::EPK_CONST<(x)>)
+
 namespace epk {
 
 enum { TP06_S = 19 };
@@ -71,70 +78,115 @@ constexpr double E5C = 148.4131591025766;         // e^(5)
 constexpr double EM1 = 0.36787944117144233;       // e^(-1)
 
 // shared-memory slots of the three batches
-enum { L_KI = 0, L_NAI, L_KS, L_CAI, N_LOG = 4 };
-enum { A_B600 = 0, A_E14, A_M, A_H, A_XR1, A_D, A_PK, A_W, A_GR, A_GS, A_G27, A_CAL, A_K1Q, A_K1Q2, A_HJ0, N_EXPA = A_HJ0 + 8 };
-enum { N_EXPB = 14 };   // 13 Rush-Larsen factors + 1 pad
-enum { N_SLOTS = N_EXPA };
-static_assert(N_EXPA % 2 == 0 && N_EXPA >= N_EXPB, "slot layout");
+constexpr int L_KI = 0, L_NAI = 1, L_KS = 2, L_CAI = 3, N_LOG = 4;
+constexpr int A_B600 = 0, A_E14 = 1, A_M = 2, A_H = 3, A_XR1 = 4, A_D = 5, A_PK = 6, A_W = 7, A_GR = 8, A_GS = 9, A_G27 = 10,
+              A_CAL = 11, A_K1Q = 12, A_K1Q2 = 13, A_HJ0 = 14, A_PAD0 = A_HJ0 + 8, N_EXPA = A_PAD0 + 2;
+constexpr int EXP_W = 4;    // exponentials evaluated side by side in the batch loops
+constexpr int N_EXPB = 16;   // 13 Rush-Larsen arguments + 3 pads, slots 0..15
+constexpr int B_INF0 = 16;   // 13 steady states, slots 16..28 (written after batch 2 has been consumed)
+constexpr int G_OLD0 = 29;   // 13 gate values at t^n, parked from the first load to the Rush-Larsen update, slots 29..41
+constexpr int N_SLOTS = 42;
+static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && N_EXPA <= G_OLD0 && B_INF0 + 13 <= G_OLD0 && G_OLD0 + 13 <= N_SLOTS, "slot layout");
 }  // namespace tp06
 
-// One step of one cell.  type: 0 endo, 1 mid, 2 epi.  istim = I_s/C_m [uA/uF], dv_diff = D_c/(chi C_m) [mV/ms].
-// col = this thread's column of the block's slot array (stride BLOCK doubles), at least tp06::N_SLOTS slots.
+// Batch 3: y_g <- inf_g + (y_g - inf_g) exp(arg_g) for the 13 Rush-Larsen variables, written straight
+// to their state rows.  Rolled, EXP_W gates per trip.
 template <int BLOCK>
-__device__ __forceinline__ void tp06_step(double (&y)[TP06_S], int type, double dt, double istim, double dv_diff,
-                                          double* col) {
+__device__ __forceinline__ void tp06_rush_larsen_slots(double* col, double* ycol, int64_t stride) {
     using namespace tp06;
-    const double v = y[Y_V];
+#pragma unroll 1
+    for (int g = 0; g < N_EXPB; g += EXP_W) {
+        double e[EXP_W];
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) e[j] = col[(g + j) * BLOCK];
+        ep_exp_wide<EXP_W>(e);
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) {
+            if (g + j < 13) {
+                const double yi = col[(B_INF0 + g + j) * BLOCK], yo = col[(G_OLD0 + g + j) * BLOCK];
+                ycol[(1 + g + j) * stride] = fma(yo - yi, e[j], yi);
+            }
+        }
+    }
+}
+
+// One step of one cell, everything on the right-hand side at t^n.  v = Vm^n of this cell, ycol = &y[0][cell] (state
+// row k at ycol[k*stride]; rows 1..18 are read and overwritten), type: 0 endo, 1 mid, 2 epi, istim = I_s/C_m [uA/uF],
+// dv_diff = D_c/(chi C_m) [mV/ms].  col = this thread's column of the block's slot array (stride BLOCK doubles,
+// tp06::N_SLOTS slots).  Returns Vm^{n+1}.
+template <int BLOCK>
+__device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stride, int type, double dt, double istim,
+                                            double dv_diff, double* col) {
+    using namespace tp06;
     const double vg = ep_clamp(v, -250.0, 250.0);   // argument of every transcendental: keeps all exponents < 700
-    const double Cai = y[Y_CAI], CaSR = y[Y_CASR], CaSS = y[Y_CASS], Nai = y[Y_NAI], Ki = y[Y_KI];
+    const double Cai = ycol[Y_CAI * stride], CaSR = ycol[Y_CASR * stride], CaSS = ycol[Y_CASS * stride],
+                 Nai = ycol[Y_NAI * stride], Ki = ycol[Y_KI * stride];
+    // gate products needed by the currents; the gate values themselves wait in shared memory for the RL update
+    double gNa, gCaL, gto, gKr, gKs, Rbar;
+    {
+        double g[13];
+#pragma unroll
+        for (int k = 0; k < 13; ++k) {
+            g[k] = ycol[(1 + k) * stride];
+            col[(G_OLD0 + k) * BLOCK] = g[k];
+        }
+        gNa = (g[Y_M - 1] * g[Y_M - 1] * g[Y_M - 1]) * g[Y_H - 1] * g[Y_J - 1];
+        gCaL = (g[Y_D - 1] * g[Y_F - 1]) * (g[Y_F2 - 1] * g[Y_FCASS - 1]);
+        gto = g[Y_R - 1] * g[Y_S - 1];
+        gKr = g[Y_XR1 - 1] * g[Y_XR2 - 1];
+        gKs = g[Y_XS - 1] * g[Y_XS - 1];
+        Rbar = g[Y_RBAR - 1];
+    }
 
     // ---- batch 1: the four logarithms of the reversal potentials
     col[L_KI * BLOCK] = Ki;
     col[L_NAI * BLOCK] = Nai;
-    col[L_KS * BLOCK] = fma(pKNa, Nai, Ki);
+    col[L_KS * BLOCK] = fma(CK(pKNa), Nai, Ki);
     col[L_CAI * BLOCK] = Cai;
     ep_log_slots<N_LOG, BLOCK>(col);
-    const double EK = RTF * (LN_KO - col[L_KI * BLOCK]);
-    const double ENa = RTF * (LN_NAO - col[L_NAI * BLOCK]);
-    const double EKs = RTF * (LN_KO_PNAO - col[L_KS * BLOCK]);
-    const double ECa = (0.5 * RTF) * (LN_CAO - col[L_CAI * BLOCK]);
+    const double EK = CK(RTF) * (CK(LN_KO) - col[L_KI * BLOCK]);
+    const double ENa = CK(RTF) * (CK(LN_NAO) - col[L_NAI * BLOCK]);
+    const double EKs = CK(RTF) * (CK(LN_KO_PNAO) - col[L_KS * BLOCK]);
+    const double ECa = CK(0.5 * RTF) * (CK(LN_CAO) - col[L_CAI * BLOCK]);
     const double u = v - EK;
     const double ug = ep_clamp(u, -300.0, 400.0);
     const bool hi = (v >= -40.0);   // reading B7
 
     // ---- batch 2: every voltage-dependent exponential that is not an integer power of another one
-    col[A_B600 * BLOCK] = vg * (1.0 / 600.0);
-    col[A_E14 * BLOCK] = vg * (1.0 / 14.0);
-    col[A_M * BLOCK] = fma(vg, -1.0 / 9.03, -56.86 / 9.03);
-    col[A_H * BLOCK] = fma(vg, 1.0 / 7.43, 71.55 / 7.43);
-    col[A_XR1 * BLOCK] = fma(vg, 1.0 / 11.5, 30.0 / 11.5);
-    col[A_D * BLOCK] = fma(vg, -1.0 / 13.0, -35.0 / 13.0);
-    col[A_PK * BLOCK] = fma(vg, -1.0 / 5.98, 25.0 / 5.98);
-    col[A_W * BLOCK] = vg * (0.05 * FRT);
-    col[A_GR * BLOCK] = (vg + 40.0) * (vg + 40.0) * (-1.0 / 1800.0);
-    col[A_GS * BLOCK] = (type == 0) ? (vg + 67.0) * (vg + 67.0) * (-1.0 / 1000.0)
-                                    : (vg + 45.0) * (vg + 45.0) * (-1.0 / 320.0);
-    col[A_G27 * BLOCK] = (vg + 27.0) * (vg + 27.0) * (-1.0 / 3600.0);
-    const double xcal = (vg - 15.0) * (2.0 * FRT);
+    col[A_B600 * BLOCK] = vg * CK(1.0 / 600.0);
+    col[A_E14 * BLOCK] = vg * CK(1.0 / 14.0);
+    col[A_M * BLOCK] = fma(vg, CK(-1.0 / 9.03), CK(-56.86 / 9.03));
+    col[A_H * BLOCK] = fma(vg, CK(1.0 / 7.43), CK(71.55 / 7.43));
+    col[A_XR1 * BLOCK] = fma(vg, CK(1.0 / 11.5), CK(30.0 / 11.5));
+    col[A_D * BLOCK] = fma(vg, CK(-1.0 / 13.0), CK(-35.0 / 13.0));
+    col[A_PK * BLOCK] = fma(vg, CK(-1.0 / 5.98), CK(25.0 / 5.98));
+    col[A_W * BLOCK] = vg * CK(0.05 * FRT);
+    col[A_GR * BLOCK] = (vg + 40.0) * (vg + 40.0) * CK(-1.0 / 1800.0);
+    col[A_GS * BLOCK] = (type == 0) ? (vg + 67.0) * (vg + 67.0) * CK(-1.0 / 1000.0)
+                                    : (vg + 45.0) * (vg + 45.0) * CK(-1.0 / 320.0);
+    col[A_G27 * BLOCK] = (vg + 27.0) * (vg + 27.0) * CK(-1.0 / 3600.0);
+    const double xcal = (vg - 15.0) * CK(2.0 * FRT);
     col[A_CAL * BLOCK] = xcal;
-    col[A_K1Q * BLOCK] = fma(ug, 0.0002, 0.02);       // 0.0002 (u + 100)
-    col[A_K1Q2 * BLOCK] = ug * 0.02;
+    col[A_K1Q * BLOCK] = fma(ug, CK(0.0002), CK(0.02));       // 0.0002 (u + 100)
+    col[A_K1Q2 * BLOCK] = ug * CK(0.02);
     if (hi) {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vg, -1.0 / 11.1, -10.66 / 11.1);
-        col[(A_HJ0 + 1) * BLOCK] = vg * 0.057;
+        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-1.0 / 11.1), CK(-10.66 / 11.1));
+        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.057);
 #pragma unroll
         for (int k = 2; k < 8; ++k) col[(A_HJ0 + k) * BLOCK] = 0.0;
     } else {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vg, -1.0 / 6.8, -80.0 / 6.8);
-        col[(A_HJ0 + 1) * BLOCK] = vg * 0.079;
-        col[(A_HJ0 + 2) * BLOCK] = vg * 0.3485;
-        col[(A_HJ0 + 3) * BLOCK] = vg * 0.2444;
-        col[(A_HJ0 + 4) * BLOCK] = vg * -0.04391;
-        col[(A_HJ0 + 5) * BLOCK] = fma(vg, 0.311, 0.311 * 79.23);
-        col[(A_HJ0 + 6) * BLOCK] = vg * -0.01052;
-        col[(A_HJ0 + 7) * BLOCK] = fma(vg, -0.1378, -0.1378 * 40.14);
+        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-1.0 / 6.8), CK(-80.0 / 6.8));
+        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.079);
+        col[(A_HJ0 + 2) * BLOCK] = vg * CK(0.3485);
+        col[(A_HJ0 + 3) * BLOCK] = vg * CK(0.2444);
+        col[(A_HJ0 + 4) * BLOCK] = vg * CK(-0.04391);
+        col[(A_HJ0 + 5) * BLOCK] = fma(vg, CK(0.311), CK(0.311 * 79.23));
+        col[(A_HJ0 + 6) * BLOCK] = vg * CK(-0.01052);
+        col[(A_HJ0 + 7) * BLOCK] = fma(vg, CK(-0.1378), CK(-0.1378 * 40.14));
     }
-    ep_exp_slots<N_EXPA, BLOCK>(col);
+    col[A_PAD0 * BLOCK] = 0.0;
+    col[(A_PAD0 + 1) * BLOCK] = 0.0;
+    ep_exp_slots<N_EXPA, BLOCK, EXP_W>(col);
 
     // ---- integer powers
     double E200, E24, E20, E15, E10, E7p5, E6, E5;
@@ -159,139 +211,141 @@ __device__ __forceinline__ void tp06_step(double (&y)[TP06_S], int type, double 
     }
 
     // ---- membrane currents
-    const double m = y[Y_M];
-    const double INa = GNa * (m * m * m) * y[Y_H] * y[Y_J] * (v - ENa);
+    const double INa = CK(GNa) * gNa * (v - ENa);
     double ICaL;
     {
         const double ex = col[A_CAL * BLOCK];
         // x/(e^x - 1), with the series 1 - x/2 inside |x| < 1e-7 (reading B6)
         const double xo = (fabs(xcal) < 1e-7) ? fma(-0.5, xcal, 1.0) : xcal * ep_rcp(ex - 1.0);
-        ICaL = (GCaL * 2.0 * F) * (y[Y_D] * y[Y_F]) * (y[Y_F2] * y[Y_FCASS]) * xo * fma(0.25 * CaSS, ex, -Cao);
+        ICaL = CK(GCaL * 2.0 * F) * gCaL * xo * fma(0.25 * CaSS, ex, -Cao);
     }
-    const double Gto = (type == 0) ? 0.073 : 0.294;
-    const double GKs = (type == 1) ? 0.098 : 0.392;
-    const double Ito = Gto * y[Y_R] * y[Y_S] * u;
-    const double IKr = GKr * y[Y_XR1] * y[Y_XR2] * u;     // sqrt(Ko/5.4) = 1
-    const double IKs = GKs * y[Y_XS] * y[Y_XS] * (v - EKs);
+    const double Gto = (type == 0) ? CK(0.073) : CK(0.294);
+    const double GKs = (type == 1) ? CK(0.098) : CK(0.392);
+    const double Ito = Gto * gto * u;
+    const double IKr = CK(GKr) * gKr * u;     // sqrt(Ko/5.4) = 1
+    const double IKs = GKs * gKs * (v - EKs);
     double IK1;
     {
         const double q = col[A_K1Q * BLOCK], Q = col[A_K1Q2 * BLOCK];
         const double Q2 = Q * Q, Q3 = Q2 * Q, Q5 = Q2 * Q3, Q10 = Q5 * Q5, Q25 = Q10 * Q10 * Q5;
-        const double t1 = fma(0.1, Q25, 0.1);                                       // 0.1 (1 + e^{-0.5u}) Q^25
-        const double t2 = fma(EM1, Q5, 3.0 * q) * fma(EM12, Q3, 1.0) * Q25;         // (3q + e^{0.1(u-10)})(1 + e^{0.06(u-200)}) Q^25
-        IK1 = GK1 * u * t1 * ep_rcp(t1 + t2);
+        const double t1 = fma(CK(0.1), Q25, CK(0.1));                                       // 0.1 (1 + e^{-0.5u}) Q^25
+        const double t2 = fma(CK(EM1), Q5, 3.0 * q) * fma(CK(EM12), Q3, 1.0) * Q25;         // (3q + e^{0.1(u-10)})(1 + e^{0.06(u-200)}) Q^25
+        IK1 = CK(GK1) * u * t1 * ep_rcp(t1 + t2);
     }
     const double Nai3 = Nai * Nai * Nai;
-    const double INaCa = (kNaCa / ((KmNai * KmNai * KmNai + Nao * Nao * Nao) * (KmCa + Cao)))
-                         * fma(W20, Nai3 * Cao, -(Nao * Nao * Nao * alpha) * Cai) * ep_rcp(W13 + ksat);
-    const double INaK = (PNaK * Ko / (Ko + KmK)) * Nai * W20
-                        * ep_rcp((Nai + KmNa) * fma(0.1245, W18, W20 + 0.0353));
-    const double IpCa = GpCa * Cai * ep_rcp(KpCa + Cai);
-    const double IpK = GpK * u * ep_rcp(1.0 + col[A_PK * BLOCK]);
-    const double IbNa = GbNa * (v - ENa);
-    const double IbCa = GbCa * (v - ECa);
+    const double INaCa = CK(kNaCa / ((KmNai * KmNai * KmNai + Nao * Nao * Nao) * (KmCa + Cao)))
+                         * fma(W20, Nai3 * Cao, CK(-(Nao * Nao * Nao * alpha)) * Cai) * ep_rcp(W13 + CK(ksat));
+    const double INaK = CK(PNaK * Ko / (Ko + KmK)) * Nai * W20
+                        * ep_rcp((Nai + KmNa) * fma(CK(0.1245), W18, W20 + CK(0.0353)));
+    const double IpCa = CK(GpCa) * Cai * ep_rcp(CK(KpCa) + Cai);
+    const double IpK = CK(GpK) * u * ep_rcp(1.0 + col[A_PK * BLOCK]);
+    const double IbNa = CK(GbNa) * (v - ENa);
+    const double IbCa = CK(GbCa) * (v - ECa);
     const double iion = INa + ICaL + Ito + IKr + IKs + IK1 + INaCa + INaK + IpCa + IpK + IbNa + IbCa;
 
     // ---- sarcoplasmic-reticulum fluxes, buffer factors (reading B3), concentration derivatives
     const double c2 = CaSR * CaSR, css2 = CaSS * CaSS, ci2 = Cai * Cai;
     const double kcasr = fma(-(maxsr - minsr) * c2, ep_rcp(c2 + EC * EC), maxsr);
-    const double O = k1p * css2 * y[Y_RBAR] * ep_rcp(fma(k3, kcasr, k1p * css2));
-    const double Irel = Vrel * O * (CaSR - CaSS);
-    const double Ileak = Vleak * (CaSR - Cai);
-    const double Iup = Vmaxup * ci2 * ep_rcp(ci2 + Kup * Kup);
-    const double Ixfer = Vxfer * (CaSS - Cai);
-    const double ti = (Cai + Kbufc) * (Cai + Kbufc), tsr = (CaSR + Kbufsr) * (CaSR + Kbufsr),
-                 tss = (CaSS + Kbufss) * (CaSS + Kbufss);
-    const double bi = ti * ep_rcp(ti + Bufc * Kbufc);
+    const double O = CK(k1p) * css2 * Rbar * ep_rcp(fma(CK(k3), kcasr, CK(k1p) * css2));
+    const double Irel = CK(Vrel) * O * (CaSR - CaSS);
+    const double Ileak = CK(Vleak) * (CaSR - Cai);
+    const double Iup = CK(Vmaxup) * ci2 * ep_rcp(ci2 + CK(Kup * Kup));
+    const double Ixfer = CK(Vxfer) * (CaSS - Cai);
+    const double ti = (Cai + CK(Kbufc)) * (Cai + CK(Kbufc)), tsr = (CaSR + CK(Kbufsr)) * (CaSR + CK(Kbufsr)),
+                 tss = (CaSS + CK(Kbufss)) * (CaSS + CK(Kbufss));
+    const double bi = ti * ep_rcp(ti + CK(Bufc * Kbufc));
     const double bsr = tsr * ep_rcp(tsr + Bufsr * Kbufsr);
-    const double bss = tss * ep_rcp(tss + Bufss * Kbufss);
-    const double dCai = bi * ((Ileak - Iup) * (Vsr / Vc) + Ixfer - (IbCa + IpCa - 2.0 * INaCa) * (Cap / (2.0 * Vc * F)));
+    const double bss = tss * ep_rcp(tss + CK(Bufss * Kbufss));
+    const double dCai = bi * ((Ileak - Iup) * CK(Vsr / Vc) + Ixfer - (IbCa + IpCa - 2.0 * INaCa) * CK(Cap / (2.0 * Vc * F)));
     const double dCaSR = bsr * (Iup - Ileak - Irel);
-    const double dCaSS = bss * (-ICaL * (Cap / (2.0 * Vss * F)) + Irel * (Vsr / Vss) - Ixfer * (Vc / Vss));
-    const double dNai = -(INa + IbNa + 3.0 * INaK + 3.0 * INaCa) * (Cap / (Vc * F));
-    const double dKi = -(IK1 + Ito + IKr + IKs - 2.0 * INaK + IpK + istim) * (Cap / (Vc * F));   // reading B8
+    const double dCaSS = bss * (-ICaL * CK(Cap / (2.0 * Vss * F)) + Irel * CK(Vsr / Vss) - Ixfer * CK(Vc / Vss));
+    const double dNai = -(INa + IbNa + 3.0 * INaK + 3.0 * INaCa) * CK(Cap / (Vc * F));
+    const double dKi = -(IK1 + Ito + IKr + IKs - 2.0 * INaK + IpK + istim) * CK(Cap / (Vc * F));   // reading B8
     const double v_new = fma(dt, dv_diff - iion - istim, v);   // eq. (7); explicit increment :172
+    ycol[Y_CAI * stride] = fma(dt, dCai, Cai);                 // forward Euler
+    ycol[Y_CASR * stride] = fma(dt, dCaSR, CaSR);
+    ycol[Y_CASS * stride] = fma(dt, dCaSS, CaSS);
+    ycol[Y_NAI * stride] = fma(dt, dNai, Nai);
+    ycol[Y_KI * stride] = fma(dt, dKi, Ki);
 
     // ---- gates: steady states and rates 1/tau, each as one rational function
     double inf[13], rate[13];   // index g = state index - 1
     {   // m: tau = s(-60-v;5) [0.1 s(v+35;5) + 0.1 s(v-50;200)],  s(z) = 1/(1+e^z)
         const double sm = ep_rcp(1.0 + col[A_M * BLOCK]);
         inf[0] = sm * sm;
-        const double P = fma(E7C, E5, 1.0), Q = fma(EM025, E200, 1.0);
-        rate[0] = (E5 + EM12) * P * Q * ep_rcp(0.1 * E5 * (P + Q));
+        const double P = fma(CK(E7C), E5, 1.0), Q = fma(CK(EM025), E200, 1.0);
+        rate[0] = (E5 + CK(EM12)) * P * Q * ep_rcp(CK(0.1) * E5 * (P + Q));
     }
     {   // h, j share the steady state
         const double sh = ep_rcp(1.0 + col[A_H * BLOCK]);
         inf[1] = inf[2] = sh * sh;
         const double s0 = col[(A_HJ0 + 0) * BLOCK], s1 = col[(A_HJ0 + 1) * BLOCK];
         if (hi) {
-            rate[1] = (0.77 / 0.13) * ep_rcp(1.0 + s0);
-            rate[2] = 0.6 * s1 * E10 * ep_rcp(E10 + EM32);
+            rate[1] = CK(0.77 / 0.13) * ep_rcp(1.0 + s0);
+            rate[2] = CK(0.6) * s1 * E10 * ep_rcp(E10 + CK(EM32));
         } else {
             const double s2 = col[(A_HJ0 + 2) * BLOCK], s3 = col[(A_HJ0 + 3) * BLOCK], s4 = col[(A_HJ0 + 4) * BLOCK],
                          s5 = col[(A_HJ0 + 5) * BLOCK], s6 = col[(A_HJ0 + 6) * BLOCK], s7 = col[(A_HJ0 + 7) * BLOCK];
-            rate[1] = fma(0.057, s0, fma(2.7, s1, 3.1e5 * s2));
-            const double N1 = fma(-2.5428e4, s3, -6.948e-6 * s4) * (vg + 37.78), D1 = 1.0 + s5;
-            const double N2 = 0.02424 * s6, D2 = 1.0 + s7;
+            rate[1] = fma(CK(0.057), s0, fma(CK(2.7), s1, 3.1e5 * s2));
+            const double N1 = fma(-2.5428e4, s3, CK(-6.948e-6) * s4) * (vg + CK(37.78)), D1 = 1.0 + s5;
+            const double N2 = CK(0.02424) * s6, D2 = 1.0 + s7;
             rate[2] = fma(N1, D2, N2 * D1) * ep_rcp(D1 * D2);
         }
     }
     {   // xr1, xr2, xs
-        inf[3] = E7 * ep_rcp(E7 + EM26_7);
-        rate[3] = (E10 + EM45) * (1.0 + col[A_XR1 * BLOCK]) * ep_rcp(2700.0 * E10);
-        inf[4] = ep_rcp(fma(E88_24, E24, 1.0));
-        rate[4] = (E20 + EM3) * fma(EM3, E20, 1.0) * ep_rcp(3.36 * E20);
-        inf[5] = E14 * ep_rcp(E14 + EM5_14);
-        const double t = ep_rsqrt((E6 + E5_6) * E6) * E6;          // 1/sqrt(1 + e^{(5-v)/6})
-        const double P15 = fma(EM35_15, E15, 1.0);
+        inf[3] = E7 * ep_rcp(E7 + CK(EM26_7));
+        rate[3] = (E10 + CK(EM45)) * (1.0 + col[A_XR1 * BLOCK]) * ep_rcp(2700.0 * E10);
+        inf[4] = ep_rcp(fma(CK(E88_24), E24, 1.0));
+        rate[4] = (E20 + CK(EM3)) * fma(CK(EM3), E20, 1.0) * ep_rcp(CK(3.36) * E20);
+        inf[5] = E14 * ep_rcp(E14 + CK(EM5_14));
+        const double t = ep_rsqrt((E6 + CK(E5_6)) * E6) * E6;          // 1/sqrt(1 + e^{(5-v)/6})
+        const double P15 = fma(CK(EM35_15), E15, 1.0);
         rate[5] = P15 * ep_rcp(fma(1400.0, t, 80.0 * P15));
     }
     {   // r, s (reading B5: endo has its own s curves)
-        inf[6] = E6 * ep_rcp(E6 + E20_6);
-        rate[6] = ep_rcp(fma(9.5, col[A_GR * BLOCK], 0.8));
+        inf[6] = E6 * ep_rcp(E6 + CK(E20_6));
+        rate[6] = ep_rcp(fma(9.5, col[A_GR * BLOCK], CK(0.8)));
         const double Gs = col[A_GS * BLOCK];
         if (type == 0) {
-            inf[7] = ep_rcp(fma(E56, E5, 1.0));
+            inf[7] = ep_rcp(fma(CK(E56), E5, 1.0));
             rate[7] = ep_rcp(fma(1000.0, Gs, 8.0));
         } else {
-            inf[7] = ep_rcp(fma(E4, E5, 1.0));
-            const double P = fma(EM4, E5, 1.0);
+            inf[7] = ep_rcp(fma(CK(E4), E5, 1.0));
+            const double P = fma(CK(EM4), E5, 1.0);
             rate[7] = P * ep_rcp(fma(fma(85.0, Gs, 3.0), P, 5.0));
         }
     }
     {   // d, f, f2
-        inf[8] = E7p5 * ep_rcp(E7p5 + EM8_75);
-        const double D = 1.0 + col[A_D * BLOCK], P5 = fma(E1, E5, 1.0), Q20 = E20 + E25;
-        rate[8] = D * P5 * Q20 * ep_rcp(fma(fma(0.25, D, 1.4) * 1.4, Q20, E20 * D * P5));
-        const double Qa = E10 + E13, Qb = fma(E3, E10, 1.0), Qc = E10 + E25;
-        inf[9] = ep_rcp(fma(E20_7, E7, 1.0));
+        inf[8] = E7p5 * ep_rcp(E7p5 + CK(EM8_75));
+        const double D = 1.0 + col[A_D * BLOCK], P5 = fma(CK(E1), E5, 1.0), Q20 = E20 + CK(E25);
+        rate[8] = D * P5 * Q20 * ep_rcp(fma(fma(0.25, D, CK(1.4)) * CK(1.4), Q20, E20 * D * P5));
+        const double Qa = E10 + CK(E13), Qb = fma(CK(E3), E10, 1.0), Qc = E10 + CK(E25);
+        inf[9] = ep_rcp(fma(CK(E20_7), E7, 1.0));
         rate[9] = Qa * Qb * ep_rcp(fma(fma(1102.5, Gf, 20.0), Qa * Qb, fma(200.0 * E10, Qb, 180.0 * Qa)));
-        inf[10] = fma(0.67, ep_rcp(fma(E5C, E7, 1.0)), 0.33);
+        inf[10] = fma(CK(0.67), ep_rcp(fma(CK(E5C), E7, 1.0)), CK(0.33));
         rate[10] = Qc * Qb * ep_rcp(fma(562.0 * Gf2, Qc * Qb, fma(31.0 * E10, Qb, 80.0 * Qc)));
     }
     {   // fCass
         const double qf = ep_rcp(fma(400.0 * CaSS, CaSS, 1.0));    // 1/(1 + (CaSS/0.05)^2)
-        inf[11] = fma(0.6, qf, 0.4);
+        inf[11] = fma(CK(0.6), qf, CK(0.4));
         rate[11] = ep_rcp(fma(80.0, qf, 2.0));
     }
     {   // Rbar: dR/dt = k4 (1 - R) - k2 CaSS R, linear in R at frozen Ca (reading B1)
-        rate[12] = fma(k2p * kcasr, CaSS, k4);
-        inf[12] = k4 * ep_rcp(rate[12]);
+        rate[12] = fma(CK(k2p) * kcasr, CaSS, CK(k4));
+        inf[12] = CK(k4) * ep_rcp(rate[12]);
     }
 
-    // ---- batch 3: Rush-Larsen factors exp(-dt/tau)
+    // ---- batch 3: Rush-Larsen (every value of batch 2 has been consumed above, so its slots are free)
 #pragma unroll
-    for (int g = 0; g < 13; ++g) col[g * BLOCK] = fmax(-dt * rate[g], -700.0);
+    for (int g = 0; g < 13; ++g) {
+        col[g * BLOCK] = fmax(-dt * rate[g], -700.0);
+        col[(B_INF0 + g) * BLOCK] = inf[g];
+    }
     col[13 * BLOCK] = 0.0;
-    ep_exp_slots<N_EXPB, BLOCK>(col);
-#pragma unroll
-    for (int g = 0; g < 13; ++g) y[1 + g] = fma(y[1 + g] - inf[g], col[g * BLOCK], inf[g]);
-    y[Y_CAI] = fma(dt, dCai, Cai);
-    y[Y_CASR] = fma(dt, dCaSR, CaSR);
-    y[Y_CASS] = fma(dt, dCaSS, CaSS);
-    y[Y_NAI] = fma(dt, dNai, Nai);
-    y[Y_KI] = fma(dt, dKi, Ki);
-    y[Y_V] = v_new;
+    col[14 * BLOCK] = 0.0;
+    col[15 * BLOCK] = 0.0;
+    tp06_rush_larsen_slots<BLOCK>(col, ycol, stride);
+    return v_new;
 }
 
 }  // namespace epk
