@@ -84,15 +84,40 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_tp
     const int64_t i = (int64_t)blockIdx.x * CELL_THREADS + threadIdx.x;
     if (i >= nc) return;
     const double v_old = a.vm_cur[i];
-    const double dv = diffusion_gather(i, stride, cidx, ccoef, a.vm_cur, a.vn, v_old);
+    // S2+S3 in two halves: indices are loaded here, the gathers are issued once the cell model has parked its gates
+    // and stay in flight while it evaluates its logarithms and first exponential batch
+    int32_t id[12];
+    double cf[12];
+#pragma unroll
+    for (int m = 0; m < 12; ++m) {
+        id[m] = __ldg(cidx + m * stride + i);
+        cf[m] = __ldg(ccoef + m * stride + i);
+    }
+    double gv[12];
+    auto issue_gather = [&]() {
+#pragma unroll
+        for (int m = 0; m < 8; ++m) gv[m] = a.vn[id[m]];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) gv[8 + j] = a.vm_cur[id[8 + j]];
+    };
+    auto finish_gather = [&]() {   // dv = sum_m a_m v_n[node_m] + sum_j b_j (v[nbr_j] - v_c)   [mV/ms]
+        double accn = 0.0, accm = 0.0, accc = 0.0;
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            accn = fma(cf[m], gv[m], accn);
+            accm = fma(cf[4 + m], gv[4 + m], accm);
+            accc = fma(cf[8 + m], gv[8 + m] - v_old, accc);
+        }
+        return (accn + accm) + accc;
+    };
     // S4: stimulus, eq. (4) PAPER.md:130-132 (window already resolved on the host into istim[k])
     const unsigned mask = a.smask[i];
     double istim = 0.0;
 #pragma unroll
     for (int k = 0; k < 8; ++k)
         if (mask & (1u << k)) istim += a.istim[k];
-    const double v_new = tp06_step<CELL_THREADS>(v_old, a.y + i, stride, a.ctype[i], a.dt, istim, dv,
-                                                 &xs[0][threadIdx.x]);
+    const double v_new = tp06_step<CELL_THREADS>(v_old, a.y + i, stride, a.ctype[i], a.dt, istim, issue_gather,
+                                                 finish_gather, &xs[0][threadIdx.x]);
     a.vm_next[i] = v_new;
     // S9: activation time = first upward crossing of 0 mV (reading A18)
     if (v_old <= 0.0 && v_new > 0.0) {

@@ -128,15 +128,38 @@ __device__ __forceinline__ void ep_exp_slots(double* col) {
     }
 }
 
-template <int N, int BLOCK>
-__device__ __forceinline__ void ep_log_slots(double* col) {
-    static_assert(N % 2 == 0, "pad the slot list to an even length");
-#pragma unroll 1
-    for (int s = 0; s < N; s += 2) {
-        const double a = col[s * BLOCK], b = col[(s + 1) * BLOCK];
-        const double la = ep_log_core(a), lb = ep_log_core(b);
-        col[s * BLOCK] = la;
-        col[(s + 1) * BLOCK] = lb;
+// W logarithms at once, stage by stage (same arithmetic as ep_log_core); arguments positive and normal.
+template <int W>
+__device__ __forceinline__ void ep_log_wide(double (&x)[W]) {
+    double m[W], s[W], z[W], p[W], ed[W];
+#pragma unroll
+    for (int j = 0; j < W; ++j) {
+        int hi = __double2hiint(x[j]);
+        const int lo = __double2loint(x[j]);
+        int e = (hi >> 20) - 1023;
+        hi = (hi & 0x000fffff) | 0x3ff00000;
+        if (hi > 0x3ff6a09e) { hi -= 0x00100000; e += 1; }    // m in [sqrt(1/2), sqrt(2))
+        m[j] = __hiloint2double(hi, lo);
+        ed[j] = (double)e;
+    }
+#pragma unroll
+    for (int j = 0; j < W; ++j) s[j] = ep_rcp(m[j] + 1.0);
+#pragma unroll
+    for (int j = 0; j < W; ++j) { s[j] *= (m[j] - 1.0); z[j] = s[j] * s[j]; }
+#pragma unroll
+    for (int j = 0; j < W; ++j) p[j] = fma(LOG_C[8], z[j], LOG_C[7]);
+#pragma unroll
+    for (int i = 6; i >= 0; --i) {
+#pragma unroll
+        for (int j = 0; j < W; ++j) p[j] = fma(p[j], z[j], LOG_C[i]);
+    }
+#pragma unroll
+    for (int j = 0; j < W; ++j) {
+        const double s2 = s[j] + s[j];
+        double res = s2 * (z[j] * p[j]);                      // summed small to large
+        res = fma(ed[j], 1.90821492927058770002e-10, res);
+        res += s2;
+        x[j] = fma(ed[j], 6.93147180369123816490e-01, res);
     }
 }
 

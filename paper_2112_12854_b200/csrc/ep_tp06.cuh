@@ -77,20 +77,21 @@ constexpr double E3 = 20.085536923187668;         // e^(3)
 constexpr double E5C = 148.4131591025766;         // e^(5)
 constexpr double EM1 = 0.36787944117144233;       // e^(-1)
 
-// shared-memory slots of the three batches
-constexpr int L_KI = 0, L_NAI = 1, L_KS = 2, L_CAI = 3, N_LOG = 4;
+// shared-memory slots of the two exponential batches
 constexpr int A_B600 = 0, A_E14 = 1, A_M = 2, A_H = 3, A_XR1 = 4, A_D = 5, A_PK = 6, A_W = 7, A_GR = 8, A_GS = 9, A_G27 = 10,
-              A_CAL = 11, A_K1Q = 12, A_K1Q2 = 13, A_HJ0 = 14, A_PAD0 = A_HJ0 + 8, N_EXPA = A_PAD0 + 2;
-constexpr int EXP_W = 4;    // exponentials evaluated side by side in the batch loops
-constexpr int N_EXPB = 16;   // 13 Rush-Larsen arguments + 3 pads, slots 0..15
-constexpr int B_INF0 = 16;   // 13 steady states, slots 16..28 (written after batch 2 has been consumed)
-constexpr int G_OLD0 = 29;   // 13 gate values at t^n, parked from the first load to the Rush-Larsen update, slots 29..41
-constexpr int N_SLOTS = 42;
-static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && N_EXPA <= G_OLD0 && B_INF0 + 13 <= G_OLD0 && G_OLD0 + 13 <= N_SLOTS, "slot layout");
+              A_CAL = 11, A_K1Q = 12, A_K1Q2 = 13, A_HJ0 = 14, A_RLF = 22, A_RLR = 23, N_EXPA = 24;
+constexpr int EXP_W = 4;     // exponentials evaluated side by side in the batch loops
+constexpr int N_RLB = 11;    // Rush-Larsen variables whose rate depends on batch 2: m h j xr1 xr2 xs r s d f f2
+constexpr int N_EXPB = 12;   // their arguments + 1 pad, slots 0..11 (fCass and Rbar ride in batch 2: rates need no exp)
+constexpr int B_INF0 = 12;   // 11 steady states, slots 12..22 (written after batch 2 has been consumed)
+constexpr int G_OLD0 = 24;   // 11 gate values at t^n, parked from the first load to the Rush-Larsen update, slots 24..34
+constexpr int N_SLOTS = 35;
+static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && N_EXPA <= G_OLD0 && B_INF0 + N_RLB <= G_OLD0 &&
+              G_OLD0 + N_RLB <= N_SLOTS, "slot layout");
 }  // namespace tp06
 
-// Batch 3: y_g <- inf_g + (y_g - inf_g) exp(arg_g) for the 13 Rush-Larsen variables, written straight
-// to their state rows.  Rolled, EXP_W gates per trip.
+// Batch 3: y_g <- inf_g + (y_g - inf_g) exp(arg_g) for the 11 voltage-driven Rush-Larsen variables,
+// written straight to their state rows 1..11.  Rolled, EXP_W gates per trip.
 template <int BLOCK>
 __device__ __forceinline__ void tp06_rush_larsen_slots(double* col, double* ycol, int64_t stride) {
     using namespace tp06;
@@ -102,7 +103,7 @@ __device__ __forceinline__ void tp06_rush_larsen_slots(double* col, double* ycol
         ep_exp_wide<EXP_W>(e);
 #pragma unroll
         for (int j = 0; j < EXP_W; ++j) {
-            if (g + j < 13) {
+            if (g + j < N_RLB) {
                 const double yi = col[(B_INF0 + g + j) * BLOCK], yo = col[(G_OLD0 + g + j) * BLOCK];
                 ycol[(1 + g + j) * stride] = fma(yo - yi, e[j], yi);
             }
@@ -111,43 +112,42 @@ __device__ __forceinline__ void tp06_rush_larsen_slots(double* col, double* ycol
 }
 
 // One step of one cell, everything on the right-hand side at t^n.  v = Vm^n of this cell, ycol = &y[0][cell] (state
-// row k at ycol[k*stride]; rows 1..18 are read and overwritten), type: 0 endo, 1 mid, 2 epi, istim = I_s/C_m [uA/uF],
-// dv_diff = D_c/(chi C_m) [mV/ms].  col = this thread's column of the block's slot array (stride BLOCK doubles,
-// tp06::N_SLOTS slots).  Returns Vm^{n+1}.
-template <int BLOCK>
+// row k at ycol[k*stride]; rows 1..18 are read and overwritten), type: 0 endo, 1 mid, 2 epi, istim = I_s/C_m [uA/uF].
+// The diffusion term D_c/(chi C_m) [mV/ms] comes from two callables so that its gathers are in flight while the
+// logarithms and the first exponential batch run: issue_gather() starts the loads, finish_gather() returns the sum.
+// col = this thread's column of the block's slot array (stride BLOCK doubles, tp06::N_SLOTS slots).  Returns Vm^{n+1}.
+template <int BLOCK, class Issue, class Finish>
 __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stride, int type, double dt, double istim,
-                                            double dv_diff, double* col) {
+                                            Issue issue_gather, Finish finish_gather, double* col) {
     using namespace tp06;
     const double vg = ep_clamp(v, -250.0, 250.0);   // argument of every transcendental: keeps all exponents < 700
     const double Cai = ycol[Y_CAI * stride], CaSR = ycol[Y_CASR * stride], CaSS = ycol[Y_CASS * stride],
                  Nai = ycol[Y_NAI * stride], Ki = ycol[Y_KI * stride];
     // gate products needed by the currents; the gate values themselves wait in shared memory for the RL update
-    double gNa, gCaL, gto, gKr, gKs, Rbar;
+    double gNa, gCaL, gto, gKr, gKs, fCass, Rbar;
     {
         double g[13];
 #pragma unroll
-        for (int k = 0; k < 13; ++k) {
-            g[k] = ycol[(1 + k) * stride];
-            col[(G_OLD0 + k) * BLOCK] = g[k];
-        }
+        for (int k = 0; k < 13; ++k) g[k] = ycol[(1 + k) * stride];
+#pragma unroll
+        for (int k = 0; k < N_RLB; ++k) col[(G_OLD0 + k) * BLOCK] = g[k];
         gNa = (g[Y_M - 1] * g[Y_M - 1] * g[Y_M - 1]) * g[Y_H - 1] * g[Y_J - 1];
-        gCaL = (g[Y_D - 1] * g[Y_F - 1]) * (g[Y_F2 - 1] * g[Y_FCASS - 1]);
+        fCass = g[Y_FCASS - 1];
+        gCaL = (g[Y_D - 1] * g[Y_F - 1]) * (g[Y_F2 - 1] * fCass);
         gto = g[Y_R - 1] * g[Y_S - 1];
         gKr = g[Y_XR1 - 1] * g[Y_XR2 - 1];
         gKs = g[Y_XS - 1] * g[Y_XS - 1];
         Rbar = g[Y_RBAR - 1];
     }
+    issue_gather();
 
-    // ---- batch 1: the four logarithms of the reversal potentials
-    col[L_KI * BLOCK] = Ki;
-    col[L_NAI * BLOCK] = Nai;
-    col[L_KS * BLOCK] = fma(CK(pKNa), Nai, Ki);
-    col[L_CAI * BLOCK] = Cai;
-    ep_log_slots<N_LOG, BLOCK>(col);
-    const double EK = CK(RTF) * (CK(LN_KO) - col[L_KI * BLOCK]);
-    const double ENa = CK(RTF) * (CK(LN_NAO) - col[L_NAI * BLOCK]);
-    const double EKs = CK(RTF) * (CK(LN_KO_PNAO) - col[L_KS * BLOCK]);
-    const double ECa = CK(0.5 * RTF) * (CK(LN_CAO) - col[L_CAI * BLOCK]);
+    // ---- batch 1: the four logarithms of the reversal potentials, side by side in registers
+    double lg[4] = {Ki, Nai, fma(CK(pKNa), Nai, Ki), Cai};
+    ep_log_wide<4>(lg);
+    const double EK = CK(RTF) * (CK(LN_KO) - lg[0]);
+    const double ENa = CK(RTF) * (CK(LN_NAO) - lg[1]);
+    const double EKs = CK(RTF) * (CK(LN_KO_PNAO) - lg[2]);
+    const double ECa = CK(0.5 * RTF) * (CK(LN_CAO) - lg[3]);
     const double u = v - EK;
     const double ug = ep_clamp(u, -300.0, 400.0);
     const bool hi = (v >= -40.0);   // reading B7
@@ -184,9 +184,18 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
         col[(A_HJ0 + 6) * BLOCK] = vg * CK(-0.01052);
         col[(A_HJ0 + 7) * BLOCK] = fma(vg, CK(-0.1378), CK(-0.1378 * 40.14));
     }
-    col[A_PAD0 * BLOCK] = 0.0;
-    col[(A_PAD0 + 1) * BLOCK] = 0.0;
+    // fCass and Rbar: their Rush-Larsen rates need no exponential, so exp(-dt/tau) rides in this batch
+    const double c2 = CaSR * CaSR, css2 = CaSS * CaSS, ci2 = Cai * Cai;
+    const double kcasr = fma(-(maxsr - minsr) * c2, ep_rcp(c2 + EC * EC), maxsr);
+    const double qf = ep_rcp(fma(400.0, css2, 1.0));              // 1/(1 + (CaSS/0.05)^2)
+    const double fCass_inf = fma(CK(0.6), qf, CK(0.4));
+    const double Rbar_rate = fma(CK(k2p) * kcasr, CaSS, CK(k4));   // dR/dt = k4 (1 - R) - k2 CaSS R (reading B1)
+    const double Rbar_inf = CK(k4) * ep_rcp(Rbar_rate);
+    col[A_RLF * BLOCK] = fmax(-dt * ep_rcp(fma(80.0, qf, 2.0)), -700.0);
+    col[A_RLR * BLOCK] = fmax(-dt * Rbar_rate, -700.0);
     ep_exp_slots<N_EXPA, BLOCK, EXP_W>(col);
+    ycol[Y_FCASS * stride] = fma(fCass - fCass_inf, col[A_RLF * BLOCK], fCass_inf);   // Rush-Larsen
+    ycol[Y_RBAR * stride] = fma(Rbar - Rbar_inf, col[A_RLR * BLOCK], Rbar_inf);
 
     // ---- integer powers
     double E200, E24, E20, E15, E10, E7p5, E6, E5;
@@ -244,8 +253,6 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double iion = INa + ICaL + Ito + IKr + IKs + IK1 + INaCa + INaK + IpCa + IpK + IbNa + IbCa;
 
     // ---- sarcoplasmic-reticulum fluxes, buffer factors (reading B3), concentration derivatives
-    const double c2 = CaSR * CaSR, css2 = CaSS * CaSS, ci2 = Cai * Cai;
-    const double kcasr = fma(-(maxsr - minsr) * c2, ep_rcp(c2 + EC * EC), maxsr);
     const double O = CK(k1p) * css2 * Rbar * ep_rcp(fma(CK(k3), kcasr, CK(k1p) * css2));
     const double Irel = CK(Vrel) * O * (CaSR - CaSS);
     const double Ileak = CK(Vleak) * (CaSR - Cai);
@@ -261,7 +268,7 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double dCaSS = bss * (-ICaL * CK(Cap / (2.0 * Vss * F)) + Irel * CK(Vsr / Vss) - Ixfer * CK(Vc / Vss));
     const double dNai = -(INa + IbNa + 3.0 * INaK + 3.0 * INaCa) * CK(Cap / (Vc * F));
     const double dKi = -(IK1 + Ito + IKr + IKs - 2.0 * INaK + IpK + istim) * CK(Cap / (Vc * F));   // reading B8
-    const double v_new = fma(dt, dv_diff - iion - istim, v);   // eq. (7); explicit increment :172
+    const double v_new = fma(dt, finish_gather() - iion - istim, v);   // eq. (7); explicit increment :172
     ycol[Y_CAI * stride] = fma(dt, dCai, Cai);                 // forward Euler
     ycol[Y_CASR * stride] = fma(dt, dCaSR, CaSR);
     ycol[Y_CASS * stride] = fma(dt, dCaSS, CaSS);
@@ -269,7 +276,7 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     ycol[Y_KI * stride] = fma(dt, dKi, Ki);
 
     // ---- gates: steady states and rates 1/tau, each as one rational function
-    double inf[13], rate[13];   // index g = state index - 1
+    double inf[N_RLB], rate[N_RLB];   // index g = state index - 1
     {   // m: tau = s(-60-v;5) [0.1 s(v+35;5) + 0.1 s(v-50;200)],  s(z) = 1/(1+e^z)
         const double sm = ep_rcp(1.0 + col[A_M * BLOCK]);
         inf[0] = sm * sm;
@@ -325,25 +332,13 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
         inf[10] = fma(CK(0.67), ep_rcp(fma(CK(E5C), E7, 1.0)), CK(0.33));
         rate[10] = Qc * Qb * ep_rcp(fma(562.0 * Gf2, Qc * Qb, fma(31.0 * E10, Qb, 80.0 * Qc)));
     }
-    {   // fCass
-        const double qf = ep_rcp(fma(400.0 * CaSS, CaSS, 1.0));    // 1/(1 + (CaSS/0.05)^2)
-        inf[11] = fma(CK(0.6), qf, CK(0.4));
-        rate[11] = ep_rcp(fma(80.0, qf, 2.0));
-    }
-    {   // Rbar: dR/dt = k4 (1 - R) - k2 CaSS R, linear in R at frozen Ca (reading B1)
-        rate[12] = fma(CK(k2p) * kcasr, CaSS, CK(k4));
-        inf[12] = CK(k4) * ep_rcp(rate[12]);
-    }
-
     // ---- batch 3: Rush-Larsen (every value of batch 2 has been consumed above, so its slots are free)
 #pragma unroll
-    for (int g = 0; g < 13; ++g) {
+    for (int g = 0; g < N_RLB; ++g) {
         col[g * BLOCK] = fmax(-dt * rate[g], -700.0);
         col[(B_INF0 + g) * BLOCK] = inf[g];
     }
-    col[13 * BLOCK] = 0.0;
-    col[14 * BLOCK] = 0.0;
-    col[15 * BLOCK] = 0.0;
+    col[N_RLB * BLOCK] = 0.0;
     tp06_rush_larsen_slots<BLOCK>(col, ycol, stride);
     return v_new;
 }
