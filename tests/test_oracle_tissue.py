@@ -1,0 +1,78 @@
+"""Tissue-level pins of the oracle (diffusion + TP06 together) against what the paper states.
+
+P11 (Fig. 11): conduction velocity along the fibres rises with mesh refinement and converges; the
+converged value lies in the physiological range for ventricular myocardium (PAPER.md:21 quotes 0.3-0.5 m/s for atria
+and faster ventricles; TP06 monodomain benchmarks sit at 0.5-0.7 m/s along fibres).
+P5 (dense brute force): the operator assembled column by column from the oracle equals the dense matrix expanded
+from the preprocessor's factored coefficients, has zero row sums, volume-weighted zero column sums and a spectrum in
+the closed left half-plane.
+"""
+import os
+
+import numpy as np
+
+from ep_inputs import meshes as M
+
+
+def _cv_along_x(oracle, h, dt, t_end=16.0):
+    nx, ny = int(round(6.0 / h)), max(2, int(round(1.0 / h)))
+    m = M.kuhn_slab(nx, ny, ny, h)
+    fib = np.tile([1.0, 0.0, 0.0], (m.n_tets, 1))
+    s = oracle.OracleSim(m.xyz, m.tets, fib, None, 1.3, 0.18, 1400.0, 1.0)
+    s.state_init(0, None)
+    cen = m.centroids()
+    s.stimulus_set(0, np.nonzero(cen[:, 0] < 0.5)[0], -52.0, 0.0, 1.0)
+    s.step(int(round(t_end / dt)), dt)
+    ta = s.activation_times()
+    assert (ta >= 0).all(), "the wave must cross the whole slab"
+    # mean activation time in two transverse slices
+    a = np.abs(cen[:, 0] - 2.0) < 0.5 * h + 1e-9
+    b = np.abs(cen[:, 0] - 4.5) < 0.5 * h + 1e-9
+    xa, xb = cen[a, 0].mean(), cen[b, 0].mean()
+    return (xb - xa) / (ta[b].mean() - ta[a].mean()) * 100.0   # mm/ms -> cm/s
+
+
+def test_plane_wave_cv_converges_under_refinement(oracle):
+    oracle.set_threads(max(1, os.cpu_count() or 1))
+    cv = [_cv_along_x(oracle, 0.5, 0.02), _cv_along_x(oracle, 0.25, 0.02), _cv_along_x(oracle, 0.125, 0.01)]
+    oracle.set_threads(1)
+    assert cv[0] < cv[1] < cv[2], cv                 # rises with refinement
+    assert (cv[2] - cv[1]) < (cv[1] - cv[0]), cv     # and the increments shrink: converging from below
+    assert abs(cv[1] - 53.7) < 1.0 and abs(cv[2] - 58.6) < 1.0, cv   # regression guard (SURVEY probe: 53.5 / 58.9)
+    assert 45.0 < cv[2] < 75.0, cv                   # physiological range along fibres
+
+
+def test_dense_assembly_matches_factored_stencil(oracle):
+    import paper_2112_12854_b200 as ep
+    m = M.kuhn_slab(4, 3, 3, 0.4)
+    M.jitter_interior(m, 0.06, 5)
+    cen = m.centroids()
+    th = np.deg2rad(-60 + 120 * cen[:, 2] / 1.2)
+    fib = np.stack([np.cos(th), np.sin(th), 0 * th], axis=1)
+    n = m.n_tets
+    s = oracle.OracleSim(m.xyz, m.tets, fib, None, 1.3, 0.18, 1400.0, 1.0)
+    A = np.empty((n, n))
+    for j in range(n):                                # brute force: one unit vector per column
+        e = np.zeros(n); e[j] = 1.0
+        A[:, j] = s.apply_diffusion(e)
+    st = ep.host_stencil(m.xyz, m.tets, fib, None, 1.3, 0.18, 1400.0, 1.0)
+    nn = m.n_nodes
+    W = np.zeros((nn, n))                             # node interpolation matrix
+    owner = np.repeat(np.arange(nn), np.diff(st["node_ptr"]))
+    W[owner, st["node_cell"]] += st["w"]
+    B = np.zeros((n, n))
+    rows = np.arange(n)
+    for k in range(8):
+        B += st["a"][:, k, None] * W[st["node"][:, k], :]
+    for k in range(4):
+        np.add.at(B, (rows, st["nbr"][:, k]), st["b"][:, k])
+        np.add.at(B, (rows, rows), -st["b"][:, k])
+    B *= 1400.0 * 1.0
+    scale = np.abs(A).max()
+    assert np.abs(A - B).max() <= 1e-12 * scale
+    assert np.abs(A.sum(axis=1)).max() <= 1e-11 * scale            # P1: row sums vanish
+    vol, _ = s.geometry()
+    assert np.abs(vol @ A).max() <= 1e-11 * scale * vol.max()      # P2: volume-weighted column sums vanish
+    assert np.all(np.diag(A) < 0)
+    lam = np.linalg.eigvals(A)
+    assert lam.real.max() <= 1e-9 * scale                          # stable with eq. (8)
