@@ -2,7 +2,8 @@
 //
 // Plain, slow, obviously-correct fp64 implementation of the explicit monodomain time step of
 // arXiv 2112.12854 (section 3.2) on a tetrahedral cell-centred finite-volume mesh, with the
-// ten Tusscher-Panfilov 2006 ventricular cell model (ref [3]) integrated by Rush-Larsen
+// ten Tusscher-Panfilov 2006 ventricular cell model (ref [3]) -- and the Courtemanche atrial model
+// (ref [1], config 5) -- integrated by Rush-Larsen
 // (gates) and forward Euler (everything else).
 //
 // Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may use this file.
@@ -188,6 +189,172 @@ void tp06_step(const double* y, int type, double dt, double istim, double dv_dif
     yn[18] = y[18] + dt * dKi;
     yn[0] = y[0] + dt * (dv_diff - c.iion - istim);  // eq. (7), explicit increment :172
 }
+
+
+// ---------------------------------------------------------------------------------------------------------
+// Courtemanche-Ramirez-Nattel 1998 human atrial cell model (ref [1] PAPER.md:352: 21 state
+// variables, 15 of them gating variables advanced by Rush-Larsen).  Equations and constants restated from the
+// published model (DESIGN.md Appendix B).  Units: mV, ms, mM; currents are per unit capacitance (pA/pF = uA/uF);
+// where the published concentration equations use whole-cell currents in pA they are multiplied by C_m = 100 pF.
+// State order: 0 V, 1 m, 2 h, 3 j, 4 oa, 5 oi, 6 ua, 7 ui, 8 xr, 9 xs, 10 d, 11 f, 12 fCa, 13 u, 14 v, 15 w,
+//              16 Na_i, 17 K_i, 18 Ca_i, 19 Ca_up, 20 Ca_rel.
+namespace crn {
+const int S = 21;
+const double R = 8.3143, T = 310.0, F = 96.4867;          // J/(K mol), K, C/mmol
+const double RTF = R * T / F;                              // mV
+const double Cm = 100.0;                                   // pF
+const double Vi = 13668.0, Vup = 1109.52, Vrel = 96.48;    // um^3
+const double Ko = 5.4, Nao = 140.0, Cao = 1.8;
+const double gNa = 7.8, gK1 = 0.09, gto = 0.1652, gKr = 0.0294, gKs = 0.129, gCaL = 0.1238, gbCa = 0.00113, gbNa = 0.000674;
+const double INaKmax = 0.60, INaCamax = 1600.0, IpCamax = 0.275, Iupmax = 0.005;
+const double KQ10 = 3.0, gam = 0.35, KmNai = 10.0, KmKo = 1.5, KmNa = 87.5, KmCa = 1.38, ksat = 0.1;
+const double krel = 30.0, Kup = 0.00092, Caupmax = 15.0, tau_tr = 180.0, tau_fCa = 2.0, tau_u = 8.0;
+const double Cmdnmax = 0.05, Trpnmax = 0.07, Csqnmax = 10.0, KmCmdn = 0.00238, KmTrpn = 0.0005, KmCsqn = 0.8;
+const double REST[S] = {-81.18, 2.91e-3, 0.965, 0.978, 0.0304, 0.999, 4.96e-3, 0.999, 3.29e-5, 0.0187, 1.37e-4, 0.999,
+                        0.775, 0.0, 1.0, 0.999, 11.17, 139.0, 1.013e-4, 1.488, 1.488};
+
+// phi(x) = x/(e^x - 1); reading B11: 1 - x/2 + x^2/12 for |x| < 1e-4 (removable singularities of the alpha/beta and
+// tau expressions at V = -47.13, -14.1, 3.3328, 19.9, -10, 7.9 mV)
+inline double phi(double x) {
+    if (std::fabs(x) < 1e-4) return 1.0 - 0.5 * x + x * x / 12.0;
+    return x / (std::exp(x) - 1.0);
+}
+
+struct Currents {
+    double INa, IK1, Ito, IKur, IKr, IKs, ICaL, IpCa, INaK, INaCa, IbNa, IbCa, iion;
+    double Irel, Itr, Iup, Iupleak, Fn;
+};
+
+void currents(const double* y, Currents& c) {
+    const double V = y[0], m = y[1], h = y[2], j = y[3], oa = y[4], oi = y[5], ua = y[6], ui = y[7], xr = y[8], xs = y[9];
+    const double d = y[10], f = y[11], fCa = y[12], u = y[13], v = y[14], w = y[15];
+    const double Nai = y[16], Ki = y[17], Cai = y[18], Caup = y[19], Carel = y[20];
+    const double ENa = RTF * std::log(Nao / Nai), EK = RTF * std::log(Ko / Ki), ECa = 0.5 * RTF * std::log(Cao / Cai);
+    c.INa = gNa * m * m * m * h * j * (V - ENa);
+    c.IK1 = gK1 * (V - EK) / (1.0 + std::exp(0.07 * (V + 80.0)));
+    c.Ito = gto * oa * oa * oa * oi * (V - EK);
+    const double gKur = 0.005 + 0.05 / (1.0 + std::exp(-(V - 15.0) / 13.0));
+    c.IKur = gKur * ua * ua * ua * ui * (V - EK);
+    c.IKr = gKr * xr * (V - EK) / (1.0 + std::exp((V + 15.0) / 22.4));
+    c.IKs = gKs * xs * xs * (V - EK);
+    c.ICaL = gCaL * d * f * fCa * (V - 65.0);
+    const double sigma = (std::exp(Nao / 67.3) - 1.0) / 7.0;
+    const double fNaK = 1.0 / (1.0 + 0.1245 * std::exp(-0.1 * V / RTF) + 0.0365 * sigma * std::exp(-V / RTF));
+    c.INaK = INaKmax * fNaK / (1.0 + std::pow(KmNai / Nai, 1.5)) * Ko / (Ko + KmKo);
+    {
+        const double e1 = std::exp(gam * V / RTF), e2 = std::exp((gam - 1.0) * V / RTF);
+        c.INaCa = INaCamax * (e1 * Nai * Nai * Nai * Cao - e2 * Nao * Nao * Nao * Cai)
+                  / ((KmNa * KmNa * KmNa + Nao * Nao * Nao) * (KmCa + Cao) * (1.0 + ksat * e2));
+    }
+    c.IbCa = gbCa * (V - ECa);
+    c.IbNa = gbNa * (V - ENa);
+    c.IpCa = IpCamax * Cai / (0.0005 + Cai);
+    c.iion = c.INa + c.IK1 + c.Ito + c.IKur + c.IKr + c.IKs + c.ICaL + c.IpCa + c.INaK + c.INaCa + c.IbNa + c.IbCa;
+    c.Irel = krel * u * u * v * w * (Carel - Cai);
+    c.Itr = (Caup - Carel) / tau_tr;
+    c.Iup = Iupmax / (1.0 + Kup / Cai);
+    c.Iupleak = Caup / Caupmax * Iupmax;
+    // flux signal driving the u and v gates; whole-cell currents in pA = C_m * (pA/pF)
+    c.Fn = 1e-12 * Vrel * c.Irel - (5e-13 / F) * (0.5 * Cm * c.ICaL - 0.2 * Cm * c.INaCa);
+}
+
+// steady states and time constants of the 15 gates, index g = state index - 1
+void gates(double V, double Cai, double Fn, double* inf, double* tau) {
+    {   // m
+        const double am = 3.2 * phi(-0.1 * (V + 47.13));     // 0.32 (V+47.13)/(1 - exp(-0.1 (V+47.13)))
+        const double bm = 0.08 * std::exp(-V / 11.0);
+        inf[0] = am / (am + bm); tau[0] = 1.0 / (am + bm);
+    }
+    {   // h, j: V >= -40 takes the high-voltage branch (reading B7)
+        double ah, bh, aj, bj;
+        if (V >= -40.0) {
+            ah = 0.0; bh = 1.0 / (0.13 * (1.0 + std::exp(-(V + 10.66) / 11.1)));
+            aj = 0.0; bj = 0.3 * std::exp(-2.535e-7 * V) / (1.0 + std::exp(-0.1 * (V + 32.0)));
+        } else {
+            ah = 0.135 * std::exp(-(V + 80.0) / 6.8);
+            bh = 3.56 * std::exp(0.079 * V) + 3.1e5 * std::exp(0.35 * V);
+            aj = (-127140.0 * std::exp(0.2444 * V) - 3.474e-5 * std::exp(-0.04391 * V)) * (V + 37.78)
+                 / (1.0 + std::exp(0.311 * (V + 79.23)));
+            bj = 0.1212 * std::exp(-0.01052 * V) / (1.0 + std::exp(-0.1378 * (V + 40.14)));
+        }
+        inf[1] = ah / (ah + bh); tau[1] = 1.0 / (ah + bh);
+        inf[2] = aj / (aj + bj); tau[2] = 1.0 / (aj + bj);
+    }
+    {   // oa, ua share alpha and beta
+        const double a = 0.65 / (std::exp(-(V + 10.0) / 8.5) + std::exp(-(V - 30.0) / 59.0));
+        const double b = 0.65 / (2.5 + std::exp((V + 82.0) / 17.0));
+        inf[3] = 1.0 / (1.0 + std::exp(-(V + 20.47) / 17.54)); tau[3] = 1.0 / (a + b) / KQ10;
+        inf[5] = 1.0 / (1.0 + std::exp(-(V + 30.3) / 9.6));     tau[5] = 1.0 / (a + b) / KQ10;
+    }
+    {   // oi
+        const double a = 1.0 / (18.53 + std::exp((V + 113.7) / 10.95));
+        const double b = 1.0 / (35.56 + std::exp(-(V + 1.26) / 7.44));
+        inf[4] = 1.0 / (1.0 + std::exp((V + 43.1) / 5.3)); tau[4] = 1.0 / (a + b) / KQ10;
+    }
+    {   // ui
+        const double a = 1.0 / (21.0 + std::exp(-(V - 185.0) / 28.0));
+        const double b = std::exp((V - 158.0) / 16.0);
+        inf[6] = 1.0 / (1.0 + std::exp((V - 99.45) / 27.48)); tau[6] = 1.0 / (a + b) / KQ10;
+    }
+    {   // xr
+        const double a = 0.0015 * phi(-(V + 14.1) / 5.0);                    // 0.0003 (V+14.1)/(1 - exp(-(V+14.1)/5))
+        const double b = 7.3898e-5 * 5.1237 * phi((V - 3.3328) / 5.1237);    // 7.3898e-5 (V-3.3328)/(exp((V-3.3328)/5.1237) - 1)
+        inf[7] = 1.0 / (1.0 + std::exp(-(V + 14.1) / 6.5)); tau[7] = 1.0 / (a + b);
+    }
+    {   // xs
+        const double a = 4e-5 * 17.0 * phi(-(V - 19.9) / 17.0);              // 4e-5 (V-19.9)/(1 - exp(-(V-19.9)/17))
+        const double b = 3.5e-5 * 9.0 * phi((V - 19.9) / 9.0);               // 3.5e-5 (V-19.9)/(exp((V-19.9)/9) - 1)
+        inf[8] = 1.0 / std::sqrt(1.0 + std::exp(-(V - 19.9) / 12.7)); tau[8] = 0.5 / (a + b);
+    }
+    {   // d: tau = (1 - e^x)/(0.035 (V+10)(1 + e^x)), x = -(V+10)/6.24
+        const double x = -(V + 10.0) / 6.24;
+        inf[9] = 1.0 / (1.0 + std::exp(-(V + 10.0) / 8.0));
+        tau[9] = 1.0 / (0.035 * 6.24 * phi(x) * (1.0 + std::exp(x)));
+    }
+    {   // f
+        inf[10] = 1.0 / (1.0 + std::exp((V + 28.0) / 6.9));
+        tau[10] = 9.0 / (0.0197 * std::exp(-0.0337 * 0.0337 * (V + 10.0) * (V + 10.0)) + 0.02);
+    }
+    inf[11] = 1.0 / (1.0 + Cai / 0.00035); tau[11] = tau_fCa;   // fCa
+    {   // u, v driven by Fn
+        const double e1 = std::exp(-(Fn - 3.4175e-13) / 13.67e-16);
+        inf[12] = 1.0 / (1.0 + e1); tau[12] = tau_u;
+        inf[13] = 1.0 - 1.0 / (1.0 + std::exp(-(Fn - 6.835e-14) / 13.67e-16));
+        tau[13] = 1.91 + 2.09 / (1.0 + e1);
+    }
+    {   // w: tau = 6 (1 - e^x)/((1 + 0.3 e^x)(V-7.9)), x = -(V-7.9)/5
+        const double x = -(V - 7.9) / 5.0;
+        inf[14] = 1.0 - 1.0 / (1.0 + std::exp(-(V - 40.0) / 17.0));
+        tau[14] = 6.0 / (5.0 * phi(x) * (1.0 + 0.3 * std::exp(x)));
+    }
+}
+
+// One explicit step of one cell: gates by Rush-Larsen, the rest by forward Euler, all from t^n.
+void step(const double* y, double dt, double istim, double dv_diff, double* yn) {
+    Currents c;
+    currents(y, c);
+    double inf[15], tau[15];
+    gates(y[0], y[18], c.Fn, inf, tau);
+    for (int g = 0; g < 15; ++g) yn[1 + g] = inf[g] + (y[1 + g] - inf[g]) * std::exp(-dt / tau[g]);
+    const double Cai = y[18], Caup = y[19], Carel = y[20];
+    const double FVi = F * Vi;
+    // whole-cell currents in pA = C_m * per-capacitance currents (reading B10: the stimulus is not counted in dK_i/dt)
+    const double dNai = Cm * (-3.0 * c.INaK - 3.0 * c.INaCa - c.IbNa - c.INa) / FVi;
+    const double dKi = Cm * (2.0 * c.INaK - c.IK1 - c.Ito - c.IKur - c.IKr - c.IKs) / FVi;
+    const double B1 = Cm * (2.0 * c.INaCa - c.IpCa - c.ICaL - c.IbCa) / (2.0 * FVi)
+                      + (Vup * (c.Iupleak - c.Iup) + c.Irel * Vrel) / Vi;
+    const double B2 = 1.0 + Trpnmax * KmTrpn / ((Cai + KmTrpn) * (Cai + KmTrpn))
+                      + Cmdnmax * KmCmdn / ((Cai + KmCmdn) * (Cai + KmCmdn));
+    const double dCaup = c.Iup - c.Iupleak - c.Itr * Vrel / Vup;
+    const double dCarel = (c.Itr - c.Irel) / (1.0 + Csqnmax * KmCsqn / ((Carel + KmCsqn) * (Carel + KmCsqn)));
+    yn[16] = y[16] + dt * dNai;
+    yn[17] = y[17] + dt * dKi;
+    yn[18] = Cai + dt * (B1 / B2);
+    yn[19] = Caup + dt * dCaup;
+    yn[20] = Carel + dt * dCarel;
+    yn[0] = y[0] + dt * (dv_diff - c.iion - istim);
+}
+}  // namespace crn
 
 }  // namespace
 
@@ -462,13 +629,14 @@ void orc_apply_diffusion(void* h, const double* v, double* D, int use_corr) { ap
 
 int orc_state_init(void* h, int model, const uint8_t* cell_type, const double* y0) {
     Sim& s = *(Sim*)h;
-    if (model != 0) return -3;
-    s.model = model; s.S = TP06_S;
+    if (model != 0 && model != 1) return -3;
+    s.model = model; s.S = (model == 0) ? TP06_S : crn::S;
+    const double* rest = (model == 0) ? TP06_REST : crn::REST;
     s.ctype.assign(s.nc, 0);
     if (cell_type) s.ctype.assign(cell_type, cell_type + s.nc);
     s.y.resize((size_t)s.S * s.nc); s.yn.resize((size_t)s.S * s.nc);
     for (int64_t c = 0; c < s.nc; ++c) {
-        const double* src = y0 ? y0 + (size_t)s.ctype[c] * s.S : TP06_REST;
+        const double* src = y0 ? y0 + (size_t)s.ctype[c] * s.S : rest;
         for (int k = 0; k < s.S; ++k) s.y[(size_t)k * s.nc + c] = src[k];
     }
     s.tact.assign(s.nc, -1.0);
@@ -508,7 +676,8 @@ int orc_step(void* h, int64_t n_steps, double dt) {
             for (int k = 0; k < s.S; ++k) y[k] = s.y[(size_t)k * nc + c];
             double Is = 0.0;   // uA/cm^2, eq. (4)
             for (int k = 0; k < 8; ++k) if (on[k] && s.stim[k].mask[c]) Is += s.stim[k].amp;
-            tp06_step(y, s.ctype[c], dt, Is / s.Cm, s.D[c] * inv_chiCm, yn);
+            if (s.model == 0) tp06_step(y, s.ctype[c], dt, Is / s.Cm, s.D[c] * inv_chiCm, yn);
+            else crn::step(y, dt, Is / s.Cm, s.D[c] * inv_chiCm, yn);
             for (int k = 0; k < s.S; ++k) s.yn[(size_t)k * nc + c] = yn[k];
             if (s.tact[c] < 0.0 && y[0] <= 0.0 && yn[0] > 0.0) s.tact[c] = (double)(n + 1) * dt;   // A18
         }
@@ -542,6 +711,28 @@ void orc_tp06_run(double* y, int type, double dt, int64_t n_steps, double istim,
     for (int64_t n = 0; n < n_steps; ++n) {
         const double is = (n_on <= n && n < n_off) ? istim : 0.0;
         tp06_step(y, type, dt, is, 0.0, yn);
+        if (freeze_v) yn[0] = y[0];
+        std::memcpy(y, yn, sizeof(yn));
+        if (vtrace) vtrace[n + 1] = y[0];
+    }
+}
+
+// ---- Courtemanche single-cell entry points (pins P8, P12)
+void orc_crn_rest(double* y) { std::memcpy(y, crn::REST, sizeof(crn::REST)); }
+void orc_crn_gates(double V, double Cai, double Fn, double* inf, double* tau) { crn::gates(V, Cai, Fn, inf, tau); }
+void orc_crn_currents(const double* y, double* out18) {
+    crn::Currents c; crn::currents(y, c);
+    const double a[18] = {c.INa, c.IK1, c.Ito, c.IKur, c.IKr, c.IKs, c.ICaL, c.IpCa, c.INaK, c.INaCa, c.IbNa, c.IbCa, c.iion,
+                          c.Irel, c.Itr, c.Iup, c.Iupleak, c.Fn};
+    std::memcpy(out18, a, sizeof(a));
+}
+void orc_crn_run(double* y, double dt, int64_t n_steps, double istim, int64_t n_on, int64_t n_off, double* vtrace,
+                 int freeze_v) {
+    double yn[crn::S];
+    if (vtrace) vtrace[0] = y[0];
+    for (int64_t n = 0; n < n_steps; ++n) {
+        const double is = (n_on <= n && n < n_off) ? istim : 0.0;
+        crn::step(y, dt, is, 0.0, yn);
         if (freeze_v) yn[0] = y[0];
         std::memcpy(y, yn, sizeof(yn));
         if (vtrace) vtrace[n + 1] = y[0];

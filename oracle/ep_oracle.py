@@ -62,6 +62,10 @@ def lib():
         L.orc_tp06_gates.argtypes = [C.c_double, C.c_int, C.c_double, C.c_double, _dp, _dp]
         L.orc_tp06_currents.argtypes = [_dp, C.c_int, _dp]
         L.orc_tp06_run.argtypes = [_dp, C.c_int, C.c_double, C.c_int64, C.c_double, C.c_int64, C.c_int64, _dp, C.c_int]
+        L.orc_crn_rest.argtypes = [_dp]
+        L.orc_crn_gates.argtypes = [C.c_double, C.c_double, C.c_double, _dp, _dp]
+        L.orc_crn_currents.argtypes = [_dp, _dp]
+        L.orc_crn_run.argtypes = [_dp, C.c_double, C.c_int64, C.c_double, C.c_int64, C.c_int64, _dp, C.c_int]
         _lib = L
     return _lib
 
@@ -206,4 +210,35 @@ def tp06_run(y, cell_type, dt, n_steps, istim=0.0, n_on=0, n_off=0, trace=False,
     tr = np.empty(n_steps + 1) if trace else None
     lib().orc_tp06_run(_p(y), int(cell_type), float(dt), int(n_steps), float(istim), int(n_on), int(n_off), _p(tr),
                        1 if freeze_v else 0)
+    return y, tr
+
+
+# ---- Courtemanche single-cell helpers
+CRN_CURRENTS = ["INa", "IK1", "Ito", "IKur", "IKr", "IKs", "ICaL", "IpCa", "INaK", "INaCa", "IbNa", "IbCa", "iion", "Irel",
+                "Itr", "Iup", "Iupleak", "Fn"]
+
+
+def crn_rest():
+    y = np.empty(21)
+    lib().orc_crn_rest(_p(y))
+    return y
+
+
+def crn_gates(V, Cai=1.013e-4, Fn=0.0):
+    inf, tau = np.empty(15), np.empty(15)
+    lib().orc_crn_gates(float(V), float(Cai), float(Fn), _p(inf), _p(tau))
+    return inf, tau
+
+
+def crn_currents(y):
+    y = np.ascontiguousarray(y, dtype=np.float64)
+    out = np.empty(18)
+    lib().orc_crn_currents(_p(y), _p(out))
+    return dict(zip(CRN_CURRENTS, out))
+
+
+def crn_run(y, dt, n_steps, istim=0.0, n_on=0, n_off=0, trace=False, freeze_v=False):
+    y = np.array(y, dtype=np.float64)
+    tr = np.empty(n_steps + 1) if trace else None
+    lib().orc_crn_run(_p(y), float(dt), int(n_steps), float(istim), int(n_on), int(n_off), _p(tr), 1 if freeze_v else 0)
     return y, tr
