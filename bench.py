@@ -230,7 +230,7 @@ def run_ours(args):
     cell_ms = prof["ms_cell"] / max(1, prof["steps"])
     node_ms = prof["ms_node"] / max(1, prof["steps"])
     achieved = cell_bytes / (cell_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "cell_step_tp06_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": "cell_step_kernel<%d>" % prob.model, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "peak_source": peak_src, "traffic": args.traffic,
                 "alg_bytes_per_launch": cell_bytes, "alg_bytes_per_cell": cell_bytes / nc,
                 "avg_launch_ms": cell_ms, "node_kernel_avg_launch_ms": node_ms,

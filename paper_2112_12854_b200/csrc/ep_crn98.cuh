@@ -1,0 +1,331 @@
+// ep_crn98.cuh -- Courtemanche-Ramirez-Nattel 1998 human atrial cell model, one explicit step of one cell (device code).
+//
+// BASELINE config 5 (ref [1] PAPER.md:352: 21 states, 15 gates advanced by Rush-Larsen, the
+// rest by forward Euler, everything on the right-hand side at t^n).  Equations and constants restated
+// from the published model (DESIGN.md Appendix B); readings B7 (v >= -40 mV takes the high-voltage h/j branch), B10 (the
+// stimulus is not counted in dK_i/dt: the published equation has no such term) and B11 (x/(e^x-1) -> 1 - x/2 + x^2/12
+// for |x| < 1e-4 at the six removable singularities) apply.
+//
+// Same production form as ep_tp06.cuh: commensurate exponentials are powers / constant multiples of one exponential
+// (V/17: oa, xs, w_inf; V/5: xr, w; 0.1 V: m, j; VF/20RT: I_NaK, I_NaCa), every tau is multiplied out to one rational
+// rate, exponentials go through the shared-memory batch loops of ep_math.cuh.
+// Units: mV, ms, mM; currents per unit capacitance (pA/pF = uA/uF); whole-cell currents are C_m = 100 pF times those.
+#pragma once
+#include "ep_tp06.cuh"   // CK(), ep_math.cuh
+
+namespace epk {
+
+enum { CRN_S = 21 };
+// state order at the ABI: V m h j oa oi ua ui xr xs d f fCa u v w Na_i K_i Ca_i Ca_up Ca_rel
+enum { C_V = 0, C_M, C_H, C_J, C_OA, C_OI, C_UA, C_UI, C_XR, C_XS, C_D, C_F, C_FCA, C_U, C_VG, C_W, C_NAI, C_KI, C_CAI,
+       C_CAUP, C_CAREL };
+
+__device__ __constant__ const double CRN_REST_STATE[CRN_S] = {
+    -81.18, 2.91e-3, 0.965, 0.978, 0.0304, 0.999, 4.96e-3, 0.999, 3.29e-5, 0.0187, 1.37e-4, 0.999,
+    0.775,  0.0,     1.0,   0.999, 11.17,  139.0, 1.013e-4, 1.488, 1.488};
+
+namespace crn {
+constexpr double R = 8.3143, T = 310.0, F = 96.4867;
+constexpr double RTF = R * T / F, FRT = F / (R * T);
+constexpr double Cm = 100.0, Vi = 13668.0, Vup = 1109.52, Vrel = 96.48;
+constexpr double Ko = 5.4, Nao = 140.0, Cao = 1.8;
+constexpr double gNa = 7.8, gK1 = 0.09, gto = 0.1652, gKr = 0.0294, gKs = 0.129, gCaL = 0.1238, gbCa = 0.00113,
+                 gbNa = 0.000674;
+constexpr double INaKmax = 0.60, INaCamax = 1600.0, IpCamax = 0.275, Iupmax = 0.005;
+constexpr double KmNai = 10.0, KmKo = 1.5, KmNa = 87.5, KmCa = 1.38, ksat = 0.1;
+constexpr double krel = 30.0, Kup = 0.00092, Caupmax = 15.0, tau_tr = 180.0;
+constexpr double Cmdnmax = 0.05, Trpnmax = 0.07, Csqnmax = 10.0, KmCmdn = 0.00238, KmTrpn = 0.0005, KmCsqn = 0.8;
+constexpr double LN_KO = 1.6863989535702288, LN_NAO = 4.941642422609304, LN_CAO = 0.5877866649021191;
+// e^c constants of the split exponents
+constexpr double E82_17 = 124.40338763970256;      // e^(82/17)
+constexpr double E199_17 = 3.22388848586336;     // e^(19.9/17)
+constexpr double E40_17 = 10.516455032989136;      // e^(40/17)
+constexpr double EM141_5 = 0.059605942708939354;    // e^(-14.1/5)
+constexpr double E79_5 = 4.854955811237433;        // e^(7.9/5)
+constexpr double E1513 = 4.540331377371345;        // e^(1.513) = e^(-0.1 (32 - 47.13))
+constexpr double SIGMA = 1.0009103049457282;       // (e^(Nao/67.3) - 1)/7
+constexpr double EM200 = 1.3838965267367376e-87;   // e^(-200) = e^(-(3.4175e-13 - 6.835e-14)/13.67e-16)
+
+// shared-memory slots
+constexpr int A_E17 = 0, A_W = 1, A_X1 = 2, A_BM = 3, A_K1 = 4, A_OA1 = 5, A_OA2 = 6, A_OAI = 7, A_UAI = 8, A_OI1 = 9,
+              A_OI2 = 10, A_OII = 11, A_UI1 = 12, A_UI2 = 13, A_UII = 14, A_KUR = 15, A_KR = 16, A_E5M = 17, A_XB = 18,
+              A_XRI = 19, A_XD = 20, A_XSI = 21, A_DX = 22, A_DI = 23, A_FG = 24, A_FI = 25, A_HJ0 = 26, A_TFCA = 34,
+              A_TU = 35, N_EXPA = 36;
+constexpr int EXP_W = 4;
+constexpr int N_RLB = 10;    // gates of the rolled Rush-Larsen loop: oa oi ua ui xr xs d f (rows 4..11), v w (rows 14, 15)
+constexpr int N_EXPB = 12;   // their arguments + 2 pads, slots 0..11
+constexpr int B_INF0 = 12;   // steady states, slots 12..21
+constexpr int G_OLD0 = 36;   // gate values at t^n of those ten, slots 36..45
+constexpr int N_SLOTS = 46;
+static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && B_INF0 + N_RLB <= G_OLD0 && N_EXPA <= G_OLD0, "slot layout");
+
+// phi(x) = x/(e^x - 1) given e^x (reading B11)
+__device__ __forceinline__ double phi(double x, double ex) {
+    const double series = fma(x, fma(x, 1.0 / 12.0, -0.5), 1.0);
+    return (fabs(x) < 1e-4) ? series : x * ep_rcp(ex - 1.0);
+}
+}  // namespace crn
+
+// y_g <- inf_g + (y_g - inf_g) exp(arg_g) for the ten gates of the rolled loop, written to their state rows.
+template <int BLOCK>
+__device__ __forceinline__ void crn_rush_larsen_slots(double* col, double* ycol, int64_t stride) {
+    using namespace crn;
+#pragma unroll 1
+    for (int g = 0; g < N_EXPB; g += EXP_W) {
+        double e[EXP_W];
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) e[j] = col[(g + j) * BLOCK];
+        ep_exp_wide<EXP_W>(e);
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) {
+            if (g + j < N_RLB) {
+                const double yi = col[(B_INF0 + g + j) * BLOCK], yo = col[(G_OLD0 + g + j) * BLOCK];
+                const int row = (g + j < 8) ? C_OA + g + j : C_VG + (g + j - 8);
+                ycol[row * stride] = fma(yo - yi, e[j], yi);
+            }
+        }
+    }
+}
+
+// One step of one cell (same contract as tp06_step).  Returns Vm^{n+1}.
+template <int BLOCK, class Issue, class Finish>
+__device__ __forceinline__ double crn_step(double v, double* ycol, int64_t stride, double dt, double istim,
+                                           Issue issue_gather, Finish finish_gather, double* col) {
+    using namespace crn;
+    const double vg = ep_clamp(v, -250.0, 250.0);   // argument of every transcendental
+    const double Nai = ycol[C_NAI * stride], Ki = ycol[C_KI * stride], Cai = ycol[C_CAI * stride],
+                 Caup = ycol[C_CAUP * stride], Carel = ycol[C_CAREL * stride];
+    // gates: products for the currents; m h j fCa u stay in registers, the other ten wait in shared memory
+    const double m = ycol[C_M * stride], h = ycol[C_H * stride], j = ycol[C_J * stride], fCa = ycol[C_FCA * stride],
+                 u = ycol[C_U * stride];
+    double gto3, gkur3, xr, xs2, gcal, uvw;
+    {
+        double g[10];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) g[k] = ycol[(C_OA + k) * stride];
+        g[8] = ycol[C_VG * stride];
+        g[9] = ycol[C_W * stride];
+#pragma unroll
+        for (int k = 0; k < 10; ++k) col[(G_OLD0 + k) * BLOCK] = g[k];
+        gto3 = (g[0] * g[0] * g[0]) * g[1];          // oa^3 oi
+        gkur3 = (g[2] * g[2] * g[2]) * g[3];         // ua^3 ui
+        xr = g[4];
+        xs2 = g[5] * g[5];
+        gcal = g[6] * g[7] * fCa;                    // d f fCa
+        uvw = (u * u) * g[8] * g[9];                 // u^2 v w
+    }
+    issue_gather();
+
+    // ---- batch 1: logarithms of the reversal potentials
+    double lg[3] = {Nai, Ki, Cai};
+    ep_log_wide<3>(lg);
+    const double ENa = CK(RTF) * (CK(LN_NAO) - lg[0]);
+    const double EK = CK(RTF) * (CK(LN_KO) - lg[1]);
+    const double ECa = CK(0.5 * RTF) * (CK(LN_CAO) - lg[2]);
+    const bool hi = (v >= -40.0);   // reading B7
+
+    // ---- batch 2: voltage-dependent exponentials (+ the two constant Rush-Larsen factors of fCa and u)
+    const double x1 = fma(vg, -0.1, CK(-0.1 * 47.13));
+    const double xb = fma(vg, CK(1.0 / 5.1237), CK(-3.3328 / 5.1237));
+    const double xd = fma(vg, CK(1.0 / 9.0), CK(-19.9 / 9.0));
+    const double dx = fma(vg, CK(-1.0 / 6.24), CK(-10.0 / 6.24));
+    col[A_E17 * BLOCK] = vg * CK(1.0 / 17.0);
+    col[A_W * BLOCK] = vg * CK(0.05 * FRT);
+    col[A_X1 * BLOCK] = x1;
+    col[A_BM * BLOCK] = vg * CK(-1.0 / 11.0);
+    col[A_K1 * BLOCK] = fma(vg, CK(0.07), CK(0.07 * 80.0));
+    col[A_OA1 * BLOCK] = fma(vg, CK(-1.0 / 8.5), CK(-10.0 / 8.5));
+    col[A_OA2 * BLOCK] = fma(vg, CK(-1.0 / 59.0), CK(30.0 / 59.0));
+    col[A_OAI * BLOCK] = fma(vg, CK(-1.0 / 17.54), CK(-20.47 / 17.54));
+    col[A_UAI * BLOCK] = fma(vg, CK(-1.0 / 9.6), CK(-30.3 / 9.6));
+    col[A_OI1 * BLOCK] = fma(vg, CK(1.0 / 10.95), CK(113.7 / 10.95));
+    col[A_OI2 * BLOCK] = fma(vg, CK(-1.0 / 7.44), CK(-1.26 / 7.44));
+    col[A_OII * BLOCK] = fma(vg, CK(1.0 / 5.3), CK(43.1 / 5.3));
+    col[A_UI1 * BLOCK] = fma(vg, CK(-1.0 / 28.0), CK(185.0 / 28.0));
+    col[A_UI2 * BLOCK] = fma(vg, 0.0625, CK(-158.0 / 16.0));
+    col[A_UII * BLOCK] = fma(vg, CK(1.0 / 27.48), CK(-99.45 / 27.48));
+    col[A_KUR * BLOCK] = fma(vg, CK(-1.0 / 13.0), CK(15.0 / 13.0));
+    col[A_KR * BLOCK] = fma(vg, CK(1.0 / 22.4), CK(15.0 / 22.4));
+    col[A_E5M * BLOCK] = vg * CK(-0.2);
+    col[A_XB * BLOCK] = xb;
+    col[A_XRI * BLOCK] = fma(vg, CK(-1.0 / 6.5), CK(-14.1 / 6.5));
+    col[A_XD * BLOCK] = xd;
+    col[A_XSI * BLOCK] = fma(vg, CK(-1.0 / 12.7), CK(19.9 / 12.7));
+    col[A_DX * BLOCK] = dx;
+    col[A_DI * BLOCK] = fma(vg, -0.125, -1.25);
+    col[A_FG * BLOCK] = (vg + 10.0) * (vg + 10.0) * CK(-0.0337 * 0.0337);
+    col[A_FI * BLOCK] = fma(vg, CK(1.0 / 6.9), CK(28.0 / 6.9));
+    if (hi) {
+        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-1.0 / 11.1), CK(-10.66 / 11.1));
+        col[(A_HJ0 + 1) * BLOCK] = vg * CK(-2.535e-7);
+#pragma unroll
+        for (int k = 2; k < 8; ++k) col[(A_HJ0 + k) * BLOCK] = 0.0;
+    } else {
+        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-1.0 / 6.8), CK(-80.0 / 6.8));
+        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.079);
+        col[(A_HJ0 + 2) * BLOCK] = vg * CK(0.35);
+        col[(A_HJ0 + 3) * BLOCK] = vg * CK(0.2444);
+        col[(A_HJ0 + 4) * BLOCK] = vg * CK(-0.04391);
+        col[(A_HJ0 + 5) * BLOCK] = fma(vg, CK(0.311), CK(0.311 * 79.23));
+        col[(A_HJ0 + 6) * BLOCK] = vg * CK(-0.01052);
+        col[(A_HJ0 + 7) * BLOCK] = fma(vg, CK(-0.1378), CK(-0.1378 * 40.14));
+    }
+    col[A_TFCA * BLOCK] = dt * -0.5;      // tau_fCa = 2 ms
+    col[A_TU * BLOCK] = dt * -0.125;      // tau_u = 8 ms
+    ep_exp_slots<N_EXPA, BLOCK, EXP_W>(col);
+
+    const double e17 = col[A_E17 * BLOCK], e5m = col[A_E5M * BLOCK], e1 = col[A_X1 * BLOCK];
+    double W13, W18, W20;
+    {
+        const double W = col[A_W * BLOCK];
+        const double W2 = W * W, W4 = W2 * W2, W8 = W4 * W4, W16 = W8 * W8;
+        W13 = W8 * W4 * W; W18 = W16 * W2; W20 = W18 * W2;
+    }
+
+    // ---- membrane currents
+    const double uK = v - EK;
+    const double INa = CK(gNa) * (m * m * m) * h * j * (v - ENa);
+    const double IK1 = CK(gK1) * uK * ep_rcp(1.0 + col[A_K1 * BLOCK]);
+    const double Ito = CK(gto) * gto3 * uK;
+    const double IKur = fma(0.05, ep_rcp(1.0 + col[A_KUR * BLOCK]), 0.005) * gkur3 * uK;
+    const double IKr = CK(gKr) * xr * uK * ep_rcp(1.0 + col[A_KR * BLOCK]);
+    const double IKs = CK(gKs) * xs2 * uK;
+    const double ICaL = CK(gCaL) * gcal * (v - 65.0);
+    const double rna = CK(KmNai) * ep_rcp(Nai);
+    const double rna15 = rna * rna * ep_rsqrt(rna);                     // (KmNai/Nai)^1.5
+    const double INaK = CK(INaKmax * Ko / (Ko + KmKo)) * W20
+                        * ep_rcp((1.0 + rna15) * fma(CK(0.1245), W18, W20 + CK(0.0365 * SIGMA)));
+    const double INaCa = CK(INaCamax / ((KmNa * KmNa * KmNa + Nao * Nao * Nao) * (KmCa + Cao)))
+                         * fma(W20, (Nai * Nai * Nai) * Cao, -(Nao * Nao * Nao) * Cai) * ep_rcp(W13 + CK(ksat));
+    const double IbCa = CK(gbCa) * (v - ECa);
+    const double IbNa = CK(gbNa) * (v - ENa);
+    const double IpCa = CK(IpCamax) * Cai * ep_rcp(CK(0.0005) + Cai);
+    const double iion = INa + IK1 + Ito + IKur + IKr + IKs + ICaL + IpCa + INaK + INaCa + IbNa + IbCa;
+    const double Irel = krel * uvw * (Carel - Cai);
+    const double Itr = (Caup - Carel) * CK(1.0 / tau_tr);
+    const double Iup = CK(Iupmax) * Cai * ep_rcp(Cai + CK(Kup));
+    const double Iupleak = Caup * CK(Iupmax / Caupmax);
+    const double Fn = fma(CK(1e-12 * Vrel), Irel, CK(-(5e-13 / F) * Cm) * fma(0.5, ICaL, CK(-0.2) * INaCa));
+
+    // ---- concentrations: forward Euler; whole-cell currents = Cm * per-capacitance currents
+    {
+        const double dNai = CK(Cm / (F * Vi)) * (-3.0 * INaK - 3.0 * INaCa - IbNa - INa);
+        const double dKi = CK(Cm / (F * Vi)) * (2.0 * INaK - IK1 - Ito - IKur - IKr - IKs);    // reading B10
+        const double B1 = fma(CK(Cm / (2.0 * F * Vi)), 2.0 * INaCa - IpCa - ICaL - IbCa,
+                              fma(CK(Vup / Vi), Iupleak - Iup, CK(Vrel / Vi) * Irel));
+        const double tt = (Cai + CK(KmTrpn)) * (Cai + CK(KmTrpn)), tc = (Cai + CK(KmCmdn)) * (Cai + CK(KmCmdn));
+        // B2 = 1 + Trpn Km/tt + Cmdn Km/tc  ->  1/B2 = tt tc / (tt tc + Trpn Km tc + Cmdn Km tt)
+        const double invB2 = tt * tc * ep_rcp(fma(tt, tc, fma(CK(Trpnmax * KmTrpn), tc, CK(Cmdnmax * KmCmdn) * tt)));
+        const double dCaup = Iup - Iupleak - Itr * CK(Vrel / Vup);
+        const double tq = (Carel + CK(KmCsqn)) * (Carel + CK(KmCsqn));
+        const double dCarel = (Itr - Irel) * tq * ep_rcp(tq + CK(Csqnmax * KmCsqn));
+        ycol[C_NAI * stride] = fma(dt, dNai, Nai);
+        ycol[C_KI * stride] = fma(dt, dKi, Ki);
+        ycol[C_CAI * stride] = fma(dt, B1 * invB2, Cai);
+        ycol[C_CAUP * stride] = fma(dt, dCaup, Caup);
+        ycol[C_CAREL * stride] = fma(dt, dCarel, Carel);
+    }
+    const double v_new = fma(dt, finish_gather() - iion - istim, v);   // eq. (7)
+
+    // ---- Rush-Larsen group 1 (registers): E1 of the release gates rides with m, h, j in one 4-wide exp
+    double m_inf, h_inf, j_inf;
+    double e4[4];
+    {
+        const double am = 3.2 * phi(x1, e1);                            // 0.32 (V+47.13)/(1 - exp(-0.1 (V+47.13)))
+        const double rm = fma(CK(0.08), col[A_BM * BLOCK], am);
+        m_inf = am * ep_rcp(rm);
+        double rh, rj;
+        const double s0 = col[(A_HJ0 + 0) * BLOCK], s1 = col[(A_HJ0 + 1) * BLOCK];
+        if (hi) {
+            h_inf = 0.0; j_inf = 0.0;
+            rh = ep_rcp(0.13 * (1.0 + s0));
+            rj = CK(0.3) * s1 * ep_rcp(fma(CK(E1513), e1, 1.0));        // exp(-0.1 (V+32)) = e^{1.513} e^{x1}
+        } else {
+            const double s2 = col[(A_HJ0 + 2) * BLOCK], s3 = col[(A_HJ0 + 3) * BLOCK], s4 = col[(A_HJ0 + 4) * BLOCK],
+                         s5 = col[(A_HJ0 + 5) * BLOCK], s6 = col[(A_HJ0 + 6) * BLOCK], s7 = col[(A_HJ0 + 7) * BLOCK];
+            const double ah = CK(0.135) * s0;
+            rh = ah + fma(CK(3.56), s1, 3.1e5 * s2);
+            h_inf = ah * ep_rcp(rh);
+            const double N1 = fma(-127140.0, s3, CK(-3.474e-5) * s4) * (vg + CK(37.78)), D1 = 1.0 + s5;
+            const double N2 = CK(0.1212) * s6, D2 = 1.0 + s7;
+            const double num = fma(N1, D2, N2 * D1);
+            rj = num * ep_rcp(D1 * D2);
+            j_inf = N1 * D2 * ep_rcp(num);
+        }
+        e4[0] = fmax(Fn * CK(-1.0 / 13.67e-16) + CK(3.4175e-13 / 13.67e-16), -700.0);
+        e4[0] = fmin(e4[0], 700.0);
+        e4[1] = fmax(-dt * rm, -700.0);
+        e4[2] = fmax(-dt * rh, -700.0);
+        e4[3] = fmax(-dt * rj, -700.0);
+    }
+    ep_exp_wide<4>(e4);
+    ycol[C_M * stride] = fma(m - m_inf, e4[1], m_inf);
+    ycol[C_H * stride] = fma(h - h_inf, e4[2], h_inf);
+    ycol[C_J * stride] = fma(j - j_inf, e4[3], j_inf);
+    {   // fCa (tau = 2 ms) and u (tau = 8 ms): constant Rush-Larsen factors from batch 2
+        const double fCa_inf = CK(0.00035) * ep_rcp(CK(0.00035) + Cai);
+        ycol[C_FCA * stride] = fma(fCa - fCa_inf, col[A_TFCA * BLOCK], fCa_inf);
+        const double u_inf = ep_rcp(1.0 + e4[0]);
+        ycol[C_U * stride] = fma(u - u_inf, col[A_TU * BLOCK], u_inf);
+    }
+
+    // ---- Rush-Larsen group 2 (rolled loop): oa oi ua ui xr xs d f v w
+    double inf[N_RLB], rate[N_RLB];
+    {   // oa, ua share alpha + beta; K_Q10 = 3 multiplies the rates
+        const double A = col[A_OA1 * BLOCK] + col[A_OA2 * BLOCK], Bq = fma(CK(E82_17), e17, 2.5);
+        const double r = 1.95 * (A + Bq) * ep_rcp(A * Bq);
+        inf[0] = ep_rcp(1.0 + col[A_OAI * BLOCK]); rate[0] = r;
+        inf[2] = ep_rcp(1.0 + col[A_UAI * BLOCK]); rate[2] = r;
+    }
+    {   // oi
+        const double P = CK(18.53) + col[A_OI1 * BLOCK], Q = CK(35.56) + col[A_OI2 * BLOCK];
+        inf[1] = ep_rcp(1.0 + col[A_OII * BLOCK]); rate[1] = 3.0 * (P + Q) * ep_rcp(P * Q);
+    }
+    {   // ui
+        const double P = 21.0 + col[A_UI1 * BLOCK];
+        inf[3] = ep_rcp(1.0 + col[A_UII * BLOCK]); rate[3] = 3.0 * fma(col[A_UI2 * BLOCK], P, 1.0) * ep_rcp(P);
+    }
+    {   // xr: alpha = 0.0015 phi(-(V+14.1)/5), beta = 7.3898e-5 * 5.1237 phi((V-3.3328)/5.1237)
+        const double xa = fma(vg, CK(-0.2), CK(-14.1 / 5.0));
+        inf[4] = ep_rcp(1.0 + col[A_XRI * BLOCK]);
+        rate[4] = fma(CK(0.0015), phi(xa, CK(EM141_5) * e5m), CK(7.3898e-5 * 5.1237) * phi(xb, col[A_XB * BLOCK]));
+    }
+    {   // xs: alpha = 6.8e-4 phi(-(V-19.9)/17), beta = 3.15e-4 phi((V-19.9)/9); tau = 0.5/(alpha+beta)
+        const double xc = fma(vg, CK(-1.0 / 17.0), CK(19.9 / 17.0));
+        const double series = fma(xc, fma(xc, 1.0 / 12.0, -0.5), 1.0);
+        const double pa = (fabs(xc) < 1e-4) ? series : xc * e17 * ep_rcp(CK(E199_17) - e17);   // e^{xc} = e^{19.9/17}/e17
+        inf[5] = ep_rsqrt(1.0 + col[A_XSI * BLOCK]);
+        rate[5] = 2.0 * fma(CK(6.8e-4), pa, CK(3.15e-4) * phi(xd, col[A_XD * BLOCK]));
+    }
+    {   // d: tau = 1/(0.035 * 6.24 phi(x)(1 + e^x)), x = -(V+10)/6.24
+        const double ex = col[A_DX * BLOCK];
+        inf[6] = ep_rcp(1.0 + col[A_DI * BLOCK]);
+        rate[6] = CK(0.035 * 6.24) * phi(dx, ex) * (1.0 + ex);
+    }
+    {   // f: tau = 9/(0.0197 G + 0.02)
+        inf[7] = ep_rcp(1.0 + col[A_FI * BLOCK]);
+        rate[7] = fma(CK(0.0197 / 9.0), col[A_FG * BLOCK], CK(0.02 / 9.0));
+    }
+    {   // v: inf = 1 - 1/(1+E2), tau = 1.91 + 2.09/(1+E1), E2 = E1 e^{-200}
+        const double E2 = e4[0] * CK(EM200);
+        inf[8] = E2 * ep_rcp(1.0 + E2);
+        rate[8] = ep_rcp(fma(CK(2.09), ep_rcp(1.0 + e4[0]), CK(1.91)));
+    }
+    {   // w: tau = 1.2/(phi(x)(1 + 0.3 e^x)), x = -(V-7.9)/5; inf = 1 - 1/(1 + e^{-(V-40)/17})
+        const double xw = fma(vg, CK(-0.2), CK(7.9 / 5.0));
+        const double ex = CK(E79_5) * e5m;
+        inf[9] = CK(E40_17) * ep_rcp(e17 + CK(E40_17));
+        rate[9] = CK(1.0 / 1.2) * phi(xw, ex) * fma(CK(0.3), ex, 1.0);
+    }
+#pragma unroll
+    for (int g = 0; g < N_RLB; ++g) {
+        col[g * BLOCK] = fmax(-dt * rate[g], -700.0);
+        col[(B_INF0 + g) * BLOCK] = inf[g];
+    }
+    col[10 * BLOCK] = 0.0;
+    col[11 * BLOCK] = 0.0;
+    crn_rush_larsen_slots<BLOCK>(col, ycol, stride);
+    return v_new;
+}
+
+}  // namespace epk

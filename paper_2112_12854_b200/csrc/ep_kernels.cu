@@ -6,6 +6,7 @@
 // and the result is deterministic.  Nothing here is a dense contraction: no tensor cores.
 #include "ep_kernels.cuh"
 #include "ep_tp06.cuh"
+#include "ep_crn98.cuh"
 
 namespace epk {
 
@@ -71,21 +72,23 @@ __global__ void __launch_bounds__(CELL_THREADS) diffusion_only_kernel(int64_t nc
     out[i] = diffusion_gather(i, stride, cidx, ccoef, vm, vn, vm[i]);
 }
 
-// S2..S9 fused, TP06.  One thread per cell; state rows are read once and written once.
+// S2..S9 fused.  One thread per cell; state rows are read once and written once.  MODEL 0: TP06, 1: Courtemanche.
 #ifndef EP_CELL_MIN_BLOCKS
 #define EP_CELL_MIN_BLOCKS 4
 #endif
-__global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_tp06_kernel(int64_t nc, int64_t stride,
-                                                                      const int32_t* __restrict__ cidx,
-                                                                      const double* __restrict__ ccoef,
-                                                                      StepArgs a) {
+template <int MODEL>
+__global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_kernel(int64_t nc, int64_t stride,
+                                                                                     const int32_t* __restrict__ cidx,
+                                                                                     const double* __restrict__ ccoef,
+                                                                                     StepArgs a) {
     // per-thread columns of the transcendental batches (ep_math.cuh): slot s of thread t at xs[s][t]
-    __shared__ double xs[tp06::N_SLOTS][CELL_THREADS];
+    constexpr int NSLOTS = (MODEL == 0) ? tp06::N_SLOTS : crn::N_SLOTS;
+    __shared__ double xs[NSLOTS][CELL_THREADS];
     const int64_t i = (int64_t)blockIdx.x * CELL_THREADS + threadIdx.x;
     if (i >= nc) return;
     const double v_old = a.vm_cur[i];
-    // S2+S3 in two halves: indices are loaded here, the gathers are issued once the cell model has parked its gates
-    // and stay in flight while it evaluates its logarithms and first exponential batch
+    // S2+S3 in two halves: indices and coefficients are loaded here, the gathers are issued once the cell model has
+    // parked its gates and stay in flight while it evaluates its logarithms and first exponential batch
     int32_t id[12];
     double cf[12];
 #pragma unroll
@@ -116,8 +119,13 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_tp
 #pragma unroll
     for (int k = 0; k < 8; ++k)
         if (mask & (1u << k)) istim += a.istim[k];
-    const double v_new = tp06_step<CELL_THREADS>(v_old, a.y + i, stride, a.ctype[i], a.dt, istim, issue_gather,
-                                                 finish_gather, &xs[0][threadIdx.x]);
+    double v_new;
+    if constexpr (MODEL == 0)
+        v_new = tp06_step<CELL_THREADS>(v_old, a.y + i, stride, a.ctype[i], a.dt, istim, issue_gather, finish_gather,
+                                        &xs[0][threadIdx.x]);
+    else
+        v_new = crn_step<CELL_THREADS>(v_old, a.y + i, stride, a.dt, istim, issue_gather, finish_gather,
+                                       &xs[0][threadIdx.x]);
     a.vm_next[i] = v_new;
     // S9: activation time = first upward crossing of 0 mV (reading A18)
     if (v_old <= 0.0 && v_new > 0.0) {
@@ -132,7 +140,7 @@ __global__ void state_fill_kernel(int S, int64_t nc, int64_t stride, const uint8
     if (i >= stride) return;
     const int t = (i < nc) ? ctype[i] : 0;
     for (int k = 0; k < S; ++k) {
-        const double val = y0 ? y0[t * S + k] : TP06_REST_STATE[k];
+        const double val = y0 ? y0[t * S + k] : (S == (int)TP06_S ? TP06_REST_STATE[k] : CRN_REST_STATE[k]);
         if (k == 0) vm[i] = val; else y[k * stride + i] = val;
     }
     tact[i] = -1.0;
@@ -187,7 +195,7 @@ inline unsigned blocks_for(int64_t n, int threads) { return (unsigned)((n + thre
 
 }  // namespace
 
-int model_n_states(int model) { return model == 0 ? (int)TP06_S : -1; }
+int model_n_states(int model) { return model == 0 ? (int)TP06_S : (model == 1 ? (int)CRN_S : -1); }
 
 void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaStream_t s) {
     const unsigned grid = blocks_for(m.n_slices, NODE_THREADS / 32);
@@ -195,8 +203,9 @@ void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaS
 }
 
 void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStream_t s) {
-    (void)model;
-    cell_step_tp06_kernel<<<blocks_for(m.nc, CELL_THREADS), CELL_THREADS, 0, s>>>(m.nc, m.nc_pad, m.cidx, m.ccoef, a);
+    const unsigned grid = blocks_for(m.nc, CELL_THREADS);
+    if (model == 0) cell_step_kernel<0><<<grid, CELL_THREADS, 0, s>>>(m.nc, m.nc_pad, m.cidx, m.ccoef, a);
+    else cell_step_kernel<1><<<grid, CELL_THREADS, 0, s>>>(m.nc, m.nc_pad, m.cidx, m.ccoef, a);
 }
 
 void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* vn, double* out, cudaStream_t s) {

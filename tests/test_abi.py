@@ -41,6 +41,7 @@ def test_model_state_counts_match_paper():
     """TP06 has 19 state variables, Courtemanche 21."""
     import paper_2112_12854_b200 as ep
     assert ep.model_n_states(ep.EP_MODEL_TP06) == 19
+    assert ep.model_n_states(ep.EP_MODEL_CRN98) == 21
     assert ep.model_n_states(99) < 0
 
 

@@ -239,3 +239,52 @@ def test_window_parity_c2(ep, oracle):
     tg, to = g.activation_times(), o.activation_times()
     assert np.array_equal(tg >= 0, to >= 0) and np.abs(tg - to).max() <= dt * (1 + 1e-12)
     g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Courtemanche model (BASELINE config 5)
+
+@pytest.mark.parametrize("case", ["c5_coarse", "jittered"])
+def test_crn_one_step_random_states(ep, oracle, case):
+    if case == "c5_coarse":
+        prob = make(5, coarsen=3.0)
+    else:
+        prob = make(5, coarsen=6.0)
+        prob.mesh = _jittered()
+        prob.mesh.cell_type = None
+        prob.stimuli[0].cell_ids = np.arange(0, prob.mesh.n_tets, 5, dtype=np.int64)
+    g, o = _pair(ep, oracle, prob)
+    assert g.n_states == 21
+    n = prob.mesh.n_tets
+    y = states.random_states(1, 177, n)
+    # removable singularities and branch points of the model (readings B7, B11)
+    sv = np.array([-47.13, -47.13 + 1e-6, -14.1, 3.3328, 19.9, 19.9 - 1e-7, -10.0, 7.9, -40.0, np.nextafter(-40.0, -50.0),
+                   -81.18, 30.0])
+    y[0, : sv.size] = sv
+    y[13, : n // 3] = 0.0                        # release gate closed in a third of the cells (Fn ~ 0 branch of u, v)
+    for k in range(21):
+        g.write_state(k, y[k]); o.write_state(k, y[k])
+    dt = 0.01
+    g.step(1, dt); o.step(1, dt)
+    err = _one_step_err(g, o, 21)
+    assert err.max() <= ONE_STEP_TOL, err
+    g.step(2, dt); o.step(2, dt)
+    err = _one_step_err(g, o, 21)
+    assert err.max() <= 10 * ONE_STEP_TOL, err
+    g.close()
+
+
+def test_crn_window_config5_coarse(ep, oracle):
+    """Config 5 twin at 2x spacing: stimulus patch fires, the wave leaves it; 1,500 steps of 0.01 ms."""
+    prob = make(5, coarsen=2.0)
+    g, o = _pair(ep, oracle, prob)
+    g.step(1500, prob.dt); o.step(1500, prob.dt)
+    vg, vo = g.read_vm(), o.read_vm()
+    assert np.abs(vg - vo).max() <= RUN_TOL_MV
+    tg, to = g.activation_times(), o.activation_times()
+    assert (to >= 0).sum() > len(prob.stimuli[0].cell_ids)       # the wave has left the stimulated patch
+    assert np.array_equal(tg >= 0, to >= 0) and np.abs(tg - to).max() <= prob.dt * (1 + 1e-12)
+    for k in range(1, 21):
+        a, b = g.read_state(k), o.read_state(k)
+        assert np.abs(a - b).max() <= 1e-8 * max(1.0, np.abs(b).max())
+    g.close()
