@@ -86,17 +86,22 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def _run_dt(prob) -> float:
+    """Time step the benchmark runs: the config's nominal dt, except where DESIGN.md reading S overrides it."""
+    return float(prob.notes.get("dt_run", prob.dt))
+
+
 def _oracle_leg(prob, budget_s: float, threads: int):
     """Time the oracle, as it stands, on this host: whole mesh, as many steps as fit the budget (at least 1)."""
     from oracle import ep_oracle as O
     O.set_threads(threads)
     o = O.OracleSim.from_problem(prob)
     t0 = time.perf_counter()
-    o.step(1, prob.dt)
+    o.step(1, _run_dt(prob))
     t1 = time.perf_counter() - t0
     n = max(1, min(50, int(budget_s / max(t1, 1e-6)) - 1))
     t0 = time.perf_counter()
-    o.step(n, prob.dt)
+    o.step(n, _run_dt(prob))
     t = time.perf_counter() - t0
     o.close()
     return prob.mesh.n_tets * n / t, n, t
@@ -115,10 +120,10 @@ def run_reference(args):
     o = O.OracleSim.from_problem(prob)
     per = max(1, args.ref_inner)
     for _ in range(args.warmup):
-        o.step(per, prob.dt)
+        o.step(per, _run_dt(prob))
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        o.step(per, prob.dt)
+        o.step(per, _run_dt(prob))
     t = time.perf_counter() - t0
     o.close()
     val = prob.mesh.n_tets * per * args.steps / t
@@ -127,7 +132,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": prob.name, "cells": prob.mesh.n_tets, "dt_ms": prob.dt, "time_steps_per_step": per},
+        "config": {"workload": prob.name, "cells": prob.mesh.n_tets, "dt_ms": _run_dt(prob), "time_steps_per_step": per},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
@@ -156,7 +161,13 @@ def run_ours(args):
     stream = torch.cuda.Stream()
     sim.set_stream(stream.cuda_stream)
     S = sim.n_states
-    inner, dt = args.inner, prob.dt
+    # explicit stability (reading S): config 2 runs at dt = nominal/4; ep_stable_dt confirms the choice
+    dt_max = sim.stable_dt()
+    dt = _run_dt(prob)
+    dt_k = int(round(prob.dt / dt))
+    if dt > dt_max:
+        raise SystemExit(f"bench.py: dt = {dt} ms exceeds the explicit stability limit {dt_max:.5f} ms of this mesh")
+    inner = args.inner
     # the config as specified: every cell at the model's resting state, the config's stimulus armed at t = 0; the
     # timed window is the start of that simulation (stimulus on, wave leaving the stimulus sites)
     pinned = torch.empty((S, nc), dtype=torch.float64).pin_memory()
@@ -179,7 +190,6 @@ def run_ours(args):
         sim.step(inner, dt)
     sim.synchronize()
     l0 = sim.launch_count
-    sim.profile(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     clocks = ClockSampler(local) if rank == 0 else None
@@ -190,10 +200,22 @@ def run_ours(args):
         e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
+    launches_timed = sim.launch_count - l0
+    # second, identical pass with a CUDA-event pair around every kernel launch (ep_profile): per-kernel durations for
+    # the roofline.  Kept out of the pass above because the extra event records cost a few us per time step.
+    sim.profile(True)
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        p0.record(stream)
+        for _ in range(args.steps):
+            sim.step(inner, dt)
+        p1.record(stream)
+    barrier()
+    ms_profiled = p0.elapsed_time(p1)
     clk = clocks.stop() if clocks else None
     prof = sim.profile_read()
     sim.profile(False)
-    launches = sim.launch_count - l0
+    launches = launches_timed
     finite = sim.check_finite()
     t_dev = torch.tensor([ms], dtype=torch.float64, device="cuda")
     if dist is not None:
@@ -235,6 +257,7 @@ def run_ours(args):
                 "alg_bytes_per_launch": cell_bytes, "alg_bytes_per_cell": cell_bytes / nc,
                 "avg_launch_ms": cell_ms, "node_kernel_avg_launch_ms": node_ms,
                 "kernel_share_of_step": cell_ms / max(1e-12, cell_ms + node_ms),
+                "profiled_pass_ms_per_step": ms_profiled / args.steps,
                 "whole_step_frac": sim.step_bytes / (ms_max * 1e-3 / (inner * args.steps)) / 1e9 / peak}
     cores = os.cpu_count() or 1
     cpu_val, cpu_n, cpu_t = _oracle_leg(prob, args.cpu_budget, cores)
@@ -242,7 +265,8 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": prob.name, "cells": nc, "nodes": mesh.n_nodes, "dt_ms": dt,
+        "config": {"workload": prob.name, "cells": nc, "nodes": mesh.n_nodes, "dt_ms": dt, "dt_nominal_ms": prob.dt,
+                   "dt_divisor": dt_k, "dt_stable_max_ms": dt_max,
                    "time_steps_per_step": inner, "states": "config initial condition (rest + stimulus at t=0), window starts after warm-up",
                    "l2": "inputs larger than L2 (%.0f MB touched per time step)" % (sim.step_bytes / 1e6),
                    "parallelism": "replicas" if world > 1 else "single"},

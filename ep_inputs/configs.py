@@ -82,7 +82,9 @@ def config2(coarsen: float = 1.0, seed: int = 1001, jitter: float = 0.2) -> Prob
     mesh.cell_type = M.thirds(zrel)
     ids = np.nonzero(np.all(cent < 1.5, axis=1))[0].astype(np.int64)
     return Problem("C2_irregular_slab", mesh, stimuli=[Stimulus(ids, -52.0, 0.0, 1.0)], dt=0.02, n_steps=5000,
-                   notes={"seed": seed, "dt_note": "nominal 0.02 ms; see DESIGN.md S-note (run at 0.02/k)"})
+                   notes={"seed": seed, "dt_run": 0.005,
+                          "dt_note": "nominal 0.02 ms is beyond the explicit stability limit of this jittered mesh "
+                                     "(DESIGN.md reading S); runs use dt_run = 0.02/4 = the paper's finest dt"})
 
 
 _LV_OUT = (35.0, 35.0, 60.0)

@@ -54,6 +54,16 @@ struct ep_sim {
     double dt = 0.0;
     int sticky = EP_OK;
     int64_t dev_bytes = 0, launches = 0;
+    // CUDA-graph replay of GRAPH_STEPS time steps (launch-bound meshes); rebuilt when dt, model or stream change
+    cudaGraphExec_t graph = nullptr;
+    double graph_dt = 0.0;
+    int graph_model = -1, graph_cur = 0;
+    cudaStream_t graph_stream = nullptr;
+    epk::StepDesc* d_desc = nullptr;
+    epk::StepDesc* h_desc = nullptr;            // pinned ring of DESC_RING x GRAPH_STEPS descriptors
+    cudaEvent_t desc_ev[8] = {};                // copy-done events guarding the reuse of a ring slot
+    bool desc_ev_used[8] = {};
+    int desc_slot = 0;
     // per-kernel event timing (ep_profile)
     bool profiling = false;
     std::vector<cudaEvent_t> ev;       // 3 per step: before node kernel, between, after cell kernel
@@ -97,6 +107,10 @@ void free_all(ep_sim* s) {
                     s->d_tmp8};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
+    if (s->graph) cudaGraphExecDestroy(s->graph);
+    if (s->d_desc) cudaFree(s->d_desc);
+    if (s->h_desc) cudaFreeHost(s->h_desc);
+    for (cudaEvent_t e : s->desc_ev) if (e) cudaEventDestroy(e);
     if (s->own_stream) cudaStreamDestroy(s->own_stream);
 }
 
@@ -121,6 +135,50 @@ int profile_event(ep_sim* s) {
         s->ev.push_back(e);
     }
     EP_CUDA(s, cudaEventRecord(s->ev[s->ev_used++], s->stream));
+    return EP_OK;
+}
+
+constexpr int GRAPH_STEPS = 32;   // even, so that the Vm double buffer is back where it started
+constexpr int DESC_RING = 8;
+
+void fill_desc(const ep_sim* s, int64_t n, double dt, const int64_t* n_on, const int64_t* n_off, epk::StepDesc& d) {
+    d.t_next = (double)(n + 1) * dt;   // reading A17: time from the integer counter
+    for (int k = 0; k < EP_MAX_STIM_SLOTS; ++k)
+        d.istim[k] = (s->stim[k].set && n_on[k] <= n && n < n_off[k]) ? s->stim[k].amp / s->Cm : 0.0;
+}
+
+epk::StepArgs step_args(ep_sim* s, int cur, double dt) {
+    epk::StepArgs a;
+    a.vm_cur = s->d_vm[cur]; a.vm_next = s->d_vm[cur ^ 1];
+    a.y = s->d_y; a.vn = s->d_vn; a.ctype = s->d_ctype; a.smask = s->d_smask; a.tact = s->d_tact;
+    a.dt = dt; a.desc = nullptr;
+    return a;
+}
+
+// capture GRAPH_STEPS (node gather, cell step) pairs whose per-step data come from d_desc[k]
+int build_graph(ep_sim* s, double dt) {
+    if (s->graph) { cudaGraphExecDestroy(s->graph); s->graph = nullptr; }
+    if (!s->d_desc) {
+        EP_CUDA(s, cudaMalloc((void**)&s->d_desc, sizeof(epk::StepDesc) * GRAPH_STEPS));
+        s->dev_bytes += (int64_t)sizeof(epk::StepDesc) * GRAPH_STEPS;
+        EP_CUDA(s, cudaHostAlloc((void**)&s->h_desc, sizeof(epk::StepDesc) * GRAPH_STEPS * DESC_RING, cudaHostAllocDefault));
+        for (int r = 0; r < DESC_RING; ++r) EP_CUDA(s, cudaEventCreateWithFlags(&s->desc_ev[r], cudaEventDisableTiming));
+    }
+    cudaGraph_t g = nullptr;
+    EP_CUDA(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
+    int cur = s->cur;
+    for (int k = 0; k < GRAPH_STEPS; ++k) {
+        epk::StepArgs a = step_args(s, cur, dt);
+        a.desc = s->d_desc + k;
+        epk::launch_node_gather(s->dm, a.vm_cur, s->d_vn, s->stream);
+        epk::launch_cell_step(s->dm, s->model, a, s->stream);
+        cur ^= 1;
+    }
+    EP_CUDA(s, cudaStreamEndCapture(s->stream, &g));
+    cudaError_t e = cudaGraphInstantiate(&s->graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { s->graph = nullptr; EP_CUDA(s, e); }
+    s->graph_dt = dt; s->graph_model = s->model; s->graph_cur = s->cur; s->graph_stream = s->stream;
     return EP_OK;
 }
 
@@ -323,14 +381,33 @@ int ep_step(ep_sim* s, int64_t n_steps, double dt) {
         n_on[k] = step_index(s->stim[k].t0, dt);
         n_off[k] = step_index(s->stim[k].t0 + s->stim[k].dur, dt);
     }
-    for (int64_t it = 0; it < n_steps; ++it) {
+    int64_t left = n_steps;
+    while (left > 0) {
+        if (!s->profiling && left >= GRAPH_STEPS) {
+            // replay path: one descriptor upload + one graph launch per GRAPH_STEPS time steps
+            if (!s->graph || s->graph_dt != dt || s->graph_model != s->model || s->graph_cur != s->cur ||
+                s->graph_stream != s->stream) {
+                if ((rc = build_graph(s, dt))) return rc;
+            }
+            // pinned ring slot: wait (normally not at all) until the copy that last used it has run, refill, enqueue the
+            // copy; stream order keeps the copy behind the previous replay and ahead of the next one
+            const int r = s->desc_slot;
+            s->desc_slot = (r + 1) % DESC_RING;
+            if (s->desc_ev_used[r]) EP_CUDA(s, cudaEventSynchronize(s->desc_ev[r]));
+            epk::StepDesc* h = s->h_desc + (size_t)r * GRAPH_STEPS;
+            for (int k = 0; k < GRAPH_STEPS; ++k) fill_desc(s, s->step + k, dt, n_on, n_off, h[k]);
+            EP_CUDA(s, cudaMemcpyAsync(s->d_desc, h, sizeof(epk::StepDesc) * GRAPH_STEPS, cudaMemcpyHostToDevice, s->stream));
+            EP_CUDA(s, cudaEventRecord(s->desc_ev[r], s->stream));
+            s->desc_ev_used[r] = true;
+            EP_CUDA(s, cudaGraphLaunch(s->graph, s->stream));
+            s->launches += 2 * GRAPH_STEPS;
+            s->step += GRAPH_STEPS;
+            left -= GRAPH_STEPS;
+            continue;
+        }
         const int64_t n = s->step;
-        epk::StepArgs a;
-        a.vm_cur = s->d_vm[s->cur]; a.vm_next = s->d_vm[s->cur ^ 1];
-        a.y = s->d_y; a.vn = s->d_vn; a.ctype = s->d_ctype; a.smask = s->d_smask; a.tact = s->d_tact;
-        a.dt = dt; a.t_next = (double)(n + 1) * dt;   // reading A17: time from the integer counter
-        for (int k = 0; k < EP_MAX_STIM_SLOTS; ++k)
-            a.istim[k] = (s->stim[k].set && n_on[k] <= n && n < n_off[k]) ? s->stim[k].amp / s->Cm : 0.0;
+        epk::StepArgs a = step_args(s, s->cur, dt);
+        fill_desc(s, n, dt, n_on, n_off, a.inl);
         if (s->profiling) {
             if (s->ev_used >= 3 * 4096 && (rc = profile_drain(s))) return rc;
             if ((rc = profile_event(s))) return rc;
@@ -345,6 +422,7 @@ int ep_step(ep_sim* s, int64_t n_steps, double dt) {
         s->launches += 2;
         s->cur ^= 1;
         s->step = n + 1;
+        --left;
     }
     EP_CUDA(s, cudaGetLastError());
     return EP_OK;

@@ -16,30 +16,41 @@ constexpr int CELL_THREADS = 128;
 constexpr int NODE_THREADS = 256;
 
 // ---------------------------------------------------------------------------------------------------------
-// S1: cell -> node interpolation.  One warp per slice of 32 nodes; lane = node; the slice is stored [k][lane].
+// S1: cell -> node interpolation.  A slice of 32 nodes is stored [k][lane]; NODE_PARTS warps share a slice, warp p
+// takes rows k = p, p + NODE_PARTS, ... (each row read is 32 consecutive entries: fully coalesced) and the partial sums
+// meet in shared memory.  Four times the threads of a warp-per-slice mapping: the kernel is a latency-bound gather and
+// needs the parallelism (profiles/r01: 40 us -> see DESIGN.md section 6).
+constexpr int NODE_PARTS = 4;
+constexpr int NODE_SLICES_PER_BLOCK = NODE_THREADS / 32 / NODE_PARTS;
 __global__ void __launch_bounds__(NODE_THREADS) node_gather_kernel(int64_t nn, int64_t n_slices,
                                                                     const int64_t* __restrict__ slice_ptr,
                                                                     const int32_t* __restrict__ nidx,
                                                                     const double* __restrict__ nw,
                                                                     const double* __restrict__ vm,
                                                                     double* __restrict__ vn) {
-    const int64_t slice = (int64_t)blockIdx.x * (NODE_THREADS / 32) + (threadIdx.x >> 5);
-    if (slice >= n_slices) return;
-    const int lane = threadIdx.x & 31;
-    const int64_t beg = slice_ptr[slice], end = slice_ptr[slice + 1];
-    double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
-    int64_t p = beg + lane;
-    for (; p + 96 < end; p += 128) {   // four independent gathers in flight
-        const int32_t i0 = nidx[p], i1 = nidx[p + 32], i2 = nidx[p + 64], i3 = nidx[p + 96];
-        const double w0 = nw[p], w1 = nw[p + 32], w2 = nw[p + 64], w3 = nw[p + 96];
-        acc0 = fma(w0, vm[i0], acc0);
-        acc1 = fma(w1, vm[i1], acc1);
-        acc2 = fma(w2, vm[i2], acc2);
-        acc3 = fma(w3, vm[i3], acc3);
+    __shared__ double part[NODE_SLICES_PER_BLOCK][NODE_PARTS][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int sl = warp / NODE_PARTS, p = warp % NODE_PARTS;
+    const int64_t slice = (int64_t)blockIdx.x * NODE_SLICES_PER_BLOCK + sl;
+    double acc0 = 0.0, acc1 = 0.0;
+    if (slice < n_slices) {
+        const int64_t beg = __ldg(slice_ptr + slice), end = __ldg(slice_ptr + slice + 1);
+        int64_t q = beg + 32 * p + lane;
+        const int64_t step = 32 * NODE_PARTS;
+        for (; q + step < end; q += 2 * step) {   // two independent gathers in flight per trip
+            const int32_t i0 = __ldg(nidx + q), i1 = __ldg(nidx + q + step);
+            const double w0 = __ldg(nw + q), w1 = __ldg(nw + q + step);
+            acc0 = fma(w0, vm[i0], acc0);
+            acc1 = fma(w1, vm[i1], acc1);
+        }
+        if (q < end) acc0 = fma(__ldg(nw + q), vm[__ldg(nidx + q)], acc0);
     }
-    for (; p < end; p += 32) acc0 = fma(nw[p], vm[nidx[p]], acc0);
-    const int64_t n = slice * 32 + lane;
-    if (n < nn) vn[n] = (acc0 + acc1) + (acc2 + acc3);
+    part[sl][p][lane] = acc0 + acc1;
+    __syncthreads();
+    if (p == 0 && slice < n_slices) {
+        const int64_t n = slice * 32 + lane;
+        if (n < nn) vn[n] = (part[sl][0][lane] + part[sl][1][lane]) + (part[sl][2][lane] + part[sl][3][lane]);
+    }
 }
 
 // S2+S3: the factored diffusion gather.  dv = sum_m a_m v_n[node_m] + sum_j b_j (v[nbr_j] - v_c)   [mV/ms]
@@ -118,7 +129,7 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     double istim = 0.0;
 #pragma unroll
     for (int k = 0; k < 8; ++k)
-        if (mask & (1u << k)) istim += a.istim[k];
+        if (mask & (1u << k)) istim += a.desc ? a.desc->istim[k] : a.inl.istim[k];
     double v_new;
     if constexpr (MODEL == 0)
         v_new = tp06_step<CELL_THREADS>(v_old, a.y + i, stride, a.ctype[i], a.dt, istim, issue_gather, finish_gather,
@@ -129,7 +140,7 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     a.vm_next[i] = v_new;
     // S9: activation time = first upward crossing of 0 mV (reading A18)
     if (v_old <= 0.0 && v_new > 0.0) {
-        if (a.tact[i] < 0.0) a.tact[i] = a.t_next;
+        if (a.tact[i] < 0.0) a.tact[i] = a.desc ? a.desc->t_next : a.inl.t_next;
     }
 }
 
@@ -198,7 +209,7 @@ inline unsigned blocks_for(int64_t n, int threads) { return (unsigned)((n + thre
 int model_n_states(int model) { return model == 0 ? (int)TP06_S : (model == 1 ? (int)CRN_S : -1); }
 
 void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaStream_t s) {
-    const unsigned grid = blocks_for(m.n_slices, NODE_THREADS / 32);
+    const unsigned grid = blocks_for(m.n_slices, NODE_SLICES_PER_BLOCK);
     node_gather_kernel<<<grid, NODE_THREADS, 0, s>>>(m.nn, m.n_slices, m.slice_ptr, m.nidx, m.nw, vm, vn);
 }
 

@@ -14,6 +14,12 @@ struct DeviceMesh {
     const double* nw = nullptr;
 };
 
+// what changes from one time step to the next
+struct StepDesc {
+    double t_next;          // (n+1)*dt, recorded on an upward crossing of 0 mV (PAPER.md:216)
+    double istim[8];        // I_s/C_m of each slot at step n (0 when the slot's window is closed)
+};
+
 struct StepArgs {
     const double* vm_cur;   // [nc_pad]
     double* vm_next;        // [nc_pad]
@@ -23,8 +29,8 @@ struct StepArgs {
     const uint8_t* smask;   // [nc_pad] bit k = cell belongs to stimulus slot k
     double* tact;           // [nc_pad]
     double dt;
-    double t_next;          // (n+1)*dt, recorded on an upward crossing of 0 mV (PAPER.md:216)
-    double istim[8];        // I_s/C_m of each slot at step n (0 when the slot's window is closed)
+    const StepDesc* desc;   // device descriptor of this step (CUDA-graph replay), or NULL: use `inl`
+    StepDesc inl;
 };
 
 // S1 of SURVEY 8(a): v_n = sum_k w_nk v_k
