@@ -258,6 +258,8 @@ def run_ours(args):
                 "avg_launch_ms": cell_ms, "node_kernel_avg_launch_ms": node_ms,
                 "kernel_share_of_step": cell_ms / max(1e-12, cell_ms + node_ms),
                 "profiled_pass_ms_per_step": ms_profiled / args.steps,
+                # the method as written is ~3.7 kFLOP of fp64 per TP06 cell-step (census view)
+                "fp64_census_frac": (nc * 3.7e3 / 37.2e12) / (cell_ms * 1e-3) if prob.model == 0 else None,
                 "whole_step_frac": sim.step_bytes / (ms_max * 1e-3 / (inner * args.steps)) / 1e9 / peak}
     cores = os.cpu_count() or 1
     cpu_val, cpu_n, cpu_t = _oracle_leg(prob, args.cpu_budget, cores)
