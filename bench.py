@@ -138,6 +138,34 @@ def run_reference(args):
     }))
 
 
+def max_over_ranks(x: float, dist, device) -> float:
+    """MAX all-reduce of one timing scalar (the only collective of the N > 1 path: replicas share no data)."""
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, cells: int, inner: int, steps: int, ms_max: float) -> float:
+    """cell-updates/s of all replicas together: every rank advances `cells` cells by inner*steps time steps."""
+    return world * cells * inner * steps / (ms_max * 1e-3)
+
+
+def run_disttest(args):
+    """CPU-only check of the N > 1 plumbing (gloo): rank r reports (r + 1) ms; the job value uses the slowest rank."""
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    dist.init_process_group("gloo")
+    dist.barrier()
+    ms_max = max_over_ranks(float(rank + 1), dist, "cpu")
+    val = whole_job_value(world, 1000, 10, 2, ms_max)
+    if rank == 0:
+        print(json.dumps({"impl": "disttest", "n_gpus": world, "ms_max": ms_max, "value": val, "scaling": "weak"}))
+    dist.destroy_process_group()
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -217,11 +245,8 @@ def run_ours(args):
     sim.profile(False)
     launches = launches_timed
     finite = sim.check_finite()
-    t_dev = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t_dev, op=dist.ReduceOp.MAX)
-    ms_max = float(t_dev.item())
-    value = world * nc * inner * args.steps / (ms_max * 1e-3)
+    ms_max = max_over_ranks(ms, dist, "cuda")
+    value = whole_job_value(world, nc, inner, args.steps, ms_max)
 
     # ---------------- end-to-end arm: host state in, Vm + activation times out, every bench step
     def e2e_step():
@@ -237,10 +262,7 @@ def run_ours(args):
     for _ in range(n_e2e):
         e2e_step()
     barrier()
-    t_e2e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
-    e2e_val = world * nc * inner * n_e2e / float(t_e2e.item())
+    e2e_val = whole_job_value(world, nc, inner, n_e2e, 1e3 * max_over_ranks(time.perf_counter() - t0, dist, "cuda"))
 
     if rank != 0:
         if dist is not None:
@@ -292,7 +314,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference", "disttest"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5")
     ap.add_argument("--inner", type=int, default=100, help="explicit time steps per bench step")
     ap.add_argument("--ref-inner", type=int, default=1, help="oracle time steps per bench step (--impl reference)")
@@ -302,7 +324,9 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
-    if args.impl == "reference":
+    if args.impl == "disttest":
+        run_disttest(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
