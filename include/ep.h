@@ -113,6 +113,10 @@ int ep_profile_read(ep_sim *sim, double *out4);
 void ep_destroy(ep_sim *sim);
 const char *ep_last_error(void);
 
+/* Diagnostic: evaluate one of the kernels' fp64 math routines (csrc/ep_math.cuh) on the device, element by element.
+ * fn 0: exp (|x| <= 700), 1: log (x positive, normal), 2: reciprocal, 3: reciprocal square root.  Host pointers. */
+int ep_math_eval(int fn, int64_t n, const double *x, double *y);
+
 /* Host-only preprocessor output for tests (no CUDA call is made).  Returns the factored stencil in the CALLER's
  * numbering: for cell c,  dv_diff[c] = sum_{m<8} a[c*8+m] * v_node[node[c*8+m]] + sum_{j<4} b[c*4+j] * (v[nbr[c*4+j]] - v[c])
  * in mV/ms (= D_c/(chi Cm)), where v_node[n] = sum_{k<node_deg[n]} w[node_ptr[n]+k] * v[node_cell[node_ptr[n]+k]].

@@ -43,6 +43,7 @@ SIGNATURES = {
     "ep_kernel_bytes": (C.c_int64, [_vp, C.c_int]),
     "ep_profile": (C.c_int, [_vp, C.c_int]),
     "ep_profile_read": (C.c_int, [_vp, _dp]),
+    "ep_math_eval": (C.c_int, [C.c_int, C.c_int64, _dp, _dp]),
     "ep_destroy": (None, [_vp]),
     "ep_last_error": (C.c_char_p, []),
     "ep_host_stencil": (C.c_int, [C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double, C.c_double,
@@ -80,6 +81,14 @@ def _chk(rc: int) -> None:
 
 def _p(a, ct=C.c_double):
     return a.ctypes.data_as(C.POINTER(ct)) if a is not None else None
+
+
+def math_eval(fn: int, x):
+    """ep_math_eval: the kernels' own exp (0), log (1), rcp (2), rsqrt (3) on the device."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    y = np.empty_like(x)
+    _chk(lib().ep_math_eval(int(fn), x.size, _p(x), _p(y)))
+    return y
 
 
 def model_n_states(model: int) -> int:

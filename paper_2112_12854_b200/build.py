@@ -1,6 +1,6 @@
 """In-tree build of libep.so (the C-ABI library of include/ep.h) with nvcc for sm_100a.
 
-    python -m paper_2112_12854_b200.build [--force] [--libm]
+    python -m paper_2112_12854_b200.build [--force] [-v]
 
 nvcc cross-compiles without a GPU; the static CUDA runtime is linked so the library loads on a machine without a
 driver (every compute entry point then returns EP_ERR_CUDA).  The .so is git-ignored but travels with the tree.
@@ -34,19 +34,17 @@ def _stale() -> bool:
     return any(os.path.exists(d) and os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, libm: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False) -> str:
     if not (force or _stale()):
         return LIB
     cmd = [_nvcc(), "-O3", "-std=c++20", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
            "-Xcompiler", "-fPIC,-O2", "-shared", "-cudart", "static"]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    if libm:
-        cmd += ["-DEP_LIBM=1"]
     cmd += ["-o", LIB] + [os.path.join(CSRC, f) for f in SOURCES]
     subprocess.check_call(cmd)
     return LIB
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, libm="--libm" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -529,6 +529,23 @@ int ep_check_finite(ep_sim* s, int* all_finite) {
     return EP_OK;
 }
 
+int ep_math_eval(int fn, int64_t n, const double* x, double* y) {
+    if (fn < 0 || fn > 3 || n < 0 || (n > 0 && (!x || !y))) return fail(EP_ERR_ARG, "bad ep_math_eval argument");
+    if (n == 0) return EP_OK;
+    double *dx = nullptr, *dy = nullptr;
+    ep_sim* none = nullptr;
+    EP_CUDA(none, cudaMalloc((void**)&dx, sizeof(double) * n));
+    if (cudaMalloc((void**)&dy, sizeof(double) * n) != cudaSuccess) { cudaFree(dx); return fail(EP_ERR_NOMEM, "cudaMalloc failed"); }
+    cudaError_t e = cudaMemcpy(dx, x, sizeof(double) * n, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        epk::launch_math_eval(fn, n, dx, dy, nullptr);
+        e = cudaMemcpy(y, dy, sizeof(double) * n, cudaMemcpyDeviceToHost);
+    }
+    cudaFree(dx); cudaFree(dy);
+    if (e != cudaSuccess) return fail(EP_ERR_CUDA, std::string("ep_math_eval: ") + cudaGetErrorString(e));
+    return EP_OK;
+}
+
 int ep_device_vm(ep_sim* s, void** vm, void** perm) {
     if (!s) return fail(EP_ERR_ARG, "null sim handle");
     if (vm) *vm = s->d_vm[s->cur];

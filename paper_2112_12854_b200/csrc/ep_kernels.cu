@@ -202,9 +202,24 @@ __global__ void scale_by_inv_norm_kernel(int64_t n, const double* __restrict__ x
     if (i < n) out[i] = x[i] / sqrt(norm2[0]);
 }
 
+__global__ void math_eval_kernel(int fn, int64_t n, const double* __restrict__ x, double* __restrict__ y) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double v[1] = {x[i]};
+    if (fn == 0) ep_exp_wide<1>(v);
+    else if (fn == 1) ep_log_wide<1>(v);
+    else if (fn == 2) v[0] = ep_rcp(v[0]);
+    else v[0] = ep_rsqrt(v[0]);
+    y[i] = v[0];
+}
+
 inline unsigned blocks_for(int64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
 
 }  // namespace
+
+void launch_math_eval(int fn, int64_t n, const double* x, double* y, cudaStream_t s) {
+    math_eval_kernel<<<blocks_for(n, 256), 256, 0, s>>>(fn, n, x, y);
+}
 
 int model_n_states(int model) { return model == 0 ? (int)TP06_S : (model == 1 ? (int)CRN_S : -1); }
 

@@ -51,5 +51,7 @@ void launch_scale_by_inv_norm(int64_t n, const double* x, const double* norm2, d
 void launch_count_nonfinite(int64_t n, const double* x, double* partial, double* out, cudaStream_t s);
 
 int model_n_states(int model);
+// diagnostics: y[i] = f(x[i]) with the kernels' own exp / log / rcp / rsqrt (device pointers)
+void launch_math_eval(int fn, int64_t n, const double* x, double* y, cudaStream_t s);
 
 }  // namespace epk

@@ -11,8 +11,9 @@
 //     them by their exponentials; the loop body exists once in the kernel and its constants stay in uniform registers;
 //   * IEEE division is ~10 fp64 instructions plus a slow-path call  ->  ep_rcp: MUFU.RCP64H seed + one third-order
 //     step (3 DFMA), arguments are finite, normal and far from the ends of the exponent range at every call site.
-// Accuracy: exp and log <= 1 ulp-ish (polynomial error 2e-17), rcp <= 1 ulp, a*rcp(b) <= 2 ulp; measured on the
-// GPU by tests/test_gpu_math.py.  No lookup tables (north_star: "precomputed-free exp paths").
+// Accuracy, measured on the GPU by tests/test_gpu_math.py through ep_math_eval(): exp <= 1 ulp on [-700, 700]
+// (polynomial error 2e-17), log <= 1 ulp where |log x| > 1 (the concentrations it is used on) and <= 2.5 ulp near
+// x = 1, rcp <= 1 ulp, rsqrt <= 2 ulp, hence a*rcp(b) <= 2 ulp.  No lookup tables (north_star: "precomputed-free exp paths").
 #pragma once
 #include <cstdint>
 

@@ -12,8 +12,8 @@
 // 0.02(v-E_K) -> 0.06, 0.1, 0.5; (v+27)^2/3600 -> /240, /225), every sigmoid product is written as one rational function
 // with a single reciprocal, and the remaining exponentials / logarithms are evaluated in shared-memory batches
 // (ep_math.cuh).  Relative differences from the literal formulas are <= ~2e-14 (120-fold powers of a 1-ulp value),
-// three orders of magnitude inside the 1e-11 one-step tolerance.  The literal transcription is kept in
-// ep_tp06_direct.cuh for A/B debugging builds (-DEP_DIRECT=1); it is not part of the product build.
+// three orders of magnitude inside the 1e-11 one-step tolerance.  (The literal transcription was the first kernel of
+// this repo -- profiles/r01a_baseline_direct_kernel.md -- and lives on only in the CPU oracle.)
 //
 // Units: mV, ms, mM, currents uA/uF, conductances nS/pF.
 #pragma once
