@@ -274,8 +274,14 @@ def run_ours(args):
     cell_ms = prof["ms_cell"] / max(1, prof["steps"])
     node_ms = prof["ms_node"] / max(1, prof["steps"])
     achieved = cell_bytes / (cell_ms * 1e-3) / 1e9
+    traffic = args.traffic
+    if traffic is None:   # dram bytes per launch from the committed ncu capture of this workload, if there is one
+        try:
+            traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))[prob.name]["bytes_per_launch"]
+        except Exception:
+            traffic = None
     roofline = {"bound": "hbm", "kernel": "cell_step_kernel<%d>" % prob.model, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "peak_source": peak_src, "traffic": args.traffic,
+                "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic,
                 "alg_bytes_per_launch": cell_bytes, "alg_bytes_per_cell": cell_bytes / nc,
                 "avg_launch_ms": cell_ms, "node_kernel_avg_launch_ms": node_ms,
                 "kernel_share_of_step": cell_ms / max(1e-12, cell_ms + node_ms),

@@ -80,6 +80,10 @@ int ep_write_state(ep_sim *sim, int var, const double *in /*[n_tets]*/);
 /* First instant Vm exceeded 0 mV (reading A18: t=(n+1)dt of the step that crossed); -1 where never. */
 int ep_activation_times(ep_sim *sim, double *out /*[n_tets]*/);
 
+/* Volume-averaged potential v_bar = sum_c V_c v_c / sum_c V_c at the current time (the paper's
+ * convergence observable).  Deterministic two-pass reduction on the device; synchronises. */
+int ep_mean_vm(ep_sim *sim, double *vbar_mV);
+
 /* Diagnostics.  D = div(M grad v) in uA/cm^3 for a host cell field v [mV], through the device gather tables. */
 int ep_apply_diffusion(ep_sim *sim, const double *v /*[n_tets]*/, double *D /*[n_tets]*/);
 /* Largest explicit step of the diffusion part alone: 2 chi Cm / rho(A), rho by power iteration on the device. */

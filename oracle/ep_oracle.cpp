@@ -693,6 +693,14 @@ void orc_get_state(void* h, int var, double* out) { Sim& s = *(Sim*)h; std::memc
 void orc_set_state(void* h, int var, const double* in) { Sim& s = *(Sim*)h; std::memcpy(&s.y[(size_t)var * s.nc], in, sizeof(double) * s.nc); }
 void orc_activation_times(void* h, double* out) { Sim& s = *(Sim*)h; std::memcpy(out, s.tact.data(), sizeof(double) * s.nc); }
 
+// volume-averaged potential: sum_c V_c v_c / sum_c V_c, cells in ascending order
+double orc_mean_vm(void* h) {
+    Sim& s = *(Sim*)h;
+    double num = 0.0, den = 0.0;
+    for (int64_t c = 0; c < s.nc; ++c) { num += s.vol[c] * s.y[c]; den += s.vol[c]; }
+    return num / den;
+}
+
 // ---- single-cell entry points (pins P8-P10)
 void orc_tp06_rest(double* y) { std::memcpy(y, TP06_REST, sizeof(TP06_REST)); }
 void orc_tp06_gates(double v, int type, double Ca_SS, double Ca_SR, double* inf, double* tau) { tp06_gates(v, type, Ca_SS, Ca_SR, inf, tau); }

@@ -58,6 +58,8 @@ def lib():
         L.orc_get_state.argtypes = [C.c_void_p, C.c_int, _dp]
         L.orc_set_state.argtypes = [C.c_void_p, C.c_int, _dp]
         L.orc_activation_times.argtypes = [C.c_void_p, _dp]
+        L.orc_mean_vm.restype = C.c_double
+        L.orc_mean_vm.argtypes = [C.c_void_p]
         L.orc_tp06_rest.argtypes = [_dp]
         L.orc_tp06_gates.argtypes = [C.c_double, C.c_int, C.c_double, C.c_double, _dp, _dp]
         L.orc_tp06_currents.argtypes = [_dp, C.c_int, _dp]
@@ -175,6 +177,9 @@ class OracleSim:
 
     def read_vm(self):
         return self.read_state(0)
+
+    def mean_vm(self):
+        return float(lib().orc_mean_vm(self._h))
 
     def activation_times(self):
         out = np.empty(self.n_tets)

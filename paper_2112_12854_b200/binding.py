@@ -28,6 +28,7 @@ SIGNATURES = {
     "ep_read_state": (C.c_int, [_vp, C.c_int, _dp]),
     "ep_write_state": (C.c_int, [_vp, C.c_int, _dp]),
     "ep_activation_times": (C.c_int, [_vp, _dp]),
+    "ep_mean_vm": (C.c_int, [_vp, _dp]),
     "ep_apply_diffusion": (C.c_int, [_vp, _dp, _dp]),
     "ep_stable_dt": (C.c_int, [_vp, _dp]),
     "ep_check_finite": (C.c_int, [_vp, C.POINTER(C.c_int)]),
@@ -182,6 +183,11 @@ class Sim:
         out = np.empty(self.n_tets) if out is None else out
         _chk(lib().ep_activation_times(self._h, _p(out)))
         return out
+
+    def mean_vm(self):
+        d = C.c_double()
+        _chk(lib().ep_mean_vm(self._h, C.byref(d)))
+        return d.value
 
     def apply_diffusion(self, v):
         v = np.ascontiguousarray(v, dtype=np.float64)

@@ -46,6 +46,8 @@ struct ep_sim {
     int64_t* d_slice_ptr = nullptr;
     double *d_vm[2] = {nullptr, nullptr}, *d_y = nullptr, *d_vn = nullptr, *d_tact = nullptr, *d_tmp = nullptr,
            *d_tmp2 = nullptr, *d_red = nullptr;
+    double* d_vol = nullptr;
+    double vol_total = 0.0;
     uint8_t *d_ctype = nullptr, *d_smask = nullptr, *d_tmp8 = nullptr;
     int cur = 0;   // d_vm[cur] holds Vm at the current time level
     cudaStream_t own_stream = nullptr, stream = nullptr;
@@ -104,7 +106,7 @@ int64_t step_index(double t, double dt) { return (int64_t)std::ceil(t / dt - 1e-
 void free_all(ep_sim* s) {
     void* ptrs[] = {s->d_cidx, s->d_nidx, s->d_perm, s->d_inv, s->d_ccoef, s->d_nw, s->d_slice_ptr, s->d_vm[0],
                     s->d_vm[1], s->d_y, s->d_vn, s->d_tact, s->d_tmp, s->d_tmp2, s->d_red, s->d_ctype, s->d_smask,
-                    s->d_tmp8};
+                    s->d_tmp8, s->d_vol};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
     if (s->graph) cudaGraphExecDestroy(s->graph);
@@ -257,6 +259,7 @@ int ep_mesh_create(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_t
         s = new ep_sim();
         s->nc = pk.nc; s->nn = pk.nn; s->nc_pad = pk.nc_pad; s->chi = chi; s->Cm = Cm;
         s->star_entries = pk.star_entries;
+        s->vol_total = pk.vol_total;
         s->perm_c = pk.perm_c; s->inv_c = pk.inv_c;
         s->smask_host.assign(s->nc_pad, 0);
         auto bail = [&](int code) { free_all(s); delete s; return code; };
@@ -266,7 +269,7 @@ int ep_mesh_create(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_t
         if ((rc = upload(s, &s->d_cidx, pk.cidx)) || (rc = upload(s, &s->d_ccoef, pk.ccoef)) ||
             (rc = upload(s, &s->d_slice_ptr, pk.slice_ptr)) || (rc = upload(s, &s->d_nidx, pk.nidx)) ||
             (rc = upload(s, &s->d_nw, pk.nw)) || (rc = upload(s, &s->d_perm, pk.perm_c)) ||
-            (rc = upload(s, &s->d_inv, pk.inv_c)))
+            (rc = upload(s, &s->d_inv, pk.inv_c)) || (rc = upload(s, &s->d_vol, pk.vol)))
             return bail(rc);
         if ((rc = dev_alloc(s, &s->d_vm[0], s->nc_pad)) || (rc = dev_alloc(s, &s->d_vm[1], s->nc_pad)) ||
             (rc = dev_alloc(s, &s->d_vn, s->nn)) || (rc = dev_alloc(s, &s->d_tact, s->nc_pad)) ||
@@ -510,6 +513,18 @@ int ep_stable_dt(ep_sim* s, double* dt_max) {
     rho = std::sqrt(n2);
     if (!(rho > 0.0) || !std::isfinite(rho)) return fail(EP_ERR_NUMERIC, "power iteration failed");
     *dt_max = 2.0 / rho;
+    return EP_OK;
+}
+
+int ep_mean_vm(ep_sim* s, double* vbar) {
+    if (!s || !vbar) return fail(EP_ERR_ARG, "null argument");
+    if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
+    epk::launch_weighted_sum(s->nc, s->d_vm[s->cur], s->d_vol, s->d_red, s->d_red + 1024, s->stream);
+    s->launches += 2;
+    double sum = 0.0;
+    EP_CUDA(s, cudaMemcpyAsync(&sum, s->d_red + 1024, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    *vbar = sum / s->vol_total;
     return EP_OK;
 }
 

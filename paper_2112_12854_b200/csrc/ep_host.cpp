@@ -199,9 +199,11 @@ int build_stencil(int64_t nn, const double* xyz, int64_t nc, const int32_t* tets
     // ---- per-cell coefficients
     out.node.resize(8 * nc); out.a.assign(8 * nc, 0.0); out.b.assign(4 * nc, 0.0);
     out.centroid.resize(3 * nc);
+    out.vol.resize(nc);
     for (int64_t c = 0; c < nc; ++c) {
         const int32_t* t = tets + 4 * c;
         const CellGeom& G = g[c];
+        out.vol[c] = G.vol;
         out.centroid[3 * c] = G.xc.x; out.centroid[3 * c + 1] = G.xc.y; out.centroid[3 * c + 2] = G.xc.z;
         int32_t slot[8];
         double a[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -260,8 +262,12 @@ int pack(const Stencil& st, const double* xyz, Packed& out, std::string& err) {
     out.nc_pad = (nc + 31) / 32 * 32;
     out.cidx.assign(12 * out.nc_pad, 0);
     out.ccoef.assign(12 * out.nc_pad, 0.0);
+    out.vol.assign(out.nc_pad, 0.0);
+    out.vol_total = 0.0;
+    for (int64_t c = 0; c < nc; ++c) out.vol_total += st.vol[c];
     for (int64_t i = 0; i < nc; ++i) {
         const int64_t c = out.perm_c[i];
+        out.vol[i] = st.vol[c];
         for (int m = 0; m < 8; ++m) {
             out.cidx[m * out.nc_pad + i] = inv_n[st.node[8 * c + m]];
             out.ccoef[m * out.nc_pad + i] = st.a[8 * c + m];

@@ -24,6 +24,7 @@ struct Stencil {              // caller numbering
     std::vector<int32_t> node_cell;// [nc*4] star cells, ascending cell id
     std::vector<double> w;         // [nc*4] inverse-distance weights, normalised per node
     std::vector<double> centroid;  // [nc*3]
+    std::vector<double> vol;       // [nc] cell volumes, mm^3
 };
 
 struct Packed {               // device numbering and device layout
@@ -41,6 +42,8 @@ struct Packed {               // device numbering and device layout
     std::vector<int32_t> nidx;       // device cell ids
     std::vector<double> nw;
     int64_t star_entries = 0;        // sum of node valences (= 4*nc), unpadded
+    std::vector<double> vol;         // [nc_pad] cell volumes in device order (0 in the padding)
+    double vol_total = 0.0;
 };
 
 // Returns 0 or a negative EP_ERR_* code; err receives a message.

@@ -169,14 +169,15 @@ __global__ void gather_u8_kernel(int64_t n, const uint8_t* __restrict__ src, con
 }
 
 // deterministic two-pass reductions: 1024 blocks x 256 threads, fixed tree
-template <int MODE>   // 0: sum of squares, 1: count of non-finite entries
+template <int MODE>   // 0: sum of squares, 1: count of non-finite entries, 2: sum of w[i] * x[i]
 __global__ void __launch_bounds__(256) reduce_partial_kernel(int64_t n, const double* __restrict__ x,
+                                                              const double* __restrict__ w,
                                                               double* __restrict__ partial) {
     __shared__ double sh[256];
     double acc = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (int64_t)gridDim.x * 256) {
         const double v = x[i];
-        acc += (MODE == 0) ? v * v : (isfinite(v) ? 0.0 : 1.0);
+        acc += (MODE == 0) ? v * v : (MODE == 1 ? (isfinite(v) ? 0.0 : 1.0) : w[i] * v);
     }
     sh[threadIdx.x] = acc;
     __syncthreads();
@@ -252,11 +253,15 @@ void launch_gather_u8(int64_t n, const uint8_t* src, const int32_t* idx, uint8_t
     gather_u8_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, src, idx, dst);
 }
 void launch_norm2(int64_t n, const double* x, double* partial, double* out, cudaStream_t s) {
-    reduce_partial_kernel<0><<<1024, 256, 0, s>>>(n, x, partial);
+    reduce_partial_kernel<0><<<1024, 256, 0, s>>>(n, x, nullptr, partial);
     reduce_final_kernel<<<1, 1024, 0, s>>>(partial, out);
 }
 void launch_count_nonfinite(int64_t n, const double* x, double* partial, double* out, cudaStream_t s) {
-    reduce_partial_kernel<1><<<1024, 256, 0, s>>>(n, x, partial);
+    reduce_partial_kernel<1><<<1024, 256, 0, s>>>(n, x, nullptr, partial);
+    reduce_final_kernel<<<1, 1024, 0, s>>>(partial, out);
+}
+void launch_weighted_sum(int64_t n, const double* x, const double* w, double* partial, double* out, cudaStream_t s) {
+    reduce_partial_kernel<2><<<1024, 256, 0, s>>>(n, x, w, partial);
     reduce_final_kernel<<<1, 1024, 0, s>>>(partial, out);
 }
 void launch_scale_by_inv_norm(int64_t n, const double* x, const double* norm2, double* out, cudaStream_t s) {

@@ -48,6 +48,8 @@ void launch_gather_u8(int64_t n, const uint8_t* src, const int32_t* idx, uint8_t
 // reductions for the power iteration and the finite check (deterministic two-pass)
 void launch_norm2(int64_t n, const double* x, double* partial /*[1024]*/, double* out /*[1]*/, cudaStream_t s);
 void launch_scale_by_inv_norm(int64_t n, const double* x, const double* norm2, double* out, cudaStream_t s);
+// out[0] = sum_i w[i] x[i], fixed summation tree (deterministic)
+void launch_weighted_sum(int64_t n, const double* x, const double* w, double* partial, double* out, cudaStream_t s);
 void launch_count_nonfinite(int64_t n, const double* x, double* partial, double* out, cudaStream_t s);
 
 int model_n_states(int model);

@@ -309,3 +309,17 @@ def test_graph_replay_equals_single_steps(ep):
     assert np.array_equal(a.read_vm(), b.read_vm())
     assert a.step_count == b.step_count == 267
     a.close(); b.close()
+
+
+def test_mean_vm_parity(ep, oracle):
+    """v_bar(t) of PAPER.md:216/:230 through ep_mean_vm, during an activation of config 1."""
+    prob = make(1)
+    g, o = _pair(ep, oracle, prob)
+    assert abs(g.mean_vm() + 86.2) < 1e-10     # two summation orders of 9,600 volumes: ~1e-13 relative
+    for _ in range(4):
+        g.step(100, prob.dt); o.step(100, prob.dt)
+        assert abs(g.mean_vm() - o.mean_vm()) <= 1e-9
+    assert g.mean_vm() > -80.0            # the wave has depolarised part of the slab
+    a = g.mean_vm(); b = g.mean_vm()
+    assert a == b                          # deterministic reduction
+    g.close()

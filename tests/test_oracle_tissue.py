@@ -76,3 +76,17 @@ def test_dense_assembly_matches_factored_stencil(oracle):
     assert np.all(np.diag(A) < 0)
     lam = np.linalg.eigvals(A)
     assert lam.real.max() <= 1e-9 * scale                          # stable with eq. (8)
+
+
+def test_volume_averaged_potential(oracle):
+    """v_bar: exact for a uniform field; for v = x on a box tiled by tets the volume-weighted mean of
+    the centroid values is the box centroid, whatever the (jittered) tetrahedra are."""
+    m = M.kuhn_slab(6, 4, 3, 0.5)
+    M.jitter_interior(m, 0.1, 3)
+    s = oracle.OracleSim(m.xyz, m.tets)
+    s.state_init(0, None)
+    assert abs(s.mean_vm() + 86.2) < 1e-12
+    s.write_state(0, m.centroids()[:, 0])
+    assert abs(s.mean_vm() - 1.5) < 1e-13
+    s.write_state(0, 2.0 * m.centroids()[:, 2] - 7.0)
+    assert abs(s.mean_vm() - (2.0 * 0.75 - 7.0)) < 1e-13
