@@ -444,17 +444,21 @@ int ep_read_state(ep_sim* s, int var, double* out) {
     if (!s || !out) return fail(EP_ERR_ARG, "null argument");
     if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
     if (var < 0 || var >= s->S) return fail(EP_ERR_ARG, "state variable index out of range");
-    const double* src = (var == 0) ? s->d_vm[s->cur] : s->d_y + (int64_t)var * s->nc_pad;
-    return read_back(s, src, out);
+    if (var == 0) return read_back(s, s->d_vm[s->cur], out);
+    epk::launch_state_row_get(s->nc, s->d_y, s->S, var, s->d_inv, s->d_tmp, s->stream);
+    s->launches++;
+    EP_CUDA(s, cudaMemcpyAsync(out, s->d_tmp, sizeof(double) * s->nc, cudaMemcpyDeviceToHost, s->stream));
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    return EP_OK;
 }
 
 int ep_write_state(ep_sim* s, int var, const double* in) {
     if (!s || !in) return fail(EP_ERR_ARG, "null argument");
     if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
     if (var < 0 || var >= s->S) return fail(EP_ERR_ARG, "state variable index out of range");
-    double* dst = (var == 0) ? s->d_vm[s->cur] : s->d_y + (int64_t)var * s->nc_pad;
     EP_CUDA(s, cudaMemcpyAsync(s->d_tmp, in, sizeof(double) * s->nc, cudaMemcpyHostToDevice, s->stream));
-    epk::launch_gather_f64(s->nc, s->d_tmp, s->d_perm, dst, s->stream);
+    if (var == 0) epk::launch_gather_f64(s->nc, s->d_tmp, s->d_perm, s->d_vm[s->cur], s->stream);
+    else epk::launch_state_row_put(s->nc, s->d_tmp, s->d_perm, s->S, var, s->d_y, s->stream);
     s->launches++;
     EP_CUDA(s, cudaStreamSynchronize(s->stream));
     return EP_OK;

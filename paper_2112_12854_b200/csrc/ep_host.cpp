@@ -259,7 +259,7 @@ int pack(const Stencil& st, const double* xyz, Packed& out, std::string& err) {
     std::vector<int32_t> inv_n(nn);
     for (int64_t i = 0; i < nn; ++i) inv_n[out.perm_n[i]] = (int32_t)i;
 
-    out.nc_pad = (nc + 31) / 32 * 32;
+    out.nc_pad = (nc + TILE - 1) / TILE * TILE;
     out.cidx.assign(12 * out.nc_pad, 0);
     out.ccoef.assign(12 * out.nc_pad, 0.0);
     out.vol.assign(out.nc_pad, 0.0);
@@ -269,12 +269,12 @@ int pack(const Stencil& st, const double* xyz, Packed& out, std::string& err) {
         const int64_t c = out.perm_c[i];
         out.vol[i] = st.vol[c];
         for (int m = 0; m < 8; ++m) {
-            out.cidx[m * out.nc_pad + i] = inv_n[st.node[8 * c + m]];
-            out.ccoef[m * out.nc_pad + i] = st.a[8 * c + m];
+            out.cidx[tile_index(i, m, 12)] = inv_n[st.node[8 * c + m]];
+            out.ccoef[tile_index(i, m, 12)] = st.a[8 * c + m];
         }
         for (int j = 0; j < 4; ++j) {
-            out.cidx[(8 + j) * out.nc_pad + i] = out.inv_c[st.nbr[4 * c + j]];
-            out.ccoef[(8 + j) * out.nc_pad + i] = st.b[4 * c + j];
+            out.cidx[tile_index(i, 8 + j, 12)] = out.inv_c[st.nbr[4 * c + j]];
+            out.ccoef[tile_index(i, 8 + j, 12)] = st.b[4 * c + j];
         }
     }
     // node table: sliced ELL (32 nodes per slice, width = largest valence in the slice)

@@ -14,6 +14,13 @@
 
 namespace ep {
 
+// Tile-major device layout of every per-cell table with several rows: cells are grouped in tiles
+// of TILE consecutive (Morton-ordered) cells, and the `rows` rows of one tile are contiguous: element (cell i, row k)
+// sits at ((i / TILE) * rows + k) * TILE + i % TILE.  One thread block works on one tile, so all its rows are at
+// compile-time offsets from one base pointer.
+constexpr int64_t TILE = 128;
+inline int64_t tile_index(int64_t i, int64_t k, int64_t rows) { return ((i / TILE) * rows + k) * TILE + i % TILE; }
+
 struct Stencil {              // caller numbering
     int64_t nn = 0, nc = 0;
     std::vector<int32_t> node;     // [nc*8] node ids touched by cell c (own 4 first), unused slots = node[c*8]
@@ -29,12 +36,12 @@ struct Stencil {              // caller numbering
 
 struct Packed {               // device numbering and device layout
     int64_t nn = 0, nc = 0;
-    int64_t nc_pad = 0;            // nc rounded up to a multiple of 32 (column stride of the cell tables)
+    int64_t nc_pad = 0;            // nc rounded up to a multiple of TILE
     std::vector<int32_t> perm_c;   // [nc] device position -> caller cell id
     std::vector<int32_t> inv_c;    // [nc] caller cell id -> device position
     std::vector<int32_t> perm_n;   // [nn]
-    std::vector<int32_t> cidx;     // [12][nc_pad]: rows 0..7 device node ids, rows 8..11 device neighbour cells
-    std::vector<double> ccoef;     // [12][nc_pad]: rows 0..7 a, rows 8..11 b
+    std::vector<int32_t> cidx;     // tile-major, 12 rows: rows 0..7 device node ids, rows 8..11 device neighbour cells
+    std::vector<double> ccoef;     // tile-major, 12 rows: rows 0..7 a, rows 8..11 b
     // node table: sliced ELL, slices of 32 nodes, entries of slice s start at slice_ptr[s] (in elements) and are laid
     // out [k][lane] with k < slice_w[s]
     int64_t n_slices = 0;

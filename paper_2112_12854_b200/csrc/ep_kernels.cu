@@ -12,7 +12,10 @@ namespace epk {
 
 namespace {
 
-constexpr int CELL_THREADS = 128;
+constexpr int CELL_THREADS = 128;   // = the tile of the tile-major layout
+__host__ __device__ inline int64_t tile_index(int64_t i, int64_t k, int64_t rows) {
+    return ((i / CELL_THREADS) * rows + k) * CELL_THREADS + i % CELL_THREADS;
+}
 constexpr int NODE_THREADS = 256;
 
 // ---------------------------------------------------------------------------------------------------------
@@ -54,15 +57,15 @@ __global__ void __launch_bounds__(NODE_THREADS) node_gather_kernel(int64_t nn, i
 }
 
 // S2+S3: the factored diffusion gather.  dv = sum_m a_m v_n[node_m] + sum_j b_j (v[nbr_j] - v_c)   [mV/ms]
-__device__ __forceinline__ double diffusion_gather(int64_t i, int64_t stride, const int32_t* __restrict__ cidx,
+__device__ __forceinline__ double diffusion_gather(int64_t i, const int32_t* __restrict__ cidx,
                                                    const double* __restrict__ ccoef, const double* __restrict__ vm,
                                                    const double* __restrict__ vn, double vc) {
     int32_t id[12];
     double cf[12];
 #pragma unroll
     for (int m = 0; m < 12; ++m) {
-        id[m] = __ldg(cidx + m * stride + i);
-        cf[m] = __ldg(ccoef + m * stride + i);
+        id[m] = __ldg(cidx + tile_index(i, m, 12));
+        cf[m] = __ldg(ccoef + tile_index(i, m, 12));
     }
     double accn = 0.0, accc = 0.0;
 #pragma unroll
@@ -72,7 +75,7 @@ __device__ __forceinline__ double diffusion_gather(int64_t i, int64_t stride, co
     return accn + accc;
 }
 
-__global__ void __launch_bounds__(CELL_THREADS) diffusion_only_kernel(int64_t nc, int64_t stride,
+__global__ void __launch_bounds__(CELL_THREADS) diffusion_only_kernel(int64_t nc,
                                                                       const int32_t* __restrict__ cidx,
                                                                       const double* __restrict__ ccoef,
                                                                       const double* __restrict__ vm,
@@ -80,7 +83,7 @@ __global__ void __launch_bounds__(CELL_THREADS) diffusion_only_kernel(int64_t nc
                                                                       double* __restrict__ out) {
     const int64_t i = (int64_t)blockIdx.x * CELL_THREADS + threadIdx.x;
     if (i >= nc) return;
-    out[i] = diffusion_gather(i, stride, cidx, ccoef, vm, vn, vm[i]);
+    out[i] = diffusion_gather(i, cidx, ccoef, vm, vn, vm[i]);
 }
 
 // S2..S9 fused.  One thread per cell; state rows are read once and written once.  MODEL 0: TP06, 1: Courtemanche.
@@ -88,7 +91,7 @@ __global__ void __launch_bounds__(CELL_THREADS) diffusion_only_kernel(int64_t nc
 #define EP_CELL_MIN_BLOCKS 4
 #endif
 template <int MODEL>
-__global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_kernel(int64_t nc, int64_t stride,
+__global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_kernel(int64_t nc,
                                                                                      const int32_t* __restrict__ cidx,
                                                                                      const double* __restrict__ ccoef,
                                                                                      StepArgs a) {
@@ -98,14 +101,19 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     const int64_t i = (int64_t)blockIdx.x * CELL_THREADS + threadIdx.x;
     if (i >= nc) return;
     const double v_old = a.vm_cur[i];
+    // tile-major tables: every row of this block's tile is at a compile-time offset from these three pointers
+    constexpr int S = (MODEL == 0) ? (int)TP06_S : (int)CRN_S;
+    const int32_t* tidx = cidx + (int64_t)blockIdx.x * (12 * CELL_THREADS) + threadIdx.x;
+    const double* tcoef = ccoef + (int64_t)blockIdx.x * (12 * CELL_THREADS) + threadIdx.x;
+    double* ycol = a.y + (int64_t)blockIdx.x * (S * CELL_THREADS) + threadIdx.x;
     // S2+S3 in two halves: indices and coefficients are loaded here, the gathers are issued once the cell model has
     // parked its gates and stay in flight while it evaluates its logarithms and first exponential batch
     int32_t id[12];
     double cf[12];
 #pragma unroll
     for (int m = 0; m < 12; ++m) {
-        id[m] = __ldg(cidx + m * stride + i);
-        cf[m] = __ldg(ccoef + m * stride + i);
+        id[m] = __ldg(tidx + m * CELL_THREADS);
+        cf[m] = __ldg(tcoef + m * CELL_THREADS);
     }
     double gv[12];
     auto issue_gather = [&]() {
@@ -132,10 +140,10 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
         if (mask & (1u << k)) istim += a.desc ? a.desc->istim[k] : a.inl.istim[k];
     double v_new;
     if constexpr (MODEL == 0)
-        v_new = tp06_step<CELL_THREADS>(v_old, a.y + i, stride, a.ctype[i], a.dt, istim, issue_gather, finish_gather,
+        v_new = tp06_step<CELL_THREADS>(v_old, ycol, CELL_THREADS, a.ctype[i], a.dt, istim, issue_gather, finish_gather,
                                         &xs[0][threadIdx.x]);
     else
-        v_new = crn_step<CELL_THREADS>(v_old, a.y + i, stride, a.dt, istim, issue_gather, finish_gather,
+        v_new = crn_step<CELL_THREADS>(v_old, ycol, CELL_THREADS, a.dt, istim, issue_gather, finish_gather,
                                        &xs[0][threadIdx.x]);
     a.vm_next[i] = v_new;
     // S9: activation time = first upward crossing of 0 mV (reading A18)
@@ -144,15 +152,15 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     }
 }
 
-__global__ void state_fill_kernel(int S, int64_t nc, int64_t stride, const uint8_t* __restrict__ ctype,
+__global__ void state_fill_kernel(int S, int64_t nc, int64_t nc_pad, const uint8_t* __restrict__ ctype,
                                   const double* __restrict__ y0, double* __restrict__ y, double* __restrict__ vm,
                                   double* __restrict__ tact) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= stride) return;
+    if (i >= nc_pad) return;
     const int t = (i < nc) ? ctype[i] : 0;
     for (int k = 0; k < S; ++k) {
         const double val = y0 ? y0[t * S + k] : (S == (int)TP06_S ? TP06_REST_STATE[k] : CRN_REST_STATE[k]);
-        if (k == 0) vm[i] = val; else y[k * stride + i] = val;
+        if (k == 0) vm[i] = val; else y[tile_index(i, k, S)] = val;
     }
     tact[i] = -1.0;
 }
@@ -161,6 +169,17 @@ __global__ void gather_f64_kernel(int64_t n, const double* __restrict__ src, con
                                   double* __restrict__ dst) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) dst[i] = src[idx[i]];
+}
+// state row k (tile-major, S rows) <-> a linear array in another numbering: dst[c] = y[(idx[c], k)] / y[(i, k)] = src[idx[i]]
+__global__ void state_row_get_kernel(int64_t n, const double* __restrict__ y, int S, int k,
+                                     const int32_t* __restrict__ idx, double* __restrict__ dst) {
+    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c < n) dst[c] = y[tile_index(idx[c], k, S)];
+}
+__global__ void state_row_put_kernel(int64_t n, const double* __restrict__ src, const int32_t* __restrict__ idx, int S,
+                                     int k, double* __restrict__ y) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) y[tile_index(i, k, S)] = src[idx[i]];
 }
 __global__ void gather_u8_kernel(int64_t n, const uint8_t* __restrict__ src, const int32_t* __restrict__ idx,
                                  uint8_t* __restrict__ dst) {
@@ -231,12 +250,12 @@ void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaS
 
 void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStream_t s) {
     const unsigned grid = blocks_for(m.nc, CELL_THREADS);
-    if (model == 0) cell_step_kernel<0><<<grid, CELL_THREADS, 0, s>>>(m.nc, m.nc_pad, m.cidx, m.ccoef, a);
-    else cell_step_kernel<1><<<grid, CELL_THREADS, 0, s>>>(m.nc, m.nc_pad, m.cidx, m.ccoef, a);
+    if (model == 0) cell_step_kernel<0><<<grid, CELL_THREADS, 0, s>>>(m.nc, m.cidx, m.ccoef, a);
+    else cell_step_kernel<1><<<grid, CELL_THREADS, 0, s>>>(m.nc, m.cidx, m.ccoef, a);
 }
 
 void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* vn, double* out, cudaStream_t s) {
-    diffusion_only_kernel<<<blocks_for(m.nc, CELL_THREADS), CELL_THREADS, 0, s>>>(m.nc, m.nc_pad, m.cidx, m.ccoef, vm,
+    diffusion_only_kernel<<<blocks_for(m.nc, CELL_THREADS), CELL_THREADS, 0, s>>>(m.nc, m.cidx, m.ccoef, vm,
                                                                                   vn, out);
 }
 
@@ -248,6 +267,12 @@ void launch_state_fill(int model, int64_t nc, int64_t nc_pad, const uint8_t* cty
 
 void launch_gather_f64(int64_t n, const double* src, const int32_t* idx, double* dst, cudaStream_t s) {
     gather_f64_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, src, idx, dst);
+}
+void launch_state_row_get(int64_t n, const double* y, int S, int k, const int32_t* inv, double* dst, cudaStream_t s) {
+    state_row_get_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, y, S, k, inv, dst);
+}
+void launch_state_row_put(int64_t n, const double* src, const int32_t* perm, int S, int k, double* y, cudaStream_t s) {
+    state_row_put_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, src, perm, S, k, y);
 }
 void launch_gather_u8(int64_t n, const uint8_t* src, const int32_t* idx, uint8_t* dst, cudaStream_t s) {
     gather_u8_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, src, idx, dst);

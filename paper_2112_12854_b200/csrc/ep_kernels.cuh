@@ -7,8 +7,8 @@ namespace epk {
 
 struct DeviceMesh {
     int64_t nc = 0, nn = 0, nc_pad = 0, n_slices = 0;
-    const int32_t* cidx = nullptr;      // [12][nc_pad]
-    const double* ccoef = nullptr;      // [12][nc_pad]
+    const int32_t* cidx = nullptr;      // tile-major [nc_pad/128][12][128]
+    const double* ccoef = nullptr;      // tile-major [nc_pad/128][12][128]
     const int64_t* slice_ptr = nullptr; // [n_slices+1]
     const int32_t* nidx = nullptr;
     const double* nw = nullptr;
@@ -23,7 +23,7 @@ struct StepDesc {
 struct StepArgs {
     const double* vm_cur;   // [nc_pad]
     double* vm_next;        // [nc_pad]
-    double* y;              // [S][nc_pad]; row 0 unused (Vm lives in vm_cur/vm_next)
+    double* y;              // tile-major [nc_pad/128][S][128]; row 0 unused (Vm lives in vm_cur/vm_next)
     double* vn;             // [nn] node values scratch
     const uint8_t* ctype;   // [nc_pad]
     const uint8_t* smask;   // [nc_pad] bit k = cell belongs to stimulus slot k
@@ -44,6 +44,9 @@ void launch_state_fill(int model, int64_t nc, int64_t nc_pad, const uint8_t* cty
                        double* vm, double* tact, cudaStream_t s);
 // permutation helpers: dst[i] = src[idx[i]]
 void launch_gather_f64(int64_t n, const double* src, const int32_t* idx, double* dst, cudaStream_t s);
+// state row k of the tile-major state array: dst[c] = y(inv[c], k)   /   y(i, k) = src[perm[i]]
+void launch_state_row_get(int64_t n, const double* y, int S, int k, const int32_t* inv, double* dst, cudaStream_t s);
+void launch_state_row_put(int64_t n, const double* src, const int32_t* perm, int S, int k, double* y, cudaStream_t s);
 void launch_gather_u8(int64_t n, const uint8_t* src, const int32_t* idx, uint8_t* dst, cudaStream_t s);
 // reductions for the power iteration and the finite check (deterministic two-pass)
 void launch_norm2(int64_t n, const double* x, double* partial /*[1024]*/, double* out /*[1]*/, cudaStream_t s);
