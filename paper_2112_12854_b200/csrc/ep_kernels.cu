@@ -135,9 +135,11 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     // S4: stimulus, eq. (4) PAPER.md:130-132 (window already resolved on the host into istim[k])
     const unsigned mask = a.smask[i];
     double istim = 0.0;
+    if (mask != 0) {   // few cells belong to a stimulus slot: one test instead of eight for the others
 #pragma unroll
-    for (int k = 0; k < 8; ++k)
-        if (mask & (1u << k)) istim += a.desc ? a.desc->istim[k] : a.inl.istim[k];
+        for (int k = 0; k < 8; ++k)
+            if (mask & (1u << k)) istim += a.desc ? a.desc->istim[k] : a.inl.istim[k];
+    }
     double v_new;
     if constexpr (MODEL == 0)
         v_new = tp06_step<CELL_THREADS>(v_old, ycol, CELL_THREADS, a.ctype[i], a.dt, istim, issue_gather, finish_gather,

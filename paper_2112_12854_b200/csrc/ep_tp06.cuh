@@ -120,7 +120,9 @@ template <int BLOCK, class Issue, class Finish>
 __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stride, int type, double dt, double istim,
                                             Issue issue_gather, Finish finish_gather, double* col) {
     using namespace tp06;
-    const double vg = ep_clamp(v, -250.0, 250.0);   // argument of every transcendental: keeps all exponents < 700
+    // Argument of every transcendental.  TP06 lives in [-100, +60] mV; inside [-120, 120] every exponent stays far below
+    // 700 and every Rush-Larsen rate except the m gate's stays below 1e3/ms, so only that one needs a clamp below.
+    const double vg = ep_clamp(v, -120.0, 120.0);
     const double Cai = ycol[Y_CAI * stride], CaSR = ycol[Y_CASR * stride], CaSS = ycol[Y_CASS * stride],
                  Nai = ycol[Y_NAI * stride], Ki = ycol[Y_KI * stride];
     // gate products needed by the currents; the gate values themselves wait in shared memory for the RL update
@@ -149,7 +151,7 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double EKs = CK(RTF) * (CK(LN_KO_PNAO) - lg[2]);
     const double ECa = CK(0.5 * RTF) * (CK(LN_CAO) - lg[3]);
     const double u = v - EK;
-    const double ug = ep_clamp(u, -300.0, 400.0);
+    const double ug = ep_clamp(u, -150.0, 300.0);
     const bool hi = (v >= -40.0);   // reading B7
 
     // ---- batch 2: every voltage-dependent exponential that is not an integer power of another one
@@ -191,8 +193,8 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double fCass_inf = fma(CK(0.6), qf, CK(0.4));
     const double Rbar_rate = fma(CK(k2p) * kcasr, CaSS, CK(k4));   // dR/dt = k4 (1 - R) - k2 CaSS R (reading B1)
     const double Rbar_inf = CK(k4) * ep_rcp(Rbar_rate);
-    col[A_RLF * BLOCK] = fmax(-dt * ep_rcp(fma(80.0, qf, 2.0)), -700.0);
-    col[A_RLR * BLOCK] = fmax(-dt * Rbar_rate, -700.0);
+    col[A_RLF * BLOCK] = -dt * ep_rcp(fma(80.0, qf, 2.0));          // tau_fCass >= 2 ms
+    col[A_RLR * BLOCK] = fmax(-dt * Rbar_rate, -700.0);             // rate grows with Ca_SS: keep the clamp
     ep_exp_slots<N_EXPA, BLOCK, EXP_W>(col);
     ycol[Y_FCASS * stride] = fma(fCass - fCass_inf, col[A_RLF * BLOCK], fCass_inf);   // Rush-Larsen
     ycol[Y_RBAR * stride] = fma(Rbar - Rbar_inf, col[A_RLR * BLOCK], Rbar_inf);
@@ -335,7 +337,7 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     // ---- batch 3: Rush-Larsen (every value of batch 2 has been consumed above, so its slots are free)
 #pragma unroll
     for (int g = 0; g < N_RLB; ++g) {
-        col[g * BLOCK] = fmax(-dt * rate[g], -700.0);
+        col[g * BLOCK] = (g == 0) ? fmax(-dt * rate[g], -700.0) : -dt * rate[g];   // tau_m reaches 1e-6 ms at -120 mV
         col[(B_INF0 + g) * BLOCK] = inf[g];
     }
     col[N_RLB * BLOCK] = 0.0;
