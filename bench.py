@@ -321,7 +321,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference", "disttest"])
-    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5")
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5; 6/7/8 = the paper's Table-1 slab at dx 0.5/0.2/0.1 mm")
     ap.add_argument("--inner", type=int, default=100, help="explicit time steps per bench step")
     ap.add_argument("--ref-inner", type=int, default=1, help="oracle time steps per bench step (--impl reference)")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")

@@ -41,6 +41,7 @@ def test_mesh_generator_matches_paper_cell_counts():
         cubes = round(20 / dx) * round(7 / dx) * round(3 / dx)
         assert 6 * cubes == n
     assert make(2).mesh.n_tets == 315000
+    assert make(6).mesh.n_tets == 20160 and make(7).mesh.n_tets == 315000      # the paper's own slab (configs 6-8)
     assert make(1).mesh.n_tets == 9600 and make(1).mesh.n_nodes == 2205
 
 
