@@ -95,25 +95,14 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
     const double vg = ep_clamp(v, -250.0, 250.0);   // argument of every transcendental
     const double Nai = ycol[C_NAI * stride], Ki = ycol[C_KI * stride], Cai = ycol[C_CAI * stride],
                  Caup = ycol[C_CAUP * stride], Carel = ycol[C_CAREL * stride];
-    // gates: products for the currents; m h j fCa u stay in registers, the other ten wait in shared memory
+    // The ten gates of the rolled Rush-Larsen loop are copied into shared memory asynchronously (no registers held); they
+    // and m h j fCa u are first touched after the first exponential batch, which hides their latency.
+#pragma unroll
+    for (int k = 0; k < 8; ++k) ep_cp_async8(col + (G_OLD0 + k) * BLOCK, ycol + (C_OA + k) * stride);
+    ep_cp_async8(col + (G_OLD0 + 8) * BLOCK, ycol + C_VG * stride);
+    ep_cp_async8(col + (G_OLD0 + 9) * BLOCK, ycol + C_W * stride);
     const double m = ycol[C_M * stride], h = ycol[C_H * stride], j = ycol[C_J * stride], fCa = ycol[C_FCA * stride],
                  u = ycol[C_U * stride];
-    double gto3, gkur3, xr, xs2, gcal, uvw;
-    {
-        double g[10];
-#pragma unroll
-        for (int k = 0; k < 8; ++k) g[k] = ycol[(C_OA + k) * stride];
-        g[8] = ycol[C_VG * stride];
-        g[9] = ycol[C_W * stride];
-#pragma unroll
-        for (int k = 0; k < 10; ++k) col[(G_OLD0 + k) * BLOCK] = g[k];
-        gto3 = (g[0] * g[0] * g[0]) * g[1];          // oa^3 oi
-        gkur3 = (g[2] * g[2] * g[2]) * g[3];         // ua^3 ui
-        xr = g[4];
-        xs2 = g[5] * g[5];
-        gcal = g[6] * g[7] * fCa;                    // d f fCa
-        uvw = (u * u) * g[8] * g[9];                 // u^2 v w
-    }
     issue_gather();
 
     // ---- batch 1: logarithms of the reversal potentials
@@ -173,6 +162,20 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
     col[A_TFCA * BLOCK] = dt * -0.5;      // tau_fCa = 2 ms
     col[A_TU * BLOCK] = dt * -0.125;      // tau_u = 8 ms
     ep_exp_slots<N_EXPA, BLOCK, EXP_W>(col);
+    const double dv_diff = finish_gather();   // the gathers have landed during the batch: 12 values -> 1
+    ep_cp_async_wait();                       // so have the gate values: products for the currents
+    double gto3, gkur3, xr, xs2, gcal, uvw;
+    {
+        double g[10];
+#pragma unroll
+        for (int k = 0; k < 10; ++k) g[k] = col[(G_OLD0 + k) * BLOCK];
+        gto3 = (g[0] * g[0] * g[0]) * g[1];          // oa^3 oi
+        gkur3 = (g[2] * g[2] * g[2]) * g[3];         // ua^3 ui
+        xr = g[4];
+        xs2 = g[5] * g[5];
+        gcal = g[6] * g[7] * fCa;                    // d f fCa
+        uvw = (u * u) * g[8] * g[9];                 // u^2 v w
+    }
 
     const double e17 = col[A_E17 * BLOCK], e5m = col[A_E5M * BLOCK], e1 = col[A_X1 * BLOCK];
     double W13, W18, W20;
@@ -225,7 +228,7 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
         ycol[C_CAUP * stride] = fma(dt, dCaup, Caup);
         ycol[C_CAREL * stride] = fma(dt, dCarel, Carel);
     }
-    const double v_new = fma(dt, finish_gather() - iion - istim, v);   // eq. (7)
+    const double v_new = fma(dt, dv_diff - iion - istim, v);   // eq. (7)
 
     // ---- Rush-Larsen group 1 (registers): E1 of the release gates rides with m, h, j in one 4-wide exp
     double m_inf, h_inf, j_inf;

@@ -96,7 +96,10 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
                                                                                      const double* __restrict__ ccoef,
                                                                                      StepArgs a) {
     // per-thread columns of the transcendental batches (ep_math.cuh): slot s of thread t at xs[s][t]
-    constexpr int NSLOTS = (MODEL == 0) ? tp06::N_SLOTS : crn::N_SLOTS;
+    // TP06 also keeps its 12 stencil coefficients there (copied in asynchronously: no registers held until they are used)
+    constexpr bool CF_SMEM = (MODEL == 0);
+    constexpr int MSLOTS = (MODEL == 0) ? tp06::N_SLOTS : crn::N_SLOTS;
+    constexpr int NSLOTS = MSLOTS + (CF_SMEM ? 12 : 0);
     __shared__ double xs[NSLOTS][CELL_THREADS];
     const int64_t i = (int64_t)blockIdx.x * CELL_THREADS + threadIdx.x;
     if (i >= nc) return;
@@ -106,6 +109,7 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     const int32_t* tidx = cidx + (int64_t)blockIdx.x * (12 * CELL_THREADS) + threadIdx.x;
     const double* tcoef = ccoef + (int64_t)blockIdx.x * (12 * CELL_THREADS) + threadIdx.x;
     double* ycol = a.y + (int64_t)blockIdx.x * (S * CELL_THREADS) + threadIdx.x;
+    static_assert(NSLOTS * CELL_THREADS * 8 <= 48 * 1024, "static shared memory limit");
     // S2+S3 in two halves: indices and coefficients are loaded here, the gathers are issued once the cell model has
     // parked its gates and stay in flight while it evaluates its logarithms and first exponential batch
     int32_t id[12];
@@ -113,7 +117,8 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
 #pragma unroll
     for (int m = 0; m < 12; ++m) {
         id[m] = __ldg(tidx + m * CELL_THREADS);
-        cf[m] = __ldg(tcoef + m * CELL_THREADS);
+        if constexpr (CF_SMEM) ep_cp_async8(&xs[MSLOTS + m][threadIdx.x], tcoef + m * CELL_THREADS);
+        else cf[m] = __ldg(tcoef + m * CELL_THREADS);
     }
     double gv[12];
     auto issue_gather = [&]() {
@@ -124,6 +129,11 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     };
     auto finish_gather = [&]() {   // dv = sum_m a_m v_n[node_m] + sum_j b_j (v[nbr_j] - v_c)   [mV/ms]
         double accn = 0.0, accm = 0.0, accc = 0.0;
+        if constexpr (CF_SMEM) {
+            ep_cp_async_wait();
+#pragma unroll
+            for (int m = 0; m < 12; ++m) cf[m] = xs[MSLOTS + m][threadIdx.x];
+        }
 #pragma unroll
         for (int m = 0; m < 4; ++m) {
             accn = fma(cf[m], gv[m], accn);

@@ -164,6 +164,16 @@ __device__ __forceinline__ void ep_log_wide(double (&x)[W]) {
     }
 }
 
+// 8-byte asynchronous global -> shared copy (LDGSTS) into the thread's own slot column: no destination register is
+// held while the load is in flight.  ep_cp_async_wait() makes every copy this thread has issued visible to it.
+__device__ __forceinline__ void ep_cp_async8(double* smem_dst, const double* gsrc) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(s), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void ep_cp_async_wait() {
+    asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
+}
+
 __device__ __forceinline__ double ep_clamp(double x, double lo, double hi) { return fmin(fmax(x, lo), hi); }
 
 }  // namespace epk

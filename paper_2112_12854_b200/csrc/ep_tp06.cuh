@@ -85,9 +85,10 @@ constexpr int N_RLB = 11;    // Rush-Larsen variables whose rate depends on batc
 constexpr int N_EXPB = 12;   // their arguments + 1 pad, slots 0..11 (fCass and Rbar ride in batch 2: rates need no exp)
 constexpr int B_INF0 = 12;   // 11 steady states, slots 12..22 (written after batch 2 has been consumed)
 constexpr int G_OLD0 = 24;   // 11 gate values at t^n, parked from the first load to the Rush-Larsen update, slots 24..34
-constexpr int N_SLOTS = 35;
+constexpr int G_RBAR = 35;   // Rbar at t^n
+constexpr int N_SLOTS = 36;
 static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && N_EXPA <= G_OLD0 && B_INF0 + N_RLB <= G_OLD0 &&
-              G_OLD0 + N_RLB <= N_SLOTS, "slot layout");
+              G_OLD0 + N_RLB <= G_RBAR && G_RBAR < N_SLOTS, "slot layout");
 }  // namespace tp06
 
 // Batch 3: y_g <- inf_g + (y_g - inf_g) exp(arg_g) for the 11 voltage-driven Rush-Larsen variables,
@@ -125,22 +126,12 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double vg = ep_clamp(v, -120.0, 120.0);
     const double Cai = ycol[Y_CAI * stride], CaSR = ycol[Y_CASR * stride], CaSS = ycol[Y_CASS * stride],
                  Nai = ycol[Y_NAI * stride], Ki = ycol[Y_KI * stride];
-    // gate products needed by the currents; the gate values themselves wait in shared memory for the RL update
-    double gNa, gCaL, gto, gKr, gKs, fCass, Rbar;
-    {
-        double g[13];
+    // The 11 voltage-driven gates and Rbar are copied into shared memory asynchronously (no registers held, nothing waits
+    // for them here); they are first touched after the first exponential batch, which hides their latency.
 #pragma unroll
-        for (int k = 0; k < 13; ++k) g[k] = ycol[(1 + k) * stride];
-#pragma unroll
-        for (int k = 0; k < N_RLB; ++k) col[(G_OLD0 + k) * BLOCK] = g[k];
-        gNa = (g[Y_M - 1] * g[Y_M - 1] * g[Y_M - 1]) * g[Y_H - 1] * g[Y_J - 1];
-        fCass = g[Y_FCASS - 1];
-        gCaL = (g[Y_D - 1] * g[Y_F - 1]) * (g[Y_F2 - 1] * fCass);
-        gto = g[Y_R - 1] * g[Y_S - 1];
-        gKr = g[Y_XR1 - 1] * g[Y_XR2 - 1];
-        gKs = g[Y_XS - 1] * g[Y_XS - 1];
-        Rbar = g[Y_RBAR - 1];
-    }
+    for (int k = 0; k < N_RLB; ++k) ep_cp_async8(col + (G_OLD0 + k) * BLOCK, ycol + (1 + k) * stride);
+    ep_cp_async8(col + G_RBAR * BLOCK, ycol + Y_RBAR * stride);
+    const double fCass = ycol[Y_FCASS * stride];
     issue_gather();
 
     // ---- batch 1: the four logarithms of the reversal potentials, side by side in registers
@@ -196,6 +187,21 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     col[A_RLF * BLOCK] = -dt * ep_rcp(fma(80.0, qf, 2.0));          // tau_fCass >= 2 ms
     col[A_RLR * BLOCK] = fmax(-dt * Rbar_rate, -700.0);             // rate grows with Ca_SS: keep the clamp
     ep_exp_slots<N_EXPA, BLOCK, EXP_W>(col);
+    const double dv_diff = finish_gather();   // the gathers have landed during the batch: 12 values -> 1
+    // gate values have landed too (finish_gather waited for this thread's asynchronous copies): products for the currents
+    ep_cp_async_wait();
+    double gNa, gCaL, gto, gKr, gKs;
+    const double Rbar = col[G_RBAR * BLOCK];
+    {
+        double g[N_RLB];
+#pragma unroll
+        for (int k = 0; k < N_RLB; ++k) g[k] = col[(G_OLD0 + k) * BLOCK];
+        gNa = (g[Y_M - 1] * g[Y_M - 1] * g[Y_M - 1]) * g[Y_H - 1] * g[Y_J - 1];
+        gCaL = (g[Y_D - 1] * g[Y_F - 1]) * (g[Y_F2 - 1] * fCass);
+        gto = g[Y_R - 1] * g[Y_S - 1];
+        gKr = g[Y_XR1 - 1] * g[Y_XR2 - 1];
+        gKs = g[Y_XS - 1] * g[Y_XS - 1];
+    }
     ycol[Y_FCASS * stride] = fma(fCass - fCass_inf, col[A_RLF * BLOCK], fCass_inf);   // Rush-Larsen
     ycol[Y_RBAR * stride] = fma(Rbar - Rbar_inf, col[A_RLR * BLOCK], Rbar_inf);
 
@@ -270,7 +276,7 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double dCaSS = bss * (-ICaL * CK(Cap / (2.0 * Vss * F)) + Irel * CK(Vsr / Vss) - Ixfer * CK(Vc / Vss));
     const double dNai = -(INa + IbNa + 3.0 * INaK + 3.0 * INaCa) * CK(Cap / (Vc * F));
     const double dKi = -(IK1 + Ito + IKr + IKs - 2.0 * INaK + IpK + istim) * CK(Cap / (Vc * F));   // reading B8
-    const double v_new = fma(dt, finish_gather() - iion - istim, v);   // eq. (7); explicit increment :172
+    const double v_new = fma(dt, dv_diff - iion - istim, v);   // eq. (7); explicit increment :172
     ycol[Y_CAI * stride] = fma(dt, dCai, Cai);                 // forward Euler
     ycol[Y_CASR * stride] = fma(dt, dCaSR, CaSR);
     ycol[Y_CASS * stride] = fma(dt, dCaSS, CaSS);
