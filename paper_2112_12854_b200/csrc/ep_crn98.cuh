@@ -103,11 +103,11 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
     ep_cp_async8(col + (G_OLD0 + 9) * BLOCK, ycol + C_W * stride);
     const double m = ycol[C_M * stride], h = ycol[C_H * stride], j = ycol[C_J * stride], fCa = ycol[C_FCA * stride],
                  u = ycol[C_U * stride];
-    issue_gather();
 
     // ---- batch 1: logarithms of the reversal potentials
     double lg[3] = {Nai, Ki, Cai};
     ep_log_wide<3>(lg);
+    issue_gather();   // the stencil indices were requested before the concentrations: they are here by now
     const double ENa = CK(RTF) * (CK(LN_NAO) - lg[0]);
     const double EK = CK(RTF) * (CK(LN_KO) - lg[1]);
     const double ECa = CK(0.5 * RTF) * (CK(LN_CAO) - lg[2]);

@@ -132,11 +132,11 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     for (int k = 0; k < N_RLB; ++k) ep_cp_async8(col + (G_OLD0 + k) * BLOCK, ycol + (1 + k) * stride);
     ep_cp_async8(col + G_RBAR * BLOCK, ycol + Y_RBAR * stride);
     const double fCass = ycol[Y_FCASS * stride];
-    issue_gather();
 
     // ---- batch 1: the four logarithms of the reversal potentials, side by side in registers
     double lg[4] = {Ki, Nai, fma(CK(pKNa), Nai, Ki), Cai};
     ep_log_wide<4>(lg);
+    issue_gather();   // the stencil indices were requested before the concentrations: they are here by now
     const double EK = CK(RTF) * (CK(LN_KO) - lg[0]);
     const double ENa = CK(RTF) * (CK(LN_NAO) - lg[1]);
     const double EKs = CK(RTF) * (CK(LN_KO_PNAO) - lg[2]);
