@@ -48,7 +48,7 @@ struct ep_sim {
            *d_tmp2 = nullptr, *d_red = nullptr;
     double* d_vol = nullptr;
     double vol_total = 0.0;
-    uint8_t *d_ctype = nullptr, *d_smask = nullptr, *d_tmp8 = nullptr;
+    uint8_t *d_ctype = nullptr, *d_smask = nullptr;
     int cur = 0;   // d_vm[cur] holds Vm at the current time level
     cudaStream_t own_stream = nullptr, stream = nullptr;
     int model = -1, S = 0;
@@ -106,7 +106,7 @@ int64_t step_index(double t, double dt) { return (int64_t)std::ceil(t / dt - 1e-
 void free_all(ep_sim* s) {
     void* ptrs[] = {s->d_cidx, s->d_nidx, s->d_perm, s->d_inv, s->d_ccoef, s->d_nw, s->d_slice_ptr, s->d_vm[0],
                     s->d_vm[1], s->d_y, s->d_vn, s->d_tact, s->d_tmp, s->d_tmp2, s->d_red, s->d_ctype, s->d_smask,
-                    s->d_tmp8, s->d_vol};
+                    s->d_vol};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
     if (s->graph) cudaGraphExecDestroy(s->graph);
@@ -275,7 +275,7 @@ int ep_mesh_create(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_t
             (rc = dev_alloc(s, &s->d_vn, s->nn)) || (rc = dev_alloc(s, &s->d_tact, s->nc_pad)) ||
             (rc = dev_alloc(s, &s->d_tmp, s->nc_pad)) || (rc = dev_alloc(s, &s->d_tmp2, s->nc_pad)) ||
             (rc = dev_alloc(s, &s->d_red, 1024 + 8)) || (rc = dev_alloc(s, &s->d_ctype, s->nc_pad)) ||
-            (rc = dev_alloc(s, &s->d_smask, s->nc_pad)) || (rc = dev_alloc(s, &s->d_tmp8, s->nc_pad)))
+            (rc = dev_alloc(s, &s->d_smask, s->nc_pad)))
             return bail(rc);
         cudaMemset(s->d_vm[0], 0, sizeof(double) * s->nc_pad);
         cudaMemset(s->d_vm[1], 0, sizeof(double) * s->nc_pad);

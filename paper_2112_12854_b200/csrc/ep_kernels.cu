@@ -193,11 +193,6 @@ __global__ void state_row_put_kernel(int64_t n, const double* __restrict__ src, 
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) y[tile_index(i, k, S)] = src[idx[i]];
 }
-__global__ void gather_u8_kernel(int64_t n, const uint8_t* __restrict__ src, const int32_t* __restrict__ idx,
-                                 uint8_t* __restrict__ dst) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) dst[i] = src[idx[i]];
-}
 
 // deterministic two-pass reductions: 1024 blocks x 256 threads, fixed tree
 template <int MODE>   // 0: sum of squares, 1: count of non-finite entries, 2: sum of w[i] * x[i]
@@ -285,9 +280,6 @@ void launch_state_row_get(int64_t n, const double* y, int S, int k, const int32_
 }
 void launch_state_row_put(int64_t n, const double* src, const int32_t* perm, int S, int k, double* y, cudaStream_t s) {
     state_row_put_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, src, perm, S, k, y);
-}
-void launch_gather_u8(int64_t n, const uint8_t* src, const int32_t* idx, uint8_t* dst, cudaStream_t s) {
-    gather_u8_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, src, idx, dst);
 }
 void launch_norm2(int64_t n, const double* x, double* partial, double* out, cudaStream_t s) {
     reduce_partial_kernel<0><<<1024, 256, 0, s>>>(n, x, nullptr, partial);

@@ -47,7 +47,6 @@ void launch_gather_f64(int64_t n, const double* src, const int32_t* idx, double*
 // state row k of the tile-major state array: dst[c] = y(inv[c], k)   /   y(i, k) = src[perm[i]]
 void launch_state_row_get(int64_t n, const double* y, int S, int k, const int32_t* inv, double* dst, cudaStream_t s);
 void launch_state_row_put(int64_t n, const double* src, const int32_t* perm, int S, int k, double* y, cudaStream_t s);
-void launch_gather_u8(int64_t n, const uint8_t* src, const int32_t* idx, uint8_t* dst, cudaStream_t s);
 // reductions for the power iteration and the finite check (deterministic two-pass)
 void launch_norm2(int64_t n, const double* x, double* partial /*[1024]*/, double* out /*[1]*/, cudaStream_t s);
 void launch_scale_by_inv_norm(int64_t n, const double* x, const double* norm2, double* out, cudaStream_t s);
