@@ -323,3 +323,25 @@ def test_mean_vm_parity(ep, oracle):
     a = g.mean_vm(); b = g.mean_vm()
     assert a == b                          # deterministic reduction
     g.close()
+
+
+def test_full_size_c5_courtemanche(ep, oracle):
+    """BASELINE config 5 at full size (about 3M cells, Courtemanche): one step from random states against the threaded
+    oracle on every cell and every one of the 21 state rows, then 3 more steps."""
+    import os
+    prob = make(5)
+    n = prob.mesh.n_tets
+    assert 2.7e6 < n < 3.3e6
+    g, o = _pair(ep, oracle, prob, threads=os.cpu_count() or 1)
+    y = states.random_states(1, 199, n)
+    for k in range(21):
+        g.write_state(k, y[k]); o.write_state(k, y[k])
+    g.step(1, prob.dt); o.step(1, prob.dt)
+    err = _one_step_err(g, o, 21)
+    assert err.max() <= ONE_STEP_TOL, err
+    g.step(3, prob.dt); o.step(3, prob.dt)
+    assert np.abs(g.read_vm() - o.read_vm()).max() <= 1e-8
+    for k in range(1, 16):                      # gates stay in [0,1]
+        s = g.read_state(k)
+        assert s.min() >= 0.0 and s.max() <= 1.0
+    g.close()
