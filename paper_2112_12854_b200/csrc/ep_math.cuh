@@ -115,11 +115,12 @@ __device__ __forceinline__ void ep_exp_wide(double (&x)[W]) {
 
 // Batched evaluation over a thread's own column of a shared-memory slot array xs[slot][BLOCK]; col = &xs[0][tid].
 // N must be a multiple of W.  The loops stay rolled on purpose (instruction-cache footprint).
+// n <= N (a multiple of W, the same for every lane of the warp) lets a caller skip trailing slots it does not need.
 template <int N, int BLOCK, int W>
-__device__ __forceinline__ void ep_exp_slots(double* col) {
+__device__ __forceinline__ void ep_exp_slots(double* col, int n = N) {
     static_assert(N % W == 0, "pad the slot list to a multiple of W");
 #pragma unroll 1
-    for (int s = 0; s < N; s += W) {
+    for (int s = 0; s < n; s += W) {
         double x[W];
 #pragma unroll
         for (int j = 0; j < W; ++j) x[j] = col[(s + j) * BLOCK];

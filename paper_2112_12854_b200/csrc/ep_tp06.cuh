@@ -79,7 +79,8 @@ constexpr double EM1 = 0.36787944117144233;       // e^(-1)
 
 // shared-memory slots of the two exponential batches
 constexpr int A_B600 = 0, A_E14 = 1, A_M = 2, A_H = 3, A_XR1 = 4, A_D = 5, A_PK = 6, A_W = 7, A_GR = 8, A_GS = 9, A_G27 = 10,
-              A_CAL = 11, A_K1Q = 12, A_K1Q2 = 13, A_HJ0 = 14, A_RLF = 22, A_RLR = 23, N_EXPA = 24;
+              A_CAL = 11, A_K1Q = 12, A_K1Q2 = 13, A_HJ0 = 14, A_RLF = 16, A_RLR = 17, A_HJ2 = 18, N_EXPA = 24;
+constexpr int N_EXPA_HI = 20;   // a warp whose cells are all above -40 mV needs no h/j slot beyond the first two
 constexpr int EXP_W = 4;     // exponentials evaluated side by side in the batch loops
 constexpr int N_RLB = 11;    // Rush-Larsen variables whose rate depends on batch 2: m h j xr1 xr2 xs r s d f f2
 constexpr int N_EXPB = 12;   // their arguments + 1 pad, slots 0..11 (fCass and Rbar ride in batch 2: rates need no exp)
@@ -166,16 +167,16 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
         col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-1.0 / 11.1), CK(-10.66 / 11.1));
         col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.057);
 #pragma unroll
-        for (int k = 2; k < 8; ++k) col[(A_HJ0 + k) * BLOCK] = 0.0;
+        for (int k = 0; k < 6; ++k) col[(A_HJ2 + k) * BLOCK] = 0.0;
     } else {
         col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-1.0 / 6.8), CK(-80.0 / 6.8));
         col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.079);
-        col[(A_HJ0 + 2) * BLOCK] = vg * CK(0.3485);
-        col[(A_HJ0 + 3) * BLOCK] = vg * CK(0.2444);
-        col[(A_HJ0 + 4) * BLOCK] = vg * CK(-0.04391);
-        col[(A_HJ0 + 5) * BLOCK] = fma(vg, CK(0.311), CK(0.311 * 79.23));
-        col[(A_HJ0 + 6) * BLOCK] = vg * CK(-0.01052);
-        col[(A_HJ0 + 7) * BLOCK] = fma(vg, CK(-0.1378), CK(-0.1378 * 40.14));
+        col[(A_HJ2 + 0) * BLOCK] = vg * CK(0.3485);
+        col[(A_HJ2 + 1) * BLOCK] = vg * CK(0.2444);
+        col[(A_HJ2 + 2) * BLOCK] = vg * CK(-0.04391);
+        col[(A_HJ2 + 3) * BLOCK] = fma(vg, CK(0.311), CK(0.311 * 79.23));
+        col[(A_HJ2 + 4) * BLOCK] = vg * CK(-0.01052);
+        col[(A_HJ2 + 5) * BLOCK] = fma(vg, CK(-0.1378), CK(-0.1378 * 40.14));
     }
     // fCass and Rbar: their Rush-Larsen rates need no exponential, so exp(-dt/tau) rides in this batch
     const double c2 = CaSR * CaSR, css2 = CaSS * CaSS, ci2 = Cai * Cai;
@@ -186,7 +187,8 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double Rbar_inf = CK(k4) * ep_rcp(Rbar_rate);
     col[A_RLF * BLOCK] = -dt * ep_rcp(fma(80.0, qf, 2.0));          // tau_fCass >= 2 ms
     col[A_RLR * BLOCK] = fmax(-dt * Rbar_rate, -700.0);             // rate grows with Ca_SS: keep the clamp
-    ep_exp_slots<N_EXPA, BLOCK, EXP_W>(col);
+    // warp-uniform trip count: during the plateau (every cell of the warp above -40 mV) the last trip is skipped
+    ep_exp_slots<N_EXPA, BLOCK, EXP_W>(col, __all_sync(__activemask(), hi) ? N_EXPA_HI : N_EXPA);
     const double dv_diff = finish_gather();   // the gathers have landed during the batch: 12 values -> 1
     // gate values have landed too (finish_gather waited for this thread's asynchronous copies): products for the currents
     ep_cp_async_wait();
@@ -299,8 +301,8 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
             rate[1] = CK(0.77 / 0.13) * ep_rcp(1.0 + s0);
             rate[2] = CK(0.6) * s1 * E10 * ep_rcp(E10 + CK(EM32));
         } else {
-            const double s2 = col[(A_HJ0 + 2) * BLOCK], s3 = col[(A_HJ0 + 3) * BLOCK], s4 = col[(A_HJ0 + 4) * BLOCK],
-                         s5 = col[(A_HJ0 + 5) * BLOCK], s6 = col[(A_HJ0 + 6) * BLOCK], s7 = col[(A_HJ0 + 7) * BLOCK];
+            const double s2 = col[(A_HJ2 + 0) * BLOCK], s3 = col[(A_HJ2 + 1) * BLOCK], s4 = col[(A_HJ2 + 2) * BLOCK],
+                         s5 = col[(A_HJ2 + 3) * BLOCK], s6 = col[(A_HJ2 + 4) * BLOCK], s7 = col[(A_HJ2 + 5) * BLOCK];
             rate[1] = fma(CK(0.057), s0, fma(CK(2.7), s1, 3.1e5 * s2));
             const double N1 = fma(-2.5428e4, s3, CK(-6.948e-6) * s4) * (vg + CK(37.78)), D1 = 1.0 + s5;
             const double N2 = CK(0.02424) * s6, D2 = 1.0 + s7;

@@ -105,6 +105,25 @@ def test_one_step_random_states(ep, oracle, case):
     g.close()
 
 
+def test_one_step_plateau_and_rest_warps(ep, oracle):
+    """Whole warps above / below -40 mV: the kernel skips the unused h/j exponentials when every cell of a warp is on the
+    high-voltage branch (reading B7), so that path needs its own inputs; mixed warps are covered by the random cases."""
+    prob = make(1)
+    prob.mesh.cell_type = (np.arange(prob.mesh.n_tets) % 3).astype(np.uint8)
+    g, o = _pair(ep, oracle, prob)
+    n = prob.mesh.n_tets
+    y = states.random_states(0, 78, n)
+    y[0] = uniform(79, np.arange(n), -39.999, 45.0)        # every cell on the plateau branch
+    y[0, n // 2:] = uniform(80, np.arange(n - n // 2), -95.0, -40.001)   # second half of the cells at rest-like voltages
+    y[0, 5] = -40.0
+    for k in range(19):
+        g.write_state(k, y[k]); o.write_state(k, y[k])
+    g.step(1, 0.02); o.step(1, 0.02)
+    err = _one_step_err(g, o, 19)
+    assert err.max() <= ONE_STEP_TOL, err
+    g.close()
+
+
 def test_full_run_config1(ep, oracle):
     """C1 as specified: 1,000 steps of 0.02 ms; the wave crosses the whole slab (all 9,600 cells activate)."""
     prob = make(1)
