@@ -364,3 +364,30 @@ def test_full_size_c5_courtemanche(ep, oracle):
         s = g.read_state(k)
         assert s.min() >= 0.0 and s.max() <= 1.0
     g.close()
+
+
+def test_slab_convergence_trend(ep, capsys):
+    """SURVEY 8(f)-1 on the paper's own slab (Fig. 11): activation time of the far corner and the time at
+    which the volume-averaged potential peaks, at dx = 0.5 / 0.2 / 0.1 mm, dt = 0.005 ms.  Trend pins (PAPER.md:216-218:
+    conduction gets faster with refinement and converges): the far-corner activation time decreases with dx and the
+    decrements shrink; every cell activates."""
+    rows = []
+    for cfg in (6, 7, 8):
+        prob = make(cfg)
+        g = ep.Sim.from_problem(prob)
+        cen = prob.mesh.centroids()
+        far = int(np.argmax(cen.sum(axis=1)))
+        vbar = []
+        for _ in range(40):                      # 40 x 2.5 ms = 100 ms
+            g.step(500, prob.dt)
+            vbar.append(g.mean_vm())
+        ta = g.activation_times()
+        assert g.check_finite() and (ta >= 0).all(), cfg
+        rows.append((prob.notes["dx"], prob.mesh.n_tets, float(ta[far]), float(ta.max()), 2.5 * (1 + int(np.argmax(vbar)))))
+        g.close()
+    with capsys.disabled():
+        for r in rows:
+            print("slab dx=%.1f mm  %8d cells  t_act(far corner)=%.3f ms  last activation=%.3f ms  v_bar peaks at %.1f ms" % r)
+    t = [r[2] for r in rows]
+    assert t[0] > t[1] > t[2]
+    assert (t[1] - t[2]) < (t[0] - t[1])
