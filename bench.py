@@ -99,7 +99,7 @@ def _oracle_leg(prob, budget_s: float, threads: int):
     t0 = time.perf_counter()
     o.step(1, _run_dt(prob))
     t1 = time.perf_counter() - t0
-    n = max(1, min(50, int(budget_s / max(t1, 1e-6)) - 1))
+    n = max(1, min(400, int(budget_s / max(t1, 1e-6)) - 1))
     t0 = time.perf_counter()
     o.step(n, _run_dt(prob))
     t = time.perf_counter() - t0
