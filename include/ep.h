@@ -64,6 +64,16 @@ int ep_state_init(ep_sim *sim, int model, const uint8_t *cell_type, const double
 int ep_stimulus_set(ep_sim *sim, int slot, int64_t n_cells, const int64_t *cell_ids, double amplitude_uA_cm2,
                     double t_start_ms, double duration_ms);
 
+/* Triggered stimulus = the paper's communication-node coupling inside one mesh: the first time any of
+ * the monitored cells exceeds 0 mV (threshold of PAPER.md:190), stimulus slot `slot` -- its cells, amplitude and duration
+ * as given to ep_stimulus_set, its own t_start ignored -- switches on delay_ms later (PAPER.md:196 uses 5 ms / 3 ms) for
+ * its duration, on integer steps: steps n_fire + ceil(delay/dt) <= n < ... + ceil(duration/dt), n_fire = index after the
+ * crossing step.  A trigger fires once; ep_state_init re-arms it.  trigger in [0, 4); n_monitor = 0 removes it.
+ * A slot can be driven by one trigger only. */
+int ep_trigger_set(ep_sim *sim, int trigger, int64_t n_monitor, const int64_t *monitor_ids, int slot, double delay_ms);
+/* Time (ms) at which the trigger fired = (crossing step + 1) * dt, or -1.  Synchronises. */
+int ep_trigger_time(ep_sim *sim, int trigger, double *t_fire_ms);
+
 /* Advance n_steps explicit steps of size dt_ms (everything on the right-hand side at t^n; gates by
  * Rush-Larsen, the rest by forward Euler; v by eq. (7)).  Asynchronous on the sim's stream; errors are sticky.
  * EP_ERR_STATE: before ep_state_init, dt <= 0, or dt different from the previous call's after the first step. */

@@ -386,6 +386,9 @@ struct Face {            // interior face, c1 = lower cell id, normal outward of
 };
 
 struct Stim { std::vector<char> mask; double amp, t0, dur; bool set; };
+// triggered stimulus = communication-node coupling inside one mesh: first crossing of 0 mV by a
+// monitored cell arms slot `slot` to start `delay` later
+struct Trigger { std::vector<int64_t> cells; int slot = 0; double delay = 0.0; bool armed = false; int64_t n_fire1 = -1; };
 
 struct Sim {
     int64_t nn = 0, nc = 0;
@@ -405,6 +408,7 @@ struct Sim {
     std::vector<double> y, yn;         // SoA [S][nc], two copies (Jacobi style, never in place)
     std::vector<double> tact;
     Stim stim[8];
+    Trigger trig[4];
     int64_t step = 0;
     double dt = 0;
     // scratch
@@ -640,6 +644,7 @@ int orc_state_init(void* h, int model, const uint8_t* cell_type, const double* y
         for (int k = 0; k < s.S; ++k) s.y[(size_t)k * s.nc + c] = src[k];
     }
     s.tact.assign(s.nc, -1.0);
+    for (int t = 0; t < 4; ++t) s.trig[t].n_fire1 = -1;
     s.step = 0; s.dt = 0;
     return 0;
 }
@@ -652,6 +657,21 @@ int orc_stimulus_set(void* h, int slot, int64_t n, const int64_t* ids, double am
     for (int64_t i = 0; i < n; ++i) { if (ids[i] < 0 || ids[i] >= s.nc) return -1; st.mask[ids[i]] = 1; }
     st.amp = amp; st.t0 = t0; st.dur = dur; st.set = (n > 0);
     return 0;
+}
+
+int orc_trigger_set(void* h, int trig, int64_t n, const int64_t* ids, int slot, double delay) {
+    Sim& s = *(Sim*)h;
+    if (trig < 0 || trig >= 4 || slot < 0 || slot >= 8) return -1;
+    Trigger& g = s.trig[trig];
+    g.cells.assign(ids, ids + n);
+    for (int64_t c : g.cells) if (c < 0 || c >= s.nc) return -1;
+    g.slot = slot; g.delay = delay; g.armed = n > 0; g.n_fire1 = -1;
+    return 0;
+}
+
+double orc_trigger_time(void* h, int trig) {
+    Sim& s = *(Sim*)h;
+    return s.trig[trig].n_fire1 < 0 ? -1.0 : (double)s.trig[trig].n_fire1 * s.dt;
 }
 
 int orc_step(void* h, int64_t n_steps, double dt) {
@@ -670,6 +690,12 @@ int orc_step(void* h, int64_t n_steps, double dt) {
             const int64_t n_on = step_index(s.stim[k].t0, dt), n_off = step_index(s.stim[k].t0 + s.stim[k].dur, dt);
             on[k] = (n_on <= n && n < n_off);
         }
+        for (int t = 0; t < 4; ++t) {   // a slot driven by a trigger ignores its own window
+            const Trigger& g = s.trig[t];
+            if (!g.armed) continue;
+            const int64_t nd = step_index(g.delay, dt), ndur = step_index(s.stim[g.slot].dur, dt);
+            on[g.slot] = s.stim[g.slot].set && g.n_fire1 >= 0 && n >= g.n_fire1 + nd && n < g.n_fire1 + nd + ndur;
+        }
 #pragma omp parallel for schedule(static)
         for (int64_t c = 0; c < nc; ++c) {
             double y[32], yn[32];
@@ -680,6 +706,12 @@ int orc_step(void* h, int64_t n_steps, double dt) {
             else crn::step(y, dt, Is / s.Cm, s.D[c] * inv_chiCm, yn);
             for (int k = 0; k < s.S; ++k) s.yn[(size_t)k * nc + c] = yn[k];
             if (s.tact[c] < 0.0 && y[0] <= 0.0 && yn[0] > 0.0) s.tact[c] = (double)(n + 1) * dt;   // A18
+        }
+        for (int t = 0; t < 4; ++t) {   // a monitored cell exceeding 0 mV fires the trigger, once
+            Trigger& g = s.trig[t];
+            if (!g.armed || g.n_fire1 >= 0) continue;
+            for (int64_t c : g.cells)
+                if (s.y[c] <= 0.0 && s.yn[c] > 0.0) { g.n_fire1 = n + 1; break; }
         }
         s.y.swap(s.yn);
         s.step = n + 1;

@@ -52,6 +52,9 @@ def lib():
         L.orc_stimulus_set.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.POINTER(C.c_int64), C.c_double, C.c_double,
                                        C.c_double]
         L.orc_step.argtypes = [C.c_void_p, C.c_int64, C.c_double]
+        L.orc_trigger_set.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.POINTER(C.c_int64), C.c_int, C.c_double]
+        L.orc_trigger_time.argtypes = [C.c_void_p, C.c_int]
+        L.orc_trigger_time.restype = C.c_double
         L.orc_n_states.argtypes = [C.c_void_p]
         L.orc_step_count.argtypes = [C.c_void_p]
         L.orc_step_count.restype = C.c_int64
@@ -159,6 +162,15 @@ class OracleSim:
         rc = lib().orc_stimulus_set(self._h, slot, ids.size, _p(ids, C.c_int64), amplitude, t_start, duration)
         if rc:
             raise ValueError(f"oracle: stimulus_set rc={rc}")
+
+    def trigger_set(self, trigger, monitor_ids, slot, delay):
+        ids = np.ascontiguousarray(monitor_ids, dtype=np.int64)
+        rc = lib().orc_trigger_set(self._h, int(trigger), ids.size, _p(ids, C.c_int64), int(slot), float(delay))
+        if rc:
+            raise ValueError(f"oracle: trigger_set rc={rc}")
+
+    def trigger_time(self, trigger):
+        return float(lib().orc_trigger_time(self._h, int(trigger)))
 
     def step(self, n_steps, dt):
         rc = lib().orc_step(self._h, int(n_steps), float(dt))

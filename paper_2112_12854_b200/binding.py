@@ -22,6 +22,8 @@ SIGNATURES = {
                                  C.c_double, C.c_double]),
     "ep_state_init": (C.c_int, [_vp, C.c_int, _u8p, _dp]),
     "ep_stimulus_set": (C.c_int, [_vp, C.c_int, C.c_int64, _i64p, C.c_double, C.c_double, C.c_double]),
+    "ep_trigger_set": (C.c_int, [_vp, C.c_int, C.c_int64, _i64p, C.c_int, C.c_double]),
+    "ep_trigger_time": (C.c_int, [_vp, C.c_int, _dp]),
     "ep_step": (C.c_int, [_vp, C.c_int64, C.c_double]),
     "ep_synchronize": (C.c_int, [_vp]),
     "ep_read_vm": (C.c_int, [_vp, _dp]),
@@ -157,6 +159,15 @@ class Sim:
     def stimulus_set(self, slot, cell_ids, amplitude, t_start, duration):
         ids = np.ascontiguousarray(cell_ids, dtype=np.int64)
         _chk(lib().ep_stimulus_set(self._h, slot, ids.size, _p(ids, C.c_int64), amplitude, t_start, duration))
+
+    def trigger_set(self, trigger, monitor_ids, slot, delay):
+        ids = np.ascontiguousarray(monitor_ids, dtype=np.int64)
+        _chk(lib().ep_trigger_set(self._h, int(trigger), ids.size, _p(ids, C.c_int64), int(slot), float(delay)))
+
+    def trigger_time(self, trigger):
+        d = C.c_double()
+        _chk(lib().ep_trigger_time(self._h, int(trigger), C.byref(d)))
+        return d.value
 
     def step(self, n_steps, dt):
         _chk(lib().ep_step(self._h, int(n_steps), float(dt)))

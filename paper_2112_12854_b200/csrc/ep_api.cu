@@ -56,6 +56,14 @@ struct ep_sim {
     double dt = 0.0;
     int sticky = EP_OK;
     int64_t dev_bytes = 0, launches = 0;
+    // triggered stimuli (ep_trigger_set)
+    struct Trig { bool armed = false; int slot = 0; double delay = 0.0; };
+    Trig trig[epk::MAX_TRIGGERS];
+    std::vector<uint8_t> tmask_host;   // device order
+    uint8_t* d_tmask = nullptr;
+    long long* d_trig_fire = nullptr;
+    epk::TrigPar* d_trig_par = nullptr;
+    bool trig_dirty = true;
     // CUDA-graph replay of GRAPH_STEPS time steps (launch-bound meshes); rebuilt when dt, model or stream change
     cudaGraphExec_t graph = nullptr;
     double graph_dt = 0.0;
@@ -106,7 +114,7 @@ int64_t step_index(double t, double dt) { return (int64_t)std::ceil(t / dt - 1e-
 void free_all(ep_sim* s) {
     void* ptrs[] = {s->d_cidx, s->d_nidx, s->d_perm, s->d_inv, s->d_ccoef, s->d_nw, s->d_slice_ptr, s->d_vm[0],
                     s->d_vm[1], s->d_y, s->d_vn, s->d_tact, s->d_tmp, s->d_tmp2, s->d_red, s->d_ctype, s->d_smask,
-                    s->d_vol};
+                    s->d_vol, s->d_tmask, s->d_trig_fire, s->d_trig_par};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
     if (s->graph) cudaGraphExecDestroy(s->graph);
@@ -144,6 +152,7 @@ constexpr int GRAPH_STEPS = 32;   // even, so that the Vm double buffer is back 
 constexpr int DESC_RING = 8;
 
 void fill_desc(const ep_sim* s, int64_t n, double dt, const int64_t* n_on, const int64_t* n_off, epk::StepDesc& d) {
+    d.n = n;
     d.t_next = (double)(n + 1) * dt;   // reading A17: time from the integer counter
     for (int k = 0; k < EP_MAX_STIM_SLOTS; ++k)
         d.istim[k] = (s->stim[k].set && n_on[k] <= n && n < n_off[k]) ? s->stim[k].amp / s->Cm : 0.0;
@@ -153,6 +162,9 @@ epk::StepArgs step_args(ep_sim* s, int cur, double dt) {
     epk::StepArgs a;
     a.vm_cur = s->d_vm[cur]; a.vm_next = s->d_vm[cur ^ 1];
     a.y = s->d_y; a.vn = s->d_vn; a.ctype = s->d_ctype; a.smask = s->d_smask; a.tact = s->d_tact;
+    a.tmask = s->d_tmask; a.trig_fire = s->d_trig_fire; a.trig_par = s->d_trig_par;
+    a.trig_slots = 0;
+    for (const ep_sim::Trig& t : s->trig) if (t.armed) a.trig_slots |= 1u << t.slot;
     a.dt = dt; a.desc = nullptr;
     return a;
 }
@@ -281,6 +293,13 @@ int ep_mesh_create(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_t
         cudaMemset(s->d_vm[1], 0, sizeof(double) * s->nc_pad);
         cudaMemset(s->d_ctype, 0, s->nc_pad);
         cudaMemset(s->d_smask, 0, s->nc_pad);
+        s->tmask_host.assign(s->nc_pad, 0);
+        if ((rc = dev_alloc(s, &s->d_tmask, s->nc_pad)) || (rc = dev_alloc(s, &s->d_trig_fire, epk::MAX_TRIGGERS)) ||
+            (rc = dev_alloc(s, &s->d_trig_par, epk::MAX_TRIGGERS)))
+            return bail(rc);
+        cudaMemset(s->d_tmask, 0, s->nc_pad);
+        cudaMemset(s->d_trig_fire, 0xff, sizeof(long long) * epk::MAX_TRIGGERS);
+        cudaMemset(s->d_trig_par, 0, sizeof(epk::TrigPar) * epk::MAX_TRIGGERS);
         s->dm.nc = s->nc; s->dm.nn = s->nn; s->dm.nc_pad = s->nc_pad; s->dm.n_slices = pk.n_slices;
         s->dm.cidx = s->d_cidx; s->dm.ccoef = s->d_ccoef; s->dm.slice_ptr = s->d_slice_ptr;
         s->dm.nidx = s->d_nidx; s->dm.nw = s->d_nw;
@@ -343,6 +362,8 @@ int ep_state_init(ep_sim* s, int model, const uint8_t* cell_type, const double* 
         EP_CUDA(s, cudaMemcpy(d_y0, y0, sizeof(double) * n_types * S, cudaMemcpyHostToDevice));
     }
     s->model = model; s->S = S; s->step = 0; s->dt = 0.0; s->cur = 0; s->sticky = EP_OK;
+    EP_CUDA(s, cudaMemset(s->d_trig_fire, 0xff, sizeof(long long) * epk::MAX_TRIGGERS));   // triggers back to "not fired"
+    s->trig_dirty = true;
     epk::launch_state_fill(model, s->nc, s->nc_pad, s->d_ctype, d_y0, s->d_y, s->d_vm[0], s->d_tact, s->stream);
     s->launches++;
     EP_CUDA(s, cudaMemcpyAsync(s->d_vm[1], s->d_vm[0], sizeof(double) * s->nc_pad, cudaMemcpyDeviceToDevice, s->stream));
@@ -364,6 +385,7 @@ int ep_stimulus_set(ep_sim* s, int slot, int64_t n_cells, const int64_t* cell_id
     for (int64_t k = 0; k < n_cells; ++k) s->smask_host[s->inv_c[cell_ids[k]]] |= bit;
     s->stim[slot].set = n_cells > 0;
     s->stim[slot].amp = amp; s->stim[slot].t0 = t0; s->stim[slot].dur = dur; s->stim[slot].n_cells = n_cells;
+    s->trig_dirty = true;   // a trigger may drive this slot: its amplitude / duration are cached on the device
     EP_CUDA(s, cudaStreamSynchronize(s->stream));
     EP_CUDA(s, cudaMemcpy(s->d_smask, s->smask_host.data(), s->nc_pad, cudaMemcpyHostToDevice));
     return EP_OK;
@@ -383,6 +405,21 @@ int ep_step(ep_sim* s, int64_t n_steps, double dt) {
         if (!s->stim[k].set) continue;
         n_on[k] = step_index(s->stim[k].t0, dt);
         n_off[k] = step_index(s->stim[k].t0 + s->stim[k].dur, dt);
+    }
+    if (s->trig_dirty) {   // trigger parameters in steps of this dt; a changed trigger set invalidates the captured graph
+        epk::TrigPar par[epk::MAX_TRIGGERS];
+        for (int t = 0; t < epk::MAX_TRIGGERS; ++t) {
+            const ep_sim::Trig& g = s->trig[t];
+            par[t].armed = g.armed ? 1 : 0;
+            par[t].slot = g.slot;
+            par[t].nd = (int32_t)step_index(g.delay, dt);
+            par[t].ndur = g.armed ? (int32_t)step_index(s->stim[g.slot].dur, dt) : 0;
+            par[t].amp_cm = g.armed ? s->stim[g.slot].amp / s->Cm : 0.0;
+        }
+        EP_CUDA(s, cudaStreamSynchronize(s->stream));
+        EP_CUDA(s, cudaMemcpy(s->d_trig_par, par, sizeof(par), cudaMemcpyHostToDevice));
+        if (s->graph) { cudaGraphExecDestroy(s->graph); s->graph = nullptr; }
+        s->trig_dirty = false;
     }
     int64_t left = n_steps;
     while (left > 0) {
@@ -517,6 +554,41 @@ int ep_stable_dt(ep_sim* s, double* dt_max) {
     rho = std::sqrt(n2);
     if (!(rho > 0.0) || !std::isfinite(rho)) return fail(EP_ERR_NUMERIC, "power iteration failed");
     *dt_max = 2.0 / rho;
+    return EP_OK;
+}
+
+int ep_trigger_set(ep_sim* s, int trigger, int64_t n_monitor, const int64_t* monitor_ids, int slot, double delay_ms) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    if (trigger < 0 || trigger >= epk::MAX_TRIGGERS) return fail(EP_ERR_ARG, "trigger index out of range");
+    if (n_monitor < 0 || (n_monitor > 0 && !monitor_ids)) return fail(EP_ERR_ARG, "bad monitor cell list");
+    if (n_monitor > 0 && (slot < 0 || slot >= EP_MAX_STIM_SLOTS)) return fail(EP_ERR_ARG, "stimulus slot out of range");
+    if (!std::isfinite(delay_ms) || delay_ms < 0.0) return fail(EP_ERR_ARG, "delay must be finite and non-negative");
+    for (int64_t k = 0; k < n_monitor; ++k)
+        if (monitor_ids[k] < 0 || monitor_ids[k] >= s->nc) return fail(EP_ERR_ARG, "monitor cell id out of range");
+    for (int t = 0; t < epk::MAX_TRIGGERS; ++t)
+        if (n_monitor > 0 && t != trigger && s->trig[t].armed && s->trig[t].slot == slot)
+            return fail(EP_ERR_ARG, "stimulus slot is already driven by another trigger");
+    const uint8_t bit = (uint8_t)(1u << trigger);
+    for (int64_t i = 0; i < s->nc; ++i) s->tmask_host[i] &= (uint8_t)~bit;
+    for (int64_t k = 0; k < n_monitor; ++k) s->tmask_host[s->inv_c[monitor_ids[k]]] |= bit;
+    s->trig[trigger].armed = n_monitor > 0;
+    s->trig[trigger].slot = slot;
+    s->trig[trigger].delay = delay_ms;
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    EP_CUDA(s, cudaMemcpy(s->d_tmask, s->tmask_host.data(), s->nc_pad, cudaMemcpyHostToDevice));
+    const long long none = -1;
+    EP_CUDA(s, cudaMemcpy(s->d_trig_fire + trigger, &none, sizeof(none), cudaMemcpyHostToDevice));
+    s->trig_dirty = true;
+    return EP_OK;
+}
+
+int ep_trigger_time(ep_sim* s, int trigger, double* t_fire_ms) {
+    if (!s || !t_fire_ms) return fail(EP_ERR_ARG, "null argument");
+    if (trigger < 0 || trigger >= epk::MAX_TRIGGERS) return fail(EP_ERR_ARG, "trigger index out of range");
+    long long n1 = -1;
+    EP_CUDA(s, cudaMemcpyAsync(&n1, s->d_trig_fire + trigger, sizeof(n1), cudaMemcpyDeviceToHost, s->stream));
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    *t_fire_ms = n1 < 0 ? -1.0 : (double)n1 * s->dt;
     return EP_OK;
 }
 

@@ -146,9 +146,23 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     const unsigned mask = a.smask[i];
     double istim = 0.0;
     if (mask != 0) {   // few cells belong to a stimulus slot: one test instead of eight for the others
+        const long long n = a.desc ? a.desc->n : a.inl.n;
 #pragma unroll
-        for (int k = 0; k < 8; ++k)
-            if (mask & (1u << k)) istim += a.desc ? a.desc->istim[k] : a.inl.istim[k];
+        for (int k = 0; k < 8; ++k) {
+            if (!(mask & (1u << k))) continue;
+            if (a.trig_slots & (1u << k)) {
+                // slot driven by a trigger: on for ndur steps starting nd steps after the monitored crossing.  A firing
+                // written by another thread of THIS launch cannot switch it on (n_on >= n + 1), so there is no race.
+                for (int t = 0; t < MAX_TRIGGERS; ++t) {
+                    const TrigPar p = a.trig_par[t];
+                    if (!p.armed || p.slot != k) continue;
+                    const long long nf = a.trig_fire[t];
+                    if (nf >= 0 && n >= nf + p.nd && n < nf + p.nd + p.ndur) istim += p.amp_cm;
+                }
+            } else {
+                istim += a.desc ? a.desc->istim[k] : a.inl.istim[k];
+            }
+        }
     }
     double v_new;
     if constexpr (MODEL == 0)
@@ -161,6 +175,13 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     // S9: activation time = first upward crossing of 0 mV (reading A18)
     if (v_old <= 0.0 && v_new > 0.0) {
         if (a.tact[i] < 0.0) a.tact[i] = a.desc ? a.desc->t_next : a.inl.t_next;
+        // communication nodes: the first monitored cell to exceed 0 mV fires its trigger, once
+        const unsigned tm = a.tmask[i];
+        if (tm != 0) {
+            const unsigned long long n1 = (unsigned long long)((a.desc ? a.desc->n : a.inl.n) + 1);
+            for (int t = 0; t < MAX_TRIGGERS; ++t)
+                if (tm & (1u << t)) atomicCAS((unsigned long long*)(a.trig_fire + t), ~0ull, n1);
+        }
     }
 }
 

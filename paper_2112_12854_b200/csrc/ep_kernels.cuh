@@ -15,7 +15,17 @@ struct DeviceMesh {
 };
 
 // what changes from one time step to the next
+// Triggered stimulus (communication-node coupling): host-written parameters of one trigger
+struct TrigPar {
+    int32_t armed;          // 0: unused
+    int32_t slot;           // stimulus slot it drives
+    int32_t nd, ndur;       // delay and duration in time steps
+    double amp_cm;          // I_s / C_m of that slot
+};
+enum { MAX_TRIGGERS = 4 };
+
 struct StepDesc {
+    long long n;            // step index
     double t_next;          // (n+1)*dt, recorded on an upward crossing of 0 mV
     double istim[8];        // I_s/C_m of each slot at step n (0 when the slot's window is closed)
 };
@@ -28,6 +38,10 @@ struct StepArgs {
     const uint8_t* ctype;   // [nc_pad]
     const uint8_t* smask;   // [nc_pad] bit k = cell belongs to stimulus slot k
     double* tact;           // [nc_pad]
+    const uint8_t* tmask;   // [nc_pad] bit t = cell is monitored by trigger t (read only on a 0 mV crossing)
+    long long* trig_fire;   // [MAX_TRIGGERS] step index (n+1) of the first crossing of a monitored cell, -1 before
+    const TrigPar* trig_par;// [MAX_TRIGGERS]
+    unsigned trig_slots;    // bit k = slot k is driven by a trigger instead of its own time window
     double dt;
     const StepDesc* desc;   // device descriptor of this step (CUDA-graph replay), or NULL: use `inl`
     StepDesc inl;

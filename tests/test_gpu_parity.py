@@ -391,3 +391,36 @@ def test_slab_convergence_trend(ep, capsys):
     t = [r[2] for r in rows]
     assert t[0] > t[1] > t[2]
     assert (t[1] - t[2]) < (t[0] - t[1])
+
+
+def test_triggered_stimulus_parity(ep, oracle):
+    """Communication-node coupling: a wave started at one end of config 1's slab reaches monitored cells
+    in the middle; 3 ms later the trigger's slot fires at the far end.  Firing time equal, fields within tolerance, across
+    graph replays (the trigger state lives on the device)."""
+    prob = make(1)
+    cen = prob.mesh.centroids()
+    mon = np.nonzero(np.abs(cen[:, 0] - 1.5) < 0.13)[0].astype(np.int64)
+    tgt = np.nonzero(cen[:, 0] > 4.5)[0].astype(np.int64)
+    g, o = _pair(ep, oracle, prob)
+    for s in (g, o):
+        s.stimulus_set(2, tgt, -52.0, 999.0, 1.0)
+        s.trigger_set(1, mon, 2, 3.0)
+    g.step(450, prob.dt); o.step(450, prob.dt)             # 9 ms: 14 graph replays + 2 single steps
+    assert g.trigger_time(1) == o.trigger_time(1) > 0
+    n_f = round(o.trigger_time(1) / prob.dt)
+    assert n_f + 150 + 50 < 450                             # the driven window lies inside the run
+    vg, vo = g.read_vm(), o.read_vm()
+    assert np.abs(vg - vo).max() <= RUN_TOL_MV
+    assert vo[tgt].min() > -60.0                            # the far end has been excited by the triggered slot
+    tg, to = g.activation_times(), o.activation_times()
+    assert np.array_equal(tg >= 0, to >= 0) and np.abs(tg - to).max() <= prob.dt * (1 + 1e-12)
+    assert to[tgt].min() < to[mon].min() + 3.0 + 2.0        # and earlier than the wave alone could have arrived
+    # re-arming: ep_state_init resets the trigger
+    g.state_init(0, prob.mesh.cell_type)
+    assert g.trigger_time(1) == -1.0
+    with pytest.raises(ep.EpError):
+        g.trigger_set(0, mon, 2, 1.0)                       # slot 2 already driven by trigger 1
+    g.trigger_set(1, np.zeros(0, np.int64), 0, 0.0)         # removed
+    g.step(40, prob.dt)
+    assert g.check_finite()
+    g.close()

@@ -90,3 +90,35 @@ def test_volume_averaged_potential(oracle):
     assert abs(s.mean_vm() - 1.5) < 1e-13
     s.write_state(0, 2.0 * m.centroids()[:, 2] - 7.0)
     assert abs(s.mean_vm() - (2.0 * 0.75 - 7.0)) < 1e-13
+
+
+def test_triggered_stimulus_timing(oracle):
+    """Communication-node coupling in the oracle, pinned on two UNCOUPLED cells (sigma scale 0, so each
+    tet is a single cell): cell 0 is paced and monitored; the trigger must fire at the step after its first crossing of
+    0 mV (read off an independent single-cell trace), and cell 1 must then follow exactly the single-cell trace of a cell
+    stimulated for the slot's duration starting `delay` after that instant."""
+    xyz = np.array([[0, 0, 0], [1, 0, 0], [0, 1, 0], [0, 0, 1], [1, 1, 1.0]])
+    tets = np.array([[0, 1, 2, 3], [1, 2, 3, 4]], np.int32)
+    s = oracle.OracleSim(xyz, tets, None, np.zeros(2))
+    s.state_init(0, None)
+    dt, delay, dur = 0.02, 5.0, 0.5                          # PAPER.md:196 orthodromic delay, S_d = 0.5 ms
+    s.stimulus_set(0, np.array([0]), -52.0, 0.0, 1.0)
+    s.stimulus_set(1, np.array([1]), -80.0, 123.0, dur)      # its own t_start must be ignored once a trigger drives it
+    s.trigger_set(0, np.array([0]), 1, delay)
+    s.step(1500, dt)
+    _, tr0 = oracle.tp06_run(oracle.tp06_rest(), 0, dt, 1500, istim=-52.0, n_on=0, n_off=50, trace=True)
+    n_cross = int(np.argmax(tr0 > 0.0))                      # first index with v > 0 = (crossing step + 1)
+    assert tr0[n_cross - 1] <= 0.0 < tr0[n_cross]
+    assert s.trigger_time(0) == n_cross * dt
+    assert s.activation_times()[0] == n_cross * dt
+    n_on = n_cross + 250                                     # 5 ms / 0.02 ms
+    y1, _ = oracle.tp06_run(oracle.tp06_rest(), 0, dt, 1500, istim=-80.0, n_on=n_on, n_off=n_on + 25)
+    got = np.array([s.read_state(k)[1] for k in range(19)])
+    assert np.array_equal(got, y1)
+    # never fired -> the driven slot stays off even inside its own window
+    s2 = oracle.OracleSim(xyz, tets, None, np.zeros(2))
+    s2.state_init(0, None)
+    s2.stimulus_set(1, np.array([1]), -80.0, 0.0, 1.0)
+    s2.trigger_set(0, np.array([0]), 1, 0.0)
+    s2.step(200, dt)
+    assert s2.trigger_time(0) == -1.0 and abs(s2.read_vm()[1] + 86.2) < 0.5
