@@ -461,3 +461,23 @@ def test_device_view_streams_and_two_sims(ep):
     assert np.array_equal(a.read_vm(), ref.read_vm())
     assert a.device_bytes > 0 and a.step_bytes == a.kernel_bytes(0) + a.kernel_bytes(1)
     a.close(); b.close(); ref.close()
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("EP_SLOW"), reason="about 6 minutes and 30 GB of host memory: set EP_SLOW=1")
+def test_full_size_c4_biventricle_scar(ep, oracle):
+    """BASELINE config 4 at full size (22.5 M cells, scar with sigma x 0.1): one step from random states against the
+    threaded oracle on every cell, then 2 more steps."""
+    import os
+    prob = make(4)
+    n = prob.mesh.n_tets
+    assert 1.8e7 < n < 2.6e7 and (prob.mesh.sigma_scale == 0.1).sum() > 1000
+    g, o = _pair(ep, oracle, prob, threads=os.cpu_count() or 1)
+    y = states.random_states(0, 404, n)
+    for k in range(19):
+        g.write_state(k, y[k]); o.write_state(k, y[k])
+    g.step(1, prob.dt); o.step(1, prob.dt)
+    err = _one_step_err(g, o, 19)
+    assert err.max() <= ONE_STEP_TOL, err
+    g.step(2, prob.dt); o.step(2, prob.dt)
+    assert np.abs(g.read_vm() - o.read_vm()).max() <= 1e-8
+    g.close()
