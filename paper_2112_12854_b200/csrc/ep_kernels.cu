@@ -1,9 +1,11 @@
-// ep_kernels.cu -- sm_100a kernels of the monodomain + TP06 step.  fp64 throughout.
+// ep_kernels.cu -- sm_100a kernels of the monodomain + cell-model step.  fp64 throughout.
 //
-// Layout: cells and nodes are in Morton order; every per-cell array is a column of length
-// nc_pad so that consecutive threads touch consecutive addresses (coalesced 8-byte loads/stores); the stencil is a
-// fixed-width gather (8 node + 4 neighbour coefficients per cell, sliced-ELL node table), so there are no atomics
-// and the result is deterministic.  Nothing here is a dense contraction: no tensor cores.
+// Layout: cells and nodes are in Morton order; consecutive threads always touch consecutive
+// addresses (coalesced 8-byte loads/stores); arrays with several rows per cell (state, stencil tables) are tile-major:
+// the rows of the 128 cells of one thread block are contiguous, so each row is at a compile-time offset from one
+// pointer.  The stencil is a fixed-width gather (8 node + 4 neighbour coefficients per cell, sliced-ELL node table), so
+// the diffusion term needs no atomics and the result is deterministic (the only atomic is the once-per-run firing of a
+// communication-node trigger).  Nothing here is a dense contraction: no tensor cores.
 #include "ep_kernels.cuh"
 #include "ep_tp06.cuh"
 #include "ep_crn98.cuh"
@@ -21,8 +23,8 @@ constexpr int NODE_THREADS = 256;
 // ---------------------------------------------------------------------------------------------------------
 // S1: cell -> node interpolation.  A slice of 32 nodes is stored [k][lane]; NODE_PARTS warps share a slice, warp p
 // takes rows k = p, p + NODE_PARTS, ... (each row read is 32 consecutive entries: fully coalesced) and the partial sums
-// meet in shared memory.  Four times the threads of a warp-per-slice mapping: the kernel is a latency-bound gather and
-// needs the parallelism (profiles/r01: 40 us -> see DESIGN.md section 6).
+// meet in shared memory.  Four times the threads of a warp-per-slice mapping; the kernel is a dependent gather (index,
+// then value) that runs at 64 % of the HBM peak (profiles/r01b_to_r01e_cell_kernel.md, node kernel section).
 constexpr int NODE_PARTS = 4;
 constexpr int NODE_SLICES_PER_BLOCK = NODE_THREADS / 32 / NODE_PARTS;
 __global__ void __launch_bounds__(NODE_THREADS) node_gather_kernel(int64_t nn, int64_t n_slices,
