@@ -481,3 +481,25 @@ def test_full_size_c4_biventricle_scar(ep, oracle):
     g.step(2, prob.dt); o.step(2, prob.dt)
     assert np.abs(g.read_vm() - o.read_vm()).max() <= 1e-8
     g.close()
+
+
+def test_operator_invariants_at_full_size(ep):
+    """Properties of the diffusion operator that hold at any size, on the full config-3 mesh through the device tables:
+    a uniform field gives zero (row sums vanish, pin P1) and the volume-weighted sum of D vanishes for any field under
+    no-flux boundaries (conservation, pin P2)."""
+    prob = make(3)
+    m = prob.mesh
+    g = ep.Sim(m.xyz, m.tets, m.fibre, m.sigma_scale)
+    x = m.xyz[m.tets]
+    vol = np.abs(np.einsum("ij,ij->i", np.cross(x[:, 1] - x[:, 0], x[:, 2] - x[:, 0]), x[:, 3] - x[:, 0])) / 6.0
+    D0 = g.apply_diffusion(np.full(m.n_tets, -86.2))
+    v = uniform(31, np.arange(m.n_tets), -90.0, 40.0)
+    D = g.apply_diffusion(v)
+    scale = np.abs(D).max()
+    assert np.abs(D0).max() <= 1e-9 * scale
+    assert abs(np.dot(vol, D)) <= 1e-11 * np.dot(vol, np.abs(D))
+    # smooth field: the operator is consistent with div(M grad v) -> small compared with a rough field's response
+    cen = m.centroids()
+    Ds = g.apply_diffusion(np.cos(cen[:, 2] / 20.0))
+    assert np.abs(Ds).max() < 1e-2 * scale
+    g.close()
