@@ -503,3 +503,27 @@ def test_operator_invariants_at_full_size(ep):
     Ds = g.apply_diffusion(np.cos(cen[:, 2] / 20.0))
     assert np.abs(Ds).max() < 1e-2 * scale
     g.close()
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("EP_SLOW"), reason="5-8 minutes each (threaded oracle): set EP_SLOW=1")
+@pytest.mark.parametrize("cfg,coarsen,dt,steps", [(2, 1.0, 0.005, 20000), (3, 2.0, 0.02, 20000), (4, 3.0, 0.01, 5000),
+                                                  (5, 2.0, 0.01, 15000)])
+def test_full_duration(ep, oracle, cfg, coarsen, dt, steps, capsys):
+    """north_star's full-run tolerance on configs 2-5: the whole specified duration (C2 100 ms on the full mesh at the
+    stable dt; C3 one 400 ms beat, C4 its 50 ms window, C5 150 ms on twins at 2-3x the lattice spacing), threaded
+    oracle.  max |dVm| <= 1e-6 mV, identical activated sets, activation times within one dt."""
+    import os
+    prob = make(cfg, coarsen=coarsen)
+    g, o = _pair(ep, oracle, prob, threads=os.cpu_count() or 1)
+    worst = 0.0
+    for _ in range(10):                       # compare along the way: a divergence shows where it starts
+        g.step(steps // 10, dt); o.step(steps // 10, dt)
+        worst = max(worst, float(np.abs(g.read_vm() - o.read_vm()).max()))
+    tg, to = g.activation_times(), o.activation_times()
+    with capsys.disabled():
+        print("config %d (coarsen %.0f): %d cells x %d steps, max|dVm| over 10 checkpoints = %.3e mV, activated %d / %d, "
+              "max|dt_act| = %.3e ms" % (cfg, coarsen, prob.mesh.n_tets, steps, worst, int((to >= 0).sum()), to.size,
+                                         float(np.abs(tg - to).max())))
+    assert worst <= RUN_TOL_MV
+    assert np.array_equal(tg >= 0, to >= 0) and np.abs(tg - to).max() <= dt * (1 + 1e-12)
+    g.close()
