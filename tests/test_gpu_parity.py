@@ -527,3 +527,22 @@ def test_full_duration(ep, oracle, cfg, coarsen, dt, steps, capsys):
     assert worst <= RUN_TOL_MV
     assert np.array_equal(tg >= 0, to >= 0) and np.abs(tg - to).max() <= dt * (1 + 1e-12)
     g.close()
+
+
+def test_checkpoint_resume(ep):
+    """ep_read_state / ep_write_state are the checkpoint format.  A run resumed in a fresh handle from the
+    19 state rows continues bit for bit (after the stimulus window has closed: the step counter itself is not restored)."""
+    prob = make(1, coarsen=2.0)
+    a = ep.Sim.from_problem(prob)
+    a.step(120, prob.dt)                              # stimulus window (50 steps) is over
+    ckpt = [a.read_state(k) for k in range(19)]
+    a.step(150, prob.dt)
+    b = ep.Sim(prob.mesh.xyz, prob.mesh.tets, prob.mesh.fibre, prob.mesh.sigma_scale, prob.sigma_l, prob.sigma_t,
+               prob.chi, prob.Cm)
+    b.state_init(prob.model, prob.mesh.cell_type)
+    for k in range(19):
+        b.write_state(k, ckpt[k])
+    b.step(150, prob.dt)
+    for k in range(19):
+        assert np.array_equal(a.read_state(k), b.read_state(k)), k
+    a.close(); b.close()
