@@ -14,6 +14,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "ep_oracle.cpp")
 _LIB = os.path.join(_HERE, "libep_oracle.so")
+# tests/test_oracle_mutations.py points this at a deliberately broken build to prove that the pins notice it
+_LIB_OVERRIDE = os.environ.get("EP_ORACLE_LIB")
 _lib = None
 
 _dp = C.POINTER(C.c_double)
@@ -34,8 +36,11 @@ def _p(a, ct=C.c_double):
 def lib():
     global _lib
     if _lib is None:
-        build()
-        L = C.CDLL(_LIB)
+        if _LIB_OVERRIDE:
+            L = C.CDLL(_LIB_OVERRIDE)
+        else:
+            build()
+            L = C.CDLL(_LIB)
         L.orc_create.restype = C.c_void_p
         L.orc_create.argtypes = [C.c_int64, _dp, C.c_int64, C.POINTER(C.c_int32), _dp, _dp, C.c_double, C.c_double,
                                  C.c_double, C.c_double]

@@ -77,3 +77,39 @@ def test_morton_order_is_local():
     bnd = st["nbr"] == np.arange(inv.size)[:, None]
     dist = np.abs(inv[st["nbr"]] - inv[:, None])[~bnd]
     assert np.median(dist) <= 8
+
+
+def test_dense_assembly_matches_factored_stencil(oracle):
+    import paper_2112_12854_b200 as ep
+    m = M.kuhn_slab(4, 3, 3, 0.4)
+    M.jitter_interior(m, 0.06, 5)
+    cen = m.centroids()
+    th = np.deg2rad(-60 + 120 * cen[:, 2] / 1.2)
+    fib = np.stack([np.cos(th), np.sin(th), 0 * th], axis=1)
+    n = m.n_tets
+    s = oracle.OracleSim(m.xyz, m.tets, fib, None, 1.3, 0.18, 1400.0, 1.0)
+    A = np.empty((n, n))
+    for j in range(n):                                # brute force: one unit vector per column
+        e = np.zeros(n); e[j] = 1.0
+        A[:, j] = s.apply_diffusion(e)
+    st = ep.host_stencil(m.xyz, m.tets, fib, None, 1.3, 0.18, 1400.0, 1.0)
+    nn = m.n_nodes
+    W = np.zeros((nn, n))                             # node interpolation matrix
+    owner = np.repeat(np.arange(nn), np.diff(st["node_ptr"]))
+    W[owner, st["node_cell"]] += st["w"]
+    B = np.zeros((n, n))
+    rows = np.arange(n)
+    for k in range(8):
+        B += st["a"][:, k, None] * W[st["node"][:, k], :]
+    for k in range(4):
+        np.add.at(B, (rows, st["nbr"][:, k]), st["b"][:, k])
+        np.add.at(B, (rows, rows), -st["b"][:, k])
+    B *= 1400.0 * 1.0
+    scale = np.abs(A).max()
+    assert np.abs(A - B).max() <= 1e-12 * scale
+    assert np.abs(A.sum(axis=1)).max() <= 1e-11 * scale            # P1: row sums vanish
+    vol, _ = s.geometry()
+    assert np.abs(vol @ A).max() <= 1e-11 * scale * vol.max()      # P2: volume-weighted column sums vanish
+    assert np.all(np.diag(A) < 0)
+    lam = np.linalg.eigvals(A)
+    assert lam.real.max() <= 1e-9 * scale                          # stable with eq. (8)

@@ -231,3 +231,75 @@ def test_scaling_and_isotropic_default(oracle):
     t2 = m.tets[:, [1, 0, 2, 3]].copy()
     flipped = oracle.OracleSim(m.xyz, t2, f, None, 0.7, 0.7)
     assert np.allclose(flipped.apply_diffusion(v), same.apply_diffusion(v), rtol=1e-12, atol=1e-9)
+
+
+def test_two_tet_flux_by_hand(oracle):
+    """Readings A6 (alpha weights) and A8 (M_f) pinned by a flux worked out by hand (numbers: tests/golden/two_tet_flux.json).
+
+    Two tets share the face ABC, A=(0,0,0), B=(1,0,0), C=(0,1,0), in the plane z=0; cell 0 has apex P1=(0,0,1), cell 1 apex
+    P2 below the plane.  v = (1, 0), sigma scale = (1, 0.1), sigma_l = 2, sigma_t = 0.5 mS/cm.  V_0 = 1/6; the area vector
+    of the face outward of cell 0 is s = (0,0,-1/2); x_f = (1/3,1/3,0); x_c0 = (1/4,1/4,1/4), |x_f - x_c0| = sqrt(11)/12.
+
+    Case A, P2=(0,0,-2), isotropic sigma_l: x_c1 = (1/4,1/4,-1/2), |x_f - x_c1| = sqrt(38)/12, so (A6)
+      alpha_c1 = sqrt38/(sqrt11+sqrt38) = 0.65018...;  e = z-hat, d = 3/4.  Eq. (8) replaces the e-component of the averaged
+      gradient by (v_c1 - v_c2)/d = 4/3 and e is parallel to s, so F = sigma_f (4/3)(-1/2) with (A8)
+      sigma_f = 2 (alpha_c1 + 0.1 alpha_c2);  D_0 = 100 F / V_0 = -400 sigma_f = -548.132...,  D_1 = -100 F/V_1 = +200 sigma_f.
+      (alpha swapped would give -331.9; a harmonic mean of the two tensors -192.8.)
+
+    Case B, P2=(1,0,-2), fibre (1,0,1)/sqrt2 in both cells: x_c1 = (1/2,1/4,-1/2), V_1 = 1/3, e = (-1,0,3)/sqrt10, d = sqrt10/4,
+      |x_f - x_c1| = sqrt(41)/12, alpha_c1 = sqrt41/(sqrt11+sqrt41) = 0.658775.
+      Node values (P1 and P2 belong to one cell each): v_P1 = 1, v_P2 = 0,
+        v_A = 3/(3+sqrt3) = 0.633975   (|A-x_c0| = sqrt3/4, |A-x_c1| = 3/4),
+        v_B = 3/(3+sqrt11) = 0.474937  (sqrt11/4, 3/4),   v_C = sqrt17/(sqrt17+sqrt11) = 0.554201  (sqrt11/4, sqrt17/4).
+      Gauss-Green with three-node face means = sum_n v_n grad(lambda_n):
+        cell 0: lambda_B = x, lambda_C = y, lambda_P1 = z       -> grad v_c0 = (v_B-v_A, v_C-v_A, 1-v_A)
+        cell 1: lambda_B = x+z/2, lambda_C = y, lambda_P2 = -z/2 -> grad v_c1 = (v_B-v_A, v_C-v_A, v_B/2)
+      gbar = alpha_c1 grad v_c0 + alpha_c2 grad v_c1 = (-0.159037, -0.079774, 0.322159);
+      eq. (8): g = gbar + [4/sqrt10 - gbar.e] e = (-0.446486, -0.079774, 1.184505);
+      M_f = (alpha_c1 + 0.1 alpha_c2) [0.5 I + 1.5 f f^T]: (M g)_z = k (0.75 g_x + 1.25 g_z), k = 0.692898;
+      F = (M_f g).s = -0.396949;  D_0 = 600 F = -238.169,  D_1 = -300 F = +119.085."""
+    gold = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "two_tet_flux.json")))
+    xyz = np.array(gold["nodes"], dtype=float)
+    v = np.array(gold["v"])
+    scale = np.array(gold["sigma_scale"])
+    for case in ("case_A", "case_B"):
+        g = gold[case]
+        tets = np.array(g["tets"], np.int32)
+        fib = None if g["fibre"] is None else np.tile(np.array(g["fibre"]), (2, 1))
+        s = oracle.OracleSim(xyz, tets, fib, scale, g["sigma_l"], g["sigma_t"])
+        D = s.apply_diffusion(v)
+        assert D == pytest.approx(np.array(g["D"]), rel=1e-13), case
+        if case == "case_B":
+            vn = s.node_values(v)
+            assert vn[:3] == pytest.approx(np.array(g["node_values_ABC"]), rel=1e-14)
+            assert vn[3] == 1.0 and vn[5] == 0.0
+            gr = s.cell_gradients(v)
+            a1 = g["alpha_c1"]
+            assert a1 * gr[0, 2] + (1 - a1) * gr[1, 2] == pytest.approx(g["gbar_z"], rel=1e-13)
+
+
+def test_rotation_invariance(oracle):
+    """div(M grad v) is a scalar: rotating the mesh and the fibres together (eq. (2)-(3): M = A M_hat A^T) must not change
+    D_c.  Checked with the two proper axis permutations on the hand-worked two-tet case B (so that every component of
+    M_f, not only the z row, meets the hand value) and with a general rotation on a jittered slab with conductivity
+    contrasts (readings A8, A9)."""
+    gold = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "two_tet_flux.json")))
+    g = gold["case_B"]
+    xyz = np.array(gold["nodes"], dtype=float)
+    fib = np.tile(np.array(g["fibre"]), (2, 1))
+    for perm in ([1, 2, 0], [2, 0, 1]):
+        s = oracle.OracleSim(xyz[:, perm], np.array(g["tets"], np.int32), fib[:, perm], np.array(gold["sigma_scale"]),
+                             g["sigma_l"], g["sigma_t"])
+        assert s.apply_diffusion(np.array(gold["v"])) == pytest.approx(np.array(g["D"]), rel=1e-13), perm
+    m, s0 = _jittered(oracle)
+    from ep_inputs.prng import uniform
+    scale = uniform(8, np.arange(m.n_tets), 0.1, 1.0)
+    a, b, c = 0.7, -1.1, 0.4
+    Rz = np.array([[np.cos(a), -np.sin(a), 0], [np.sin(a), np.cos(a), 0], [0, 0, 1]])
+    Ry = np.array([[np.cos(b), 0, np.sin(b)], [0, 1, 0], [-np.sin(b), 0, np.cos(b)]])
+    Rx = np.array([[1, 0, 0], [0, np.cos(c), -np.sin(c)], [0, np.sin(c), np.cos(c)]])
+    R = Rz @ Ry @ Rx
+    s1 = oracle.OracleSim(m.xyz @ R.T, m.tets, m.fibre @ R.T, scale, 1.3, 0.18)
+    v = np.random.default_rng(9).uniform(-90, 40, m.n_tets)
+    D0, D1 = s0.apply_diffusion(v), s1.apply_diffusion(v)
+    assert np.abs(D0 - D1).max() <= 1e-10 * np.abs(D0).max()
