@@ -199,14 +199,12 @@ def run_ours(args):
     # the config as specified: every cell at the model's resting state, the config's stimulus armed at t = 0; the
     # timed window is the start of that simulation (stimulus on, wave leaving the stimulus sites)
     pinned = torch.empty((S, nc), dtype=torch.float64).pin_memory()
-    for k in range(S):
-        sim.read_state(k, pinned.numpy()[k])
+    sim.read_states(pinned.numpy())
     out_vm = torch.empty(nc, dtype=torch.float64).pin_memory()
     out_ta = torch.empty(nc, dtype=torch.float64).pin_memory()
 
     def upload():
-        for k in range(S):
-            sim.write_state(k, pinned.numpy()[k])
+        sim.write_states(pinned.numpy())      # all S rows, one call: pipelined copies + permutation kernels, one sync
 
     def barrier():
         if dist is not None:

@@ -25,6 +25,15 @@ class Stimulus:
 
 
 @dataclass
+class Trigger:
+    """Communication-node coupling inside one mesh: the first monitored cell to exceed 0 mV switches
+    stimulus slot `slot` on `delay` ms later (ep_trigger_set)."""
+    monitor_ids: np.ndarray   # int64
+    slot: int
+    delay: float              # ms
+
+
+@dataclass
 class Problem:
     name: str
     mesh: M.TetMesh
@@ -37,6 +46,7 @@ class Problem:
     dt: float = 0.02          # ms
     n_steps: int = 1000
     notes: dict = field(default_factory=dict)
+    triggers: list = field(default_factory=list)   # trigger k drives stimuli[triggers[k].slot]
 
 
 def _pick(seed: int, pool: np.ndarray, k: int) -> np.ndarray:
@@ -47,10 +57,13 @@ def _pick(seed: int, pool: np.ndarray, k: int) -> np.ndarray:
 
 
 def _balls(cent: np.ndarray, centres: np.ndarray, radius: float) -> np.ndarray:
+    """Ids (ascending) of the cells whose centroid lies within `radius` of any of `centres`."""
+    order = np.argsort(cent[:, 0], kind="stable")
+    xs = cent[order, 0]
     hit = np.zeros(cent.shape[0], dtype=bool)
     for c in centres:
-        box = np.all(np.abs(cent - c[None, :]) <= radius, axis=1)
-        idx = np.nonzero(box)[0]
+        lo, hi = np.searchsorted(xs, [c[0] - radius, c[0] + radius])
+        idx = order[lo:hi]
         d2 = ((cent[idx] - c[None, :]) ** 2).sum(axis=1)
         hit[idx[d2 <= radius * radius]] = True
     return np.nonzero(hit)[0].astype(np.int64)
@@ -132,10 +145,10 @@ def config4(coarsen: float = 1.0, seed: int = 1004, h: float = 0.345) -> Problem
     mesh = M.carve_lattice(inside, (-35.0, -35.0, -60.0), (60.0, 35.0, _LV_ZCUT), h)
     cent = mesh.centroids()
     is_lv = _lv_inside(cent)
-    f_lv, d_lv = M.helical_fibres(cent, (0, 0, 0), _LV_IN, _LV_OUT)
-    f_rv, d_rv = M.helical_fibres(cent, _RV_C, _RV_IN, _RV_OUT)
-    mesh.fibre = np.where(is_lv[:, None], f_lv, f_rv)
-    d = np.where(is_lv, d_lv, d_rv)
+    mesh.fibre = np.empty((mesh.n_tets, 3))
+    d = np.empty(mesh.n_tets)
+    mesh.fibre[is_lv], d[is_lv] = M.helical_fibres(cent[is_lv], (0, 0, 0), _LV_IN, _LV_OUT)
+    mesh.fibre[~is_lv], d[~is_lv] = M.helical_fibres(cent[~is_lv], _RV_C, _RV_IN, _RV_OUT)
     mesh.cell_type = M.thirds(d)
     mid_pool = np.nonzero(is_lv & (np.abs(d - 0.5) < 0.1))[0]
     scar_c = cent[_pick(seed + 7, mid_pool, 1)[0]]
@@ -173,9 +186,21 @@ def config5(coarsen: float = 1.0, seed: int = 1005, h: float = 0.55) -> Problem:
     mesh.fibre = circ
     mesh.cell_type = np.zeros(mesh.n_tets, dtype=np.uint8)
     pt = _pick(seed, np.nonzero(left)[0], 1)
-    ids = _balls(cent, cent[pt], max(2.0, 2.0 * coarsen))
-    return Problem("C5_atrial_shell", mesh, model=MODEL_CRN98, stimuli=[Stimulus(ids, -52.0, 0.0, 2.5)], dt=0.01,
-                   n_steps=15000, notes={"seed": seed, "h": h})
+    r = max(2.0, 2.0 * coarsen)
+    ids = _balls(cent, cent[pt], r)
+    stimuli = [Stimulus(ids, -52.0, 0.0, 2.5)]
+    # Reading G1: the 2 mm patch alone excites the wall and the wave travels at ~0.3 m/s along the fibres, which reaches
+    # ~5 % of the cells in 150 ms; in the paper the atria are activated within 140 ms because the 1D internodal pathways and
+    # Bachmann's bundle (1.5 m/s) re-excite the myocardium through communication nodes.  Those
+    # bundles are outside this path, so they are stood in for by two trigger-driven slots (ep_trigger_set): 12 seeded sites
+    # on the shell of the sinus node 10 ms after the patch fires, 12 on the other shell 30 ms after it.
+    triggers = []
+    for k, (pool, delay) in enumerate(((np.nonzero(left)[0], 10.0), (np.nonzero(~left)[0], 30.0))):
+        sites = _pick(seed + 1 + k, pool, 12)
+        stimuli.append(Stimulus(_balls(cent, cent[sites], r), -52.0, 1e9, 2.5))
+        triggers.append(Trigger(ids, 1 + k, delay))
+    return Problem("C5_atrial_shell", mesh, model=MODEL_CRN98, stimuli=stimuli, dt=0.01, n_steps=15000,
+                   notes={"seed": seed, "h": h}, triggers=triggers)
 
 
 def paper_slab(dx: float = 0.1, coarsen: float = 1.0) -> Problem:

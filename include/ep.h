@@ -87,8 +87,25 @@ int ep_synchronize(ep_sim *sim);
 int ep_read_vm(ep_sim *sim, double *out /*[n_tets]*/);
 int ep_read_state(ep_sim *sim, int var /*0..S-1, 0 = Vm*/, double *out /*[n_tets]*/);
 int ep_write_state(ep_sim *sim, int var, const double *in /*[n_tets]*/);
+/* All S state rows in one call, row-major [S][n_tets] in the caller's cell order (row 0 = Vm).  The rows move through a
+ * two-slot device staging buffer: the host<->device copy of row k overlaps the permutation kernel of row k-1 on a second
+ * stream, and the host is synchronised once, at the end.  Pinned host memory makes the copies asynchronous. */
+int ep_write_states(ep_sim *sim, const double *in /*[S*n_tets]*/);
+int ep_read_states(ep_sim *sim, double *out /*[S*n_tets]*/);
 /* First instant Vm exceeded 0 mV (reading A18: t=(n+1)dt of the step that crossed); -1 where never. */
 int ep_activation_times(ep_sim *sim, double *out /*[n_tets]*/);
+
+/* Checkpoint / resume.  A run is the S state rows (ep_read_states) PLUS the clock, the activation times recorded so far
+ * and the firing state of the triggers; stimulus windows and trigger delays are counted on the integer step index
+ * (readings A16, A17), so a resumed run needs that index back.  Restore order: ep_state_init, ep_stimulus_set /
+ * ep_trigger_set as in the original run, ep_write_states, ep_set_step_count, ep_write_activation_times,
+ * ep_trigger_restore.  The continuation is then bit-identical to the uninterrupted run.
+ *   ep_set_step_count: step counter n (t = n dt) and the dt the run uses; ep_step keeps refusing any other dt.
+ *   ep_write_activation_times: [n_tets], -1 where not yet activated (what ep_activation_times returned).
+ *   ep_trigger_restore: the value ep_trigger_time returned (-1: not fired yet). */
+int ep_set_step_count(ep_sim *sim, int64_t step_count, double dt_ms);
+int ep_write_activation_times(ep_sim *sim, const double *in /*[n_tets]*/);
+int ep_trigger_restore(ep_sim *sim, int trigger, double t_fire_ms);
 
 /* Volume-averaged potential v_bar = sum_c V_c v_c / sum_c V_c at the current time (the paper's
  * convergence observable).  Deterministic two-pass reduction on the device; synchronises. */
@@ -98,7 +115,9 @@ int ep_mean_vm(ep_sim *sim, double *vbar_mV);
 int ep_apply_diffusion(ep_sim *sim, const double *v /*[n_tets]*/, double *D /*[n_tets]*/);
 /* Largest explicit step of the diffusion part alone: 2 chi Cm / rho(A), rho by power iteration on the device. */
 int ep_stable_dt(ep_sim *sim, double *dt_max_ms);
-/* Sets *all_finite = 0 and the sticky error EP_ERR_NUMERIC if any Vm is NaN/Inf. Synchronises. */
+/* Scans Vm and every state row: sets *all_finite = 0 and the sticky error EP_ERR_NUMERIC if any value is NaN/Inf or any
+ * ion concentration is <= 0 (forward Euler at an unstable dt; the kernels' logarithms need positive arguments and their
+ * clamps would otherwise keep producing finite, meaningless numbers).  Synchronises. */
 int ep_check_finite(ep_sim *sim, int *all_finite);
 
 /* Stream interop: cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL => the sim's own stream. */
@@ -128,7 +147,8 @@ void ep_destroy(ep_sim *sim);
 const char *ep_last_error(void);
 
 /* Diagnostic: evaluate one of the kernels' fp64 math routines (csrc/ep_math.cuh) on the device, element by element.
- * fn 0: exp (|x| <= 700), 1: log (x positive, normal), 2: reciprocal, 3: reciprocal square root.  Host pointers. */
+ * fn 0: 2^x (|x| <= 1000; the kernels form every exponent in base-2 units), 1: log (x positive, normal), 2: reciprocal,
+ * 3: reciprocal square root.  Host pointers. */
 int ep_math_eval(int fn, int64_t n, const double *x, double *y);
 
 /* Host-only preprocessor output for tests (no CUDA call is made).  Returns the factored stencil in the CALLER's

@@ -111,6 +111,8 @@ class OracleSim:
         s.state_init(prob.model, m.cell_type)
         for k, st in enumerate(prob.stimuli):
             s.stimulus_set(k, st.cell_ids, st.amplitude, st.t_start, st.duration)
+        for k, tr in enumerate(getattr(prob, "triggers", [])):
+            s.trigger_set(k, tr.monitor_ids, tr.slot, tr.delay)
         return s
 
     def close(self):

@@ -29,7 +29,12 @@ SIGNATURES = {
     "ep_read_vm": (C.c_int, [_vp, _dp]),
     "ep_read_state": (C.c_int, [_vp, C.c_int, _dp]),
     "ep_write_state": (C.c_int, [_vp, C.c_int, _dp]),
+    "ep_write_states": (C.c_int, [_vp, _dp]),
+    "ep_read_states": (C.c_int, [_vp, _dp]),
     "ep_activation_times": (C.c_int, [_vp, _dp]),
+    "ep_set_step_count": (C.c_int, [_vp, C.c_int64, C.c_double]),
+    "ep_write_activation_times": (C.c_int, [_vp, _dp]),
+    "ep_trigger_restore": (C.c_int, [_vp, C.c_int, C.c_double]),
     "ep_mean_vm": (C.c_int, [_vp, _dp]),
     "ep_apply_diffusion": (C.c_int, [_vp, _dp, _dp]),
     "ep_stable_dt": (C.c_int, [_vp, _dp]),
@@ -137,6 +142,8 @@ class Sim:
         s.state_init(prob.model, m.cell_type)
         for k, st in enumerate(prob.stimuli):
             s.stimulus_set(k, st.cell_ids, st.amplitude, st.t_start, st.duration)
+        for k, tr in enumerate(getattr(prob, "triggers", [])):
+            s.trigger_set(k, tr.monitor_ids, tr.slot, tr.delay)
         return s
 
     def close(self):
@@ -189,6 +196,29 @@ class Sim:
         arr = np.ascontiguousarray(arr, dtype=np.float64)
         assert arr.size == self.n_tets
         _chk(lib().ep_write_state(self._h, int(var), _p(arr)))
+
+    def write_states(self, arr):
+        """All S rows at once, [S, n_tets] row-major (pinned memory makes the copies asynchronous)."""
+        arr = np.ascontiguousarray(arr, dtype=np.float64)
+        assert arr.size == self.n_states * self.n_tets
+        _chk(lib().ep_write_states(self._h, _p(arr)))
+
+    def read_states(self, out=None):
+        out = np.empty((self.n_states, self.n_tets)) if out is None else out
+        assert out.size == self.n_states * self.n_tets and out.flags.c_contiguous
+        _chk(lib().ep_read_states(self._h, _p(out)))
+        return out
+
+    def set_step_count(self, step_count, dt):
+        _chk(lib().ep_set_step_count(self._h, int(step_count), float(dt)))
+
+    def write_activation_times(self, arr):
+        arr = np.ascontiguousarray(arr, dtype=np.float64)
+        assert arr.size == self.n_tets
+        _chk(lib().ep_write_activation_times(self._h, _p(arr)))
+
+    def trigger_restore(self, trigger, t_fire):
+        _chk(lib().ep_trigger_restore(self._h, int(trigger), float(t_fire)))
 
     def activation_times(self, out=None):
         out = np.empty(self.n_tets) if out is None else out

@@ -2,8 +2,10 @@
 // There is no CPU fallback: every compute entry point needs a CUDA device and fails with EP_ERR_CUDA otherwise.
 #include "../../include/ep.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -64,11 +66,17 @@ struct ep_sim {
     long long* d_trig_fire = nullptr;
     epk::TrigPar* d_trig_par = nullptr;
     bool trig_dirty = true;
-    // CUDA-graph replay of GRAPH_STEPS time steps (launch-bound meshes); rebuilt when dt, model or stream change
-    cudaGraphExec_t graph = nullptr;
+    // CUDA-graph replay of GRAPH_STEPS time steps (launch-bound meshes), one graph per parity of the Vm double buffer;
+    // rebuilt when dt, model or stream change
+    cudaGraphExec_t graph[2] = {nullptr, nullptr};
     double graph_dt = 0.0;
-    int graph_model = -1, graph_cur = 0;
+    int graph_model = -1;
     cudaStream_t graph_stream = nullptr;
+    int device = 0;                             // the device the handle was created on
+    bool pdl = true;                            // programmatic dependent launch of the step kernels (EP_NO_PDL=1 disables)
+    // bulk state I/O (ep_write_states / ep_read_states): second stream + events for a two-slot staging pipeline
+    cudaStream_t io_stream = nullptr;
+    cudaEvent_t io_copied[2] = {}, io_consumed[2] = {}, io_fence = nullptr;
     epk::StepDesc* d_desc = nullptr;
     epk::StepDesc* h_desc = nullptr;            // pinned ring of DESC_RING x GRAPH_STEPS descriptors
     cudaEvent_t desc_ev[8] = {};                // copy-done events guarding the reuse of a ring slot
@@ -117,8 +125,14 @@ void free_all(ep_sim* s) {
                     s->d_vol, s->d_tmask, s->d_trig_fire, s->d_trig_par};
     for (void* p : ptrs) if (p) cudaFree(p);
     for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
-    if (s->graph) cudaGraphExecDestroy(s->graph);
+    for (cudaGraphExec_t g : s->graph) if (g) cudaGraphExecDestroy(g);
     if (s->d_desc) cudaFree(s->d_desc);
+    for (int k = 0; k < 2; ++k) {
+        if (s->io_copied[k]) cudaEventDestroy(s->io_copied[k]);
+        if (s->io_consumed[k]) cudaEventDestroy(s->io_consumed[k]);
+    }
+    if (s->io_fence) cudaEventDestroy(s->io_fence);
+    if (s->io_stream) cudaStreamDestroy(s->io_stream);
     if (s->h_desc) cudaFreeHost(s->h_desc);
     for (cudaEvent_t e : s->desc_ev) if (e) cudaEventDestroy(e);
     if (s->own_stream) cudaStreamDestroy(s->own_stream);
@@ -170,8 +184,14 @@ epk::StepArgs step_args(ep_sim* s, int cur, double dt) {
 }
 
 // capture GRAPH_STEPS (node gather, cell step) pairs whose per-step data come from d_desc[k]
+void drop_graphs(ep_sim* s) {
+    for (cudaGraphExec_t& g : s->graph) if (g) { cudaGraphExecDestroy(g); g = nullptr; }
+}
+
 int build_graph(ep_sim* s, double dt) {
-    if (s->graph) { cudaGraphExecDestroy(s->graph); s->graph = nullptr; }
+    if (s->graph_dt != dt || s->graph_model != s->model || s->graph_stream != s->stream) drop_graphs(s);
+    cudaGraphExec_t& slot = s->graph[s->cur];
+    if (slot) { cudaGraphExecDestroy(slot); slot = nullptr; }
     if (!s->d_desc) {
         EP_CUDA(s, cudaMalloc((void**)&s->d_desc, sizeof(epk::StepDesc) * GRAPH_STEPS));
         s->dev_bytes += (int64_t)sizeof(epk::StepDesc) * GRAPH_STEPS;
@@ -184,20 +204,34 @@ int build_graph(ep_sim* s, double dt) {
     for (int k = 0; k < GRAPH_STEPS; ++k) {
         epk::StepArgs a = step_args(s, cur, dt);
         a.desc = s->d_desc + k;
-        epk::launch_node_gather(s->dm, a.vm_cur, s->d_vn, s->stream);
-        epk::launch_cell_step(s->dm, s->model, a, s->stream);
+        epk::launch_node_gather(s->dm, a.vm_cur, s->d_vn, s->stream, s->pdl);
+        epk::launch_cell_step(s->dm, s->model, a, s->stream, s->pdl);
         cur ^= 1;
     }
     EP_CUDA(s, cudaStreamEndCapture(s->stream, &g));
-    cudaError_t e = cudaGraphInstantiate(&s->graph, g, 0);
+    cudaError_t e = cudaGraphInstantiate(&slot, g, 0);
     cudaGraphDestroy(g);
-    if (e != cudaSuccess) { s->graph = nullptr; EP_CUDA(s, e); }
-    s->graph_dt = dt; s->graph_model = s->model; s->graph_cur = s->cur; s->graph_stream = s->stream;
+    if (e != cudaSuccess) { slot = nullptr; EP_CUDA(s, e); }
+    s->graph_dt = dt; s->graph_model = s->model; s->graph_stream = s->stream;
+    return EP_OK;
+}
+
+// every entry point that touches the device goes through this: the handle's device becomes the current one
+int use_device(ep_sim* s) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != s->device) {
+        if (cudaSetDevice(s->device) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(EP_ERR_CUDA, "cannot make the handle's device current");
+        }
+    }
     return EP_OK;
 }
 
 int check_sim(ep_sim* s) {
-    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    int rc = use_device(s);
+    if (rc) return rc;
     if (s->sticky != EP_OK) return fail(s->sticky, "sim is in a sticky error state: " + g_err);
     return EP_OK;
 }
@@ -269,6 +303,8 @@ int ep_mesh_create(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_t
         rc = ep::pack(st, xyz, pk, err);
         if (rc) return fail(rc, err);
         s = new ep_sim();
+        cudaGetDevice(&s->device);
+        s->pdl = (std::getenv("EP_NO_PDL") == nullptr);
         s->nc = pk.nc; s->nn = pk.nn; s->nc_pad = pk.nc_pad; s->chi = chi; s->Cm = Cm;
         s->star_entries = pk.star_entries;
         s->vol_total = pk.vol_total;
@@ -330,45 +366,58 @@ int ep_set_stream(ep_sim* s, void* cuda_stream) {
 }
 
 int ep_state_init(ep_sim* s, int model, const uint8_t* cell_type, const double* y0) {
-    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    int rc = use_device(s);
+    if (rc) return rc;
+    if (s->sticky == EP_ERR_CUDA) return fail(EP_ERR_CUDA, "sim is in a sticky CUDA error state");
     const int S = epk::model_n_states(model);
     if (S < 0) return fail(EP_ERR_ARG, "unknown cell model");
     const int n_types = (model == EP_MODEL_TP06) ? 3 : 1;
+    if (y0)
+        for (int k = 0; k < n_types * S; ++k)
+            if (!std::isfinite(y0[k])) return fail(EP_ERR_ARG, "non-finite initial state");
+    // ep_step is asynchronous on a non-blocking stream: nothing below may overtake a step kernel still in flight
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
     try {
+        std::vector<uint8_t> ct(s->nc_pad, 0);
         if (cell_type) {
-            std::vector<uint8_t> ct(s->nc_pad, 0);
             for (int64_t i = 0; i < s->nc; ++i) {
                 const uint8_t t = cell_type[s->perm_c[i]];
                 if (t >= n_types) return fail(EP_ERR_ARG, "cell_type out of range for this model");
                 ct[i] = t;
             }
-            EP_CUDA(s, cudaMemcpy(s->d_ctype, ct.data(), s->nc_pad, cudaMemcpyHostToDevice));
-        } else {
-            EP_CUDA(s, cudaMemset(s->d_ctype, 0, s->nc_pad));
         }
+        EP_CUDA(s, cudaMemcpyAsync(s->d_ctype, ct.data(), s->nc_pad, cudaMemcpyHostToDevice, s->stream));
+        EP_CUDA(s, cudaStreamSynchronize(s->stream));   // ct goes out of scope
     } catch (const std::bad_alloc&) {
         return fail(EP_ERR_NOMEM, "host allocation failed");
     }
     if (s->S != S) {
-        if (s->d_y) { cudaFree(s->d_y); s->dev_bytes -= (int64_t)sizeof(double) * s->S * s->nc_pad; s->d_y = nullptr; }
-        int rc = dev_alloc(s, &s->d_y, (int64_t)S * s->nc_pad);
+        if (s->d_y) { cudaFree(s->d_y); s->dev_bytes -= (int64_t)sizeof(double) * s->S * s->nc_pad; s->d_y = nullptr; s->S = 0; }
+        rc = dev_alloc(s, &s->d_y, (int64_t)S * s->nc_pad);
         if (rc) return rc;
+        // row 0 of the state array is never used (Vm lives in vm[2]): define it so that whole-array checks see numbers
+        EP_CUDA(s, cudaMemsetAsync(s->d_y, 0, sizeof(double) * (size_t)S * s->nc_pad, s->stream));
     }
-    double* d_y0 = nullptr;
-    if (y0) {
-        for (int k = 0; k < n_types * S; ++k)
-            if (!std::isfinite(y0[k])) return fail(EP_ERR_ARG, "non-finite initial state");
-        EP_CUDA(s, cudaMalloc((void**)&d_y0, sizeof(double) * n_types * S));
-        EP_CUDA(s, cudaMemcpy(d_y0, y0, sizeof(double) * n_types * S, cudaMemcpyHostToDevice));
-    }
-    s->model = model; s->S = S; s->step = 0; s->dt = 0.0; s->cur = 0; s->sticky = EP_OK;
-    EP_CUDA(s, cudaMemset(s->d_trig_fire, 0xff, sizeof(long long) * epk::MAX_TRIGGERS));   // triggers back to "not fired"
+    s->model = model; s->S = S; s->step = 0; s->dt = 0.0; s->cur = 0;
+    if (s->sticky == EP_ERR_NUMERIC) s->sticky = EP_OK;   // a fresh state clears a numerical failure, not a CUDA one
     s->trig_dirty = true;
-    epk::launch_state_fill(model, s->nc, s->nc_pad, s->d_ctype, d_y0, s->d_y, s->d_vm[0], s->d_tact, s->stream);
-    s->launches++;
-    EP_CUDA(s, cudaMemcpyAsync(s->d_vm[1], s->d_vm[0], sizeof(double) * s->nc_pad, cudaMemcpyDeviceToDevice, s->stream));
-    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    double* d_y0 = nullptr;
+    cudaError_t e = cudaSuccess;
+    if (y0) {
+        e = cudaMalloc((void**)&d_y0, sizeof(double) * n_types * S);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(d_y0, y0, sizeof(double) * n_types * S, cudaMemcpyHostToDevice, s->stream);
+    }
+    if (e == cudaSuccess)   // triggers back to "not fired"
+        e = cudaMemsetAsync(s->d_trig_fire, 0xff, sizeof(long long) * epk::MAX_TRIGGERS, s->stream);
+    if (e == cudaSuccess) {
+        epk::launch_state_fill(model, s->nc, s->nc_pad, s->d_ctype, d_y0, s->d_y, s->d_vm[0], s->d_tact, s->stream);
+        s->launches++;
+        e = cudaMemcpyAsync(s->d_vm[1], s->d_vm[0], sizeof(double) * s->nc_pad, cudaMemcpyDeviceToDevice, s->stream);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
     if (d_y0) cudaFree(d_y0);
+    EP_CUDA(s, e);
     return EP_OK;
 }
 
@@ -418,15 +467,14 @@ int ep_step(ep_sim* s, int64_t n_steps, double dt) {
         }
         EP_CUDA(s, cudaStreamSynchronize(s->stream));
         EP_CUDA(s, cudaMemcpy(s->d_trig_par, par, sizeof(par), cudaMemcpyHostToDevice));
-        if (s->graph) { cudaGraphExecDestroy(s->graph); s->graph = nullptr; }
+        drop_graphs(s);
         s->trig_dirty = false;
     }
     int64_t left = n_steps;
     while (left > 0) {
         if (!s->profiling && left >= GRAPH_STEPS) {
             // replay path: one descriptor upload + one graph launch per GRAPH_STEPS time steps
-            if (!s->graph || s->graph_dt != dt || s->graph_model != s->model || s->graph_cur != s->cur ||
-                s->graph_stream != s->stream) {
+            if (!s->graph[s->cur] || s->graph_dt != dt || s->graph_model != s->model || s->graph_stream != s->stream) {
                 if ((rc = build_graph(s, dt))) return rc;
             }
             // pinned ring slot: wait (normally not at all) until the copy that last used it has run, refill, enqueue the
@@ -439,7 +487,7 @@ int ep_step(ep_sim* s, int64_t n_steps, double dt) {
             EP_CUDA(s, cudaMemcpyAsync(s->d_desc, h, sizeof(epk::StepDesc) * GRAPH_STEPS, cudaMemcpyHostToDevice, s->stream));
             EP_CUDA(s, cudaEventRecord(s->desc_ev[r], s->stream));
             s->desc_ev_used[r] = true;
-            EP_CUDA(s, cudaGraphLaunch(s->graph, s->stream));
+            EP_CUDA(s, cudaGraphLaunch(s->graph[s->cur], s->stream));
             s->launches += 2 * GRAPH_STEPS;
             s->step += GRAPH_STEPS;
             left -= GRAPH_STEPS;
@@ -456,8 +504,8 @@ int ep_step(ep_sim* s, int64_t n_steps, double dt) {
             epk::launch_cell_step(s->dm, s->model, a, s->stream);
             if ((rc = profile_event(s))) return rc;
         } else {
-            epk::launch_node_gather(s->dm, a.vm_cur, s->d_vn, s->stream);
-            epk::launch_cell_step(s->dm, s->model, a, s->stream);
+            epk::launch_node_gather(s->dm, a.vm_cur, s->d_vn, s->stream, s->pdl);
+            epk::launch_cell_step(s->dm, s->model, a, s->stream, s->pdl);
         }
         s->launches += 2;
         s->cur ^= 1;
@@ -504,7 +552,101 @@ int ep_write_state(ep_sim* s, int var, const double* in) {
 int ep_activation_times(ep_sim* s, double* out) {
     if (!s || !out) return fail(EP_ERR_ARG, "null argument");
     if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
+    int rc = use_device(s);
+    if (rc) return rc;
     return read_back(s, s->d_tact, out);
+}
+
+int ep_write_activation_times(ep_sim* s, const double* in) {
+    if (!s || !in) return fail(EP_ERR_ARG, "null argument");
+    if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
+    int rc = use_device(s);
+    if (rc) return rc;
+    EP_CUDA(s, cudaMemcpyAsync(s->d_tmp, in, sizeof(double) * s->nc, cudaMemcpyHostToDevice, s->stream));
+    epk::launch_gather_f64(s->nc, s->d_tmp, s->d_perm, s->d_tact, s->stream);
+    s->launches++;
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    return EP_OK;
+}
+
+int ep_set_step_count(ep_sim* s, int64_t step_count, double dt_ms) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
+    if (step_count < 0) return fail(EP_ERR_ARG, "step_count must be non-negative");
+    if (step_count > 0 && (!(dt_ms > 0.0) || !std::isfinite(dt_ms))) return fail(EP_ERR_ARG, "dt must be positive");
+    s->step = step_count;
+    s->dt = step_count > 0 ? dt_ms : 0.0;
+    return EP_OK;
+}
+
+int ep_trigger_restore(ep_sim* s, int trigger, double t_fire_ms) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    if (trigger < 0 || trigger >= epk::MAX_TRIGGERS) return fail(EP_ERR_ARG, "trigger index out of range");
+    if (t_fire_ms >= 0.0 && !(s->dt > 0.0)) return fail(EP_ERR_STATE, "set the clock first (ep_set_step_count)");
+    int rc = use_device(s);
+    if (rc) return rc;
+    const long long n1 = t_fire_ms < 0.0 ? -1 : (long long)std::llround(t_fire_ms / s->dt);
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    EP_CUDA(s, cudaMemcpy(s->d_trig_fire + trigger, &n1, sizeof(n1), cudaMemcpyHostToDevice));
+    return EP_OK;
+}
+
+// Two-slot pipeline between the I/O stream (copies) and the sim's stream (permutation kernels): row k is copied while
+// row k-1 is permuted; nothing synchronises with the host until the last row.
+static int io_setup(ep_sim* s) {
+    if (s->io_stream) return EP_OK;
+    EP_CUDA(s, cudaStreamCreateWithFlags(&s->io_stream, cudaStreamNonBlocking));
+    for (int k = 0; k < 2; ++k) {
+        EP_CUDA(s, cudaEventCreateWithFlags(&s->io_copied[k], cudaEventDisableTiming));
+        EP_CUDA(s, cudaEventCreateWithFlags(&s->io_consumed[k], cudaEventDisableTiming));
+    }
+    EP_CUDA(s, cudaEventCreateWithFlags(&s->io_fence, cudaEventDisableTiming));
+    return EP_OK;
+}
+
+int ep_write_states(ep_sim* s, const double* in) {
+    if (!s || !in) return fail(EP_ERR_ARG, "null argument");
+    if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
+    int rc = use_device(s);
+    if (rc || (rc = io_setup(s))) return rc;
+    double* stage[2] = {s->d_tmp, s->d_tmp2};
+    EP_CUDA(s, cudaEventRecord(s->io_fence, s->stream));          // the staging buffers may still be in use by the sim's stream
+    EP_CUDA(s, cudaStreamWaitEvent(s->io_stream, s->io_fence, 0));
+    for (int k = 0; k < s->S; ++k) {
+        const int b = k & 1;
+        if (k >= 2) EP_CUDA(s, cudaStreamWaitEvent(s->io_stream, s->io_consumed[b], 0));
+        EP_CUDA(s, cudaMemcpyAsync(stage[b], in + (size_t)k * s->nc, sizeof(double) * s->nc, cudaMemcpyHostToDevice, s->io_stream));
+        EP_CUDA(s, cudaEventRecord(s->io_copied[b], s->io_stream));
+        EP_CUDA(s, cudaStreamWaitEvent(s->stream, s->io_copied[b], 0));
+        if (k == 0) epk::launch_gather_f64(s->nc, stage[b], s->d_perm, s->d_vm[s->cur], s->stream);
+        else epk::launch_state_row_put(s->nc, stage[b], s->d_perm, s->S, k, s->d_y, s->stream);
+        s->launches++;
+        EP_CUDA(s, cudaEventRecord(s->io_consumed[b], s->stream));
+    }
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    return EP_OK;
+}
+
+int ep_read_states(ep_sim* s, double* out) {
+    if (!s || !out) return fail(EP_ERR_ARG, "null argument");
+    if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
+    int rc = use_device(s);
+    if (rc || (rc = io_setup(s))) return rc;
+    double* stage[2] = {s->d_tmp, s->d_tmp2};
+    for (int k = 0; k < s->S; ++k) {
+        const int b = k & 1;
+        if (k >= 2) EP_CUDA(s, cudaStreamWaitEvent(s->stream, s->io_consumed[b], 0));
+        if (k == 0) epk::launch_gather_f64(s->nc, s->d_vm[s->cur], s->d_inv, stage[b], s->stream);
+        else epk::launch_state_row_get(s->nc, s->d_y, s->S, k, s->d_inv, stage[b], s->stream);
+        s->launches++;
+        EP_CUDA(s, cudaEventRecord(s->io_copied[b], s->stream));
+        EP_CUDA(s, cudaStreamWaitEvent(s->io_stream, s->io_copied[b], 0));
+        EP_CUDA(s, cudaMemcpyAsync(out + (size_t)k * s->nc, stage[b], sizeof(double) * s->nc, cudaMemcpyDeviceToHost, s->io_stream));
+        EP_CUDA(s, cudaEventRecord(s->io_consumed[b], s->io_stream));
+    }
+    EP_CUDA(s, cudaStreamSynchronize(s->io_stream));
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    return EP_OK;
 }
 
 int ep_apply_diffusion(ep_sim* s, const double* v, double* D) {
@@ -537,10 +679,20 @@ int ep_stable_dt(ep_sim* s, double* dt_max) {
     } catch (const std::bad_alloc&) {
         return fail(EP_ERR_NOMEM, "host allocation failed");
     }
-    double rho = 0.0;
-    const int iters = 300;
-    for (int it = 0; it < iters; ++it) {
+    // |Bx_k| with |x_k| = 1 settles at rho; read it back every CHECK iterations and stop once it has stopped moving
+    // (relative change below 1e-4 over CHECK iterations) or after MAX_ITERS.
+    double rho = 0.0, rho_prev = 0.0;
+    const int MAX_ITERS = 300, CHECK = 20;
+    for (int it = 0; it < MAX_ITERS; ++it) {
         epk::launch_norm2(s->nc, s->d_tmp, s->d_red, s->d_red + 1024, s->stream);
+        if (it > 0 && it % CHECK == 0) {
+            double n2 = 0.0;
+            EP_CUDA(s, cudaMemcpyAsync(&n2, s->d_red + 1024, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+            EP_CUDA(s, cudaStreamSynchronize(s->stream));
+            rho = std::sqrt(n2);
+            if (it > CHECK && std::fabs(rho - rho_prev) <= 1e-4 * rho) break;
+            rho_prev = rho;
+        }
         epk::launch_scale_by_inv_norm(s->nc, s->d_tmp, s->d_red + 1024, s->d_tmp2, s->stream);
         epk::launch_node_gather(s->dm, s->d_tmp2, s->d_vn, s->stream);
         epk::launch_diffusion_only(s->dm, s->d_tmp2, s->d_vn, s->d_tmp, s->stream);
@@ -551,7 +703,7 @@ int ep_stable_dt(ep_sim* s, double* dt_max) {
     double n2 = 0.0;
     EP_CUDA(s, cudaMemcpyAsync(&n2, s->d_red + 1024, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
     EP_CUDA(s, cudaStreamSynchronize(s->stream));
-    rho = std::sqrt(n2);
+    rho = std::max(rho, std::sqrt(n2));
     if (!(rho > 0.0) || !std::isfinite(rho)) return fail(EP_ERR_NUMERIC, "power iteration failed");
     *dt_max = 2.0 / rho;
     return EP_OK;
@@ -607,15 +759,22 @@ int ep_mean_vm(ep_sim* s, double* vbar) {
 int ep_check_finite(ep_sim* s, int* all_finite) {
     if (!s || !all_finite) return fail(EP_ERR_ARG, "null argument");
     if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
-    epk::launch_count_nonfinite(s->nc, s->d_vm[s->cur], s->d_red, s->d_red + 1024, s->stream);
-    s->launches += 2;
-    double bad = 0.0;
-    EP_CUDA(s, cudaMemcpyAsync(&bad, s->d_red + 1024, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    int rc = use_device(s);
+    if (rc) return rc;
+    unsigned long long* d_cnt = reinterpret_cast<unsigned long long*>(s->d_red);
+    EP_CUDA(s, cudaMemsetAsync(d_cnt, 0, 2 * sizeof(unsigned long long), s->stream));
+    epk::launch_state_scan(s->model, s->nc, s->d_vm[s->cur], s->d_y, d_cnt, s->stream);
+    s->launches += 1;
+    unsigned long long cnt[2] = {0, 0};
+    EP_CUDA(s, cudaMemcpyAsync(cnt, d_cnt, sizeof(cnt), cudaMemcpyDeviceToHost, s->stream));
     EP_CUDA(s, cudaStreamSynchronize(s->stream));
-    *all_finite = (bad == 0.0);
-    if (bad != 0.0) {
+    *all_finite = (cnt[0] == 0 && cnt[1] == 0);
+    if (!*all_finite) {
         s->sticky = EP_ERR_NUMERIC;
-        return fail(EP_ERR_NUMERIC, "non-finite membrane potential (explicit step unstable? see ep_stable_dt)");
+        char msg[200];
+        std::snprintf(msg, sizeof msg, "%llu non-finite state values, %llu non-positive concentrations (explicit step unstable? "
+                      "see ep_stable_dt)", cnt[0], cnt[1]);
+        return fail(EP_ERR_NUMERIC, msg);
     }
     return EP_OK;
 }

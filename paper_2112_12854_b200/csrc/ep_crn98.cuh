@@ -75,7 +75,7 @@ __device__ __forceinline__ void crn_rush_larsen_slots(double* col, double* ycol,
         double e[EXP_W];
 #pragma unroll
         for (int j = 0; j < EXP_W; ++j) e[j] = col[(g + j) * BLOCK];
-        ep_exp_wide<EXP_W>(e);
+        ep_exp2_wide<EXP_W>(e);
 #pragma unroll
         for (int j = 0; j < EXP_W; ++j) {
             if (g + j < N_RLB) {
@@ -93,6 +93,7 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
                                            Issue issue_gather, Finish finish_gather, double* col) {
     using namespace crn;
     const double vg = ep_clamp(v, -250.0, 250.0);   // argument of every transcendental
+    const double dtl = dt * L2E;                    // Rush-Larsen exponents in base-2 units (the primitive is 2^x)
     const double Nai = ycol[C_NAI * stride], Ki = ycol[C_KI * stride], Cai = ycol[C_CAI * stride],
                  Caup = ycol[C_CAUP * stride], Carel = ycol[C_CAREL * stride];
     // The ten gates of the rolled Rush-Larsen loop are copied into shared memory asynchronously (no registers held); they
@@ -118,50 +119,50 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
     const double xb = fma(vg, CK(1.0 / 5.1237), CK(-3.3328 / 5.1237));
     const double xd = fma(vg, CK(1.0 / 9.0), CK(-19.9 / 9.0));
     const double dx = fma(vg, CK(-1.0 / 6.24), CK(-10.0 / 6.24));
-    col[A_E17 * BLOCK] = vg * CK(1.0 / 17.0);
-    col[A_W * BLOCK] = vg * CK(0.05 * FRT);
-    col[A_X1 * BLOCK] = x1;
-    col[A_BM * BLOCK] = vg * CK(-1.0 / 11.0);
-    col[A_K1 * BLOCK] = fma(vg, CK(0.07), CK(0.07 * 80.0));
-    col[A_OA1 * BLOCK] = fma(vg, CK(-1.0 / 8.5), CK(-10.0 / 8.5));
-    col[A_OA2 * BLOCK] = fma(vg, CK(-1.0 / 59.0), CK(30.0 / 59.0));
-    col[A_OAI * BLOCK] = fma(vg, CK(-1.0 / 17.54), CK(-20.47 / 17.54));
-    col[A_UAI * BLOCK] = fma(vg, CK(-1.0 / 9.6), CK(-30.3 / 9.6));
-    col[A_OI1 * BLOCK] = fma(vg, CK(1.0 / 10.95), CK(113.7 / 10.95));
-    col[A_OI2 * BLOCK] = fma(vg, CK(-1.0 / 7.44), CK(-1.26 / 7.44));
-    col[A_OII * BLOCK] = fma(vg, CK(1.0 / 5.3), CK(43.1 / 5.3));
-    col[A_UI1 * BLOCK] = fma(vg, CK(-1.0 / 28.0), CK(185.0 / 28.0));
-    col[A_UI2 * BLOCK] = fma(vg, 0.0625, CK(-158.0 / 16.0));
-    col[A_UII * BLOCK] = fma(vg, CK(1.0 / 27.48), CK(-99.45 / 27.48));
-    col[A_KUR * BLOCK] = fma(vg, CK(-1.0 / 13.0), CK(15.0 / 13.0));
-    col[A_KR * BLOCK] = fma(vg, CK(1.0 / 22.4), CK(15.0 / 22.4));
-    col[A_E5M * BLOCK] = vg * CK(-0.2);
-    col[A_XB * BLOCK] = xb;
-    col[A_XRI * BLOCK] = fma(vg, CK(-1.0 / 6.5), CK(-14.1 / 6.5));
-    col[A_XD * BLOCK] = xd;
-    col[A_XSI * BLOCK] = fma(vg, CK(-1.0 / 12.7), CK(19.9 / 12.7));
-    col[A_DX * BLOCK] = dx;
-    col[A_DI * BLOCK] = fma(vg, -0.125, -1.25);
-    col[A_FG * BLOCK] = (vg + 10.0) * (vg + 10.0) * CK(-0.0337 * 0.0337);
-    col[A_FI * BLOCK] = fma(vg, CK(1.0 / 6.9), CK(28.0 / 6.9));
+    col[A_E17 * BLOCK] = vg * CK(L2E / 17.0);
+    col[A_W * BLOCK] = vg * CK(0.05 * FRT * L2E);
+    col[A_X1 * BLOCK] = x1 * CK(L2E);
+    col[A_BM * BLOCK] = vg * CK(-L2E / 11.0);
+    col[A_K1 * BLOCK] = fma(vg, CK(0.07 * L2E), CK(0.07 * 80.0 * L2E));
+    col[A_OA1 * BLOCK] = fma(vg, CK(-L2E / 8.5), CK(-10.0 * L2E / 8.5));
+    col[A_OA2 * BLOCK] = fma(vg, CK(-L2E / 59.0), CK(30.0 * L2E / 59.0));
+    col[A_OAI * BLOCK] = fma(vg, CK(-L2E / 17.54), CK(-20.47 * L2E / 17.54));
+    col[A_UAI * BLOCK] = fma(vg, CK(-L2E / 9.6), CK(-30.3 * L2E / 9.6));
+    col[A_OI1 * BLOCK] = fma(vg, CK(L2E / 10.95), CK(113.7 * L2E / 10.95));
+    col[A_OI2 * BLOCK] = fma(vg, CK(-L2E / 7.44), CK(-1.26 * L2E / 7.44));
+    col[A_OII * BLOCK] = fma(vg, CK(L2E / 5.3), CK(43.1 * L2E / 5.3));
+    col[A_UI1 * BLOCK] = fma(vg, CK(-L2E / 28.0), CK(185.0 * L2E / 28.0));
+    col[A_UI2 * BLOCK] = fma(vg, CK(L2E / 16.0), CK(-158.0 * L2E / 16.0));
+    col[A_UII * BLOCK] = fma(vg, CK(L2E / 27.48), CK(-99.45 * L2E / 27.48));
+    col[A_KUR * BLOCK] = fma(vg, CK(-L2E / 13.0), CK(15.0 * L2E / 13.0));
+    col[A_KR * BLOCK] = fma(vg, CK(L2E / 22.4), CK(15.0 * L2E / 22.4));
+    col[A_E5M * BLOCK] = vg * CK(-0.2 * L2E);
+    col[A_XB * BLOCK] = xb * CK(L2E);
+    col[A_XRI * BLOCK] = fma(vg, CK(-L2E / 6.5), CK(-14.1 * L2E / 6.5));
+    col[A_XD * BLOCK] = xd * CK(L2E);
+    col[A_XSI * BLOCK] = fma(vg, CK(-L2E / 12.7), CK(19.9 * L2E / 12.7));
+    col[A_DX * BLOCK] = dx * CK(L2E);
+    col[A_DI * BLOCK] = fma(vg, CK(-0.125 * L2E), CK(-1.25 * L2E));
+    col[A_FG * BLOCK] = (vg + 10.0) * (vg + 10.0) * CK(-0.0337 * 0.0337 * L2E);
+    col[A_FI * BLOCK] = fma(vg, CK(L2E / 6.9), CK(28.0 * L2E / 6.9));
     if (hi) {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-1.0 / 11.1), CK(-10.66 / 11.1));
-        col[(A_HJ0 + 1) * BLOCK] = vg * CK(-2.535e-7);
+        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
+        col[(A_HJ0 + 1) * BLOCK] = vg * CK(-2.535e-7 * L2E);
 #pragma unroll
         for (int k = 2; k < 8; ++k) col[(A_HJ0 + k) * BLOCK] = 0.0;
     } else {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-1.0 / 6.8), CK(-80.0 / 6.8));
-        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.079);
-        col[(A_HJ0 + 2) * BLOCK] = vg * CK(0.35);
-        col[(A_HJ0 + 3) * BLOCK] = vg * CK(0.2444);
-        col[(A_HJ0 + 4) * BLOCK] = vg * CK(-0.04391);
-        col[(A_HJ0 + 5) * BLOCK] = fma(vg, CK(0.311), CK(0.311 * 79.23));
-        col[(A_HJ0 + 6) * BLOCK] = vg * CK(-0.01052);
-        col[(A_HJ0 + 7) * BLOCK] = fma(vg, CK(-0.1378), CK(-0.1378 * 40.14));
+        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));
+        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.079 * L2E);
+        col[(A_HJ0 + 2) * BLOCK] = vg * CK(0.35 * L2E);
+        col[(A_HJ0 + 3) * BLOCK] = vg * CK(0.2444 * L2E);
+        col[(A_HJ0 + 4) * BLOCK] = vg * CK(-0.04391 * L2E);
+        col[(A_HJ0 + 5) * BLOCK] = fma(vg, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
+        col[(A_HJ0 + 6) * BLOCK] = vg * CK(-0.01052 * L2E);
+        col[(A_HJ0 + 7) * BLOCK] = fma(vg, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
     }
-    col[A_TFCA * BLOCK] = dt * -0.5;      // tau_fCa = 2 ms
-    col[A_TU * BLOCK] = dt * -0.125;      // tau_u = 8 ms
-    ep_exp_slots<N_EXPA, BLOCK, EXP_W>(col);
+    col[A_TFCA * BLOCK] = dtl * -0.5;     // tau_fCa = 2 ms
+    col[A_TU * BLOCK] = dtl * -0.125;     // tau_u = 8 ms
+    ep_exp2_slots<N_EXPA, BLOCK, EXP_W>(col);
     const double dv_diff = finish_gather();   // the gathers have landed during the batch: 12 values -> 1
     ep_cp_async_wait();                       // so have the gate values: products for the currents
     double gto3, gkur3, xr, xs2, gcal, uvw;
@@ -255,13 +256,13 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
             rj = num * ep_rcp(D1 * D2);
             j_inf = N1 * D2 * ep_rcp(num);
         }
-        e4[0] = fmax(Fn * CK(-1.0 / 13.67e-16) + CK(3.4175e-13 / 13.67e-16), -700.0);
-        e4[0] = fmin(e4[0], 700.0);
-        e4[1] = fmax(-dt * rm, -700.0);
-        e4[2] = fmax(-dt * rh, -700.0);
-        e4[3] = fmax(-dt * rj, -700.0);
+        e4[0] = fmax(Fn * CK(-L2E / 13.67e-16) + CK(3.4175e-13 * L2E / 13.67e-16), -1000.0);
+        e4[0] = fmin(e4[0], 1000.0);
+        e4[1] = fmax(-dtl * rm, -1000.0);
+        e4[2] = fmax(-dtl * rh, -1000.0);
+        e4[3] = fmax(-dtl * rj, -1000.0);
     }
-    ep_exp_wide<4>(e4);
+    ep_exp2_wide<4>(e4);
     ycol[C_M * stride] = fma(m - m_inf, e4[1], m_inf);
     ycol[C_H * stride] = fma(h - h_inf, e4[2], h_inf);
     ycol[C_J * stride] = fma(j - j_inf, e4[3], j_inf);
@@ -322,7 +323,7 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
     }
 #pragma unroll
     for (int g = 0; g < N_RLB; ++g) {
-        col[g * BLOCK] = fmax(-dt * rate[g], -700.0);
+        col[g * BLOCK] = fmax(-dtl * rate[g], -1000.0);
         col[(B_INF0 + g) * BLOCK] = inf[g];
     }
     col[10 * BLOCK] = 0.0;

@@ -14,6 +14,17 @@ namespace epk {
 
 namespace {
 
+// Programmatic dependent launch (PDL): the two step kernels are launched with programmatic stream serialisation, so the
+// next kernel's blocks may start while the previous kernel drains its last wave.  pdl_wait() blocks until the previous
+// kernel has completed and its writes are visible; pdl_launch_dependents() lets the next kernel in the stream start its
+// prologue.  Both are no-ops for a kernel launched without the attribute.  Order of the chain cell(n-1) -> node(n) ->
+// cell(n): node(n) waits first and only then releases cell(n), so cell(n) may read everything cell(n-1) wrote (state rows,
+// Vm) as soon as it starts; it waits only before it touches the node values v_n that node(n) is still writing.  cell(n)
+// releases node(n+1) at once: that kernel reads nothing but its slice pointers before its own wait, and it overwrites v_n
+// only after cell(n) has completed.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 constexpr int CELL_THREADS = 128;   // = the tile of the tile-major layout
 __host__ __device__ inline int64_t tile_index(int64_t i, int64_t k, int64_t rows) {
     return ((i / CELL_THREADS) * rows + k) * CELL_THREADS + i % CELL_THREADS;
@@ -38,8 +49,11 @@ __global__ void __launch_bounds__(NODE_THREADS) node_gather_kernel(int64_t nn, i
     const int sl = warp / NODE_PARTS, p = warp % NODE_PARTS;
     const int64_t slice = (int64_t)blockIdx.x * NODE_SLICES_PER_BLOCK + sl;
     double acc0 = 0.0, acc1 = 0.0;
+    int64_t beg = 0, end = 0;
+    if (slice < n_slices) { beg = __ldg(slice_ptr + slice); end = __ldg(slice_ptr + slice + 1); }
+    pdl_wait();                  // Vm of this time level is complete (previous cell kernel); v_n is free to overwrite
+    pdl_launch_dependents();     // the cell kernel may start its state loads now
     if (slice < n_slices) {
-        const int64_t beg = __ldg(slice_ptr + slice), end = __ldg(slice_ptr + slice + 1);
         int64_t q = beg + 32 * p + lane;
         const int64_t step = 32 * NODE_PARTS;
         for (; q + step < end; q += 2 * step) {   // two independent gathers in flight per trip
@@ -104,6 +118,7 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     constexpr int NSLOTS = MSLOTS + (CF_SMEM ? 12 : 0);
     __shared__ double xs[NSLOTS][CELL_THREADS];
     const int64_t i = (int64_t)blockIdx.x * CELL_THREADS + threadIdx.x;
+    pdl_launch_dependents();
     if (i >= nc) return;
     const double v_old = a.vm_cur[i];
     // tile-major tables: every row of this block's tile is at a compile-time offset from these three pointers
@@ -125,9 +140,10 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     double gv[12];
     auto issue_gather = [&]() {
 #pragma unroll
-        for (int m = 0; m < 8; ++m) gv[m] = a.vn[id[m]];
-#pragma unroll
         for (int j = 0; j < 4; ++j) gv[8 + j] = a.vm_cur[id[8 + j]];
+        pdl_wait();              // the node kernel of this step has finished writing v_n
+#pragma unroll
+        for (int m = 0; m < 8; ++m) gv[m] = a.vn[id[m]];
     };
     auto finish_gather = [&]() {   // dv = sum_m a_m v_n[node_m] + sum_j b_j (v[nbr_j] - v_c)   [mV/ms]
         double accn = 0.0, accm = 0.0, accc = 0.0;
@@ -246,6 +262,29 @@ __global__ void __launch_bounds__(1024) reduce_final_kernel(const double* __rest
     }
     if (threadIdx.x == 0) out[0] = sh[0];
 }
+// Failure detection over the WHOLE state (not only Vm): counts[0] += non-finite entries of Vm and of state rows 1..S-1,
+// counts[1] += concentrations (rows conc0..S-1) that are not positive -- forward Euler at an unstable dt can drive them
+// through zero, after which the logarithms of the reversal potentials mean nothing.  Integer counts: atomics are exact.
+__global__ void __launch_bounds__(256) state_scan_kernel(int S, int conc0, int64_t nc, const double* __restrict__ vm,
+                                                          const double* __restrict__ y,
+                                                          unsigned long long* __restrict__ counts) {
+    unsigned bad = 0, nonpos = 0;
+    for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < nc; i += (int64_t)gridDim.x * 256) {
+        bad += !isfinite(vm[i]);
+        for (int k = 1; k < S; ++k) {
+            const double v = y[tile_index(i, k, S)];
+            bad += !isfinite(v);
+            if (k >= conc0) nonpos += !(v > 0.0);
+        }
+    }
+    bad = __reduce_add_sync(0xffffffffu, bad);
+    nonpos = __reduce_add_sync(0xffffffffu, nonpos);
+    if ((threadIdx.x & 31) == 0) {
+        if (bad) atomicAdd(counts, (unsigned long long)bad);
+        if (nonpos) atomicAdd(counts + 1, (unsigned long long)nonpos);
+    }
+}
+
 __global__ void scale_by_inv_norm_kernel(int64_t n, const double* __restrict__ x, const double* __restrict__ norm2,
                                          double* __restrict__ out) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -256,7 +295,7 @@ __global__ void math_eval_kernel(int fn, int64_t n, const double* __restrict__ x
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     double v[1] = {x[i]};
-    if (fn == 0) ep_exp_wide<1>(v);
+    if (fn == 0) ep_exp2_wide<1>(v);
     else if (fn == 1) ep_log_wide<1>(v);
     else if (fn == 2) v[0] = ep_rcp(v[0]);
     else v[0] = ep_rsqrt(v[0]);
@@ -273,15 +312,27 @@ void launch_math_eval(int fn, int64_t n, const double* x, double* y, cudaStream_
 
 int model_n_states(int model) { return model == 0 ? (int)TP06_S : (model == 1 ? (int)CRN_S : -1); }
 
-void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaStream_t s) {
-    const unsigned grid = blocks_for(m.n_slices, NODE_SLICES_PER_BLOCK);
-    node_gather_kernel<<<grid, NODE_THREADS, 0, s>>>(m.nn, m.n_slices, m.slice_ptr, m.nidx, m.nw, vm, vn);
+// kernel launch with the programmatic-stream-serialisation attribute (see the PDL note at the top of this file)
+template <class... KArgs, class... Args>
+void launch_pdl(void (*kernel)(KArgs...), unsigned grid, unsigned block, cudaStream_t s, bool pdl, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
-void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStream_t s) {
+void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaStream_t s, bool pdl) {
+    const unsigned grid = blocks_for(m.n_slices, NODE_SLICES_PER_BLOCK);
+    launch_pdl(node_gather_kernel, grid, NODE_THREADS, s, pdl, m.nn, m.n_slices, m.slice_ptr, m.nidx, m.nw, vm, vn);
+}
+
+void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStream_t s, bool pdl) {
     const unsigned grid = blocks_for(m.nc, CELL_THREADS);
-    if (model == 0) cell_step_kernel<0><<<grid, CELL_THREADS, 0, s>>>(m.nc, m.cidx, m.ccoef, a);
-    else cell_step_kernel<1><<<grid, CELL_THREADS, 0, s>>>(m.nc, m.cidx, m.ccoef, a);
+    if (model == 0) launch_pdl(cell_step_kernel<0>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
+    else launch_pdl(cell_step_kernel<1>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
 }
 
 void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* vn, double* out, cudaStream_t s) {
@@ -315,6 +366,11 @@ void launch_count_nonfinite(int64_t n, const double* x, double* partial, double*
 void launch_weighted_sum(int64_t n, const double* x, const double* w, double* partial, double* out, cudaStream_t s) {
     reduce_partial_kernel<2><<<1024, 256, 0, s>>>(n, x, w, partial);
     reduce_final_kernel<<<1, 1024, 0, s>>>(partial, out);
+}
+void launch_state_scan(int model, int64_t nc, const double* vm, const double* y, unsigned long long* counts,
+                       cudaStream_t s) {
+    const int S = model_n_states(model), conc0 = (model == 0) ? (int)Y_CAI : (int)C_NAI;
+    state_scan_kernel<<<1184, 256, 0, s>>>(S, conc0, nc, vm, y, counts);
 }
 void launch_scale_by_inv_norm(int64_t n, const double* x, const double* norm2, double* out, cudaStream_t s) {
     scale_by_inv_norm_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, x, norm2, out);

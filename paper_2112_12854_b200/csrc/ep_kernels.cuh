@@ -48,9 +48,10 @@ struct StepArgs {
 };
 
 // S1 of SURVEY 8(a): v_n = sum_k w_nk v_k
-void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaStream_t s);
+// pdl: launch with programmatic stream serialisation (the kernel's prologue may overlap the previous kernel's tail)
+void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaStream_t s, bool pdl = false);
 // S2..S9 fused: diffusion gather + stimulus + cell model + RL/FE updates + Vm write + activation record
-void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStream_t s);
+void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStream_t s, bool pdl = false);
 // diagnostics: out[i] = D_c/(chi Cm) [mV/ms] from vm and vn
 void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* vn, double* out, cudaStream_t s);
 // fill y rows with one state vector per cell type; y0 is a DEVICE pointer [n_types*S]; NULL = built-in rest state
@@ -66,6 +67,9 @@ void launch_norm2(int64_t n, const double* x, double* partial /*[1024]*/, double
 void launch_scale_by_inv_norm(int64_t n, const double* x, const double* norm2, double* out, cudaStream_t s);
 // out[0] = sum_i w[i] x[i], fixed summation tree (deterministic)
 void launch_weighted_sum(int64_t n, const double* x, const double* w, double* partial, double* out, cudaStream_t s);
+// counts[0] += non-finite entries of Vm and all state rows, counts[1] += non-positive concentrations (device, zeroed by caller)
+void launch_state_scan(int model, int64_t nc, const double* vm, const double* y, unsigned long long* counts,
+                       cudaStream_t s);
 void launch_count_nonfinite(int64_t n, const double* x, double* partial, double* out, cudaStream_t s);
 
 int model_n_states(int model);

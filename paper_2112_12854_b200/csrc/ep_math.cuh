@@ -11,20 +11,36 @@
 //     them by their exponentials; the loop body exists once in the kernel and its constants stay in uniform registers;
 //   * IEEE division is ~10 fp64 instructions plus a slow-path call  ->  ep_rcp: MUFU.RCP64H seed + one third-order
 //     step (3 DFMA), arguments are finite, normal and far from the ends of the exponent range at every call site.
-// Accuracy, measured on the GPU by tests/test_gpu_math.py through ep_math_eval(): exp <= 1 ulp on [-700, 700]
-// (polynomial error 2e-17), log <= 1 ulp where |log x| > 1 (the concentrations it is used on) and <= 2.5 ulp near
+//   * every exponential of the cell models has an argument of the form (compile-time constant) x (run-time value), so the
+//     factor log2(e) is folded into those constants and the primitive is 2^x: the reduction x = k + r is one exact
+//     subtraction instead of the two-constant Cody-Waite pair of a natural exponential (one fp64 instruction less per
+//     call, 36 calls per TP06 cell-step).
+// Accuracy, measured on the GPU by tests/test_gpu_math.py through ep_math_eval(): 2^x <= 1 ulp on [-1000, 1000]
+// (polynomial error 8e-18), log <= 1 ulp where |log x| > 1 (the concentrations it is used on) and <= 2.5 ulp near
 // x = 1, rcp <= 1 ulp, rsqrt <= 2 ulp, hence a*rcp(b) <= 2 ulp.  No lookup tables (north_star: "precomputed-free exp paths").
 #pragma once
 #include <cstdint>
 
 namespace epk {
 
-// e^r = 1 + r + r^2 q(r) on |r| <= ln2/2; q = degree-9 Chebyshev interpolant of (e^r - 1 - r)/r^2
-// (max relative error of the reconstructed e^r: 1.6e-17, computed in 60-digit arithmetic).
-__constant__ double EXP_Q[10] = {0.5000000000000001,     0.16666666666666669,   0.04166666666662396,
-                                 0.00833333333333005,    0.0013888888917294928, 0.00019841269863116068,
-                                 2.48015211698282e-05,   2.755726836300438e-06, 2.762014840966706e-07,
-                                 2.5100431608666542e-08};
+// 2^r = 1 + r P(r) on |r| <= 1/2; P = degree-10 Chebyshev interpolant of (2^r - 1)/r (max relative error of the
+// reconstructed 2^r: 8.4e-18, computed in 80-digit arithmetic).  EP_EXP2_DEG = 9 selects the degree-9 interpolant
+// (5.8e-16, one instruction less per call); it is an experiment switch, the shipped build uses 10.
+#ifndef EP_EXP2_DEG
+#define EP_EXP2_DEG 10
+#endif
+constexpr double L2E = 1.4426950408889634;   // log2(e): folded into the compile-time slopes of every exponent
+#if EP_EXP2_DEG == 10
+__constant__ double EXP2_P[11] = {0.6931471805599453,     0.24022650695910097,   0.0555041086648216,
+                                  0.009618129107606888,   0.0013333558146416936, 0.0001540353044173605,
+                                  1.525273382983612e-05,  1.321544258792169e-06, 1.0178062445845774e-07,
+                                  7.072585949269223e-09,  4.4549605981865186e-10};
+#else
+__constant__ double EXP2_P[10] = {0.6931471805599462,     0.24022650695910075,   0.05550410866465167,
+                                  0.009618129107618665,   0.0013333558200794592, 0.00015403530424776529,
+                                  1.5252672924850737e-05, 1.3215451633221434e-06, 1.0205905413765595e-07,
+                                  7.070977866508138e-09};
+#endif
 // log m = 2 s (1 + z/3 + z^2/5 + ... + z^9/19), s = (m-1)/(m+1), z = s^2 <= 0.0295 (next term z^10/21 < 2.4e-17)
 __constant__ double LOG_C[9] = {1.0 / 3.0, 1.0 / 5.0, 1.0 / 7.0, 1.0 / 9.0, 1.0 / 11.0, 1.0 / 13.0, 1.0 / 15.0,
                                 1.0 / 17.0, 1.0 / 19.0};
@@ -46,19 +62,16 @@ __device__ __forceinline__ double ep_rsqrt(double x) {
     return fma(y, t, y);
 }
 
-// exp of a finite argument with |x| <= 700 (callers clamp); no overflow / underflow / NaN handling
-__device__ __forceinline__ double ep_exp_core(double x) {
+// 2^x of a finite argument with |x| <= 1000 (callers clamp); no overflow / underflow / NaN handling
+__device__ __forceinline__ double ep_exp2_core(double x) {
     const double shift = 6755399441055744.0;                  // 2^52 + 2^51: round-to-nearest-integer trick
-    const double t = fma(x, 1.4426950408889634, shift);
+    const double t = x + shift;
     const int k = __double2loint(t);
-    const double kd = t - shift;
-    double r = fma(kd, -6.93147180369123816490e-01, x);       // ln2 high part (low bits zero: kd*hi is exact)
-    r = fma(kd, -1.90821492927058770002e-10, r);              // ln2 low part
-    double q = EXP_Q[9];
+    const double r = x - (t - shift);                         // exact: |r| <= 1/2
+    double q = EXP2_P[EP_EXP2_DEG];
 #pragma unroll
-    for (int i = 8; i >= 0; --i) q = fma(q, r, EXP_Q[i]);
-    double p = fma(r, q, 1.0);
-    p = fma(r, p, 1.0);
+    for (int i = EP_EXP2_DEG - 1; i >= 0; --i) q = fma(q, r, EXP2_P[i]);
+    const double p = fma(r, q, 1.0);
     return __hiloint2double(__double2hiint(p) + k * 1048576, __double2loint(p));   // * 2^k via the exponent field
 }
 
@@ -83,30 +96,26 @@ __device__ __forceinline__ double ep_log_core(double x) {
     return fma(ed, 6.93147180369123816490e-01, res);
 }
 
-// W exponentials at once, written stage by stage so that the W dependency chains are interleaved in issue order
-// (the fp64 pipe needs several independent chains per warp to stay busy).  Same arithmetic as ep_exp_core.
+// W powers of two at once, written stage by stage so that the W dependency chains are interleaved in issue order
+// (the fp64 pipe needs several independent chains per warp to stay busy).  Same arithmetic as ep_exp2_core.
 template <int W>
-__device__ __forceinline__ void ep_exp_wide(double (&x)[W]) {
+__device__ __forceinline__ void ep_exp2_wide(double (&x)[W]) {
     const double shift = 6755399441055744.0;
     double t[W], r[W], q[W];
     int k[W];
 #pragma unroll
-    for (int j = 0; j < W; ++j) t[j] = fma(x[j], 1.4426950408889634, shift);
+    for (int j = 0; j < W; ++j) t[j] = x[j] + shift;
 #pragma unroll
     for (int j = 0; j < W; ++j) { k[j] = __double2loint(t[j]); t[j] -= shift; }
 #pragma unroll
-    for (int j = 0; j < W; ++j) r[j] = fma(t[j], -6.93147180369123816490e-01, x[j]);
+    for (int j = 0; j < W; ++j) r[j] = x[j] - t[j];
 #pragma unroll
-    for (int j = 0; j < W; ++j) r[j] = fma(t[j], -1.90821492927058770002e-10, r[j]);
+    for (int j = 0; j < W; ++j) q[j] = fma(EXP2_P[EP_EXP2_DEG], r[j], EXP2_P[EP_EXP2_DEG - 1]);
 #pragma unroll
-    for (int j = 0; j < W; ++j) q[j] = fma(EXP_Q[9], r[j], EXP_Q[8]);
+    for (int i = EP_EXP2_DEG - 2; i >= 0; --i) {
 #pragma unroll
-    for (int i = 7; i >= 0; --i) {
-#pragma unroll
-        for (int j = 0; j < W; ++j) q[j] = fma(q[j], r[j], EXP_Q[i]);
+        for (int j = 0; j < W; ++j) q[j] = fma(q[j], r[j], EXP2_P[i]);
     }
-#pragma unroll
-    for (int j = 0; j < W; ++j) q[j] = fma(r[j], q[j], 1.0);
 #pragma unroll
     for (int j = 0; j < W; ++j) q[j] = fma(r[j], q[j], 1.0);
 #pragma unroll
@@ -117,14 +126,14 @@ __device__ __forceinline__ void ep_exp_wide(double (&x)[W]) {
 // N must be a multiple of W.  The loops stay rolled on purpose (instruction-cache footprint).
 // n <= N (a multiple of W, the same for every lane of the warp) lets a caller skip trailing slots it does not need.
 template <int N, int BLOCK, int W>
-__device__ __forceinline__ void ep_exp_slots(double* col, int n = N) {
+__device__ __forceinline__ void ep_exp2_slots(double* col, int n = N) {
     static_assert(N % W == 0, "pad the slot list to a multiple of W");
 #pragma unroll 1
     for (int s = 0; s < n; s += W) {
         double x[W];
 #pragma unroll
         for (int j = 0; j < W; ++j) x[j] = col[(s + j) * BLOCK];
-        ep_exp_wide<W>(x);
+        ep_exp2_wide<W>(x);
 #pragma unroll
         for (int j = 0; j < W; ++j) col[(s + j) * BLOCK] = x[j];
     }

@@ -102,7 +102,7 @@ __device__ __forceinline__ void tp06_rush_larsen_slots(double* col, double* ycol
         double e[EXP_W];
 #pragma unroll
         for (int j = 0; j < EXP_W; ++j) e[j] = col[(g + j) * BLOCK];
-        ep_exp_wide<EXP_W>(e);
+        ep_exp2_wide<EXP_W>(e);
 #pragma unroll
         for (int j = 0; j < EXP_W; ++j) {
             if (g + j < N_RLB) {
@@ -122,9 +122,13 @@ template <int BLOCK, class Issue, class Finish>
 __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stride, int type, double dt, double istim,
                                             Issue issue_gather, Finish finish_gather, double* col) {
     using namespace tp06;
-    // Argument of every transcendental.  TP06 lives in [-100, +60] mV; inside [-120, 120] every exponent stays far below
-    // 700 and every Rush-Larsen rate except the m gate's stays below 1e3/ms, so only that one needs a clamp below.
-    const double vg = ep_clamp(v, -120.0, 120.0);
+    // Argument of every transcendental (reading T2).  TP06 lives in [-100, +60] mV; for |v| <= 200 mV every
+    // exponent stays below 90 in magnitude, so the clamp is inert there and the kernel follows the (unclamped) oracle;
+    // beyond it the exponentials are frozen at their +-200 mV values while the ohmic factors (v - E) keep the true v.
+    // Inside that range four Rush-Larsen rates can exceed 700/dt (m: 8e12, h: 3e6, j: 5e4, xr1: 2e5 per ms at -200 mV):
+    // their base-2 exponents are clamped to -1000 below (2^-1000 = 1e-301 stands for the oracle's underflow to 0).
+    const double vg = ep_clamp(v, -200.0, 200.0);
+    const double dtl = dt * L2E;   // Rush-Larsen exponents -dt/tau in base-2 units (the exponential primitive is 2^x)
     const double Cai = ycol[Y_CAI * stride], CaSR = ycol[Y_CASR * stride], CaSS = ycol[Y_CASS * stride],
                  Nai = ycol[Y_NAI * stride], Ki = ycol[Y_KI * stride];
     // The 11 voltage-driven gates and Rbar are copied into shared memory asynchronously (no registers held, nothing waits
@@ -147,36 +151,36 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const bool hi = (v >= -40.0);   // reading B7
 
     // ---- batch 2: every voltage-dependent exponential that is not an integer power of another one
-    col[A_B600 * BLOCK] = vg * CK(1.0 / 600.0);
-    col[A_E14 * BLOCK] = vg * CK(1.0 / 14.0);
-    col[A_M * BLOCK] = fma(vg, CK(-1.0 / 9.03), CK(-56.86 / 9.03));
-    col[A_H * BLOCK] = fma(vg, CK(1.0 / 7.43), CK(71.55 / 7.43));
-    col[A_XR1 * BLOCK] = fma(vg, CK(1.0 / 11.5), CK(30.0 / 11.5));
-    col[A_D * BLOCK] = fma(vg, CK(-1.0 / 13.0), CK(-35.0 / 13.0));
-    col[A_PK * BLOCK] = fma(vg, CK(-1.0 / 5.98), CK(25.0 / 5.98));
-    col[A_W * BLOCK] = vg * CK(0.05 * FRT);
-    col[A_GR * BLOCK] = (vg + 40.0) * (vg + 40.0) * CK(-1.0 / 1800.0);
-    col[A_GS * BLOCK] = (type == 0) ? (vg + 67.0) * (vg + 67.0) * CK(-1.0 / 1000.0)
-                                    : (vg + 45.0) * (vg + 45.0) * CK(-1.0 / 320.0);
-    col[A_G27 * BLOCK] = (vg + 27.0) * (vg + 27.0) * CK(-1.0 / 3600.0);
+    col[A_B600 * BLOCK] = vg * CK(L2E / 600.0);
+    col[A_E14 * BLOCK] = vg * CK(L2E / 14.0);
+    col[A_M * BLOCK] = fma(vg, CK(-L2E / 9.03), CK(-56.86 * L2E / 9.03));
+    col[A_H * BLOCK] = fma(vg, CK(L2E / 7.43), CK(71.55 * L2E / 7.43));
+    col[A_XR1 * BLOCK] = fma(vg, CK(L2E / 11.5), CK(30.0 * L2E / 11.5));
+    col[A_D * BLOCK] = fma(vg, CK(-L2E / 13.0), CK(-35.0 * L2E / 13.0));
+    col[A_PK * BLOCK] = fma(vg, CK(-L2E / 5.98), CK(25.0 * L2E / 5.98));
+    col[A_W * BLOCK] = vg * CK(0.05 * FRT * L2E);
+    col[A_GR * BLOCK] = (vg + 40.0) * (vg + 40.0) * CK(-L2E / 1800.0);
+    col[A_GS * BLOCK] = (type == 0) ? (vg + 67.0) * (vg + 67.0) * CK(-L2E / 1000.0)
+                                    : (vg + 45.0) * (vg + 45.0) * CK(-L2E / 320.0);
+    col[A_G27 * BLOCK] = (vg + 27.0) * (vg + 27.0) * CK(-L2E / 3600.0);
     const double xcal = (vg - 15.0) * CK(2.0 * FRT);
-    col[A_CAL * BLOCK] = xcal;
-    col[A_K1Q * BLOCK] = fma(ug, CK(0.0002), CK(0.02));       // 0.0002 (u + 100)
-    col[A_K1Q2 * BLOCK] = ug * CK(0.02);
+    col[A_CAL * BLOCK] = fma(vg, CK(2.0 * FRT * L2E), CK(-30.0 * FRT * L2E));   // xcal in base-2 units
+    col[A_K1Q * BLOCK] = fma(ug, CK(0.0002 * L2E), CK(0.02 * L2E));   // 0.0002 (u + 100)
+    col[A_K1Q2 * BLOCK] = ug * CK(0.02 * L2E);
     if (hi) {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-1.0 / 11.1), CK(-10.66 / 11.1));
-        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.057);
+        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
+        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.057 * L2E);
 #pragma unroll
         for (int k = 0; k < 6; ++k) col[(A_HJ2 + k) * BLOCK] = 0.0;
     } else {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-1.0 / 6.8), CK(-80.0 / 6.8));
-        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.079);
-        col[(A_HJ2 + 0) * BLOCK] = vg * CK(0.3485);
-        col[(A_HJ2 + 1) * BLOCK] = vg * CK(0.2444);
-        col[(A_HJ2 + 2) * BLOCK] = vg * CK(-0.04391);
-        col[(A_HJ2 + 3) * BLOCK] = fma(vg, CK(0.311), CK(0.311 * 79.23));
-        col[(A_HJ2 + 4) * BLOCK] = vg * CK(-0.01052);
-        col[(A_HJ2 + 5) * BLOCK] = fma(vg, CK(-0.1378), CK(-0.1378 * 40.14));
+        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));
+        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.079 * L2E);
+        col[(A_HJ2 + 0) * BLOCK] = vg * CK(0.3485 * L2E);
+        col[(A_HJ2 + 1) * BLOCK] = vg * CK(0.2444 * L2E);
+        col[(A_HJ2 + 2) * BLOCK] = vg * CK(-0.04391 * L2E);
+        col[(A_HJ2 + 3) * BLOCK] = fma(vg, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
+        col[(A_HJ2 + 4) * BLOCK] = vg * CK(-0.01052 * L2E);
+        col[(A_HJ2 + 5) * BLOCK] = fma(vg, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
     }
     // fCass and Rbar: their Rush-Larsen rates need no exponential, so exp(-dt/tau) rides in this batch
     const double c2 = CaSR * CaSR, css2 = CaSS * CaSS, ci2 = Cai * Cai;
@@ -185,10 +189,10 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double fCass_inf = fma(CK(0.6), qf, CK(0.4));
     const double Rbar_rate = fma(CK(k2p) * kcasr, CaSS, CK(k4));   // dR/dt = k4 (1 - R) - k2 CaSS R (reading B1)
     const double Rbar_inf = CK(k4) * ep_rcp(Rbar_rate);
-    col[A_RLF * BLOCK] = -dt * ep_rcp(fma(80.0, qf, 2.0));          // tau_fCass >= 2 ms
-    col[A_RLR * BLOCK] = fmax(-dt * Rbar_rate, -700.0);             // rate grows with Ca_SS: keep the clamp
+    col[A_RLF * BLOCK] = -dtl * ep_rcp(fma(80.0, qf, 2.0));         // tau_fCass >= 2 ms
+    col[A_RLR * BLOCK] = fmax(-dtl * Rbar_rate, -1000.0);           // rate grows with Ca_SS: keep the clamp
     // warp-uniform trip count: during the plateau (every cell of the warp above -40 mV) the last trip is skipped
-    ep_exp_slots<N_EXPA, BLOCK, EXP_W>(col, __all_sync(__activemask(), hi) ? N_EXPA_HI : N_EXPA);
+    ep_exp2_slots<N_EXPA, BLOCK, EXP_W>(col, __all_sync(__activemask(), hi) ? N_EXPA_HI : N_EXPA);
     const double dv_diff = finish_gather();   // the gathers have landed during the batch: 12 values -> 1
     // gate values have landed too (finish_gather waited for this thread's asynchronous copies): products for the currents
     ep_cp_async_wait();
@@ -345,7 +349,7 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     // ---- batch 3: Rush-Larsen (every value of batch 2 has been consumed above, so its slots are free)
 #pragma unroll
     for (int g = 0; g < N_RLB; ++g) {
-        col[g * BLOCK] = (g == 0) ? fmax(-dt * rate[g], -700.0) : -dt * rate[g];   // tau_m reaches 1e-6 ms at -120 mV
+        col[g * BLOCK] = (g <= 3) ? fmax(-dtl * rate[g], -1000.0) : -dtl * rate[g];   // m, h, j, xr1: see the clamp note above
         col[(B_INF0 + g) * BLOCK] = inf[g];
     }
     col[N_RLB * BLOCK] = 0.0;

@@ -3,8 +3,13 @@
 Tolerances are north_star's (BASELINE.json): one step, per state variable, max|g-o| / max|o| <= 1e-11;
 full run max|dVm| <= 1e-6 mV, activation times equal to within one dt and identical activated sets.
 """
+import os
+import sys
+
 import numpy as np
 import pytest
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))      # tests/wavestate.py
 
 from ep_inputs import make, states
 from ep_inputs import meshes as M
@@ -32,11 +37,22 @@ def _pair(ep, oracle, prob, threads=0):
     return g, o
 
 
-def _one_step_err(g, o, S):
+PER_CELL = {"rel": 1e-10, "floor": 1e-14}
+
+
+def _one_step_err(g, o, S, per_cell=True):
+    """north_star's metric per state variable, max|g-o| / max|o| over the mesh -- and, so that an error confined to small
+    entries (a gate near 0, a concentration orders of magnitude below the largest) cannot hide behind the field maximum, a
+    per-cell bound |g-o| <= 1e-10 |o| + 1e-14 max|o| on every entry."""
     errs = []
     for k in range(S):
         a, b = g.read_state(k), o.read_state(k)
-        errs.append(np.abs(a - b).max() / np.abs(b).max())
+        d = np.abs(a - b)
+        scale = np.abs(b).max()
+        errs.append(d.max() / scale)
+        if per_cell:
+            bad = d > PER_CELL["rel"] * np.abs(b) + PER_CELL["floor"] * scale
+            assert not bad.any(), (k, int(bad.sum()), float((d / np.maximum(np.abs(b), 1e-300))[bad].max()))
     return np.array(errs)
 
 
@@ -107,20 +123,63 @@ def test_one_step_random_states(ep, oracle, case):
 
 def test_one_step_plateau_and_rest_warps(ep, oracle):
     """Whole warps above / below -40 mV: the kernel skips the unused h/j exponentials when every cell of a warp is on the
-    high-voltage branch (reading B7), so that path needs its own inputs; mixed warps are covered by the random cases."""
+    high-voltage branch (reading B7).  Warps are 32 consecutive cells in DEVICE (Morton) order, so the voltages are laid
+    out through the preprocessor's permutation: device cells [0, n/2) all above -40 mV, one warp mixed, the rest below."""
     prob = make(1)
     prob.mesh.cell_type = (np.arange(prob.mesh.n_tets) % 3).astype(np.uint8)
     g, o = _pair(ep, oracle, prob)
     n = prob.mesh.n_tets
+    m = prob.mesh
+    perm = ep.host_stencil(m.xyz, m.tets, m.fibre, m.sigma_scale, prob.sigma_l, prob.sigma_t, prob.chi, prob.Cm)["perm"]
+    assert sorted(perm.tolist()) == list(range(n))
     y = states.random_states(0, 78, n)
-    y[0] = uniform(79, np.arange(n), -39.999, 45.0)        # every cell on the plateau branch
-    y[0, n // 2:] = uniform(80, np.arange(n - n // 2), -95.0, -40.001)   # second half of the cells at rest-like voltages
-    y[0, 5] = -40.0
+    v_dev = np.empty(n)
+    half = (n // 2 // 32) * 32
+    v_dev[:half] = uniform(79, np.arange(half), -39.999, 45.0)               # full warps on the plateau branch
+    v_dev[half:] = uniform(80, np.arange(n - half), -95.0, -40.001)          # full warps at rest-like voltages
+    v_dev[half:half + 32:2] = uniform(81, np.arange(16), -39.0, 30.0)        # one mixed warp
+    v_dev[5] = -40.0                                                         # the branch point itself (>= -40: high)
+    y[0, perm] = v_dev                                                       # perm[device position] = caller's cell id
     for k in range(19):
         g.write_state(k, y[k]); o.write_state(k, y[k])
     g.step(1, 0.02); o.step(1, 0.02)
     err = _one_step_err(g, o, 19)
     assert err.max() <= ONE_STEP_TOL, err
+    g.close()
+
+
+def test_one_step_beyond_physiological_voltages(ep, oracle):
+    """Reading T2: the kernel clamps the ARGUMENTS of its exponentials to |v| <= 200 mV (Rush-Larsen exponents to -700).
+    Inside that range the clamp is inert and the one-step tolerance holds against the unclamped oracle, including
+    |v| in (120, 200] where the m / h / j / xr1 rates reach 1e5 .. 1e13 per ms.  Beyond it the two sides part (documented,
+    not a parity claim): the kernel stays finite with gates in [0,1]; the oracle, which has no clamp, keeps its formulas."""
+    prob = make(1, coarsen=2.0)
+    prob.mesh.cell_type = (np.arange(prob.mesh.n_tets) % 3).astype(np.uint8)
+    prob.mesh.sigma_scale = np.zeros(prob.mesh.n_tets)        # uncoupled cells: this is about the cell model only
+    prob.stimuli = []
+    g, o = _pair(ep, oracle, prob)
+    n = prob.mesh.n_tets
+    y = states.random_states(0, 91, n)
+    y[0] = np.where(np.arange(n) % 2 == 0, uniform(92, np.arange(n), 120.0, 200.0), uniform(93, np.arange(n), -200.0, -120.0))
+    y[0, :4] = [200.0, -200.0, 120.0, -120.0]
+    for k in range(19):
+        g.write_state(k, y[k]); o.write_state(k, y[k])
+    g.step(1, 0.02); o.step(1, 0.02)
+    err = _one_step_err(g, o, 19)
+    assert err.max() <= ONE_STEP_TOL, err
+    # outside the clamp range: finite, gates in [0,1]; Vm moves by the ohmic currents evaluated with frozen exponentials
+    y[0] = np.where(np.arange(n) % 2 == 0, 260.0, -260.0)
+    g.state_init(0, prob.mesh.cell_type); o.state_init(0, prob.mesh.cell_type)
+    for k in range(19):
+        g.write_state(k, y[k]); o.write_state(k, y[k])
+    g.step(1, 0.02); o.step(1, 0.02)
+    for k in range(19):
+        assert np.isfinite(g.read_state(k)).all(), k
+    for k in range(1, 14):
+        sk = g.read_state(k)
+        assert sk.min() >= 0.0 and sk.max() <= 1.0, k
+    d = np.abs(g.read_vm() - o.read_vm()).max()
+    assert d > 1e-6                      # the clamp is visible here: the two sides are NOT claimed to agree
     g.close()
 
 
@@ -271,6 +330,7 @@ def test_crn_one_step_random_states(ep, oracle, case):
         prob = make(5, coarsen=6.0)
         prob.mesh = _jittered()
         prob.mesh.cell_type = None
+        prob.stimuli, prob.triggers = prob.stimuli[:1], []
         prob.stimuli[0].cell_ids = np.arange(0, prob.mesh.n_tets, 5, dtype=np.int64)
     g, o = _pair(ep, oracle, prob)
     assert g.n_states == 21
@@ -463,24 +523,89 @@ def test_device_view_streams_and_two_sims(ep):
     a.close(); b.close(); ref.close()
 
 
-@pytest.mark.skipif(not __import__("os").environ.get("EP_SLOW"), reason="about 6 minutes and 30 GB of host memory: set EP_SLOW=1")
-def test_full_size_c4_biventricle_scar(ep, oracle):
-    """BASELINE config 4 at full size (22.5 M cells, scar with sigma x 0.1): one step from random states against the
-    threaded oracle on every cell, then 2 more steps."""
+def _window(ep, oracle, prob, n_steps, dt, frac, t_span, capsys, label, chunks=4):
+    """Window parity from a seeded 'wave in progress' state (tests/wavestate.py): same painted state into both sides, n_steps
+    explicit steps, compared at `chunks` checkpoints; returns the oracle's final Vm and both activation-time arrays."""
     import os
+    import wavestate
+    g, o = _pair(ep, oracle, prob, threads=os.cpu_count() or 1)
+    y, phase = wavestate.paint(oracle, prob, frac, t_span)
+    S = y.shape[0]
+    g.write_states(y)
+    for k in range(S):
+        o.write_state(k, y[k])
+    excited0 = float((y[0] > -60.0).mean())
+    worst = 0.0
+    for _ in range(chunks):
+        g.step(n_steps // chunks, dt); o.step(n_steps // chunks, dt)
+        worst = max(worst, float(np.abs(g.read_vm() - o.read_vm()).max()))
+    tg, to = g.activation_times(), o.activation_times()
+    vo = o.read_vm()
+    with capsys.disabled():
+        print("%s: %d cells x %d steps from a painted wave (%.0f %% of the cells excited at the start, %d cells crossed 0 mV "
+              "in the window): max|dVm| = %.3e mV, max|dt_act| = %.3e ms"
+              % (label, prob.mesh.n_tets, n_steps, 100 * excited0, int((to >= 0).sum()), worst, float(np.abs(tg - to).max())))
+    assert excited0 >= 0.30
+    assert worst <= RUN_TOL_MV
+    assert np.array_equal(tg >= 0, to >= 0) and np.abs(tg - to).max() <= dt * (1 + 1e-12)
+    assert (to >= 0).sum() > 100                      # fronts moved: cells were activated inside the window
+    assert g.check_finite()
+    for k in range(1, S):
+        a, b = g.read_state(k), o.read_state(k)
+        assert np.abs(a - b).max() <= 1e-8 * max(1.0, np.abs(b).max()), k
+    g.close(); o.close()
+
+
+def test_window_full_c3(ep, oracle, capsys):
+    """1,000-step window on the FULL config-3 mesh (2,014,530 cells), threaded oracle, starting from a state
+    with wavefronts, plateau and repolarising tissue everywhere (not from rest)."""
+    prob = make(3)
+    _window(ep, oracle, prob, 1000, prob.dt, 0.45, 350.0, capsys, "C3 full mesh")
+
+
+def test_window_full_c5(ep, oracle, capsys):
+    """1,000-step window on the FULL config-5 mesh (2,992,968 cells, Courtemanche), wave in progress on both shells."""
+    prob = make(5)
+    _window(ep, oracle, prob, 1000, prob.dt, 0.45, 300.0, capsys, "C5 full mesh")
+
+
+def test_full_size_c4_biventricle_scar(ep, oracle, capsys):
+    """BASELINE config 4 at full size (22.5 M cells, scar with sigma x 0.1): one step from random states against the
+    threaded oracle on every cell and every state row, 2 more steps, then a 48-step window from a painted wave state
+    (fronts crossing the low-conductivity zone included)."""
+    import os
+    import wavestate
     prob = make(4)
     n = prob.mesh.n_tets
     assert 1.8e7 < n < 2.6e7 and (prob.mesh.sigma_scale == 0.1).sum() > 1000
     g, o = _pair(ep, oracle, prob, threads=os.cpu_count() or 1)
     y = states.random_states(0, 404, n)
+    g.write_states(y)
     for k in range(19):
-        g.write_state(k, y[k]); o.write_state(k, y[k])
+        o.write_state(k, y[k])
     g.step(1, prob.dt); o.step(1, prob.dt)
     err = _one_step_err(g, o, 19)
     assert err.max() <= ONE_STEP_TOL, err
     g.step(2, prob.dt); o.step(2, prob.dt)
     assert np.abs(g.read_vm() - o.read_vm()).max() <= 1e-8
-    g.close()
+    del y
+    # window: re-initialise both sides, paint, run
+    g.state_init(0, prob.mesh.cell_type); o.state_init(0, prob.mesh.cell_type)
+    y, _ = wavestate.paint(oracle, prob, 0.45, 350.0)
+    excited0 = float((y[0] > -60.0).mean())
+    g.write_states(y)
+    for k in range(19):
+        o.write_state(k, y[k])
+    del y
+    g.step(48, prob.dt); o.step(48, prob.dt)
+    worst = float(np.abs(g.read_vm() - o.read_vm()).max())
+    tg, to = g.activation_times(), o.activation_times()
+    with capsys.disabled():
+        print("C4 full mesh: %d cells, one-step max rel err %.2e; 48-step window from a painted wave (%.0f %% excited, %d cells "
+              "crossed 0 mV): max|dVm| = %.3e mV" % (n, err.max(), 100 * excited0, int((to >= 0).sum()), worst))
+    assert excited0 >= 0.30 and worst <= RUN_TOL_MV
+    assert np.array_equal(tg >= 0, to >= 0) and np.abs(tg - to).max() <= prob.dt * (1 + 1e-12)
+    g.close(); o.close()
 
 
 def test_operator_invariants_at_full_size(ep):
@@ -505,13 +630,18 @@ def test_operator_invariants_at_full_size(ep):
     g.close()
 
 
-@pytest.mark.skipif(not __import__("os").environ.get("EP_SLOW"), reason="5-8 minutes each (threaded oracle): set EP_SLOW=1")
-@pytest.mark.parametrize("cfg,coarsen,dt,steps", [(2, 1.0, 0.005, 20000), (3, 2.0, 0.02, 20000), (4, 3.0, 0.01, 5000),
-                                                  (5, 2.0, 0.01, 15000)])
-def test_full_duration(ep, oracle, cfg, coarsen, dt, steps, capsys):
-    """north_star's full-run tolerance on configs 2-5: the whole specified duration (C2 100 ms on the full mesh at the
-    stable dt; C3 one 400 ms beat, C4 its 50 ms window, C5 150 ms on twins at 2-3x the lattice spacing), threaded
-    oracle.  max |dVm| <= 1e-6 mV, identical activated sets, activation times within one dt."""
+_SLOW = pytest.mark.skipif(not __import__("os").environ.get("EP_SLOW"), reason="6-10 minutes each (threaded oracle): set EP_SLOW=1")
+
+
+@pytest.mark.parametrize("cfg,coarsen,dt,steps,min_frac", [
+    (2, 1.0, 0.005, 20000, 0.99), (3, 2.0, 0.02, 20000, 0.99),
+    pytest.param(4, 3.0, 0.01, 5000, 0.5, marks=_SLOW), pytest.param(5, 1.5, 0.01, 15000, 0.3, marks=_SLOW)])
+def test_full_duration(ep, oracle, cfg, coarsen, dt, steps, min_frac, capsys):
+    """north_star's full-run tolerance over the whole specified duration: C2 100 ms on the FULL mesh at the stable dt and
+    C3 one 400 ms beat on its twin at 2x the lattice spacing run by default; C4's 50 ms window (3x) and C5's 150 ms
+    (1.5x, with the bundle stand-ins of reading G1) need EP_SLOW=1.  Threaded oracle; compared at 10 checkpoints.
+    max |dVm| <= 1e-6 mV, identical activated sets, activation times within one dt, and the wave must really have
+    travelled (activated fraction >= min_frac)."""
     import os
     prob = make(cfg, coarsen=coarsen)
     g, o = _pair(ep, oracle, prob, threads=os.cpu_count() or 1)
@@ -521,28 +651,88 @@ def test_full_duration(ep, oracle, cfg, coarsen, dt, steps, capsys):
         worst = max(worst, float(np.abs(g.read_vm() - o.read_vm()).max()))
     tg, to = g.activation_times(), o.activation_times()
     with capsys.disabled():
-        print("config %d (coarsen %.0f): %d cells x %d steps, max|dVm| over 10 checkpoints = %.3e mV, activated %d / %d, "
+        print("config %d (coarsen %.1f): %d cells x %d steps, max|dVm| over 10 checkpoints = %.3e mV, activated %d / %d, "
               "max|dt_act| = %.3e ms" % (cfg, coarsen, prob.mesh.n_tets, steps, worst, int((to >= 0).sum()), to.size,
                                          float(np.abs(tg - to).max())))
     assert worst <= RUN_TOL_MV
     assert np.array_equal(tg >= 0, to >= 0) and np.abs(tg - to).max() <= dt * (1 + 1e-12)
-    g.close()
+    assert (to >= 0).mean() >= min_frac
+    g.close(); o.close()
 
 
 def test_checkpoint_resume(ep):
-    """ep_read_state / ep_write_state are the checkpoint format.  A run resumed in a fresh handle from the
-    19 state rows continues bit for bit (after the stimulus window has closed: the step counter itself is not restored)."""
+    """Checkpoint = the S state rows + the clock + the activation times + the trigger state (include/ep.h).  Checkpoints are
+    taken INSIDE an open stimulus window and while a trigger has fired but its delayed slot has not yet switched on; the run
+    resumed in a fresh handle continues bit for bit, and reports the same times."""
     prob = make(1, coarsen=2.0)
-    a = ep.Sim.from_problem(prob)
-    a.step(120, prob.dt)                              # stimulus window (50 steps) is over
-    ckpt = [a.read_state(k) for k in range(19)]
-    a.step(150, prob.dt)
-    b = ep.Sim(prob.mesh.xyz, prob.mesh.tets, prob.mesh.fibre, prob.mesh.sigma_scale, prob.sigma_l, prob.sigma_t,
-               prob.chi, prob.Cm)
-    b.state_init(prob.model, prob.mesh.cell_type)
+    cen = prob.mesh.centroids()
+    mon = np.nonzero(cen[:, 0] < 0.6)[0].astype(np.int64)
+    tgt = np.nonzero(cen[:, 0] > 4.4)[0].astype(np.int64)
+
+    def fresh():
+        s = ep.Sim.from_problem(prob)
+        s.stimulus_set(2, tgt, -52.0, 999.0, 1.0)
+        s.trigger_set(0, mon, 2, 4.0)
+        return s
+
+    a = fresh()
+    for n_ckpt in (30, 120):                          # 30: slot 0 (50 steps) still on; 120: trigger fired, slot 2 pending
+        a.step(n_ckpt - a.step_count, prob.dt)
+        states_ck = a.read_states()
+        tact_ck, tfire_ck = a.activation_times(), a.trigger_time(0)
+        if n_ckpt == 120:
+            assert tfire_ck > 0 and tfire_ck + 4.0 > a.time       # fired, delayed slot not yet on
+        b = fresh()
+        b.write_states(states_ck)
+        b.set_step_count(n_ckpt, prob.dt)
+        b.write_activation_times(tact_ck)
+        b.trigger_restore(0, tfire_ck)
+        assert b.step_count == n_ckpt and b.time == a.time and b.trigger_time(0) == tfire_ck
+        ref = fresh()
+        ref.step(n_ckpt + 300, prob.dt)               # uninterrupted
+        b.step(300, prob.dt)
+        assert np.array_equal(ref.read_states(), b.read_states()), n_ckpt
+        assert np.array_equal(ref.activation_times(), b.activation_times())
+        assert ref.trigger_time(0) == b.trigger_time(0) and ref.time == b.time
+        assert (b.activation_times()[tgt] >= 0).all()              # the delayed slot did fire in the resumed run
+        with pytest.raises(ep.EpError):
+            b.step(1, 0.5 * prob.dt)                               # the restored clock keeps its dt
+        b.close(); ref.close()
+    a.close()
+
+
+def test_bulk_state_io_equals_row_io(ep):
+    """ep_write_states / ep_read_states (pipelined, one synchronisation) move exactly what the row calls move."""
+    prob = make(3, coarsen=4.0)
+    n = prob.mesh.n_tets
+    a = ep.Sim.from_problem(prob); b = ep.Sim.from_problem(prob)
+    y = states.random_states(0, 5, n)
+    a.write_states(y)
     for k in range(19):
-        b.write_state(k, ckpt[k])
-    b.step(150, prob.dt)
+        b.write_state(k, y[k])
+    ra = a.read_states()
+    assert np.array_equal(ra, y)
     for k in range(19):
-        assert np.array_equal(a.read_state(k), b.read_state(k)), k
+        assert np.array_equal(b.read_state(k), y[k])
+    a.step(3, prob.dt); b.step(3, prob.dt)
+    assert np.array_equal(a.read_states(), np.stack([b.read_state(k) for k in range(19)]))
     a.close(); b.close()
+
+
+def test_check_finite_sees_every_state_row(ep):
+    """ep_check_finite scans Vm and all state rows and flags non-positive concentrations (sticky EP_ERR_NUMERIC)."""
+    prob = make(1, coarsen=2.0)
+    for var, val in ((0, np.nan), (7, np.inf), (18, -1.0), (14, 0.0)):
+        g = ep.Sim.from_problem(prob)
+        assert g.check_finite()
+        row = g.read_state(var)
+        row[prob.mesh.n_tets // 2] = val
+        g.write_state(var, row)
+        assert not g.check_finite(), var
+        with pytest.raises(ep.EpError) as e:
+            g.step(1, prob.dt)
+        assert e.value.code == -6
+        g.state_init(0, prob.mesh.cell_type)           # a fresh state clears the numerical failure
+        g.step(1, prob.dt)
+        assert g.check_finite()
+        g.close()
