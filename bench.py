@@ -272,20 +272,35 @@ def run_ours(args):
     cell_ms = prof["ms_cell"] / max(1, prof["steps"])
     node_ms = prof["ms_node"] / max(1, prof["steps"])
     achieved = cell_bytes / (cell_ms * 1e-3) / 1e9
-    traffic = args.traffic
-    if traffic is None:   # dram bytes per launch from the committed ncu capture of this workload, if there is one
-        try:
-            traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))[prob.name]["bytes_per_launch"]
-        except Exception:
-            traffic = None
+    # figures read from the committed ncu capture of this workload (profiles/traffic.json names the capture): DRAM bytes
+    # per launch and fp64 warp instructions per warp (= fp64 instructions per cell-step) of the dominant kernel
+    cap = {}
+    try:
+        cap = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(prob.name, {})
+    except Exception:
+        cap = {}
+    traffic = args.traffic if args.traffic is not None else cap.get("bytes_per_launch")
+    fp64_inst = cap.get("fp64_inst_per_cell_step")
+    hbm_floor_ms = cell_bytes / (peak * 1e9) * 1e3
+    # the other roof (t_roof = max(bytes / BW_HBM, I_alg / R_fp64)): fp64 instructions the kernel executes
+    # (ncu) over the DFMA issue rate of this GPU measured in this run, after the timed region, at whatever clock the
+    # power cap then allows (ep_fp64_rate: a DFMA-only kernel)
+    fp64_rate = ep.fp64_rate()
+    fp64_floor_ms = (nc / 32.0) * fp64_inst / fp64_rate * 1e3 if fp64_inst else None
+    roof_ms = max(hbm_floor_ms, fp64_floor_ms or 0.0)
     roofline = {"bound": "hbm", "kernel": "cell_step_kernel<%d>" % prob.model, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic,
                 "alg_bytes_per_launch": cell_bytes, "alg_bytes_per_cell": cell_bytes / nc,
                 "avg_launch_ms": cell_ms, "node_kernel_avg_launch_ms": node_ms,
                 "kernel_share_of_step": cell_ms / max(1e-12, cell_ms + node_ms),
                 "profiled_pass_ms_per_step": ms_profiled / args.steps,
-                # the method as written is ~3.7 kFLOP of fp64 per TP06 cell-step (census view)
-                "fp64_census_frac": (nc * 3.7e3 / 37.2e12) / (cell_ms * 1e-3) if prob.model == 0 else None,
+                "hbm_floor_ms": hbm_floor_ms,
+                "fp64": {"warp_dfma_per_s_measured": fp64_rate, "tflops_measured": fp64_rate * 64 / 1e12,
+                         "inst_per_cell_step": fp64_inst, "inst_source": cap.get("source"),
+                         "floor_ms": fp64_floor_ms,
+                         "frac": (fp64_floor_ms / cell_ms) if fp64_floor_ms else None},
+                "roof": "fp64" if (fp64_floor_ms or 0.0) > hbm_floor_ms else "hbm",
+                "roof_ms": roof_ms, "roof_frac": roof_ms / cell_ms,
                 "whole_step_frac": sim.step_bytes / (ms_max * 1e-3 / (inner * args.steps)) / 1e9 / peak}
     cores = os.cpu_count() or 1
     cpu_val, cpu_n, cpu_t = _oracle_leg(prob, args.cpu_budget, cores)

@@ -151,6 +151,12 @@ const char *ep_last_error(void);
  * 3: reciprocal square root.  Host pointers. */
 int ep_math_eval(int fn, int64_t n, const double *x, double *y);
 
+/* Diagnostic: measured throughput of the plain fp64 pipe of the current device, in warp-wide DFMA instructions per second
+ * (a DFMA-only kernel, four independent chains per thread, 16 warps per SM sub-partition, best of three ~2 ms launches on
+ * the default stream).  This is the denominator of the "alu" roof of DESIGN.md section 6: the fused step executes a
+ * counted number of fp64 warp instructions per 32 cells (t_roof = max(bytes/BW_HBM, I_alg/R_fp64)). */
+int ep_fp64_rate(double *warp_dfma_per_s);
+
 /* Host-only preprocessor output for tests (no CUDA call is made).  Returns the factored stencil in the CALLER's
  * numbering: for cell c,  dv_diff[c] = sum_{m<8} a[c*8+m] * v_node[node[c*8+m]] + sum_{j<4} b[c*4+j] * (v[nbr[c*4+j]] - v[c])
  * in mV/ms (= D_c/(chi Cm)), where v_node[n] = sum_{k<node_deg[n]} w[node_ptr[n]+k] * v[node_cell[node_ptr[n]+k]].

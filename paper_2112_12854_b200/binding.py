@@ -52,6 +52,7 @@ SIGNATURES = {
     "ep_profile": (C.c_int, [_vp, C.c_int]),
     "ep_profile_read": (C.c_int, [_vp, _dp]),
     "ep_math_eval": (C.c_int, [C.c_int, C.c_int64, _dp, _dp]),
+    "ep_fp64_rate": (C.c_int, [_dp]),
     "ep_destroy": (None, [_vp]),
     "ep_last_error": (C.c_char_p, []),
     "ep_host_stencil": (C.c_int, [C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double, C.c_double,
@@ -97,6 +98,13 @@ def math_eval(fn: int, x):
     y = np.empty_like(x)
     _chk(lib().ep_math_eval(int(fn), x.size, _p(x), _p(y)))
     return y
+
+
+def fp64_rate() -> float:
+    """ep_fp64_rate: measured warp-wide DFMA instructions per second of the current device's fp64 pipe."""
+    r = C.c_double(0.0)
+    _chk(lib().ep_fp64_rate(C.byref(r)))
+    return float(r.value)
 
 
 def model_n_states(model: int) -> int:

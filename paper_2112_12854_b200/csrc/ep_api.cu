@@ -796,6 +796,36 @@ int ep_math_eval(int fn, int64_t n, const double* x, double* y) {
     return EP_OK;
 }
 
+int ep_fp64_rate(double* warp_dfma_per_s) {
+    if (!warp_dfma_per_s) return fail(EP_ERR_ARG, "null argument");
+    ep_sim* none = nullptr;
+    const int64_t len = 592 * 512;
+    double* scratch = nullptr;
+    EP_CUDA(none, cudaMalloc((void**)&scratch, sizeof(double) * len));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaError_t e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    double best = 0.0;
+    if (e == cudaSuccess) {
+        epk::launch_dfma_rate(scratch, len, 2000, nullptr);   // warm-up: clocks up, code resident
+        for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {
+            cudaEventRecord(e0, nullptr);
+            const double n = epk::launch_dfma_rate(scratch, len, 4000, nullptr);   // about 2.3 ms
+            cudaEventRecord(e1, nullptr);
+            e = cudaEventSynchronize(e1);
+            float ms = 0.f;
+            if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+            if (e == cudaSuccess && ms > 0.f) best = std::max(best, n / (ms * 1e-3));
+        }
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(scratch);
+    if (e != cudaSuccess) return fail(EP_ERR_CUDA, std::string("ep_fp64_rate: ") + cudaGetErrorString(e));
+    *warp_dfma_per_s = best;
+    return EP_OK;
+}
+
 int ep_device_vm(ep_sim* s, void** vm, void** perm) {
     if (!s) return fail(EP_ERR_ARG, "null sim handle");
     if (vm) *vm = s->d_vm[s->cur];

@@ -7,6 +7,7 @@
 // the diffusion term needs no atomics and the result is deterministic (the only atomic is the once-per-run firing of a
 // communication-node trigger).  Nothing here is a dense contraction: no tensor cores.
 #include "ep_kernels.cuh"
+#include <algorithm>
 #include "ep_tp06.cuh"
 #include "ep_crn98.cuh"
 
@@ -302,12 +303,38 @@ __global__ void math_eval_kernel(int fn, int64_t n, const double* __restrict__ x
     y[i] = v[0];
 }
 
+// Plain fp64-pipe throughput probe (the "alu" roof of DESIGN.md section 6): every thread runs `iters` x 8 x 4 DFMAs in four
+// independent chains, 16 warps per SM sub-partition, no memory traffic.  Returns nothing useful in `out` (it only keeps
+// the chains alive); the launcher times the kernel.
+__global__ void __launch_bounds__(512) dfma_rate_kernel(double* out, int iters, double a, double b) {
+    double x[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) x[j] = threadIdx.x * 1e-9 + j;
+#pragma unroll 1
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) x[j] = fma(x[j], a, b);
+        }
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = (x[0] + x[1]) + (x[2] + x[3]);
+}
+
 inline unsigned blocks_for(int64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
 
 }  // namespace
 
 void launch_math_eval(int fn, int64_t n, const double* x, double* y, cudaStream_t s) {
     math_eval_kernel<<<blocks_for(n, 256), 256, 0, s>>>(fn, n, x, y);
+}
+
+double launch_dfma_rate(double* scratch, int64_t scratch_len, int iters, cudaStream_t s) {
+    const int threads = 512;
+    const unsigned blocks = (unsigned)std::min<int64_t>(592, scratch_len / threads);
+    if (blocks == 0) return 0.0;
+    dfma_rate_kernel<<<blocks, threads, 0, s>>>(scratch, iters, 0.999999, 1e-7);
+    return (double)blocks * (threads / 32) * (double)iters * 32.0;   // warp-wide DFMAs issued
 }
 
 int model_n_states(int model) { return model == 0 ? (int)TP06_S : (model == 1 ? (int)CRN_S : -1); }

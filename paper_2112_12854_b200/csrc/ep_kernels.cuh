@@ -73,6 +73,9 @@ void launch_state_scan(int model, int64_t nc, const double* vm, const double* y,
 void launch_count_nonfinite(int64_t n, const double* x, double* partial, double* out, cudaStream_t s);
 
 int model_n_states(int model);
+// fp64-pipe probe: launches a DFMA-only kernel on up to 592 blocks x 512 threads (scratch must hold that many doubles),
+// returns the number of warp-wide DFMAs it issues; the caller times it
+double launch_dfma_rate(double* scratch, int64_t scratch_len, int iters, cudaStream_t s);
 // diagnostics: y[i] = f(x[i]) with the kernels' own exp / log / rcp / rsqrt (device pointers)
 void launch_math_eval(int fn, int64_t n, const double* x, double* y, cudaStream_t s);
 
