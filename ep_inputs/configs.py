@@ -14,6 +14,7 @@ from .prng import splitmix64
 
 MODEL_TP06 = 0
 MODEL_CRN98 = 1
+MODEL_STEWART = 2
 
 
 @dataclass
@@ -218,9 +219,43 @@ def paper_slab(dx: float = 0.1, coarsen: float = 1.0) -> Problem:
                    notes={"dx": dx})
 
 
+# Table 2: 2D Purkinje network, Stewart model, isotropic monodomain, 3.95 mS/mm = 39.5 mS/cm
+SIGMA_PURKINJE = 39.5
+
+
+def purkinje_strip(dx: float = 0.2, jitter: float = 0.0, seed: int = 2001, lx: float = 20.0, ly: float = 7.0) -> Problem:
+    """The paper's 2D benchmark domain (rectangle 20 x 7 mm, uniform grid) as a triangulated sheet with the
+    Purkinje parameters of Table 2 (Stewart model, isotropic 39.5 mS/cm).  Stimulus: the strip x < 1.5 mm (the corner square
+    of PAPER.md:214 does not reach the liminal size at this conductivity), -52 uA/cm^2 for 2 ms."""
+    nx, ny = int(round(lx / dx)), int(round(ly / dx))
+    mesh = M.rect_tri(nx, ny, dx)
+    if jitter:
+        M.jitter_interior_tri(mesh, jitter * dx, seed, out_of_plane=0.5 * jitter * dx)
+    cent = mesh.centroids()
+    ids = np.nonzero(cent[:, 0] < 1.5)[0].astype(np.int64)
+    return Problem("purkinje_strip_dx%g" % dx, mesh, sigma_l=SIGMA_PURKINJE, sigma_t=SIGMA_PURKINJE, model=MODEL_STEWART,
+                   stimuli=[Stimulus(ids, -52.0, 0.0, 2.0)], dt=0.001, n_steps=10000, notes={"dx": dx, "dim": 2})
+
+
+def purkinje_sheet(coarsen: float = 1.0, seed: int = 2002, h: float = 0.45) -> Problem:
+    """A Purkinje layer on the endocardium of config 3's left ventricle: the inner ellipsoid 25/25/50 mm below z = 20 mm as a
+    triangulated surface, ~97,000 triangles at h = 0.45 mm (54,000 triangles at 0.45 mm for one ventricle,
+    108,000 for both), Stewart model, isotropic 39.5 mS/cm.  Stimulus: the triangles within 3 mm of a seeded point on the
+    base ring (where the bundle branch enters), 2 ms."""
+    h = h * coarsen
+    mesh = M.ellipsoid_surface(_LV_IN, _LV_ZCUT, h)
+    cent = mesh.centroids()
+    pool = np.nonzero(cent[:, 2] > _LV_ZCUT - 2.0)[0]
+    pt = _pick(seed, pool, 1)
+    ids = _balls(cent, cent[pt], 3.0)
+    return Problem("purkinje_sheet", mesh, sigma_l=SIGMA_PURKINJE, sigma_t=SIGMA_PURKINJE, model=MODEL_STEWART,
+                   stimuli=[Stimulus(ids, -52.0, 0.0, 2.0)], dt=0.001, n_steps=30000, notes={"seed": seed, "h": h, "dim": 2})
+
+
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5,
            6: lambda coarsen=1.0: paper_slab(0.5, coarsen), 7: lambda coarsen=1.0: paper_slab(0.2, coarsen),
-           8: lambda coarsen=1.0: paper_slab(0.1, coarsen)}
+           8: lambda coarsen=1.0: paper_slab(0.1, coarsen),
+           9: lambda coarsen=1.0: purkinje_strip(0.2 * coarsen), 10: purkinje_sheet}
 
 
 def make(cfg: int, coarsen: float = 1.0) -> Problem:

@@ -203,3 +203,97 @@ def validate(mesh: TetMesh) -> dict:
         raise ValueError("face shared by more than two cells")
     return {"n_faces": int(cnt.size), "n_boundary_faces": int((cnt == 1).sum()), "min_vol": float(vol.min()),
             "mean_vol": float(vol.mean())}
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Triangulated surfaces: the two-dimensional media of the paper (Purkinje network).
+@dataclass
+class TriMesh:
+    xyz: np.ndarray            # [n_nodes,3] float64, mm (a flat mesh has z = 0)
+    tris: np.ndarray           # [n_tris,3] int32, 0-based
+    fibre: np.ndarray | None = None        # [n_tris,3] or None = isotropic (Table 2)
+    sigma_scale: np.ndarray | None = None  # [n_tris] or None
+    cell_type: np.ndarray | None = None
+    meta: dict = field(default_factory=dict)
+
+    @property
+    def n_nodes(self) -> int:
+        return int(self.xyz.shape[0])
+
+    @property
+    def n_tris(self) -> int:
+        return int(self.tris.shape[0])
+
+    @property
+    def n_tets(self) -> int:       # "number of cells" under the name the 3D code paths use
+        return self.n_tris
+
+    def centroids(self) -> np.ndarray:
+        return self.xyz[self.tris].mean(axis=1)
+
+
+def rect_tri(nx: int, ny: int, h: float) -> TriMesh:
+    """nx x ny squares of side h in the plane z = 0, each cut along its (0,0)-(1,1) diagonal: 2 nx ny triangles (the
+    paper's 2D benchmark domain is such a rectangle, 20 x 7 mm)."""
+    i, j = np.meshgrid(np.arange(nx + 1), np.arange(ny + 1), indexing="ij")
+    xyz = np.stack([i.ravel() * h, j.ravel() * h, np.zeros(i.size)], axis=1).astype(np.float64)
+    nid = lambda a, b: a * (ny + 1) + b
+    ci, cj = np.meshgrid(np.arange(nx), np.arange(ny), indexing="ij")
+    ci, cj = ci.ravel(), cj.ravel()
+    t1 = np.stack([nid(ci, cj), nid(ci + 1, cj), nid(ci + 1, cj + 1)], axis=1)
+    t2 = np.stack([nid(ci, cj), nid(ci + 1, cj + 1), nid(ci, cj + 1)], axis=1)
+    tris = np.empty((2 * ci.size, 3), dtype=np.int32)
+    tris[0::2] = t1
+    tris[1::2] = t2
+    return TriMesh(xyz, tris, meta={"kind": "rect", "nx": nx, "ny": ny, "h": h})
+
+
+def jitter_interior_tri(mesh: TriMesh, amplitude: float, seed: int, out_of_plane: float = 0.0) -> None:
+    """Move the interior nodes of a rect_tri mesh by U(-a, a) per in-plane axis (and optionally out of the plane)."""
+    nx, ny, h = mesh.meta["nx"], mesh.meta["ny"], mesh.meta["h"]
+    x, y = mesh.xyz[:, 0], mesh.xyz[:, 1]
+    interior = (x > 0.5 * h) & (x < (nx - 0.5) * h) & (y > 0.5 * h) & (y < (ny - 0.5) * h)
+    ids = np.nonzero(interior)[0]
+    for d, amp in ((0, amplitude), (1, amplitude), (2, out_of_plane)):
+        if amp:
+            mesh.xyz[ids, d] += uniform(seed + d, ids, -amp, amp)
+
+
+def ellipsoid_surface(axes, z_cut: float, h: float, apex_hole: float = 1.0) -> TriMesh:
+    """Triangulated open ellipsoidal surface x^2/a^2 + y^2/b^2 + z^2/c^2 = 1 between the plane z = z_cut (base) and a small
+    hole around the apex (lowest point), on a structured (ring, azimuth) grid whose rings are about h apart and whose rings
+    carry a number of points proportional to their circumference (rounded to a multiple of 8).  Stand-in for the Purkinje
+    layer on a ventricular endocardium (a thin layer in the subendocardium)."""
+    a, b, c = axes
+    t_top = np.arccos(np.clip(z_cut / c, -1.0, 1.0))              # polar angle from +z of the base ring
+    t_bot = np.pi - apex_hole / max(a, b)                         # ring of radius ~apex_hole around the apex
+    # arc length along a meridian, numerically, to place rings ~h apart
+    tt = np.linspace(t_top, t_bot, 4001)
+    ds = np.hypot(a * np.cos(tt), c * np.sin(tt))
+    s = np.concatenate([[0.0], np.cumsum(0.5 * (ds[1:] + ds[:-1]) * np.diff(tt))])
+    n_rings = max(2, int(round(s[-1] / h)) + 1)
+    ring_t = np.interp(np.linspace(0.0, s[-1], n_rings), s, tt)
+    pts, ring_start, ring_n = [], [], []
+    for t in ring_t:
+        r = 0.5 * (a + b) * np.sin(t)
+        n = max(8, int(round(2.0 * np.pi * r / h / 8.0)) * 8)
+        ph = 2.0 * np.pi * np.arange(n) / n
+        ring_start.append(sum(ring_n))
+        ring_n.append(n)
+        pts.append(np.stack([a * np.sin(t) * np.cos(ph), b * np.sin(t) * np.sin(ph), np.full(n, c * np.cos(t))], axis=1))
+    xyz = np.concatenate(pts, axis=0)
+    tris = []
+    for k in range(n_rings - 1):        # stitch ring k (n0 points) to ring k+1 (n1 points) by advancing the lagging side
+        n0, n1, s0, s1 = ring_n[k], ring_n[k + 1], ring_start[k], ring_start[k + 1]
+        i = j = 0
+        while i < n0 or j < n1:
+            # next azimuth on each ring (as a fraction of the circle)
+            fi, fj = (i + 1) / n0, (j + 1) / n1
+            if j >= n1 or (i < n0 and fi <= fj):
+                tris.append((s0 + i % n0, s0 + (i + 1) % n0, s1 + j % n1))
+                i += 1
+            else:
+                tris.append((s0 + i % n0, s1 + (j + 1) % n1, s1 + j % n1))
+                j += 1
+    return TriMesh(xyz.astype(np.float64), np.array(tris, dtype=np.int32),
+                   meta={"kind": "ellipsoid_surface", "axes": tuple(axes), "z_cut": z_cut, "h": h})

@@ -56,7 +56,7 @@ constexpr int N_RLB = 10;    // gates of the rolled Rush-Larsen loop: oa oi ua u
 constexpr int N_EXPB = 12;   // their arguments + 2 pads, slots 0..11
 constexpr int B_INF0 = 12;   // steady states, slots 12..21
 constexpr int G_OLD0 = 36;   // gate values at t^n of those ten, slots 36..45
-constexpr int N_SLOTS = 46;
+constexpr int N_SLOTS = 48;   // 46, 47: pads read (not used) by the last trip of the Rush-Larsen loop
 static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && B_INF0 + N_RLB <= G_OLD0 && N_EXPA <= G_OLD0, "slot layout");
 
 // phi(x) = x/(e^x - 1) given e^x (reading B11)
@@ -70,26 +70,37 @@ __device__ __forceinline__ double phi(double x, double ex) {
 template <int BLOCK>
 __device__ __forceinline__ void crn_rush_larsen_slots(double* col, double* ycol, int64_t stride) {
     using namespace crn;
+    // software-pipelined like ep_exp2_slots (ep_math.cuh): next trip's exponents and this trip's steady states / old gate
+    // values are read before the polynomials run.  Slots B_INF0 + 10, 11 and G_OLD0 + 10, 11 are read but not used.
+    double e[EXP_W];
+#pragma unroll
+    for (int j = 0; j < EXP_W; ++j) e[j] = col[j * BLOCK];
 #pragma unroll 1
     for (int g = 0; g < N_EXPB; g += EXP_W) {
-        double e[EXP_W];
+        const int gn = (g + EXP_W < N_EXPB) ? g + EXP_W : g;
+        double ne[EXP_W], yi[EXP_W], yo[EXP_W];
 #pragma unroll
-        for (int j = 0; j < EXP_W; ++j) e[j] = col[(g + j) * BLOCK];
+        for (int j = 0; j < EXP_W; ++j) {
+            ne[j] = col[(gn + j) * BLOCK];
+            yi[j] = col[(B_INF0 + g + j) * BLOCK];
+            yo[j] = col[(G_OLD0 + g + j) * BLOCK];
+        }
         ep_exp2_wide<EXP_W>(e);
 #pragma unroll
         for (int j = 0; j < EXP_W; ++j) {
             if (g + j < N_RLB) {
-                const double yi = col[(B_INF0 + g + j) * BLOCK], yo = col[(G_OLD0 + g + j) * BLOCK];
                 const int row = (g + j < 8) ? C_OA + g + j : C_VG + (g + j - 8);
-                ycol[row * stride] = fma(yo - yi, e[j], yi);
+                ycol[row * stride] = fma(yo[j] - yi[j], e[j], yi[j]);
             }
         }
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) e[j] = ne[j];
     }
 }
 
 // One step of one cell (same contract as tp06_step).  Returns Vm^{n+1}.
-template <int BLOCK, class Issue, class Finish>
-__device__ __forceinline__ double crn_step(double v, double* ycol, int64_t stride, double dt, double istim,
+template <int BLOCK, class Stim, class Issue, class Finish>
+__device__ __forceinline__ double crn_step(double v, double* ycol, int64_t stride, double dt, Stim stimulus,
                                            Issue issue_gather, Finish finish_gather, double* col) {
     using namespace crn;
     const double vg = ep_clamp(v, -250.0, 250.0);   // argument of every transcendental
@@ -164,6 +175,7 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
     col[A_TU * BLOCK] = dtl * -0.125;     // tau_u = 8 ms
     ep_exp2_slots<N_EXPA, BLOCK, EXP_W>(col);
     const double dv_diff = finish_gather();   // the gathers have landed during the batch: 12 values -> 1
+    const double istim = stimulus();          // late on purpose: see tp06_step
     ep_cp_async_wait();                       // so have the gate values: products for the currents
     double gto3, gkur3, xr, xs2, gcal, uvw;
     {

@@ -161,34 +161,38 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
         }
         return (accn + accm) + accc;
     };
-    // S4: stimulus, eq. (4) PAPER.md:130-132 (window already resolved on the host into istim[k])
+    // S4: stimulus, eq. (4) PAPER.md:130-132 (window already resolved on the host into istim[k]).  The mask is requested
+    // here with the other loads; the cell model calls stimulus() after its first exponential batch, so nothing waits for it.
     const unsigned mask = a.smask[i];
-    double istim = 0.0;
-    if (mask != 0) {   // few cells belong to a stimulus slot: one test instead of eight for the others
-        const long long n = a.desc ? a.desc->n : a.inl.n;
+    auto stimulus = [&]() {
+        double istim = 0.0;
+        if (mask != 0) {   // few cells belong to a stimulus slot: one test instead of eight for the others
+            const long long n = a.desc ? a.desc->n : a.inl.n;
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            if (!(mask & (1u << k))) continue;
-            if (a.trig_slots & (1u << k)) {
-                // slot driven by a trigger: on for ndur steps starting nd steps after the monitored crossing.  A firing
-                // written by another thread of THIS launch cannot switch it on (n_on >= n + 1), so there is no race.
-                for (int t = 0; t < MAX_TRIGGERS; ++t) {
-                    const TrigPar p = a.trig_par[t];
-                    if (!p.armed || p.slot != k) continue;
-                    const long long nf = a.trig_fire[t];
-                    if (nf >= 0 && n >= nf + p.nd && n < nf + p.nd + p.ndur) istim += p.amp_cm;
+            for (int k = 0; k < 8; ++k) {
+                if (!(mask & (1u << k))) continue;
+                if (a.trig_slots & (1u << k)) {
+                    // slot driven by a trigger: on for ndur steps starting nd steps after the monitored crossing.  A firing
+                    // written by another thread of THIS launch cannot switch it on (n_on >= n + 1), so there is no race.
+                    for (int t = 0; t < MAX_TRIGGERS; ++t) {
+                        const TrigPar p = a.trig_par[t];
+                        if (!p.armed || p.slot != k) continue;
+                        const long long nf = a.trig_fire[t];
+                        if (nf >= 0 && n >= nf + p.nd && n < nf + p.nd + p.ndur) istim += p.amp_cm;
+                    }
+                } else {
+                    istim += a.desc ? a.desc->istim[k] : a.inl.istim[k];
                 }
-            } else {
-                istim += a.desc ? a.desc->istim[k] : a.inl.istim[k];
             }
         }
-    }
+        return istim;
+    };
     double v_new;
     if constexpr (MODEL == 0)
-        v_new = tp06_step<CELL_THREADS>(v_old, ycol, CELL_THREADS, a.ctype[i], a.dt, istim, issue_gather, finish_gather,
+        v_new = tp06_step<CELL_THREADS>(v_old, ycol, CELL_THREADS, a.ctype[i], a.dt, stimulus, issue_gather, finish_gather,
                                         &xs[0][threadIdx.x]);
     else
-        v_new = crn_step<CELL_THREADS>(v_old, ycol, CELL_THREADS, a.dt, istim, issue_gather, finish_gather,
+        v_new = crn_step<CELL_THREADS>(v_old, ycol, CELL_THREADS, a.dt, stimulus, issue_gather, finish_gather,
                                        &xs[0][threadIdx.x]);
     a.vm_next[i] = v_new;
     // S9: activation time = first upward crossing of 0 mV (reading A18)

@@ -128,6 +128,7 @@ __device__ __forceinline__ void ep_exp2_wide(double (&x)[W]) {
 template <int N, int BLOCK, int W>
 __device__ __forceinline__ void ep_exp2_slots(double* col, int n = N) {
     static_assert(N % W == 0, "pad the slot list to a multiple of W");
+#ifdef EP_SLOTS_UNPIPELINED
 #pragma unroll 1
     for (int s = 0; s < n; s += W) {
         double x[W];
@@ -137,6 +138,25 @@ __device__ __forceinline__ void ep_exp2_slots(double* col, int n = N) {
 #pragma unroll
         for (int j = 0; j < W; ++j) col[(s + j) * BLOCK] = x[j];
     }
+#else
+    // software-pipelined: the arguments of the next trip are read from shared memory before this trip's polynomials are
+    // evaluated, so no trip starts by waiting for its own loads (the last trip prefetches itself: values unused)
+    double x[W];
+#pragma unroll
+    for (int j = 0; j < W; ++j) x[j] = col[j * BLOCK];
+#pragma unroll 1
+    for (int s = 0; s < n; s += W) {
+        const int sn = (s + W < n) ? s + W : s;
+        double nx[W];
+#pragma unroll
+        for (int j = 0; j < W; ++j) nx[j] = col[(sn + j) * BLOCK];
+        ep_exp2_wide<W>(x);
+#pragma unroll
+        for (int j = 0; j < W; ++j) col[(s + j) * BLOCK] = x[j];
+#pragma unroll
+        for (int j = 0; j < W; ++j) x[j] = nx[j];
+    }
+#endif
 }
 
 // W logarithms at once, stage by stage (same arithmetic as ep_log_core); arguments positive and normal.

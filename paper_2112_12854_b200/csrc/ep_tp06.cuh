@@ -97,6 +97,7 @@ static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && N_EXPA <= G_OLD0 && 
 template <int BLOCK>
 __device__ __forceinline__ void tp06_rush_larsen_slots(double* col, double* ycol, int64_t stride) {
     using namespace tp06;
+#ifdef EP_SLOTS_UNPIPELINED
 #pragma unroll 1
     for (int g = 0; g < N_EXPB; g += EXP_W) {
         double e[EXP_W];
@@ -111,15 +112,40 @@ __device__ __forceinline__ void tp06_rush_larsen_slots(double* col, double* ycol
             }
         }
     }
+#else
+    // software-pipelined like ep_exp2_slots: next trip's exponents, and this trip's steady states / old gate values, are
+    // read before the polynomials run
+    double e[EXP_W];
+#pragma unroll
+    for (int j = 0; j < EXP_W; ++j) e[j] = col[j * BLOCK];
+#pragma unroll 1
+    for (int g = 0; g < N_EXPB; g += EXP_W) {
+        const int gn = (g + EXP_W < N_EXPB) ? g + EXP_W : g;
+        double ne[EXP_W], yi[EXP_W], yo[EXP_W];
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) {
+            ne[j] = col[(gn + j) * BLOCK];
+            yi[j] = col[(B_INF0 + g + j) * BLOCK];      // slot B_INF0 + 11 is the (unused) pad of the last trip
+            yo[j] = col[(G_OLD0 + g + j) * BLOCK];      // slot G_OLD0 + 11 = G_RBAR: read, not used
+        }
+        ep_exp2_wide<EXP_W>(e);
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j)
+            if (g + j < N_RLB) ycol[(1 + g + j) * stride] = fma(yo[j] - yi[j], e[j], yi[j]);
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) e[j] = ne[j];
+    }
+#endif
 }
 
 // One step of one cell, everything on the right-hand side at t^n.  v = Vm^n of this cell, ycol = &y[0][cell] (state
-// row k at ycol[k*stride]; rows 1..18 are read and overwritten), type: 0 endo, 1 mid, 2 epi, istim = I_s/C_m [uA/uF].
+// row k at ycol[k*stride]; rows 1..18 are read and overwritten), type: 0 endo, 1 mid, 2 epi, stimulus() returns
+// I_s/C_m [uA/uF] of this cell and step.
 // The diffusion term D_c/(chi C_m) [mV/ms] comes from two callables so that its gathers are in flight while the
 // logarithms and the first exponential batch run: issue_gather() starts the loads, finish_gather() returns the sum.
 // col = this thread's column of the block's slot array (stride BLOCK doubles, tp06::N_SLOTS slots).  Returns Vm^{n+1}.
-template <int BLOCK, class Issue, class Finish>
-__device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stride, int type, double dt, double istim,
+template <int BLOCK, class Stim, class Issue, class Finish>
+__device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stride, int type, double dt, Stim stimulus,
                                             Issue issue_gather, Finish finish_gather, double* col) {
     using namespace tp06;
     // Argument of every transcendental (reading T2).  TP06 lives in [-100, +60] mV; for |v| <= 200 mV every
@@ -194,6 +220,10 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     // warp-uniform trip count: during the plateau (every cell of the warp above -40 mV) the last trip is skipped
     ep_exp2_slots<N_EXPA, BLOCK, EXP_W>(col, __all_sync(__activemask(), hi) ? N_EXPA_HI : N_EXPA);
     const double dv_diff = finish_gather();   // the gathers have landed during the batch: 12 values -> 1
+    // I_s/C_m of this cell and step.  Evaluated here, not before the loads above: its first instruction waits for the
+    // cell's stimulus mask, and a wait at the top of the kernel would delay the issue of every other load by one DRAM
+    // round trip (profiles/r02a: two serialised long-scoreboard waits in the prologue, 12 % of all stall samples).
+    const double istim = stimulus();
     // gate values have landed too (finish_gather waited for this thread's asynchronous copies): products for the currents
     ep_cp_async_wait();
     double gNa, gCaL, gto, gKr, gKs;
