@@ -17,10 +17,14 @@ TP06_RANGES = [(-95.0, 45.0)] + [(0.0, 1.0)] * 13 + [(4e-5, 1.5e-3), (0.5, 4.5),
 CRN98_RANGES = [(-90.0, 35.0)] + [(0.0, 1.0)] * 15 + [(9.0, 14.0), (130.0, 142.0), (6e-5, 1.2e-3), (0.8, 2.2),
                                                        (0.3, 2.0)]
 
+# Stewart order: V y xr1 xr2 xs m h j d f f2 fCass s r R' Ca_i Ca_SR Ca_SS Na_i K_i
+STEWART_RANGES = [(-95.0, 50.0)] + [(0.0, 1.0)] * 14 + [(4e-5, 1.5e-3), (0.5, 4.5), (4e-5, 5e-3), (6.0, 12.0),
+                                                          (125.0, 142.0)]
+
 
 def random_states(model: int, seed: int, n: int) -> np.ndarray:
     """[S, n] float64; variable k of cell c is uniform in its range, from counter k*n + c."""
-    ranges = TP06_RANGES if model == 0 else CRN98_RANGES
+    ranges = TP06_RANGES if model == 0 else (CRN98_RANGES if model == 1 else STEWART_RANGES)
     out = np.empty((len(ranges), n))
     ctr = np.arange(n, dtype=np.uint64)
     for k, (lo, hi) in enumerate(ranges):

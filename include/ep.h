@@ -31,10 +31,11 @@ typedef struct ep_sim ep_sim; /* opaque; owns all host and device memory it allo
 
 enum { EP_OK = 0, EP_ERR_ARG = -1, EP_ERR_MESH = -2, EP_ERR_STATE = -3, EP_ERR_CUDA = -4, EP_ERR_NOMEM = -5,
        EP_ERR_NUMERIC = -6 };
-enum { EP_MODEL_TP06 = 0, EP_MODEL_CRN98 = 1 };
+enum { EP_MODEL_TP06 = 0, EP_MODEL_CRN98 = 1, EP_MODEL_STEWART = 2 };
 enum { EP_MAX_STIM_SLOTS = 8 };
 
-/* Number of state variables of a cell model, Vm included (TP06 19, Courtemanche 21); <0 if unknown. */
+/* Number of state variables of a cell model, Vm included (TP06 19, Courtemanche 21, Stewart 20); <0 if
+ * unknown. */
 int ep_model_n_states(int model);
 
 /* Build the simulation object: validate the mesh, run the one-time preprocessor (geometry, face matching, node stars,
@@ -52,9 +53,20 @@ int ep_mesh_create(ep_sim **out, int64_t n_nodes, const double *xyz_mm, int64_t 
                    const double *fibre, const double *sigma_scale, double sigma_l, double sigma_t, double chi,
                    double Cm);
 
+/* The same for a two-dimensional medium (the Purkinje network): a triangulated surface embedded in 3D,
+ * tris [n_tris*3].  PAPER.md:170: "a similar FV approach is used to discretize the ... equations over 1D and 2D media": the
+ * chain of PAPER.md:164-168 with edges for faces, edge lengths for face areas and triangle areas for cell volumes (a uniform
+ * layer thickness cancels); readings D1-D3 of DESIGN.md section 3.  Every other call works on the handle unchanged ("n_tets"
+ * then means the number of triangles, ep_mean_vm is area-weighted).  Errors as ep_mesh_create; EP_ERR_MESH also for an edge
+ * shared by more than two triangles. */
+int ep_mesh_create_tri(ep_sim **out, int64_t n_nodes, const double *xyz_mm, int64_t n_tris, const int32_t *tris,
+                       const double *fibre, const double *sigma_scale, double sigma_l, double sigma_t, double chi,
+                       double Cm);
+
 /* Choose the cell model and set every cell to an initial state.
  *   cell_type [n_tets] TP06: 0 endo, 1 mid, 2 epi (reading B5); NULL => 0
- *   y0        [n_types*S] one state vector per cell type (n_types = 3 for TP06, 1 for CRN98); NULL => built-in rest state
+ *   y0        [n_types*S] one state vector per cell type (n_types = 3 for TP06, 1 for CRN98 and STEWART); NULL => built-in
+ *             rest state (Stewart: the published initial state, a point of its spontaneous cycle -- the model has no rest)
  * Resets the step counter, the activation times (to -1) and keeps the stimulus slots. */
 int ep_state_init(ep_sim *sim, int model, const uint8_t *cell_type, const double *y0);
 
@@ -69,10 +81,21 @@ int ep_stimulus_set(ep_sim *sim, int slot, int64_t n_cells, const int64_t *cell_
  * as given to ep_stimulus_set, its own t_start ignored -- switches on delay_ms later (PAPER.md:196 uses 5 ms / 3 ms) for
  * its duration, on integer steps: steps n_fire + ceil(delay/dt) <= n < ... + ceil(duration/dt), n_fire = index after the
  * crossing step.  A trigger fires once; ep_state_init re-arms it.  trigger in [0, 4); n_monitor = 0 removes it.
- * A slot can be driven by one trigger only. */
+ * A slot can be driven by one trigger only.  slot = -1: monitor only -- the trigger records its firing time and drives no
+ * slot of this mesh (the coupling then goes to another handle through ep_couple). */
 int ep_trigger_set(ep_sim *sim, int trigger, int64_t n_monitor, const int64_t *monitor_ids, int slot, double delay_ms);
 /* Time (ms) at which the trigger fired = (crossing step + 1) * dt, or -1.  Synchronises. */
 int ep_trigger_time(ep_sim *sim, int trigger, double *t_fire_ms);
+
+/* Communication-node coupling ACROSS two handles (the 2D Purkinje sheet excites the 3D ventricular
+ * myocardium through the Purkinje-muscle junctions with an orthodromic delay of 5 ms; the bundles excite the
+ * atria; with the roles exchanged the same call gives the antidromic direction).  If trigger `trigger` of
+ * `src` has fired at t_f, stimulus slot `slot` of `dst` -- cells, amplitude and duration as given to ep_stimulus_set, e.g.
+ * the cells within R_S of the junction -- is scheduled to switch on at t_f + delay_ms; *scheduled = 1 from then on, 0 before.
+ * Call it between ep_step calls, both handles at the same time level, at intervals no longer than delay_ms: the trigger time
+ * is read from the device (synchronises src), the window is resolved on dst's integer steps (reading A16).
+ * EP_ERR_STATE if dst has already passed t_f + delay_ms (polled too late) or its slot has no cells. */
+int ep_couple(ep_sim *src, int trigger, ep_sim *dst, int slot, double delay_ms, int *scheduled);
 
 /* Advance n_steps explicit steps of size dt_ms (everything on the right-hand side at t^n; gates by
  * Rush-Larsen, the rest by forward Euler; v by eq. (7)).  Asynchronous on the sim's stream; errors are sticky.
@@ -167,6 +190,13 @@ int ep_host_stencil(int64_t n_nodes, const double *xyz_mm, int64_t n_tets, const
                     const double *sigma_scale, double sigma_l, double sigma_t, double chi, double Cm, int32_t *node,
                     double *a, int32_t *nbr, double *b, int64_t *node_ptr, int32_t *node_cell, double *w,
                     int32_t *perm);
+
+/* The same for a triangulated surface (ep_mesh_create_tri): node [n_tris*8] (3 own + up to 3 opposite nodes, rest unused),
+ * nbr / b [n_tris*4] (slot 3 unused), node_cell / w [n_tris*3]. */
+int ep_host_stencil_tri(int64_t n_nodes, const double *xyz_mm, int64_t n_tris, const int32_t *tris, const double *fibre,
+                        const double *sigma_scale, double sigma_l, double sigma_t, double chi, double Cm, int32_t *node,
+                        double *a, int32_t *nbr, double *b, int64_t *node_ptr, int32_t *node_cell, double *w,
+                        int32_t *perm);
 
 #ifdef __cplusplus
 }

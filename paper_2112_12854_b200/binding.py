@@ -8,7 +8,7 @@ import numpy as np
 
 from . import build as _build
 
-EP_MODEL_TP06, EP_MODEL_CRN98 = 0, 1
+EP_MODEL_TP06, EP_MODEL_CRN98, EP_MODEL_STEWART = 0, 1, 2
 _dp = C.POINTER(C.c_double)
 _i32p = C.POINTER(C.c_int32)
 _i64p = C.POINTER(C.c_int64)
@@ -20,10 +20,13 @@ SIGNATURES = {
     "ep_model_n_states": (C.c_int, [C.c_int]),
     "ep_mesh_create": (C.c_int, [C.POINTER(_vp), C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double,
                                  C.c_double, C.c_double]),
+    "ep_mesh_create_tri": (C.c_int, [C.POINTER(_vp), C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double,
+                                     C.c_double, C.c_double]),
     "ep_state_init": (C.c_int, [_vp, C.c_int, _u8p, _dp]),
     "ep_stimulus_set": (C.c_int, [_vp, C.c_int, C.c_int64, _i64p, C.c_double, C.c_double, C.c_double]),
     "ep_trigger_set": (C.c_int, [_vp, C.c_int, C.c_int64, _i64p, C.c_int, C.c_double]),
     "ep_trigger_time": (C.c_int, [_vp, C.c_int, _dp]),
+    "ep_couple": (C.c_int, [_vp, C.c_int, _vp, C.c_int, C.c_double, C.POINTER(C.c_int)]),
     "ep_step": (C.c_int, [_vp, C.c_int64, C.c_double]),
     "ep_synchronize": (C.c_int, [_vp]),
     "ep_read_vm": (C.c_int, [_vp, _dp]),
@@ -57,6 +60,8 @@ SIGNATURES = {
     "ep_last_error": (C.c_char_p, []),
     "ep_host_stencil": (C.c_int, [C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double, C.c_double,
                                   C.c_double, _i32p, _dp, _i32p, _dp, _i64p, _i32p, _dp, _i32p]),
+    "ep_host_stencil_tri": (C.c_int, [C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double, C.c_double,
+                                      C.c_double, _i32p, _dp, _i32p, _dp, _i64p, _i32p, _dp, _i32p]),
 }
 
 _lib = None
@@ -128,8 +133,26 @@ def host_stencil(xyz, tets, fibre=None, sigma_scale=None, sigma_l=1.3, sigma_t=0
     return out
 
 
+def host_stencil_tri(xyz, tris, fibre=None, sigma_scale=None, sigma_l=1.3, sigma_t=0.18, chi=1400.0, Cm=1.0):
+    """ep_host_stencil_tri: the factored stencil of a triangulated surface in the caller's numbering (no GPU needed)."""
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+    tris = np.ascontiguousarray(tris, dtype=np.int32)
+    fibre = None if fibre is None else np.ascontiguousarray(fibre, dtype=np.float64)
+    sigma_scale = None if sigma_scale is None else np.ascontiguousarray(sigma_scale, dtype=np.float64)
+    nn, nc = xyz.shape[0], tris.shape[0]
+    out = dict(node=np.empty((nc, 8), np.int32), a=np.empty((nc, 8)), nbr=np.empty((nc, 4), np.int32),
+               b=np.empty((nc, 4)), node_ptr=np.empty(nn + 1, np.int64), node_cell=np.empty(3 * nc, np.int32),
+               w=np.empty(3 * nc), perm=np.empty(nc, np.int32))
+    _chk(lib().ep_host_stencil_tri(nn, _p(xyz), nc, _p(tris, C.c_int32), _p(fibre), _p(sigma_scale), sigma_l, sigma_t,
+                                   chi, Cm, _p(out["node"], C.c_int32), _p(out["a"]), _p(out["nbr"], C.c_int32),
+                                   _p(out["b"]), _p(out["node_ptr"], C.c_int64), _p(out["node_cell"], C.c_int32),
+                                   _p(out["w"]), _p(out["perm"], C.c_int32)))
+    return out
+
+
 class Sim:
-    """One simulation handle (ep_sim*).  Method names follow the C-ABI calls."""
+    """One simulation handle (ep_sim*).  Method names follow the C-ABI calls.  cells [n,4]: tetrahedra (ep_mesh_create);
+    cells [n,3]: a triangulated surface (ep_mesh_create_tri)."""
 
     def __init__(self, xyz, tets, fibre=None, sigma_scale=None, sigma_l=1.3, sigma_t=0.18, chi=1400.0, Cm=1.0):
         xyz = np.ascontiguousarray(xyz, dtype=np.float64)
@@ -137,8 +160,9 @@ class Sim:
         fibre = None if fibre is None else np.ascontiguousarray(fibre, dtype=np.float64)
         sigma_scale = None if sigma_scale is None else np.ascontiguousarray(sigma_scale, dtype=np.float64)
         self._h = _vp()
-        _chk(lib().ep_mesh_create(C.byref(self._h), xyz.shape[0], _p(xyz), tets.shape[0], _p(tets, C.c_int32),
-                                  _p(fibre), _p(sigma_scale), sigma_l, sigma_t, chi, Cm))
+        create = lib().ep_mesh_create if tets.shape[1] == 4 else lib().ep_mesh_create_tri
+        _chk(create(C.byref(self._h), xyz.shape[0], _p(xyz), tets.shape[0], _p(tets, C.c_int32),
+                    _p(fibre), _p(sigma_scale), sigma_l, sigma_t, chi, Cm))
         self.n_tets = int(lib().ep_n_cells(self._h))
         self.n_nodes = int(lib().ep_n_nodes(self._h))
         self.n_states = 0
@@ -146,7 +170,8 @@ class Sim:
     @classmethod
     def from_problem(cls, prob):
         m = prob.mesh
-        s = cls(m.xyz, m.tets, m.fibre, m.sigma_scale, prob.sigma_l, prob.sigma_t, prob.chi, prob.Cm)
+        cells = m.tets if hasattr(m, "tets") else m.tris          # TetMesh or TriMesh (ep_inputs.meshes)
+        s = cls(m.xyz, cells, m.fibre, m.sigma_scale, prob.sigma_l, prob.sigma_t, prob.chi, prob.Cm)
         s.state_init(prob.model, m.cell_type)
         for k, st in enumerate(prob.stimuli):
             s.stimulus_set(k, st.cell_ids, st.amplitude, st.t_start, st.duration)
@@ -183,6 +208,12 @@ class Sim:
         d = C.c_double()
         _chk(lib().ep_trigger_time(self._h, int(trigger), C.byref(d)))
         return d.value
+
+    def couple(self, trigger, dst, slot, delay):
+        """ep_couple(self -> dst): True once dst's slot has been scheduled."""
+        f = C.c_int()
+        _chk(lib().ep_couple(self._h, int(trigger), dst._h, int(slot), float(delay), C.byref(f)))
+        return bool(f.value)
 
     def step(self, n_steps, dt):
         _chk(lib().ep_step(self._h, int(n_steps), float(dt)))

@@ -73,6 +73,7 @@ struct ep_sim {
     int graph_model = -1;
     cudaStream_t graph_stream = nullptr;
     int device = 0;                             // the device the handle was created on
+    int dim = 3;                                // 3: tetrahedra, 2: triangulated surface
     bool pdl = true;                            // programmatic dependent launch of the step kernels (EP_NO_PDL=1 disables)
     // bulk state I/O (ep_write_states / ep_read_states): second stream + events for a two-slot staging pipeline
     cudaStream_t io_stream = nullptr;
@@ -178,7 +179,7 @@ epk::StepArgs step_args(ep_sim* s, int cur, double dt) {
     a.y = s->d_y; a.vn = s->d_vn; a.ctype = s->d_ctype; a.smask = s->d_smask; a.tact = s->d_tact;
     a.tmask = s->d_tmask; a.trig_fire = s->d_trig_fire; a.trig_par = s->d_trig_par;
     a.trig_slots = 0;
-    for (const ep_sim::Trig& t : s->trig) if (t.armed) a.trig_slots |= 1u << t.slot;
+    for (const ep_sim::Trig& t : s->trig) if (t.armed && t.slot >= 0) a.trig_slots |= 1u << t.slot;
     a.dt = dt; a.desc = nullptr;
     return a;
 }
@@ -283,9 +284,10 @@ int ep_host_stencil(int64_t n_nodes, const double* xyz, int64_t n_tets, const in
     }
 }
 
-int ep_mesh_create(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_tets, const int32_t* tets,
-                   const double* fibre, const double* sigma_scale, double sigma_l, double sigma_t, double chi,
-                   double Cm) {
+// dim = 3: tetrahedra (cells [n*4]); dim = 2: triangles (cells [n*3])
+static int mesh_create_impl(ep_sim** out, int dim, int64_t n_nodes, const double* xyz, int64_t n_tets, const int32_t* tets,
+                            const double* fibre, const double* sigma_scale, double sigma_l, double sigma_t, double chi,
+                            double Cm) {
     if (!out) return fail(EP_ERR_ARG, "out is NULL");
     *out = nullptr;
     ep_sim* s = nullptr;
@@ -298,11 +300,13 @@ int ep_mesh_create(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_t
         ep::Stencil st;
         ep::Packed pk;
         std::string err;
-        int rc = ep::build_stencil(n_nodes, xyz, n_tets, tets, fibre, sigma_scale, sigma_l, sigma_t, chi, Cm, st, err);
+        int rc = dim == 3 ? ep::build_stencil(n_nodes, xyz, n_tets, tets, fibre, sigma_scale, sigma_l, sigma_t, chi, Cm, st, err)
+                          : ep::build_stencil_tri(n_nodes, xyz, n_tets, tets, fibre, sigma_scale, sigma_l, sigma_t, chi, Cm, st, err);
         if (rc) return fail(rc, err);
         rc = ep::pack(st, xyz, pk, err);
         if (rc) return fail(rc, err);
         s = new ep_sim();
+        s->dim = dim;
         cudaGetDevice(&s->device);
         s->pdl = (std::getenv("EP_NO_PDL") == nullptr);
         s->nc = pk.nc; s->nn = pk.nn; s->nc_pad = pk.nc_pad; s->chi = chi; s->Cm = Cm;
@@ -351,6 +355,48 @@ int ep_mesh_create(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_t
     }
 }
 
+int ep_host_stencil_tri(int64_t n_nodes, const double* xyz, int64_t n_tris, const int32_t* tris, const double* fibre,
+                        const double* sigma_scale, double sigma_l, double sigma_t, double chi, double Cm, int32_t* node,
+                        double* a, int32_t* nbr, double* b, int64_t* node_ptr, int32_t* node_cell, double* w,
+                        int32_t* perm) {
+    try {
+        ep::Stencil st;
+        std::string err;
+        int rc = ep::build_stencil_tri(n_nodes, xyz, n_tris, tris, fibre, sigma_scale, sigma_l, sigma_t, chi, Cm, st, err);
+        if (rc) return fail(rc, err);
+        if (node) std::memcpy(node, st.node.data(), sizeof(int32_t) * st.node.size());
+        if (a) std::memcpy(a, st.a.data(), sizeof(double) * st.a.size());
+        if (nbr) std::memcpy(nbr, st.nbr.data(), sizeof(int32_t) * st.nbr.size());
+        if (b) std::memcpy(b, st.b.data(), sizeof(double) * st.b.size());
+        if (node_ptr) std::memcpy(node_ptr, st.node_ptr.data(), sizeof(int64_t) * st.node_ptr.size());
+        if (node_cell) std::memcpy(node_cell, st.node_cell.data(), sizeof(int32_t) * st.node_cell.size());
+        if (w) std::memcpy(w, st.w.data(), sizeof(double) * st.w.size());
+        if (perm) {
+            ep::Packed pk;
+            rc = ep::pack(st, xyz, pk, err);
+            if (rc) return fail(rc, err);
+            std::memcpy(perm, pk.perm_c.data(), sizeof(int32_t) * pk.perm_c.size());
+        }
+        return EP_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(EP_ERR_NOMEM, "host allocation failed");
+    } catch (...) {
+        return fail(EP_ERR_ARG, "unexpected exception in preprocessor");
+    }
+}
+
+int ep_mesh_create(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_tets, const int32_t* tets,
+                   const double* fibre, const double* sigma_scale, double sigma_l, double sigma_t, double chi,
+                   double Cm) {
+    return mesh_create_impl(out, 3, n_nodes, xyz, n_tets, tets, fibre, sigma_scale, sigma_l, sigma_t, chi, Cm);
+}
+
+int ep_mesh_create_tri(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_tris, const int32_t* tris,
+                       const double* fibre, const double* sigma_scale, double sigma_l, double sigma_t, double chi,
+                       double Cm) {
+    return mesh_create_impl(out, 2, n_nodes, xyz, n_tris, tris, fibre, sigma_scale, sigma_l, sigma_t, chi, Cm);
+}
+
 void ep_destroy(ep_sim* s) {
     if (!s) return;
     cudaStreamSynchronize(s->stream);
@@ -371,7 +417,7 @@ int ep_state_init(ep_sim* s, int model, const uint8_t* cell_type, const double* 
     if (s->sticky == EP_ERR_CUDA) return fail(EP_ERR_CUDA, "sim is in a sticky CUDA error state");
     const int S = epk::model_n_states(model);
     if (S < 0) return fail(EP_ERR_ARG, "unknown cell model");
-    const int n_types = (model == EP_MODEL_TP06) ? 3 : 1;
+    const int n_types = (model == EP_MODEL_TP06) ? 3 : 1;   // Courtemanche and Stewart have one cell type
     if (y0)
         for (int k = 0; k < n_types * S; ++k)
             if (!std::isfinite(y0[k])) return fail(EP_ERR_ARG, "non-finite initial state");
@@ -459,11 +505,12 @@ int ep_step(ep_sim* s, int64_t n_steps, double dt) {
         epk::TrigPar par[epk::MAX_TRIGGERS];
         for (int t = 0; t < epk::MAX_TRIGGERS; ++t) {
             const ep_sim::Trig& g = s->trig[t];
+            const bool drives = g.armed && g.slot >= 0;   // slot -1: monitor only (cross-handle coupling, ep_couple)
             par[t].armed = g.armed ? 1 : 0;
             par[t].slot = g.slot;
             par[t].nd = (int32_t)step_index(g.delay, dt);
-            par[t].ndur = g.armed ? (int32_t)step_index(s->stim[g.slot].dur, dt) : 0;
-            par[t].amp_cm = g.armed ? s->stim[g.slot].amp / s->Cm : 0.0;
+            par[t].ndur = drives ? (int32_t)step_index(s->stim[g.slot].dur, dt) : 0;
+            par[t].amp_cm = drives ? s->stim[g.slot].amp / s->Cm : 0.0;
         }
         EP_CUDA(s, cudaStreamSynchronize(s->stream));
         EP_CUDA(s, cudaMemcpy(s->d_trig_par, par, sizeof(par), cudaMemcpyHostToDevice));
@@ -713,12 +760,12 @@ int ep_trigger_set(ep_sim* s, int trigger, int64_t n_monitor, const int64_t* mon
     if (!s) return fail(EP_ERR_ARG, "null sim handle");
     if (trigger < 0 || trigger >= epk::MAX_TRIGGERS) return fail(EP_ERR_ARG, "trigger index out of range");
     if (n_monitor < 0 || (n_monitor > 0 && !monitor_ids)) return fail(EP_ERR_ARG, "bad monitor cell list");
-    if (n_monitor > 0 && (slot < 0 || slot >= EP_MAX_STIM_SLOTS)) return fail(EP_ERR_ARG, "stimulus slot out of range");
+    if (n_monitor > 0 && (slot < -1 || slot >= EP_MAX_STIM_SLOTS)) return fail(EP_ERR_ARG, "stimulus slot out of range");
     if (!std::isfinite(delay_ms) || delay_ms < 0.0) return fail(EP_ERR_ARG, "delay must be finite and non-negative");
     for (int64_t k = 0; k < n_monitor; ++k)
         if (monitor_ids[k] < 0 || monitor_ids[k] >= s->nc) return fail(EP_ERR_ARG, "monitor cell id out of range");
     for (int t = 0; t < epk::MAX_TRIGGERS; ++t)
-        if (n_monitor > 0 && t != trigger && s->trig[t].armed && s->trig[t].slot == slot)
+        if (n_monitor > 0 && slot >= 0 && t != trigger && s->trig[t].armed && s->trig[t].slot == slot)
             return fail(EP_ERR_ARG, "stimulus slot is already driven by another trigger");
     const uint8_t bit = (uint8_t)(1u << trigger);
     for (int64_t i = 0; i < s->nc; ++i) s->tmask_host[i] &= (uint8_t)~bit;
@@ -741,6 +788,27 @@ int ep_trigger_time(ep_sim* s, int trigger, double* t_fire_ms) {
     EP_CUDA(s, cudaMemcpyAsync(&n1, s->d_trig_fire + trigger, sizeof(n1), cudaMemcpyDeviceToHost, s->stream));
     EP_CUDA(s, cudaStreamSynchronize(s->stream));
     *t_fire_ms = n1 < 0 ? -1.0 : (double)n1 * s->dt;
+    return EP_OK;
+}
+
+int ep_couple(ep_sim* src, int trigger, ep_sim* dst, int slot, double delay_ms, int* scheduled) {
+    if (!src || !dst || !scheduled) return fail(EP_ERR_ARG, "null argument");
+    if (slot < 0 || slot >= EP_MAX_STIM_SLOTS) return fail(EP_ERR_ARG, "stimulus slot out of range");
+    if (!std::isfinite(delay_ms) || delay_ms < 0.0) return fail(EP_ERR_ARG, "delay must be finite and non-negative");
+    if (!dst->stim[slot].set) return fail(EP_ERR_STATE, "destination slot has no cells: call ep_stimulus_set first");
+    *scheduled = 0;
+    double t_fire = -1.0;
+    int rc = ep_trigger_time(src, trigger, &t_fire);
+    if (rc) return rc;
+    if (t_fire < 0.0) return EP_OK;
+    const double t_on = t_fire + delay_ms;
+    if (dst->stim[slot].t0 == t_on) { *scheduled = 1; return EP_OK; }     // already scheduled by an earlier poll
+    // windows live on integer steps of the destination (reading A16): the first active step must not be in its past
+    if (dst->dt > 0.0 && step_index(t_on, dst->dt) < dst->step)
+        return fail(EP_ERR_STATE, "ep_couple polled too late: the stimulus would have started in the destination's past");
+    dst->stim[slot].t0 = t_on;
+    dst->trig_dirty = true;   // (a trigger of dst driving this slot caches its parameters)
+    *scheduled = 1;
     return EP_OK;
 }
 

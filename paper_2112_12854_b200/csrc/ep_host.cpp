@@ -248,6 +248,180 @@ int build_stencil(int64_t nn, const double* xyz, int64_t nc, const int32_t* tets
     return 0;
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// Two-dimensional media ("a similar FV approach is used to discretize the bidomain/monodomain equations over
+// 1D and 2D media"): triangles for tetrahedra, edges for faces, edge lengths for face areas, triangle areas for cell volumes.
+// The chain of PAPER.md:164-168 folds into the same factored form with 3 own + <= 3 opposite nodes and 3 edge neighbours, so
+// the tables keep their 8 + 4 width (unused slots: coefficient 0) and the device kernels are the three-dimensional ones.
+// Readings D1-D3 of DESIGN.md: edge value = mean of its two nodal values; each cell gradient lies in its own triangle's
+// plane, neighbouring gradients are combined as 3D vectors and the flux uses the in-plane outward edge normal of the cell
+// being summed; M_c = scale [sigma_t I + (sigma_l - sigma_t) f f^T].
+int build_stencil_tri(int64_t nn, const double* xyz, int64_t nc, const int32_t* tris, const double* fibre,
+                      const double* scale, double sigma_l, double sigma_t, double chi, double Cm, Stencil& out,
+                      std::string& err) {
+    if (nn <= 0 || nc <= 0 || !xyz || !tris) { err = "null pointer or non-positive mesh size"; return ERR_ARG; }
+    if (nn > 2000000000LL || nc > 500000000LL) { err = "mesh too large for int32 device indices"; return ERR_ARG; }
+    if (!(sigma_l > 0.0) || !(sigma_t > 0.0) || !(chi > 0.0) || !(Cm > 0.0)) {
+        err = "sigma_l, sigma_t, chi and Cm must be positive";
+        return ERR_ARG;
+    }
+    for (int64_t i = 0; i < 3 * nn; ++i)
+        if (!std::isfinite(xyz[i])) { err = "non-finite node coordinate"; return ERR_MESH; }
+    auto P = [&](int32_t n) { return V3{xyz[3 * (int64_t)n], xyz[3 * (int64_t)n + 1], xyz[3 * (int64_t)n + 2]}; };
+    struct TriGeom { V3 xc; double area; V3 opp[3]; V3 glam[3]; V3 xm[3]; };
+    std::vector<TriGeom> g(nc);
+    std::vector<Tensor> M(nc);
+    for (int64_t c = 0; c < nc; ++c) {
+        const int32_t* t = tris + 3 * c;
+        for (int k = 0; k < 3; ++k)
+            if (t[k] < 0 || t[k] >= nn) { err = "triangle node index out of range"; return ERR_MESH; }
+        if (t[0] == t[1] || t[1] == t[2] || t[0] == t[2]) { err = "triangle with a repeated node"; return ERR_MESH; }
+        const V3 p[3] = {P(t[0]), P(t[1]), P(t[2])};
+        TriGeom& G = g[c];
+        G.xc = scl(1.0 / 3.0, add(add(p[0], p[1]), p[2]));
+        const V3 N = crs(sub(p[1], p[0]), sub(p[2], p[0]));
+        const double n2 = len(N);
+        G.area = 0.5 * n2;
+        if (!(G.area > 0.0)) { err = "degenerate triangle (zero area)"; return ERR_MESH; }
+        const V3 nu = scl(1.0 / n2, N);
+        for (int n = 0; n < 3; ++n) {
+            const V3 a = p[(n + 1) % 3], b = p[(n + 2) % 3];
+            V3 s = crs(sub(b, a), nu);                                   // in-plane normal of the edge opposite vertex n
+            if (dot(s, sub(p[n], a)) > 0.0) s = scl(-1.0, s);            // the opposite vertex lies inside
+            G.opp[n] = s;
+            G.glam[n] = scl(-1.0 / (2.0 * G.area), s);                   // gradient of the barycentric function of vertex n
+            G.xm[n] = scl(0.5, add(a, b));
+        }
+        double sc = scale ? scale[c] : 1.0;
+        if (!std::isfinite(sc) || sc < 0.0) { err = "sigma_scale must be finite and non-negative"; return ERR_ARG; }
+        double sl = sigma_l, st = sigma_t;
+        V3 f = {0, 0, 0};
+        if (fibre) {
+            f = {fibre[3 * c], fibre[3 * c + 1], fibre[3 * c + 2]};
+            const double n = len(f);
+            if (!(n > 0.0) || !std::isfinite(n)) { err = "zero or non-finite fibre vector"; return ERR_MESH; }
+            f = scl(1.0 / n, f);
+        } else {
+            st = sl;
+        }
+        const double dl = sl - st;
+        M[c] = {sc * (st + dl * f.x * f.x), sc * dl * f.x * f.y, sc * dl * f.x * f.z,
+                sc * (st + dl * f.y * f.y), sc * dl * f.y * f.z, sc * (st + dl * f.z * f.z)};
+    }
+    // ---- edge matching, bucketed by the smaller node id
+    out.nn = nn; out.nc = nc;
+    out.nbr.assign(4 * nc, -1);
+    {
+        struct EdgeRec { int32_t b; int32_t cell; int32_t j; };
+        std::vector<int64_t> ptr(nn + 1, 0);
+        auto ends = [&](int64_t c, int j, int32_t& a, int32_t& b) {
+            a = tris[3 * c + (j + 1) % 3]; b = tris[3 * c + (j + 2) % 3];
+            if (a > b) std::swap(a, b);
+        };
+        for (int64_t c = 0; c < nc; ++c)
+            for (int j = 0; j < 3; ++j) { int32_t a, b; ends(c, j, a, b); ptr[a + 1]++; }
+        for (int64_t n = 0; n < nn; ++n) ptr[n + 1] += ptr[n];
+        std::vector<EdgeRec> rec(3 * nc);
+        std::vector<int64_t> fill(ptr.begin(), ptr.end() - 1);
+        for (int64_t c = 0; c < nc; ++c)
+            for (int j = 0; j < 3; ++j) { int32_t a, b; ends(c, j, a, b); rec[fill[a]++] = {b, (int32_t)c, j}; }
+        for (int64_t n = 0; n < nn; ++n) {
+            EdgeRec* lo = rec.data() + ptr[n];
+            EdgeRec* hi = rec.data() + ptr[n + 1];
+            std::sort(lo, hi, [](const EdgeRec& p, const EdgeRec& q) { return p.b != q.b ? p.b < q.b : p.cell < q.cell; });
+            for (EdgeRec* r = lo; r < hi;) {
+                EdgeRec* e = r + 1;
+                while (e < hi && e->b == r->b) ++e;
+                if (e - r > 2) { err = "edge shared by more than two triangles"; return ERR_MESH; }
+                if (e - r == 2) {
+                    out.nbr[4 * (int64_t)r[0].cell + r[0].j] = r[1].cell;
+                    out.nbr[4 * (int64_t)r[1].cell + r[1].j] = r[0].cell;
+                }
+                r = e;
+            }
+        }
+    }
+    // ---- node stars with normalised inverse-distance weights
+    out.node_ptr.assign(nn + 1, 0);
+    for (int64_t c = 0; c < nc; ++c) for (int k = 0; k < 3; ++k) out.node_ptr[tris[3 * c + k] + 1]++;
+    for (int64_t n = 0; n < nn; ++n) out.node_ptr[n + 1] += out.node_ptr[n];
+    out.node_cell.resize(3 * nc); out.w.resize(3 * nc);
+    {
+        std::vector<int64_t> fill(out.node_ptr.begin(), out.node_ptr.end() - 1);
+        for (int64_t c = 0; c < nc; ++c)
+            for (int k = 0; k < 3; ++k) {
+                const int32_t n = tris[3 * c + k];
+                const int64_t p = fill[n]++;
+                out.node_cell[p] = (int32_t)c;
+                out.w[p] = 1.0 / len(sub(P(n), g[c].xc));
+            }
+        for (int64_t n = 0; n < nn; ++n) {
+            double s = 0.0;
+            for (int64_t p = out.node_ptr[n]; p < out.node_ptr[n + 1]; ++p) s += out.w[p];
+            for (int64_t p = out.node_ptr[n]; p < out.node_ptr[n + 1]; ++p) out.w[p] /= s;
+        }
+    }
+    // ---- per-cell coefficients: same algebra as in three dimensions
+    out.node.resize(8 * nc); out.a.assign(8 * nc, 0.0); out.b.assign(4 * nc, 0.0);
+    out.centroid.resize(3 * nc);
+    out.vol.resize(nc);
+    for (int64_t c = 0; c < nc; ++c) {
+        const int32_t* t = tris + 3 * c;
+        const TriGeom& G = g[c];
+        out.vol[c] = G.area;
+        out.centroid[3 * c] = G.xc.x; out.centroid[3 * c + 1] = G.xc.y; out.centroid[3 * c + 2] = G.xc.z;
+        int32_t slot[8];
+        double a[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        int ns = 3;
+        for (int k = 0; k < 3; ++k) slot[k] = t[k];
+        const double unit = 100.0 / (G.area * chi * Cm);
+        out.nbr[4 * c + 3] = (int32_t)c;                                    // fourth neighbour slot is never used
+        for (int j = 0; j < 3; ++j) {
+            const int64_t c2 = out.nbr[4 * c + j];
+            if (c2 < 0) { out.nbr[4 * c + j] = (int32_t)c; continue; }      // boundary edge: zero flux
+            const TriGeom& H = g[c2];
+            // reading D2: the flux through an edge uses the in-plane edge normal of the LOWER-numbered of its two cells
+            // (single-valued flux, conservative on a curved surface); from the other side it is that vector reversed
+            V3 s = G.opp[j];
+            if (c2 < c) {
+                const int32_t ea = t[(j + 1) % 3], eb = t[(j + 2) % 3];
+                const int32_t* u2 = tris + 3 * c2;
+                int j2 = 0;
+                for (int q = 0; q < 3; ++q) {
+                    const int32_t fa = u2[(q + 1) % 3], fb = u2[(q + 2) % 3];
+                    if ((fa == ea && fb == eb) || (fa == eb && fb == ea)) j2 = q;
+                }
+                s = scl(-1.0, H.opp[j2]);
+            }
+            const double d1 = len(sub(G.xm[j], G.xc)), d2 = len(sub(G.xm[j], H.xc));
+            const double al1 = d2 / (d1 + d2), al2 = d1 / (d1 + d2);
+            const Tensor& A = M[c]; const Tensor& B = M[c2];
+            const Tensor Mf = {al1 * A.xx + al2 * B.xx, al1 * A.xy + al2 * B.xy, al1 * A.xz + al2 * B.xz,
+                               al1 * A.yy + al2 * B.yy, al1 * A.yz + al2 * B.yz, al1 * A.zz + al2 * B.zz};
+            const V3 dc = sub(G.xc, H.xc);
+            const double d = len(dc);
+            const V3 e = scl(1.0 / d, dc);
+            const V3 q = apply(Mf, s);
+            const double qe = dot(q, e);
+            const V3 p = sub(q, scl(qe, e));
+            out.b[4 * c + j] = -unit * qe / d;
+            for (int k = 0; k < 3; ++k) a[k] += unit * al1 * dot(p, G.glam[k]);
+            const int32_t* t2 = tris + 3 * c2;
+            for (int k = 0; k < 3; ++k) {
+                int m = 0;
+                while (m < ns && slot[m] != t2[k]) ++m;
+                if (m == ns) slot[ns++] = t2[k];                            // at most 3 + 3 distinct nodes
+                a[m] += unit * al2 * dot(p, H.glam[k]);
+            }
+        }
+        for (int m = 0; m < 8; ++m) {
+            out.node[8 * c + m] = m < ns ? slot[m] : slot[0];
+            out.a[8 * c + m] = m < ns ? a[m] : 0.0;
+        }
+    }
+    return 0;
+}
+
 int pack(const Stencil& st, const double* xyz, Packed& out, std::string& err) {
     (void)err;
     const int64_t nc = st.nc, nn = st.nn;

@@ -28,8 +28,8 @@ struct Stencil {              // caller numbering
     std::vector<int32_t> nbr;      // [nc*4] face-neighbour cell (face j is opposite vertex j); boundary => c itself
     std::vector<double> b;         // [nc*4] (0 on boundary faces: no-flux, reading A11)
     std::vector<int64_t> node_ptr; // [nn+1]
-    std::vector<int32_t> node_cell;// [nc*4] star cells, ascending cell id
-    std::vector<double> w;         // [nc*4] inverse-distance weights, normalised per node
+    std::vector<int32_t> node_cell;// [nc*4] ([nc*3] for triangles) star cells, ascending cell id
+    std::vector<double> w;         // same length: inverse-distance weights, normalised per node
     std::vector<double> centroid;  // [nc*3]
     std::vector<double> vol;       // [nc] cell volumes, mm^3
 };
@@ -57,6 +57,10 @@ struct Packed {               // device numbering and device layout
 int build_stencil(int64_t nn, const double* xyz, int64_t nc, const int32_t* tets, const double* fibre,
                   const double* scale, double sigma_l, double sigma_t, double chi, double Cm, Stencil& out,
                   std::string& err);
+// The same for a triangulated surface (tris [nc*3]); the tables keep the 8 + 4 layout, unused slots have coefficient 0.
+int build_stencil_tri(int64_t nn, const double* xyz, int64_t nc, const int32_t* tris, const double* fibre,
+                      const double* scale, double sigma_l, double sigma_t, double chi, double Cm, Stencil& out,
+                      std::string& err);
 int pack(const Stencil& st, const double* xyz, Packed& out, std::string& err);
 
 }  // namespace ep

@@ -10,6 +10,7 @@
 #include <algorithm>
 #include "ep_tp06.cuh"
 #include "ep_crn98.cuh"
+#include "ep_stewart.cuh"
 
 namespace epk {
 
@@ -103,7 +104,8 @@ __global__ void __launch_bounds__(CELL_THREADS) diffusion_only_kernel(int64_t nc
     out[i] = diffusion_gather(i, cidx, ccoef, vm, vn, vm[i]);
 }
 
-// S2..S9 fused.  One thread per cell; state rows are read once and written once.  MODEL 0: TP06, 1: Courtemanche.
+// S2..S9 fused.  One thread per cell; state rows are read once and written once.  MODEL 0: TP06, 1: Courtemanche,
+// 2: Stewart (Purkinje).
 #ifndef EP_CELL_MIN_BLOCKS
 #define EP_CELL_MIN_BLOCKS 4
 #endif
@@ -114,8 +116,8 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
                                                                                      StepArgs a) {
     // per-thread columns of the transcendental batches (ep_math.cuh): slot s of thread t at xs[s][t]
     // TP06 also keeps its 12 stencil coefficients there (copied in asynchronously: no registers held until they are used)
-    constexpr bool CF_SMEM = (MODEL == 0);
-    constexpr int MSLOTS = (MODEL == 0) ? tp06::N_SLOTS : crn::N_SLOTS;
+    constexpr bool CF_SMEM = (MODEL != 1);
+    constexpr int MSLOTS = (MODEL == 0) ? tp06::N_SLOTS : (MODEL == 1 ? crn::N_SLOTS : stw::N_SLOTS);
     constexpr int NSLOTS = MSLOTS + (CF_SMEM ? 12 : 0);
     __shared__ double xs[NSLOTS][CELL_THREADS];
     const int64_t i = (int64_t)blockIdx.x * CELL_THREADS + threadIdx.x;
@@ -123,7 +125,7 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     if (i >= nc) return;
     const double v_old = a.vm_cur[i];
     // tile-major tables: every row of this block's tile is at a compile-time offset from these three pointers
-    constexpr int S = (MODEL == 0) ? (int)TP06_S : (int)CRN_S;
+    constexpr int S = (MODEL == 0) ? (int)TP06_S : (MODEL == 1 ? (int)CRN_S : (int)STW_S);
     const int32_t* tidx = cidx + (int64_t)blockIdx.x * (12 * CELL_THREADS) + threadIdx.x;
     const double* tcoef = ccoef + (int64_t)blockIdx.x * (12 * CELL_THREADS) + threadIdx.x;
     double* ycol = a.y + (int64_t)blockIdx.x * (S * CELL_THREADS) + threadIdx.x;
@@ -191,8 +193,11 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     if constexpr (MODEL == 0)
         v_new = tp06_step<CELL_THREADS>(v_old, ycol, CELL_THREADS, a.ctype[i], a.dt, stimulus, issue_gather, finish_gather,
                                         &xs[0][threadIdx.x]);
-    else
+    else if constexpr (MODEL == 1)
         v_new = crn_step<CELL_THREADS>(v_old, ycol, CELL_THREADS, a.dt, stimulus, issue_gather, finish_gather,
+                                       &xs[0][threadIdx.x]);
+    else
+        v_new = stw_step<CELL_THREADS>(v_old, ycol, CELL_THREADS, a.dt, stimulus, issue_gather, finish_gather,
                                        &xs[0][threadIdx.x]);
     a.vm_next[i] = v_new;
     // S9: activation time = first upward crossing of 0 mV (reading A18)
@@ -215,7 +220,8 @@ __global__ void state_fill_kernel(int S, int64_t nc, int64_t nc_pad, const uint8
     if (i >= nc_pad) return;
     const int t = (i < nc) ? ctype[i] : 0;
     for (int k = 0; k < S; ++k) {
-        const double val = y0 ? y0[t * S + k] : (S == (int)TP06_S ? TP06_REST_STATE[k] : CRN_REST_STATE[k]);
+        const double val = y0 ? y0[t * S + k]
+                              : (S == (int)TP06_S ? TP06_REST_STATE[k] : (S == (int)CRN_S ? CRN_REST_STATE[k] : STW_INIT_STATE[k]));
         if (k == 0) vm[i] = val; else y[tile_index(i, k, S)] = val;
     }
     tact[i] = -1.0;
@@ -341,7 +347,7 @@ double launch_dfma_rate(double* scratch, int64_t scratch_len, int iters, cudaStr
     return (double)blocks * (threads / 32) * (double)iters * 32.0;   // warp-wide DFMAs issued
 }
 
-int model_n_states(int model) { return model == 0 ? (int)TP06_S : (model == 1 ? (int)CRN_S : -1); }
+int model_n_states(int model) { return model == 0 ? (int)TP06_S : (model == 1 ? (int)CRN_S : (model == 2 ? (int)STW_S : -1)); }
 
 // kernel launch with the programmatic-stream-serialisation attribute (see the PDL note at the top of this file)
 template <class... KArgs, class... Args>
@@ -363,7 +369,8 @@ void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaS
 void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStream_t s, bool pdl) {
     const unsigned grid = blocks_for(m.nc, CELL_THREADS);
     if (model == 0) launch_pdl(cell_step_kernel<0>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
-    else launch_pdl(cell_step_kernel<1>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
+    else if (model == 1) launch_pdl(cell_step_kernel<1>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
+    else launch_pdl(cell_step_kernel<2>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
 }
 
 void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* vn, double* out, cudaStream_t s) {
@@ -400,7 +407,7 @@ void launch_weighted_sum(int64_t n, const double* x, const double* w, double* pa
 }
 void launch_state_scan(int model, int64_t nc, const double* vm, const double* y, unsigned long long* counts,
                        cudaStream_t s) {
-    const int S = model_n_states(model), conc0 = (model == 0) ? (int)Y_CAI : (int)C_NAI;
+    const int S = model_n_states(model), conc0 = (model == 0) ? (int)Y_CAI : (model == 1 ? (int)C_NAI : (int)W_CAI);
     state_scan_kernel<<<1184, 256, 0, s>>>(S, conc0, nc, vm, y, counts);
 }
 void launch_scale_by_inv_norm(int64_t n, const double* x, const double* norm2, double* out, cudaStream_t s) {

@@ -113,3 +113,54 @@ def test_dense_assembly_matches_factored_stencil(oracle):
     assert np.all(np.diag(A) < 0)
     lam = np.linalg.eigvals(A)
     assert lam.real.max() <= 1e-9 * scale                          # stable with eq. (8)
+
+
+def _tri_cases():
+    m = M.rect_tri(13, 9, 0.3)
+    M.jitter_interior_tri(m, 0.06, 5, out_of_plane=0.05)
+    cen = m.centroids()
+    th = np.deg2rad(10 + 50 * cen[:, 1] / 2.7)
+    m.fibre = np.stack([np.cos(th), np.sin(th), 0 * th], axis=1)
+    m.sigma_scale = uniform(14, np.arange(m.n_tris), 0.1, 1.0)
+    yield "bumpy_sheet", m, 2.0, 0.5
+    yield "purkinje_surface_coarse", M.ellipsoid_surface((25.0, 25.0, 50.0), 20.0, 3.0), 39.5, 39.5
+
+
+@pytest.mark.parametrize("name,mesh,sl,st_", list(_tri_cases()))
+def test_factored_stencil_of_a_triangulated_surface_equals_the_2d_oracle(name, mesh, sl, st_):
+    """ep_host_stencil_tri against the edge-walking 2D oracle on random fields; table structure."""
+    import paper_2112_12854_b200 as ep
+    from oracle import ep_oracle2d as O2
+    chi, Cm = 1400.0, 1.0
+    st = ep.host_stencil_tri(mesh.xyz, mesh.tris, mesh.fibre, mesh.sigma_scale, sl, st_, chi, Cm)
+    osim = O2.OracleSim2D(mesh.xyz, mesh.tris, mesh.fibre, mesh.sigma_scale, sl, st_, chi, Cm)
+    for seed in (1, 2):
+        v = uniform(seed, np.arange(mesh.n_tris), -90.0, 40.0)
+        D_o = osim.apply_diffusion(v)
+        D_h, vn = _apply(st, v, chi * Cm)
+        assert np.abs(D_h - D_o).max() <= 1e-12 * np.abs(D_o).max(), name
+        assert np.abs(vn - osim.node_values(v)).max() <= 1e-13 * 90.0
+    nc = mesh.n_tris
+    assert np.all(st["node"][:, :3] == mesh.tris)                  # own nodes first
+    assert np.all(st["a"][:, 6:] == 0.0) and np.all(st["b"][:, 3] == 0.0)     # 3 + 3 nodes, 3 neighbours
+    bnd = st["nbr"] == np.arange(nc)[:, None]
+    assert np.all(st["b"][bnd] == 0.0)
+    assert np.abs(st["a"].sum(axis=1)).max() <= 1e-9 * np.abs(st["a"]).max()  # uniform field -> zero
+    deg = np.diff(st["node_ptr"])
+    assert deg.sum() == 3 * nc and deg.min() >= 1
+    assert sorted(st["perm"].tolist()) == list(range(nc))
+
+
+def test_triangle_mesh_errors():
+    import paper_2112_12854_b200 as ep
+    m = M.rect_tri(2, 2, 1.0)
+    bad = m.tris.copy(); bad[0, 0] = 99
+    with pytest.raises(ep.EpError) as e:
+        ep.host_stencil_tri(m.xyz, bad)
+    assert e.value.code == -2
+    flat = m.xyz.copy(); flat[:, 1] = 0.0                          # every triangle degenerate
+    with pytest.raises(ep.EpError):
+        ep.host_stencil_tri(flat, m.tris)
+    three = np.vstack([m.tris, [[0, 1, 8]], [[0, 1, 7]]]).astype(np.int32)     # edge (0,1) now in three triangles
+    with pytest.raises(ep.EpError):
+        ep.host_stencil_tri(m.xyz, three)
