@@ -414,6 +414,9 @@ struct Sim {
     // scratch
     std::vector<double> vn, D, flux;
     std::vector<Vec3> grad;
+    // bidomain (eq. (1) / (6)): extra right-hand-side term div(M_int grad v_ext)/(chi C_m) per cell,
+    // in mV/ms, supplied by the caller (oracle/ep_oracle_bidomain.py); empty = monodomain
+    std::vector<double> dv_src;
 };
 
 const int FACE_NODES[4][3] = {{1, 2, 3}, {0, 2, 3}, {0, 1, 3}, {0, 1, 2}};  // face j is opposite vertex j
@@ -702,8 +705,9 @@ int orc_step(void* h, int64_t n_steps, double dt) {
             for (int k = 0; k < s.S; ++k) y[k] = s.y[(size_t)k * nc + c];
             double Is = 0.0;   // uA/cm^2, eq. (4)
             for (int k = 0; k < 8; ++k) if (on[k] && s.stim[k].mask[c]) Is += s.stim[k].amp;
-            if (s.model == 0) tp06_step(y, s.ctype[c], dt, Is / s.Cm, s.D[c] * inv_chiCm, yn);
-            else crn::step(y, dt, Is / s.Cm, s.D[c] * inv_chiCm, yn);
+            const double dvd = s.D[c] * inv_chiCm + (s.dv_src.empty() ? 0.0 : s.dv_src[c]);
+            if (s.model == 0) tp06_step(y, s.ctype[c], dt, Is / s.Cm, dvd, yn);
+            else crn::step(y, dt, Is / s.Cm, dvd, yn);
             for (int k = 0; k < s.S; ++k) s.yn[(size_t)k * nc + c] = yn[k];
             if (s.tact[c] < 0.0 && y[0] <= 0.0 && yn[0] > 0.0) s.tact[c] = (double)(n + 1) * dt;   // A18
         }
@@ -717,6 +721,12 @@ int orc_step(void* h, int64_t n_steps, double dt) {
         s.step = n + 1;
     }
     return 0;
+}
+
+// bidomain coupling term for the following steps: src [nc] in mV/ms, or NULL to remove it
+void orc_set_source(void* h, const double* src) {
+    Sim& s = *(Sim*)h;
+    if (src) s.dv_src.assign(src, src + s.nc); else s.dv_src.clear();
 }
 
 int orc_n_states(void* h) { return ((Sim*)h)->S; }

@@ -57,6 +57,7 @@ def lib():
         L.orc_stimulus_set.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.POINTER(C.c_int64), C.c_double, C.c_double,
                                        C.c_double]
         L.orc_step.argtypes = [C.c_void_p, C.c_int64, C.c_double]
+        L.orc_set_source.argtypes = [C.c_void_p, _dp]
         L.orc_trigger_set.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.POINTER(C.c_int64), C.c_int, C.c_double]
         L.orc_trigger_time.argtypes = [C.c_void_p, C.c_int]
         L.orc_trigger_time.restype = C.c_double
@@ -178,6 +179,12 @@ class OracleSim:
 
     def trigger_time(self, trigger):
         return float(lib().orc_trigger_time(self._h, int(trigger)))
+
+    def set_source(self, src):
+        """Extra right-hand side per cell in mV/ms (bidomain: div(M_int grad v_ext)/(chi C_m)); None removes it."""
+        src = None if src is None else np.ascontiguousarray(src, dtype=np.float64)
+        assert src is None or src.size == self.n_tets
+        lib().orc_set_source(self._h, _p(src))
 
     def step(self, n_steps, dt):
         rc = lib().orc_step(self._h, int(n_steps), float(dt))
