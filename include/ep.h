@@ -63,6 +63,24 @@ int ep_mesh_create_tri(ep_sim **out, int64_t n_nodes, const double *xyz_mm, int6
                        const double *fibre, const double *sigma_scale, double sigma_l, double sigma_t, double chi,
                        double Cm);
 
+/* Bidomain model, eq. (1) / (6) of the paper: intracellular and extracellular conductivities along /
+ * across the fibres in mS/cm (Table 2: 1.7 / 0.19 and 6.2 / 2.4).  Time stepping as PAPER.md:176-178: ep_step
+ * advances v explicitly from v, v_ext, I_ion, I_s at t^n with the fused kernel (the term div(M_int grad v_ext) enters as a
+ * per-cell source), then solves  div((M_int + M_ext) grad v_ext) = -div(M_int grad v)  for v_ext at t^{n+1} by restarted GMRES
+ * entirely on the device, first estimate = v_ext of the previous step.  Readings E1-E4 of DESIGN.md: the system is singular
+ * under no-flux boundaries and v_ext is the solution with zero volume-weighted mean; v_ext at t = 0 solves the same equation
+ * for the initial potential; defaults restart 30, relative residual 1e-10, no preconditioner.  Tetrahedra only.
+ * A solve that does not reach the tolerance within max_cycles restarts sets the sticky error EP_ERR_NUMERIC. */
+int ep_mesh_create_bidomain(ep_sim **out, int64_t n_nodes, const double *xyz_mm, int64_t n_tets, const int32_t *tets,
+                            const double *fibre, const double *sigma_scale, double sigma_int_l, double sigma_int_t,
+                            double sigma_ext_l, double sigma_ext_t, double chi, double Cm);
+/* Solver settings: restart length in [1, 63], restarts allowed per solve, relative residual |b - A x| / |b|. */
+int ep_bidomain_solver(ep_sim *sim, int restart, int max_cycles, double rel_tol);
+/* Extracellular potential at the current time, [n_tets] in the caller's order, zero volume-weighted mean; synchronises. */
+int ep_read_vext(ep_sim *sim, double *out);
+/* GMRES iterations of the last solve / of all solves, number of solves, last relative residual; any pointer may be NULL. */
+int ep_bidomain_stats(ep_sim *sim, int64_t *iters_last, int64_t *iters_total, int64_t *solves, double *rel_res_last);
+
 /* Choose the cell model and set every cell to an initial state.
  *   cell_type [n_tets] TP06: 0 endo, 1 mid, 2 epi (reading B5); NULL => 0
  *   y0        [n_types*S] one state vector per cell type (n_types = 3 for TP06, 1 for CRN98 and STEWART); NULL => built-in

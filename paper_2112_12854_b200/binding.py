@@ -22,6 +22,11 @@ SIGNATURES = {
                                  C.c_double, C.c_double]),
     "ep_mesh_create_tri": (C.c_int, [C.POINTER(_vp), C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double,
                                      C.c_double, C.c_double]),
+    "ep_mesh_create_bidomain": (C.c_int, [C.POINTER(_vp), C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double,
+                                          C.c_double, C.c_double, C.c_double, C.c_double]),
+    "ep_bidomain_solver": (C.c_int, [_vp, C.c_int, C.c_int, C.c_double]),
+    "ep_read_vext": (C.c_int, [_vp, _dp]),
+    "ep_bidomain_stats": (C.c_int, [_vp, _i64p, _i64p, _i64p, _dp]),
     "ep_state_init": (C.c_int, [_vp, C.c_int, _u8p, _dp]),
     "ep_stimulus_set": (C.c_int, [_vp, C.c_int, C.c_int64, _i64p, C.c_double, C.c_double, C.c_double]),
     "ep_trigger_set": (C.c_int, [_vp, C.c_int, C.c_int64, _i64p, C.c_int, C.c_double]),
@@ -154,15 +159,22 @@ class Sim:
     """One simulation handle (ep_sim*).  Method names follow the C-ABI calls.  cells [n,4]: tetrahedra (ep_mesh_create);
     cells [n,3]: a triangulated surface (ep_mesh_create_tri)."""
 
-    def __init__(self, xyz, tets, fibre=None, sigma_scale=None, sigma_l=1.3, sigma_t=0.18, chi=1400.0, Cm=1.0):
+    def __init__(self, xyz, tets, fibre=None, sigma_scale=None, sigma_l=1.3, sigma_t=0.18, chi=1400.0, Cm=1.0,
+                 sigma_ext=None):
+        """sigma_ext = (l, t): bidomain (ep_mesh_create_bidomain); sigma_l / sigma_t are then the intracellular values."""
         xyz = np.ascontiguousarray(xyz, dtype=np.float64)
         tets = np.ascontiguousarray(tets, dtype=np.int32)
         fibre = None if fibre is None else np.ascontiguousarray(fibre, dtype=np.float64)
         sigma_scale = None if sigma_scale is None else np.ascontiguousarray(sigma_scale, dtype=np.float64)
         self._h = _vp()
-        create = lib().ep_mesh_create if tets.shape[1] == 4 else lib().ep_mesh_create_tri
-        _chk(create(C.byref(self._h), xyz.shape[0], _p(xyz), tets.shape[0], _p(tets, C.c_int32),
-                    _p(fibre), _p(sigma_scale), sigma_l, sigma_t, chi, Cm))
+        if sigma_ext is not None:
+            _chk(lib().ep_mesh_create_bidomain(C.byref(self._h), xyz.shape[0], _p(xyz), tets.shape[0], _p(tets, C.c_int32),
+                                               _p(fibre), _p(sigma_scale), sigma_l, sigma_t, float(sigma_ext[0]),
+                                               float(sigma_ext[1]), chi, Cm))
+        else:
+            create = lib().ep_mesh_create if tets.shape[1] == 4 else lib().ep_mesh_create_tri
+            _chk(create(C.byref(self._h), xyz.shape[0], _p(xyz), tets.shape[0], _p(tets, C.c_int32),
+                        _p(fibre), _p(sigma_scale), sigma_l, sigma_t, chi, Cm))
         self.n_tets = int(lib().ep_n_cells(self._h))
         self.n_nodes = int(lib().ep_n_nodes(self._h))
         self.n_states = 0
@@ -208,6 +220,19 @@ class Sim:
         d = C.c_double()
         _chk(lib().ep_trigger_time(self._h, int(trigger), C.byref(d)))
         return d.value
+
+    def bidomain_solver(self, restart=30, max_cycles=200, rel_tol=1e-10):
+        _chk(lib().ep_bidomain_solver(self._h, int(restart), int(max_cycles), float(rel_tol)))
+
+    def read_vext(self, out=None):
+        out = np.empty(self.n_tets) if out is None else out
+        _chk(lib().ep_read_vext(self._h, _p(out)))
+        return out
+
+    def bidomain_stats(self):
+        a, b, c, r = C.c_int64(), C.c_int64(), C.c_int64(), C.c_double()
+        _chk(lib().ep_bidomain_stats(self._h, C.byref(a), C.byref(b), C.byref(c), C.byref(r)))
+        return {"iters_last": a.value, "iters_total": b.value, "solves": c.value, "rel_res_last": r.value}
 
     def couple(self, trigger, dst, slot, delay):
         """ep_couple(self -> dst): True once dst's slot has been scheduled."""

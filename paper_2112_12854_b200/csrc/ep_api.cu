@@ -74,6 +74,15 @@ struct ep_sim {
     cudaStream_t graph_stream = nullptr;
     int device = 0;                             // the device the handle was created on
     int dim = 3;                                // 3: tetrahedra, 2: triangulated surface
+    // bidomain (ep_mesh_create_bidomain): the mesh's own tables hold M_int; second coefficient table for M_int + M_ext
+    bool bidomain = false;
+    double *d_ccoef_ie = nullptr, *d_vext = nullptr, *d_src = nullptr, *d_b = nullptr;
+    epk::Gmres gm;
+    int bd_restart = 30, bd_max_cycles = 200, bd_check = 5;
+    double bd_tol = 1e-10;
+    bool vext_valid = false;
+    int64_t bd_iters_last = 0, bd_iters_total = 0, bd_solves = 0;
+    double bd_res_last = 0.0;
     bool pdl = true;                            // programmatic dependent launch of the step kernels (EP_NO_PDL=1 disables)
     // bulk state I/O (ep_write_states / ep_read_states): second stream + events for a two-slot staging pipeline
     cudaStream_t io_stream = nullptr;
@@ -123,7 +132,8 @@ int64_t step_index(double t, double dt) { return (int64_t)std::ceil(t / dt - 1e-
 void free_all(ep_sim* s) {
     void* ptrs[] = {s->d_cidx, s->d_nidx, s->d_perm, s->d_inv, s->d_ccoef, s->d_nw, s->d_slice_ptr, s->d_vm[0],
                     s->d_vm[1], s->d_y, s->d_vn, s->d_tact, s->d_tmp, s->d_tmp2, s->d_red, s->d_ctype, s->d_smask,
-                    s->d_vol, s->d_tmask, s->d_trig_fire, s->d_trig_par};
+                    s->d_vol, s->d_tmask, s->d_trig_fire, s->d_trig_par, s->d_ccoef_ie, s->d_vext, s->d_src, s->d_b};
+    epk::gmres_free(s->gm);
     for (void* p : ptrs) if (p) cudaFree(p);
     for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
     for (cudaGraphExec_t g : s->graph) if (g) cudaGraphExecDestroy(g);
@@ -181,6 +191,7 @@ epk::StepArgs step_args(ep_sim* s, int cur, double dt) {
     a.trig_slots = 0;
     for (const ep_sim::Trig& t : s->trig) if (t.armed && t.slot >= 0) a.trig_slots |= 1u << t.slot;
     a.dt = dt; a.desc = nullptr;
+    a.dv_extra = s->bidomain ? s->d_src : nullptr;
     return a;
 }
 
@@ -246,6 +257,50 @@ int read_back(ep_sim* s, const double* d_src, double* out) {
     return EP_OK;
 }
 
+// Bidomain: v_ext for the potential in d_vm[cur] (second equation of (6)), then the coupling term of the next
+// step.  Both sides are multiplied by the cell volumes (flux form: the operator then has the constants as left AND right
+// null vectors, which is what makes GMRES safe on this singular, compatible system); gauge: zero volume-weighted mean.
+int bidomain_solve(ep_sim* s) {
+    if (!s->gm.V) {
+        if (epk::gmres_alloc(s->gm, s->nc, s->bd_restart) != 0) {
+            epk::gmres_free(s->gm);
+            cudaGetLastError();
+            return fail(EP_ERR_NOMEM, "cannot allocate the Krylov basis of the bidomain solver");
+        }
+        s->dev_bytes += s->gm.bytes;
+    }
+    const double* v = s->d_vm[s->cur];
+    epk::launch_node_gather(s->dm, v, s->d_vn, s->stream);
+    epk::launch_diffusion_only(s->dm, v, s->d_vn, s->d_b, s->stream, nullptr, s->d_vol, -1.0);   // b = -V A_i v
+    s->launches += 2;
+    epk::GmresOp op;
+    op.launches = 2;
+    op.f = [s](const double* x, double* out, cudaStream_t st) {
+        epk::launch_node_gather(s->dm, x, s->d_vn, st);
+        epk::launch_diffusion_only(s->dm, x, s->d_vn, out, st, s->d_ccoef_ie, s->d_vol, 1.0);      // V A_ie x
+    };
+    double rel = 0.0;
+    const int it = epk::gmres_solve(s->gm, op, s->d_b, s->d_vext, s->bd_tol, s->bd_max_cycles, s->bd_check, s->stream, &rel,
+                                    &s->launches);
+    if (it < 0) {
+        s->sticky = EP_ERR_CUDA;
+        return fail(EP_ERR_CUDA, std::string("bidomain solver: ") + cudaGetErrorString(cudaGetLastError()));
+    }
+    s->bd_iters_last = it; s->bd_iters_total += it; s->bd_solves += 1; s->bd_res_last = rel;
+    if (!(rel <= s->bd_tol)) {
+        s->sticky = EP_ERR_NUMERIC;
+        char msg[160];
+        std::snprintf(msg, sizeof msg, "bidomain solver did not converge: relative residual %.3e after %d iterations", rel, it);
+        return fail(EP_ERR_NUMERIC, msg);
+    }
+    epk::launch_remove_weighted_mean(s->gm, s->d_vext, s->d_vol, s->vol_total, s->stream);
+    epk::launch_node_gather(s->dm, s->d_vext, s->d_vn, s->stream);
+    epk::launch_diffusion_only(s->dm, s->d_vext, s->d_vn, s->d_src, s->stream);                  // A_i v_ext/(chi Cm), mV/ms
+    s->launches += 5;
+    s->vext_valid = true;
+    return EP_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -285,9 +340,10 @@ int ep_host_stencil(int64_t n_nodes, const double* xyz, int64_t n_tets, const in
 }
 
 // dim = 3: tetrahedra (cells [n*4]); dim = 2: triangles (cells [n*3])
+// ext_l, ext_t > 0: bidomain; (sigma_l, sigma_t) are then the intracellular conductivities
 static int mesh_create_impl(ep_sim** out, int dim, int64_t n_nodes, const double* xyz, int64_t n_tets, const int32_t* tets,
                             const double* fibre, const double* sigma_scale, double sigma_l, double sigma_t, double chi,
-                            double Cm) {
+                            double Cm, double ext_l = 0.0, double ext_t = 0.0) {
     if (!out) return fail(EP_ERR_ARG, "out is NULL");
     *out = nullptr;
     ep_sim* s = nullptr;
@@ -343,6 +399,23 @@ static int mesh_create_impl(ep_sim** out, int dim, int64_t n_nodes, const double
         s->dm.nc = s->nc; s->dm.nn = s->nn; s->dm.nc_pad = s->nc_pad; s->dm.n_slices = pk.n_slices;
         s->dm.cidx = s->d_cidx; s->dm.ccoef = s->d_ccoef; s->dm.slice_ptr = s->d_slice_ptr;
         s->dm.nidx = s->d_nidx; s->dm.nw = s->d_nw;
+        if (ext_l > 0.0 || ext_t > 0.0) {
+            if (!(ext_l > 0.0) || !(ext_t > 0.0)) return bail(fail(EP_ERR_ARG, "extracellular conductivities must be positive"));
+            ep::Stencil st2;
+            ep::Packed pk2;
+            rc = ep::build_stencil(n_nodes, xyz, n_tets, tets, fibre, sigma_scale, sigma_l + ext_l, sigma_t + ext_t, chi, Cm, st2, err);
+            if (rc) return bail(fail(rc, err));
+            rc = ep::pack(st2, xyz, pk2, err);
+            if (rc) return bail(fail(rc, err));
+            if (pk2.cidx != pk.cidx) return bail(fail(EP_ERR_MESH, "internal: index tables of the two operators differ"));
+            if ((rc = upload(s, &s->d_ccoef_ie, pk2.ccoef)) || (rc = dev_alloc(s, &s->d_vext, s->nc_pad)) ||
+                (rc = dev_alloc(s, &s->d_src, s->nc_pad)) || (rc = dev_alloc(s, &s->d_b, s->nc_pad)))
+                return bail(rc);
+            cudaMemset(s->d_vext, 0, sizeof(double) * s->nc_pad);
+            cudaMemset(s->d_src, 0, sizeof(double) * s->nc_pad);
+            cudaMemset(s->d_b, 0, sizeof(double) * s->nc_pad);
+            s->bidomain = true;
+        }
         if (cudaDeviceSynchronize() != cudaSuccess) return bail(fail(EP_ERR_CUDA, "upload failed"));
         *out = s;
         return EP_OK;
@@ -397,6 +470,14 @@ int ep_mesh_create_tri(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t
     return mesh_create_impl(out, 2, n_nodes, xyz, n_tris, tris, fibre, sigma_scale, sigma_l, sigma_t, chi, Cm);
 }
 
+int ep_mesh_create_bidomain(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_tets, const int32_t* tets,
+                            const double* fibre, const double* sigma_scale, double sigma_int_l, double sigma_int_t,
+                            double sigma_ext_l, double sigma_ext_t, double chi, double Cm) {
+    if (!(sigma_ext_l > 0.0) || !(sigma_ext_t > 0.0)) return fail(EP_ERR_ARG, "extracellular conductivities must be positive");
+    return mesh_create_impl(out, 3, n_nodes, xyz, n_tets, tets, fibre, sigma_scale, sigma_int_l, sigma_int_t, chi, Cm,
+                            sigma_ext_l, sigma_ext_t);
+}
+
 void ep_destroy(ep_sim* s) {
     if (!s) return;
     cudaStreamSynchronize(s->stream);
@@ -445,6 +526,11 @@ int ep_state_init(ep_sim* s, int model, const uint8_t* cell_type, const double* 
         EP_CUDA(s, cudaMemsetAsync(s->d_y, 0, sizeof(double) * (size_t)S * s->nc_pad, s->stream));
     }
     s->model = model; s->S = S; s->step = 0; s->dt = 0.0; s->cur = 0;
+    if (s->bidomain) {
+        s->vext_valid = false;
+        EP_CUDA(s, cudaMemsetAsync(s->d_vext, 0, sizeof(double) * s->nc_pad, s->stream));
+        EP_CUDA(s, cudaMemsetAsync(s->d_src, 0, sizeof(double) * s->nc_pad, s->stream));
+    }
     if (s->sticky == EP_ERR_NUMERIC) s->sticky = EP_OK;   // a fresh state clears a numerical failure, not a CUDA one
     s->trig_dirty = true;
     double* d_y0 = nullptr;
@@ -518,6 +604,22 @@ int ep_step(ep_sim* s, int64_t n_steps, double dt) {
         s->trig_dirty = false;
     }
     int64_t left = n_steps;
+    if (s->bidomain) {
+        // v^{n+1} explicit from v, v_ext, I_ion, I_s at t^n, then the elliptic solve for v_ext^{n+1}
+        if (left > 0 && !s->vext_valid && (rc = bidomain_solve(s))) return rc;     // reading E2: v_ext^0 from v^0
+        for (; left > 0; --left) {
+            epk::StepArgs a = step_args(s, s->cur, dt);
+            fill_desc(s, s->step, dt, n_on, n_off, a.inl);
+            epk::launch_node_gather(s->dm, a.vm_cur, s->d_vn, s->stream);
+            epk::launch_cell_step(s->dm, s->model, a, s->stream);
+            s->launches += 2;
+            s->cur ^= 1;
+            s->step += 1;
+            if ((rc = bidomain_solve(s))) return rc;
+        }
+        EP_CUDA(s, cudaGetLastError());
+        return EP_OK;
+    }
     while (left > 0) {
         if (!s->profiling && left >= GRAPH_STEPS) {
             // replay path: one descriptor upload + one graph launch per GRAPH_STEPS time steps
@@ -592,6 +694,7 @@ int ep_write_state(ep_sim* s, int var, const double* in) {
     if (var == 0) epk::launch_gather_f64(s->nc, s->d_tmp, s->d_perm, s->d_vm[s->cur], s->stream);
     else epk::launch_state_row_put(s->nc, s->d_tmp, s->d_perm, s->S, var, s->d_y, s->stream);
     s->launches++;
+    if (var == 0) s->vext_valid = false;
     EP_CUDA(s, cudaStreamSynchronize(s->stream));
     return EP_OK;
 }
@@ -670,6 +773,7 @@ int ep_write_states(ep_sim* s, const double* in) {
         s->launches++;
         EP_CUDA(s, cudaEventRecord(s->io_consumed[b], s->stream));
     }
+    s->vext_valid = false;
     EP_CUDA(s, cudaStreamSynchronize(s->stream));
     return EP_OK;
 }
@@ -809,6 +913,41 @@ int ep_couple(ep_sim* src, int trigger, ep_sim* dst, int slot, double delay_ms, 
     dst->stim[slot].t0 = t_on;
     dst->trig_dirty = true;   // (a trigger of dst driving this slot caches its parameters)
     *scheduled = 1;
+    return EP_OK;
+}
+
+int ep_read_vext(ep_sim* s, double* out) {
+    if (!s || !out) return fail(EP_ERR_ARG, "null argument");
+    if (!s->bidomain) return fail(EP_ERR_STATE, "not a bidomain sim (ep_mesh_create_bidomain)");
+    if (s->model < 0) return fail(EP_ERR_STATE, "no state: call ep_state_init first");
+    int rc = check_sim(s);
+    if (rc) return rc;
+    if (!s->vext_valid && (rc = bidomain_solve(s))) return rc;
+    return read_back(s, s->d_vext, out);
+}
+
+int ep_bidomain_solver(ep_sim* s, int restart, int max_cycles, double rel_tol) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    if (!s->bidomain) return fail(EP_ERR_STATE, "not a bidomain sim (ep_mesh_create_bidomain)");
+    if (restart < 1 || restart > 63 || max_cycles < 1 || !(rel_tol > 0.0) || !(rel_tol < 1.0))
+        return fail(EP_ERR_ARG, "restart in [1, 63], max_cycles >= 1, 0 < rel_tol < 1");
+    if (restart != s->bd_restart && s->gm.V) {
+        cudaStreamSynchronize(s->stream);
+        s->dev_bytes -= s->gm.bytes;
+        epk::gmres_free(s->gm);
+    }
+    s->bd_restart = restart; s->bd_max_cycles = max_cycles; s->bd_tol = rel_tol;
+    s->bd_check = std::min(5, restart);
+    return EP_OK;
+}
+
+int ep_bidomain_stats(ep_sim* s, int64_t* iters_last, int64_t* iters_total, int64_t* solves, double* rel_res_last) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    if (!s->bidomain) return fail(EP_ERR_STATE, "not a bidomain sim (ep_mesh_create_bidomain)");
+    if (iters_last) *iters_last = s->bd_iters_last;
+    if (iters_total) *iters_total = s->bd_iters_total;
+    if (solves) *solves = s->bd_solves;
+    if (rel_res_last) *rel_res_last = s->bd_res_last;
     return EP_OK;
 }
 

@@ -98,10 +98,12 @@ __global__ void __launch_bounds__(CELL_THREADS) diffusion_only_kernel(int64_t nc
                                                                       const double* __restrict__ ccoef,
                                                                       const double* __restrict__ vm,
                                                                       const double* __restrict__ vn,
-                                                                      double* __restrict__ out) {
+                                                                      double* __restrict__ out,
+                                                                      const double* __restrict__ vol, double scale) {
     const int64_t i = (int64_t)blockIdx.x * CELL_THREADS + threadIdx.x;
     if (i >= nc) return;
-    out[i] = diffusion_gather(i, cidx, ccoef, vm, vn, vm[i]);
+    const double d = diffusion_gather(i, cidx, ccoef, vm, vn, vm[i]);
+    out[i] = scale * (vol ? vol[i] * d : d);
 }
 
 // S2..S9 fused.  One thread per cell; state rows are read once and written once.  MODEL 0: TP06, 1: Courtemanche,
@@ -161,7 +163,8 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
             accm = fma(cf[4 + m], gv[4 + m], accm);
             accc = fma(cf[8 + m], gv[8 + m] - v_old, accc);
         }
-        return (accn + accm) + accc;
+        const double dv = (accn + accm) + accc;
+        return a.dv_extra ? dv + a.dv_extra[i] : dv;     // bidomain: + div(M_int grad v_ext)/(chi C_m), eq. (1)
     };
     // S4: stimulus, eq. (4) PAPER.md:130-132 (window already resolved on the host into istim[k]).  The mask is requested
     // here with the other loads; the cell model calls stimulus() after its first exponential batch, so nothing waits for it.
@@ -373,9 +376,10 @@ void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStr
     else launch_pdl(cell_step_kernel<2>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
 }
 
-void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* vn, double* out, cudaStream_t s) {
-    diffusion_only_kernel<<<blocks_for(m.nc, CELL_THREADS), CELL_THREADS, 0, s>>>(m.nc, m.cidx, m.ccoef, vm,
-                                                                                  vn, out);
+void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* vn, double* out, cudaStream_t s,
+                           const double* ccoef, const double* vol, double scale) {
+    diffusion_only_kernel<<<blocks_for(m.nc, CELL_THREADS), CELL_THREADS, 0, s>>>(m.nc, m.cidx, ccoef ? ccoef : m.ccoef, vm,
+                                                                                  vn, out, vol, scale);
 }
 
 void launch_state_fill(int model, int64_t nc, int64_t nc_pad, const uint8_t* ctype, const double* y0_dev, double* y,

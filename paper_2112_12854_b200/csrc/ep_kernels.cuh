@@ -1,6 +1,7 @@
 // ep_kernels.cuh -- launch interface between the C-ABI layer (ep_api.cu) and the sm_100a kernels (ep_kernels.cu).
 #pragma once
 #include <cstdint>
+#include <functional>
 #include <cuda_runtime.h>
 
 namespace epk {
@@ -43,6 +44,7 @@ struct StepArgs {
     const TrigPar* trig_par;// [MAX_TRIGGERS]
     unsigned trig_slots;    // bit k = slot k is driven by a trigger instead of its own time window
     double dt;
+    const double* dv_extra; // [nc_pad] extra right-hand side in mV/ms (bidomain: div(M_int grad v_ext)/(chi C_m)), or NULL
     const StepDesc* desc;   // device descriptor of this step (CUDA-graph replay), or NULL: use `inl`
     StepDesc inl;
 };
@@ -52,8 +54,10 @@ struct StepArgs {
 void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaStream_t s, bool pdl = false);
 // S2..S9 fused: diffusion gather + stimulus + cell model + RL/FE updates + Vm write + activation record
 void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStream_t s, bool pdl = false);
-// diagnostics: out[i] = D_c/(chi Cm) [mV/ms] from vm and vn
-void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* vn, double* out, cudaStream_t s);
+// out[i] = scale * (vol ? vol[i] : 1) * D_c/(chi Cm) [mV/ms] from vm and vn with the coefficient table `ccoef` (NULL: the mesh's
+// own).  Diagnostics, and the operator applications of the bidomain solver.
+void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* vn, double* out, cudaStream_t s,
+                           const double* ccoef = nullptr, const double* vol = nullptr, double scale = 1.0);
 // fill y rows with one state vector per cell type; y0 is a DEVICE pointer [n_types*S]; NULL = built-in rest state
 void launch_state_fill(int model, int64_t nc, int64_t nc_pad, const uint8_t* ctype, const double* y0_dev, double* y,
                        double* vm, double* tact, cudaStream_t s);
@@ -78,5 +82,26 @@ int model_n_states(int model);
 double launch_dfma_rate(double* scratch, int64_t scratch_len, int iters, cudaStream_t s);
 // diagnostics: y[i] = f(x[i]) with the kernels' own exp / log / rcp / rsqrt (device pointers)
 void launch_math_eval(int fn, int64_t n, const double* x, double* y, cudaStream_t s);
+
+// ---- restarted GMRES on the device (ep_elliptic.cu): bidomain elliptic equation
+struct GmresOp {           // out = A x on stream s; `launches` = kernels one application issues
+    std::function<void(const double*, double*, cudaStream_t)> f;
+    int launches = 0;
+    void operator()(const double* x, double* out, cudaStream_t s) const { f(x, out, s); }
+};
+struct Gmres {
+    int m = 0;
+    int64_t n = 0, stride = 0, bytes = 0;
+    double *V = nullptr, *w = nullptr, *small = nullptr, *partial = nullptr;
+    double *H = nullptr, *cs = nullptr, *sn = nullptr, *g = nullptr, *y = nullptr, *hcol = nullptr, *scal = nullptr;
+};
+int gmres_alloc(Gmres& G, int64_t n, int restart);      // 0, or negative on allocation failure / bad restart length
+void gmres_free(Gmres& G);
+// x: first estimate in, solution out.  Stops when the residual estimate <= rel_tol * |b|.  Returns the number of
+// iterations, or a negative value on a CUDA error; *rel_res_out = last residual estimate / |b|.
+int gmres_solve(Gmres& G, const GmresOp& apply, const double* b, double* x, double rel_tol, int max_cycles, int check_every,
+                cudaStream_t s, double* rel_res_out, int64_t* launches);
+// x -= (sum_i weight[i] x[i]) / total
+void launch_remove_weighted_mean(const Gmres& G, double* x, const double* weight, double total, cudaStream_t s);
 
 }  // namespace epk
