@@ -28,11 +28,16 @@ __global__ void __launch_bounds__(256) multi_dot_partial_kernel(int64_t n, const
     __shared__ double sh[4][256];
     const int q0 = 4 * blockIdx.y;
     double acc[4] = {0.0, 0.0, 0.0, 0.0};
-    for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (int64_t)NB * 256) {
-        const double wi = w[i];
+    if (k < 0) {            // plain sum of w into slot 0
+        for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (int64_t)NB * 256) acc[0] += w[i];
+        k = 1;
+    } else {
+        for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (int64_t)NB * 256) {
+            const double wi = w[i];
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
-            if (q0 + q < k) acc[q] = fma(wi, V[(int64_t)(q0 + q) * stride + i], acc[q]);
+            for (int q = 0; q < 4; ++q)
+                if (q0 + q < k) acc[q] = fma(wi, V[(int64_t)(q0 + q) * stride + i], acc[q]);
+        }
     }
 #pragma unroll
     for (int q = 0; q < 4; ++q) sh[q][threadIdx.x] = acc[q];
@@ -177,8 +182,8 @@ static void norm2_into(const Gmres& G, const double* x, double* out, cudaStream_
 }
 
 // Solves A x = b (A through `apply`), x holds the first estimate.  Returns iterations used (>= 0) or a negative CUDA error.
-int gmres_solve(Gmres& G, const GmresOp& apply, const double* b, double* x, double rel_tol, int max_cycles, int check_every,
-                cudaStream_t s, double* rel_res_out, int64_t* launches) {
+int gmres_solve(Gmres& G, const GmresOp& apply, const double* b, double* x, double rel_tol, double abs_tol, int max_cycles,
+                int check_every, cudaStream_t s, double* rel_res_out, int64_t* launches) {
     const int m = G.m;
     const int64_t n = G.n;
     const unsigned gb = blocks256(n);
@@ -193,7 +198,7 @@ int gmres_solve(Gmres& G, const GmresOp& apply, const double* b, double* x, doub
         if (rel_res_out) *rel_res_out = 0.0;
         return 0;
     }
-    const double tol = rel_tol * bnorm;
+    const double tol = std::max(rel_tol * bnorm, abs_tol);
     int iters = 0;
     double res = 0.0;
     for (int cycle = 0; cycle < max_cycles; ++cycle) {
@@ -234,9 +239,16 @@ int gmres_solve(Gmres& G, const GmresOp& apply, const double* b, double* x, doub
         *launches += 2;
         if (res <= tol) break;
     }
-    if (rel_res_out) *rel_res_out = res / bnorm;
+    if (rel_res_out) *rel_res_out = res <= abs_tol ? std::min(res / bnorm, rel_tol) : res / bnorm;
     if (cudaGetLastError() != cudaSuccess) return -1;
     return iters;
+}
+
+// x -= (sum_i x[i]) / n: makes a right-hand side compatible with an operator whose left null vector is the constant
+void launch_remove_mean(const Gmres& G, double* x, cudaStream_t s) {
+    multi_dot_partial_kernel<<<dim3(NB, 1), 256, 0, s>>>(G.n, x, nullptr, G.stride, -1, G.partial);
+    multi_dot_final_kernel<<<1, 256, 0, s>>>(G.partial, G.scal + 2, 0);
+    shift_kernel<<<blocks256(G.n), 256, 0, s>>>(G.n, x, G.scal + 2, 1.0 / (double)G.n);
 }
 
 void launch_remove_weighted_mean(const Gmres& G, double* x, const double* weight, double total, cudaStream_t s) {

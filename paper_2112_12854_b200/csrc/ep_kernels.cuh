@@ -99,8 +99,11 @@ int gmres_alloc(Gmres& G, int64_t n, int restart);      // 0, or negative on all
 void gmres_free(Gmres& G);
 // x: first estimate in, solution out.  Stops when the residual estimate <= rel_tol * |b|.  Returns the number of
 // iterations, or a negative value on a CUDA error; *rel_res_out = last residual estimate / |b|.
-int gmres_solve(Gmres& G, const GmresOp& apply, const double* b, double* x, double rel_tol, int max_cycles, int check_every,
-                cudaStream_t s, double* rel_res_out, int64_t* launches);
+// Also stops when the residual estimate <= abs_tol (a right-hand side that is round-off noise has no meaningful relative scale).
+int gmres_solve(Gmres& G, const GmresOp& apply, const double* b, double* x, double rel_tol, double abs_tol, int max_cycles,
+                int check_every, cudaStream_t s, double* rel_res_out, int64_t* launches);
+// x -= (sum_i x[i]) / n
+void launch_remove_mean(const Gmres& G, double* x, cudaStream_t s);
 // x -= (sum_i weight[i] x[i]) / total
 void launch_remove_weighted_mean(const Gmres& G, double* x, const double* weight, double total, cudaStream_t s);
 
