@@ -120,6 +120,16 @@ int ep_couple(ep_sim *src, int trigger, ep_sim *dst, int slot, double delay_ms, 
  * EP_ERR_STATE: before ep_state_init, dt <= 0, or dt different from the previous call's after the first step. */
 int ep_step(ep_sim *sim, int64_t n_steps, double dt_ms);
 
+/* Order of the time stepping.  1 (default): the paper's scheme, Rush-Larsen gates + forward Euler.
+ * 2: the improvement PAPER.md:232 names -- second-order Adams-Bashforth for v and the concentrations, and a second-order
+ * Rush-Larsen step for the gates (steady state and time constant taken at arguments extrapolated to t^{n+1/2}; DESIGN.md
+ * reading H1); the stimulus, piecewise constant on steps, is integrated exactly.  TP06 only (EP_ERR_ARG otherwise).  The first
+ * step after ep_state_init / ep_write_state(s) / this call has no history and is a first-order step.  The explicit stability
+ * limit of the diffusion part halves (AB2: dt <= chi Cm / rho(A), half of what ep_stable_dt reports).  Eight more state
+ * rows per cell are read and written (64 + 64 B).  The history is not part of a checkpoint: a resumed run restarts with one
+ * first-order step. */
+int ep_set_time_order(ep_sim *sim, int order);
+
 /* Wait for all queued work of this sim; returns the sticky error if any (EP_ERR_NUMERIC if a non-finite Vm was seen by
  * ep_check_finite). */
 int ep_synchronize(ep_sim *sim);

@@ -32,6 +32,7 @@ SIGNATURES = {
     "ep_trigger_set": (C.c_int, [_vp, C.c_int, C.c_int64, _i64p, C.c_int, C.c_double]),
     "ep_trigger_time": (C.c_int, [_vp, C.c_int, _dp]),
     "ep_couple": (C.c_int, [_vp, C.c_int, _vp, C.c_int, C.c_double, C.POINTER(C.c_int)]),
+    "ep_set_time_order": (C.c_int, [_vp, C.c_int]),
     "ep_step": (C.c_int, [_vp, C.c_int64, C.c_double]),
     "ep_synchronize": (C.c_int, [_vp]),
     "ep_read_vm": (C.c_int, [_vp, _dp]),
@@ -239,6 +240,9 @@ class Sim:
         f = C.c_int()
         _chk(lib().ep_couple(self._h, int(trigger), dst._h, int(slot), float(delay), C.byref(f)))
         return bool(f.value)
+
+    def set_time_order(self, order):
+        _chk(lib().ep_set_time_order(self._h, int(order)))
 
     def step(self, n_steps, dt):
         _chk(lib().ep_step(self._h, int(n_steps), float(dt)))

@@ -81,6 +81,10 @@ struct ep_sim {
     int bd_restart = 30, bd_max_cycles = 200, bd_check = 5;
     double bd_tol = 1e-10;
     bool vext_valid = false;
+    // second-order time stepping (ep_set_time_order): history rows and whether they hold t^{n-1} of the current state
+    int order = 1;
+    double* d_hist = nullptr;
+    bool o2_have = false;
     int64_t bd_iters_last = 0, bd_iters_total = 0, bd_solves = 0;
     double bd_res_last = 0.0;
     bool pdl = true;                            // programmatic dependent launch of the step kernels (EP_NO_PDL=1 disables)
@@ -132,7 +136,7 @@ int64_t step_index(double t, double dt) { return (int64_t)std::ceil(t / dt - 1e-
 void free_all(ep_sim* s) {
     void* ptrs[] = {s->d_cidx, s->d_nidx, s->d_perm, s->d_inv, s->d_ccoef, s->d_nw, s->d_slice_ptr, s->d_vm[0],
                     s->d_vm[1], s->d_y, s->d_vn, s->d_tact, s->d_tmp, s->d_tmp2, s->d_red, s->d_ctype, s->d_smask,
-                    s->d_vol, s->d_tmask, s->d_trig_fire, s->d_trig_par, s->d_ccoef_ie, s->d_vext, s->d_src, s->d_b};
+                    s->d_vol, s->d_tmask, s->d_trig_fire, s->d_trig_par, s->d_ccoef_ie, s->d_vext, s->d_src, s->d_b, s->d_hist};
     epk::gmres_free(s->gm);
     for (void* p : ptrs) if (p) cudaFree(p);
     for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
@@ -192,6 +196,8 @@ epk::StepArgs step_args(ep_sim* s, int cur, double dt) {
     for (const ep_sim::Trig& t : s->trig) if (t.armed && t.slot >= 0) a.trig_slots |= 1u << t.slot;
     a.dt = dt; a.desc = nullptr;
     a.dv_extra = s->bidomain ? s->d_src : nullptr;
+    a.hist = (s->order == 2) ? s->d_hist : nullptr;
+    a.o2_have = s->o2_have ? 1 : 0;
     return a;
 }
 
@@ -534,6 +540,8 @@ int ep_state_init(ep_sim* s, int model, const uint8_t* cell_type, const double* 
         EP_CUDA(s, cudaMemsetAsync(s->d_y, 0, sizeof(double) * (size_t)S * s->nc_pad, s->stream));
     }
     s->model = model; s->S = S; s->step = 0; s->dt = 0.0; s->cur = 0;
+    s->o2_have = false;
+    if (s->order == 2 && model != EP_MODEL_TP06) s->order = 1;   // the second-order scheme exists for TP06 only
     if (s->bidomain) {
         s->vext_valid = false;
         EP_CUDA(s, cudaMemsetAsync(s->d_vext, 0, sizeof(double) * s->nc_pad, s->stream));
@@ -623,13 +631,14 @@ int ep_step(ep_sim* s, int64_t n_steps, double dt) {
             s->launches += 2;
             s->cur ^= 1;
             s->step += 1;
+            if (s->order == 2) s->o2_have = true;
             if ((rc = bidomain_solve(s))) return rc;
         }
         EP_CUDA(s, cudaGetLastError());
         return EP_OK;
     }
     while (left > 0) {
-        if (!s->profiling && left >= GRAPH_STEPS) {
+        if (!s->profiling && left >= GRAPH_STEPS && !(s->order == 2 && !s->o2_have)) {
             // replay path: one descriptor upload + one graph launch per GRAPH_STEPS time steps
             if (!s->graph[s->cur] || s->graph_dt != dt || s->graph_model != s->model || s->graph_stream != s->stream) {
                 if ((rc = build_graph(s, dt))) return rc;
@@ -668,6 +677,7 @@ int ep_step(ep_sim* s, int64_t n_steps, double dt) {
         s->cur ^= 1;
         s->step = n + 1;
         --left;
+        if (s->order == 2 && !s->o2_have) { s->o2_have = true; drop_graphs(s); }   // graphs bake the flag in
     }
     EP_CUDA(s, cudaGetLastError());
     return EP_OK;
@@ -703,6 +713,7 @@ int ep_write_state(ep_sim* s, int var, const double* in) {
     else epk::launch_state_row_put(s->nc, s->d_tmp, s->d_perm, s->S, var, s->d_y, s->stream);
     s->launches++;
     if (var == 0) s->vext_valid = false;
+    s->o2_have = false;      // a rewritten state has no history
     EP_CUDA(s, cudaStreamSynchronize(s->stream));
     return EP_OK;
 }
@@ -782,6 +793,7 @@ int ep_write_states(ep_sim* s, const double* in) {
         EP_CUDA(s, cudaEventRecord(s->io_consumed[b], s->stream));
     }
     s->vext_valid = false;
+    s->o2_have = false;
     EP_CUDA(s, cudaStreamSynchronize(s->stream));
     return EP_OK;
 }
@@ -956,6 +968,25 @@ int ep_bidomain_stats(ep_sim* s, int64_t* iters_last, int64_t* iters_total, int6
     if (iters_total) *iters_total = s->bd_iters_total;
     if (solves) *solves = s->bd_solves;
     if (rel_res_last) *rel_res_last = s->bd_res_last;
+    return EP_OK;
+}
+
+int ep_set_time_order(ep_sim* s, int order) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    if (order != 1 && order != 2) return fail(EP_ERR_ARG, "time order must be 1 or 2");
+    if (order == 2 && s->model >= 0 && s->model != EP_MODEL_TP06)
+        return fail(EP_ERR_ARG, "the second-order scheme is implemented for the TP06 model only");
+    int rc = use_device(s);
+    if (rc) return rc;
+    EP_CUDA(s, cudaStreamSynchronize(s->stream));
+    if (order == 2 && !s->d_hist) {
+        rc = dev_alloc(s, &s->d_hist, (int64_t)epk::O2_ROWS * s->nc_pad);
+        if (rc) return rc;
+        EP_CUDA(s, cudaMemset(s->d_hist, 0, sizeof(double) * (size_t)epk::O2_ROWS * s->nc_pad));
+    }
+    if (order != s->order) drop_graphs(s);
+    s->order = order;
+    s->o2_have = false;
     return EP_OK;
 }
 

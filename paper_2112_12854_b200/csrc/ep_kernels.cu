@@ -111,7 +111,7 @@ __global__ void __launch_bounds__(CELL_THREADS) diffusion_only_kernel(int64_t nc
 #ifndef EP_CELL_MIN_BLOCKS
 #define EP_CELL_MIN_BLOCKS 4
 #endif
-template <int MODEL>
+template <int MODEL, int ORDER = 1>
 __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_kernel(int64_t nc,
                                                                                      const int32_t* __restrict__ cidx,
                                                                                      const double* __restrict__ ccoef,
@@ -193,9 +193,17 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
         return istim;
     };
     double v_new;
-    if constexpr (MODEL == 0)
-        v_new = tp06_step<CELL_THREADS>(v_old, ycol, CELL_THREADS, a.ctype[i], a.dt, stimulus, issue_gather, finish_gather,
-                                        &xs[0][threadIdx.x]);
+    if constexpr (MODEL == 0 && ORDER == 2) {
+        O2Hist h;
+        h.hcol = a.hist + (int64_t)blockIdx.x * (O2_ROWS * CELL_THREADS) + threadIdx.x;
+        h.stride = CELL_THREADS;
+        h.v_prev = a.vm_next[i];          // the buffer about to be overwritten still holds v^{n-1}
+        h.have = a.o2_have;
+        v_new = tp06_step<2, CELL_THREADS>(v_old, ycol, CELL_THREADS, a.ctype[i], a.dt, stimulus, issue_gather,
+                                           finish_gather, &xs[0][threadIdx.x], h);
+    } else if constexpr (MODEL == 0)
+        v_new = tp06_step<1, CELL_THREADS>(v_old, ycol, CELL_THREADS, a.ctype[i], a.dt, stimulus, issue_gather, finish_gather,
+                                           &xs[0][threadIdx.x]);
     else if constexpr (MODEL == 1)
         v_new = crn_step<CELL_THREADS>(v_old, ycol, CELL_THREADS, a.dt, stimulus, issue_gather, finish_gather,
                                        &xs[0][threadIdx.x]);
@@ -371,7 +379,8 @@ void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaS
 
 void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStream_t s, bool pdl) {
     const unsigned grid = blocks_for(m.nc, CELL_THREADS);
-    if (model == 0) launch_pdl(cell_step_kernel<0>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
+    if (model == 0 && a.hist) launch_pdl(cell_step_kernel<0, 2>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
+    else if (model == 0) launch_pdl(cell_step_kernel<0>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
     else if (model == 1) launch_pdl(cell_step_kernel<1>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
     else launch_pdl(cell_step_kernel<2>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
 }

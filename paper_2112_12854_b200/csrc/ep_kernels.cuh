@@ -24,6 +24,7 @@ struct TrigPar {
     double amp_cm;          // I_s / C_m of that slot
 };
 enum { MAX_TRIGGERS = 4 };
+enum { O2_ROWS = 8 };     // history rows of the second-order scheme: f^{n-1} of v Ca_i Ca_SR Ca_SS Na_i K_i, Ca_SS^{n-1}, Ca_SR^{n-1}
 
 struct StepDesc {
     long long n;            // step index
@@ -44,6 +45,8 @@ struct StepArgs {
     const TrigPar* trig_par;// [MAX_TRIGGERS]
     unsigned trig_slots;    // bit k = slot k is driven by a trigger instead of its own time window
     double dt;
+    double* hist;           // second-order stepping (TP06): tile-major [nc_pad/128][O2_ROWS][128] history of t^{n-1}, or NULL
+    int o2_have;            // 0 on the first step after an initialisation (no history yet: first-order step)
     const double* dv_extra; // [nc_pad] extra right-hand side in mV/ms (bidomain: div(M_int grad v_ext)/(chi C_m)), or NULL
     const StepDesc* desc;   // device descriptor of this step (CUDA-graph replay), or NULL: use `inl`
     StepDesc inl;

@@ -144,9 +144,20 @@ __device__ __forceinline__ void tp06_rush_larsen_slots(double* col, double* ycol
 // The diffusion term D_c/(chi C_m) [mV/ms] comes from two callables so that its gathers are in flight while the
 // logarithms and the first exponential batch run: issue_gather() starts the loads, finish_gather() returns the sum.
 // col = this thread's column of the block's slot array (stride BLOCK doubles, tp06::N_SLOTS slots).  Returns Vm^{n+1}.
-template <int BLOCK, class Stim, class Issue, class Finish>
+//
+// ORDER == 2 (reading H1): second-order Adams-Bashforth for v and the five concentrations, and the
+// gates relax towards y_inf(*) with tau(*), (*) = arguments extrapolated to t^{n+1/2} (v* = 3/2 v^n - 1/2 v^{n-1}, likewise
+// Ca_SS*, Ca_SR* for fCass and Rbar); the stimulus is piecewise constant on steps and is integrated exactly, outside the
+// extrapolation.  hist.have == 0 (first step after an initialisation): the first-order step, history recorded.
+struct O2Hist {
+    double* hcol = nullptr;   // this cell's column of the history rows: 0..5 f^{n-1} of v Ca_i Ca_SR Ca_SS Na_i K_i, 6 Ca_SS^{n-1}, 7 Ca_SR^{n-1}
+    int64_t stride = 0;
+    double v_prev = 0.0;      // v^{n-1}
+    int have = 0;
+};
+template <int ORDER, int BLOCK, class Stim, class Issue, class Finish>
 __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stride, int type, double dt, Stim stimulus,
-                                            Issue issue_gather, Finish finish_gather, double* col) {
+                                            Issue issue_gather, Finish finish_gather, double* col, O2Hist hist = O2Hist()) {
     using namespace tp06;
     // Argument of every transcendental (reading T2).  TP06 lives in [-100, +60] mV; for |v| <= 200 mV every
     // exponent stays below 90 in magnitude, so the clamp is inert there and the kernel follows the (unclamped) oracle;
@@ -157,6 +168,19 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double dtl = dt * L2E;   // Rush-Larsen exponents -dt/tau in base-2 units (the exponential primitive is 2^x)
     const double Cai = ycol[Y_CAI * stride], CaSR = ycol[Y_CASR * stride], CaSS = ycol[Y_CASS * stride],
                  Nai = ycol[Y_NAI * stride], Ki = ycol[Y_KI * stride];
+    // arguments of the gate functions: the values at t^n (first order) or extrapolated to t^{n+1/2} (second order)
+    double vs = v, vgs = vg, CaSSs = CaSS, CaSRs = CaSR;
+    double fprev[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    if constexpr (ORDER == 2) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) fprev[k] = hist.hcol[k * hist.stride];
+        if (hist.have) {
+            vs = fma(1.5, v, -0.5 * hist.v_prev);
+            CaSSs = fma(1.5, CaSS, -0.5 * hist.hcol[6 * hist.stride]);
+            CaSRs = fma(1.5, CaSR, -0.5 * hist.hcol[7 * hist.stride]);
+            vgs = ep_clamp(vs, -200.0, 200.0);
+        }
+    }
     // The 11 voltage-driven gates and Rbar are copied into shared memory asynchronously (no registers held, nothing waits
     // for them here); they are first touched after the first exponential batch, which hides their latency.
 #pragma unroll
@@ -174,46 +198,52 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double ECa = CK(0.5 * RTF) * (CK(LN_CAO) - lg[3]);
     const double u = v - EK;
     const double ug = ep_clamp(u, -150.0, 300.0);
-    const bool hi = (v >= -40.0);   // reading B7
+    const bool hi = (vs >= -40.0);   // reading B7 (on the gates' own argument)
 
     // ---- batch 2: every voltage-dependent exponential that is not an integer power of another one
-    col[A_B600 * BLOCK] = vg * CK(L2E / 600.0);
-    col[A_E14 * BLOCK] = vg * CK(L2E / 14.0);
-    col[A_M * BLOCK] = fma(vg, CK(-L2E / 9.03), CK(-56.86 * L2E / 9.03));
-    col[A_H * BLOCK] = fma(vg, CK(L2E / 7.43), CK(71.55 * L2E / 7.43));
-    col[A_XR1 * BLOCK] = fma(vg, CK(L2E / 11.5), CK(30.0 * L2E / 11.5));
-    col[A_D * BLOCK] = fma(vg, CK(-L2E / 13.0), CK(-35.0 * L2E / 13.0));
+    col[A_B600 * BLOCK] = vgs * CK(L2E / 600.0);
+    col[A_E14 * BLOCK] = vgs * CK(L2E / 14.0);
+    col[A_M * BLOCK] = fma(vgs, CK(-L2E / 9.03), CK(-56.86 * L2E / 9.03));
+    col[A_H * BLOCK] = fma(vgs, CK(L2E / 7.43), CK(71.55 * L2E / 7.43));
+    col[A_XR1 * BLOCK] = fma(vgs, CK(L2E / 11.5), CK(30.0 * L2E / 11.5));
+    col[A_D * BLOCK] = fma(vgs, CK(-L2E / 13.0), CK(-35.0 * L2E / 13.0));
     col[A_PK * BLOCK] = fma(vg, CK(-L2E / 5.98), CK(25.0 * L2E / 5.98));
     col[A_W * BLOCK] = vg * CK(0.05 * FRT * L2E);
-    col[A_GR * BLOCK] = (vg + 40.0) * (vg + 40.0) * CK(-L2E / 1800.0);
-    col[A_GS * BLOCK] = (type == 0) ? (vg + 67.0) * (vg + 67.0) * CK(-L2E / 1000.0)
-                                    : (vg + 45.0) * (vg + 45.0) * CK(-L2E / 320.0);
-    col[A_G27 * BLOCK] = (vg + 27.0) * (vg + 27.0) * CK(-L2E / 3600.0);
+    col[A_GR * BLOCK] = (vgs + 40.0) * (vgs + 40.0) * CK(-L2E / 1800.0);
+    col[A_GS * BLOCK] = (type == 0) ? (vgs + 67.0) * (vgs + 67.0) * CK(-L2E / 1000.0)
+                                    : (vgs + 45.0) * (vgs + 45.0) * CK(-L2E / 320.0);
+    col[A_G27 * BLOCK] = (vgs + 27.0) * (vgs + 27.0) * CK(-L2E / 3600.0);
     const double xcal = (vg - 15.0) * CK(2.0 * FRT);
     col[A_CAL * BLOCK] = fma(vg, CK(2.0 * FRT * L2E), CK(-30.0 * FRT * L2E));   // xcal in base-2 units
     col[A_K1Q * BLOCK] = fma(ug, CK(0.0002 * L2E), CK(0.02 * L2E));   // 0.0002 (u + 100)
     col[A_K1Q2 * BLOCK] = ug * CK(0.02 * L2E);
     if (hi) {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
-        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.057 * L2E);
+        col[(A_HJ0 + 0) * BLOCK] = fma(vgs, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
+        col[(A_HJ0 + 1) * BLOCK] = vgs * CK(0.057 * L2E);
 #pragma unroll
         for (int k = 0; k < 6; ++k) col[(A_HJ2 + k) * BLOCK] = 0.0;
     } else {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));
-        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.079 * L2E);
-        col[(A_HJ2 + 0) * BLOCK] = vg * CK(0.3485 * L2E);
-        col[(A_HJ2 + 1) * BLOCK] = vg * CK(0.2444 * L2E);
-        col[(A_HJ2 + 2) * BLOCK] = vg * CK(-0.04391 * L2E);
-        col[(A_HJ2 + 3) * BLOCK] = fma(vg, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
-        col[(A_HJ2 + 4) * BLOCK] = vg * CK(-0.01052 * L2E);
-        col[(A_HJ2 + 5) * BLOCK] = fma(vg, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
+        col[(A_HJ0 + 0) * BLOCK] = fma(vgs, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));
+        col[(A_HJ0 + 1) * BLOCK] = vgs * CK(0.079 * L2E);
+        col[(A_HJ2 + 0) * BLOCK] = vgs * CK(0.3485 * L2E);
+        col[(A_HJ2 + 1) * BLOCK] = vgs * CK(0.2444 * L2E);
+        col[(A_HJ2 + 2) * BLOCK] = vgs * CK(-0.04391 * L2E);
+        col[(A_HJ2 + 3) * BLOCK] = fma(vgs, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
+        col[(A_HJ2 + 4) * BLOCK] = vgs * CK(-0.01052 * L2E);
+        col[(A_HJ2 + 5) * BLOCK] = fma(vgs, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
     }
     // fCass and Rbar: their Rush-Larsen rates need no exponential, so exp(-dt/tau) rides in this batch
     const double c2 = CaSR * CaSR, css2 = CaSS * CaSS, ci2 = Cai * Cai;
     const double kcasr = fma(-(maxsr - minsr) * c2, ep_rcp(c2 + EC * EC), maxsr);
-    const double qf = ep_rcp(fma(400.0, css2, 1.0));              // 1/(1 + (CaSS/0.05)^2)
+    double kcasr_s = kcasr, css2_s = css2;      // the same at the gates' arguments (second order: Ca_SR*, Ca_SS*)
+    if constexpr (ORDER == 2) {
+        const double c2s = CaSRs * CaSRs;
+        kcasr_s = fma(-(maxsr - minsr) * c2s, ep_rcp(c2s + EC * EC), maxsr);
+        css2_s = CaSSs * CaSSs;
+    }
+    const double qf = ep_rcp(fma(400.0, css2_s, 1.0));              // 1/(1 + (CaSS/0.05)^2)
     const double fCass_inf = fma(CK(0.6), qf, CK(0.4));
-    const double Rbar_rate = fma(CK(k2p) * kcasr, CaSS, CK(k4));   // dR/dt = k4 (1 - R) - k2 CaSS R (reading B1)
+    const double Rbar_rate = fma(CK(k2p) * kcasr_s, CaSSs, CK(k4));   // dR/dt = k4 (1 - R) - k2 CaSS R (reading B1)
     const double Rbar_inf = CK(k4) * ep_rcp(Rbar_rate);
     col[A_RLF * BLOCK] = -dtl * ep_rcp(fma(80.0, qf, 2.0));         // tau_fCass >= 2 ms
     col[A_RLR * BLOCK] = fmax(-dtl * Rbar_rate, -1000.0);           // rate grows with Ca_SS: keep the clamp
@@ -311,13 +341,34 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double dCaSR = bsr * (Iup - Ileak - Irel);
     const double dCaSS = bss * (-ICaL * CK(Cap / (2.0 * Vss * F)) + Irel * CK(Vsr / Vss) - Ixfer * CK(Vc / Vss));
     const double dNai = -(INa + IbNa + 3.0 * INaK + 3.0 * INaCa) * CK(Cap / (Vc * F));
-    const double dKi = -(IK1 + Ito + IKr + IKs - 2.0 * INaK + IpK + istim) * CK(Cap / (Vc * F));   // reading B8
-    const double v_new = fma(dt, dv_diff - iion - istim, v);   // eq. (7); explicit increment :172
-    ycol[Y_CAI * stride] = fma(dt, dCai, Cai);                 // forward Euler
-    ycol[Y_CASR * stride] = fma(dt, dCaSR, CaSR);
-    ycol[Y_CASS * stride] = fma(dt, dCaSS, CaSS);
-    ycol[Y_NAI * stride] = fma(dt, dNai, Nai);
-    ycol[Y_KI * stride] = fma(dt, dKi, Ki);
+    double v_new;
+    if constexpr (ORDER == 1) {
+        const double dKi = -(IK1 + Ito + IKr + IKs - 2.0 * INaK + IpK + istim) * CK(Cap / (Vc * F));   // reading B8
+        v_new = fma(dt, dv_diff - iion - istim, v);            // eq. (7); explicit increment :172
+        ycol[Y_CAI * stride] = fma(dt, dCai, Cai);             // forward Euler
+        ycol[Y_CASR * stride] = fma(dt, dCaSR, CaSR);
+        ycol[Y_CASS * stride] = fma(dt, dCaSS, CaSS);
+        ycol[Y_NAI * stride] = fma(dt, dNai, Nai);
+        ycol[Y_KI * stride] = fma(dt, dKi, Ki);
+    } else {
+        // right-hand sides without the stimulus; AB2 where there is a history, the stimulus added as its exact integral
+        const double f[6] = {dv_diff - iion, dCai, dCaSR, dCaSS, dNai,
+                             -(IK1 + Ito + IKr + IKs - 2.0 * INaK + IpK) * CK(Cap / (Vc * F))};
+        double w[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            w[k] = hist.have ? fma(1.5, f[k], -0.5 * fprev[k]) : f[k];
+            hist.hcol[k * hist.stride] = f[k];
+        }
+        hist.hcol[6 * hist.stride] = CaSS;
+        hist.hcol[7 * hist.stride] = CaSR;
+        v_new = fma(dt, w[0] - istim, v);
+        ycol[Y_CAI * stride] = fma(dt, w[1], Cai);
+        ycol[Y_CASR * stride] = fma(dt, w[2], CaSR);
+        ycol[Y_CASS * stride] = fma(dt, w[3], CaSS);
+        ycol[Y_NAI * stride] = fma(dt, w[4], Nai);
+        ycol[Y_KI * stride] = fma(dt, w[5] - istim * CK(Cap / (Vc * F)), Ki);      // reading B8
+    }
 
     // ---- gates: steady states and rates 1/tau, each as one rational function
     double inf[N_RLB], rate[N_RLB];   // index g = state index - 1
@@ -338,7 +389,7 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
             const double s2 = col[(A_HJ2 + 0) * BLOCK], s3 = col[(A_HJ2 + 1) * BLOCK], s4 = col[(A_HJ2 + 2) * BLOCK],
                          s5 = col[(A_HJ2 + 3) * BLOCK], s6 = col[(A_HJ2 + 4) * BLOCK], s7 = col[(A_HJ2 + 5) * BLOCK];
             rate[1] = fma(CK(0.057), s0, fma(CK(2.7), s1, 3.1e5 * s2));
-            const double N1 = fma(-2.5428e4, s3, CK(-6.948e-6) * s4) * (vg + CK(37.78)), D1 = 1.0 + s5;
+            const double N1 = fma(-2.5428e4, s3, CK(-6.948e-6) * s4) * (vgs + CK(37.78)), D1 = 1.0 + s5;
             const double N2 = CK(0.02424) * s6, D2 = 1.0 + s7;
             rate[2] = fma(N1, D2, N2 * D1) * ep_rcp(D1 * D2);
         }
