@@ -81,6 +81,38 @@ int ep_read_vext(ep_sim *sim, double *out);
 /* GMRES iterations of the last solve / of all solves, number of solves, last relative residual; any pointer may be NULL. */
 int ep_bidomain_stats(ep_sim *sim, int64_t *iters_last, int64_t *iters_total, int64_t *solves, double *rel_res_last);
 
+/* Intra-mesh sharding (the paper itself uses one GPU per chamber).  The cells of ONE mesh are
+ * cut into n_parts contiguous ranges of the Morton curve through their centroids.  Part p owns one range and keeps, as halo,
+ * every other cell within two node-rings of an owned cell -- the reach of the stencil (the nodes of a cell and
+ * of its face neighbours, and the cells around those nodes).  ep_step advances the owned cells only; between two steps every
+ * part needs the new Vm of its halo cells from their owners: one neighbour exchange per step, no global reduction.
+ *
+ * ep_shard_create takes the GLOBAL mesh (every rank holds it on the host) and builds part `part`: a handle whose cells are
+ * numbered locally -- owned cells first (ascending global id), then halo cells (ascending global id); every other call
+ * (ep_state_init, ep_stimulus_set, ep_read_vm ...) works in that local numbering with n_tets = n_local.  Values read back for
+ * halo cells are the last received copies; activation times and ep_mean_vm cover the owned cells (ep_mean_vm: owned volume
+ * weights, so the global mean is the volume-weighted mean of the parts').
+ * ep_shard_info: sizes, the global id of every local cell [n_local], and the per-peer segments [n_parts+1] of the two
+ * exchange buffers (any pointer may be NULL).  The segment a part sends to peer q lists the same cells in the same order
+ * (ascending global id) as q's receive segment from that part.
+ * ep_shard_buffers: DEVICE pointers of the send / receive buffers (doubles), for NCCL send/recv or peer copies.
+ * One step of a sharded run: ep_step(sim, 1, dt); ep_halo_pack(sim); <exchange the segments>; ep_halo_unpack(sim).
+ * ep_halo_exchange_local does pack + exchange + unpack for all parts living in ONE process (device-to-device copies).
+ * ep_shard_plan is the host-only partitioner (no device needed): counts[4] = {n_owned, n_local, n_send, n_recv}, local_cells
+ * [n_local], send/recv segment pointers [n_parts+1] and the cells of both buffers as GLOBAL ids; arrays of capacity n_tets are
+ * always large enough; any of them may be NULL.  n_parts <= 64.  Not available for bidomain handles. */
+int ep_shard_plan(int64_t n_nodes, const double *xyz_mm, int64_t n_tets, const int32_t *tets, int part, int n_parts,
+                  int64_t *counts, int64_t *local_cells, int64_t *send_ptr, int64_t *send_global, int64_t *recv_ptr,
+                  int64_t *recv_global);
+int ep_shard_create(ep_sim **out, int64_t n_nodes, const double *xyz_mm, int64_t n_tets, const int32_t *tets,
+                    const double *fibre, const double *sigma_scale, double sigma_l, double sigma_t, double chi, double Cm,
+                    int part, int n_parts);
+int ep_shard_info(ep_sim *sim, int64_t *n_owned, int64_t *n_local, int64_t *global_ids, int64_t *send_ptr, int64_t *recv_ptr);
+int ep_shard_buffers(ep_sim *sim, void **send_dptr, void **recv_dptr);
+int ep_halo_pack(ep_sim *sim);
+int ep_halo_unpack(ep_sim *sim);
+int ep_halo_exchange_local(ep_sim **sims, int n_parts);
+
 /* Choose the cell model and set every cell to an initial state.
  *   cell_type [n_tets] TP06: 0 endo, 1 mid, 2 epi (reading B5); NULL => 0
  *   y0        [n_types*S] one state vector per cell type (n_types = 3 for TP06, 1 for CRN98 and STEWART); NULL => built-in

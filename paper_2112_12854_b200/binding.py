@@ -27,6 +27,14 @@ SIGNATURES = {
     "ep_bidomain_solver": (C.c_int, [_vp, C.c_int, C.c_int, C.c_double]),
     "ep_read_vext": (C.c_int, [_vp, _dp]),
     "ep_bidomain_stats": (C.c_int, [_vp, _i64p, _i64p, _i64p, _dp]),
+    "ep_shard_plan": (C.c_int, [C.c_int64, _dp, C.c_int64, _i32p, C.c_int, C.c_int, _i64p, _i64p, _i64p, _i64p, _i64p, _i64p]),
+    "ep_shard_create": (C.c_int, [C.POINTER(_vp), C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double,
+                                  C.c_double, C.c_double, C.c_int, C.c_int]),
+    "ep_shard_info": (C.c_int, [_vp, _i64p, _i64p, _i64p, _i64p, _i64p]),
+    "ep_shard_buffers": (C.c_int, [_vp, C.POINTER(_vp), C.POINTER(_vp)]),
+    "ep_halo_pack": (C.c_int, [_vp]),
+    "ep_halo_unpack": (C.c_int, [_vp]),
+    "ep_halo_exchange_local": (C.c_int, [C.POINTER(_vp), C.c_int]),
     "ep_state_init": (C.c_int, [_vp, C.c_int, _u8p, _dp]),
     "ep_stimulus_set": (C.c_int, [_vp, C.c_int, C.c_int64, _i64p, C.c_double, C.c_double, C.c_double]),
     "ep_trigger_set": (C.c_int, [_vp, C.c_int, C.c_int64, _i64p, C.c_int, C.c_double]),
@@ -156,6 +164,27 @@ def host_stencil_tri(xyz, tris, fibre=None, sigma_scale=None, sigma_l=1.3, sigma
     return out
 
 
+def shard_plan(xyz, tets, part, n_parts):
+    """ep_shard_plan: the host-only partitioner (no GPU needed).  Returns n_owned, the global ids of the local cells (owned
+    first), and the per-peer segments + global cell ids of the send and receive buffers."""
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+    tets = np.ascontiguousarray(tets, dtype=np.int32)
+    nc = tets.shape[0]
+    counts = np.zeros(4, np.int64)
+    local = np.empty(nc, np.int64); sg = np.empty(nc, np.int64); rg = np.empty(nc, np.int64)
+    sp = np.empty(n_parts + 1, np.int64); rp = np.empty(n_parts + 1, np.int64)
+    _chk(lib().ep_shard_plan(xyz.shape[0], _p(xyz), nc, _p(tets, C.c_int32), int(part), int(n_parts), _p(counts, C.c_int64),
+                             _p(local, C.c_int64), _p(sp, C.c_int64), _p(sg, C.c_int64), _p(rp, C.c_int64), _p(rg, C.c_int64)))
+    return dict(n_owned=int(counts[0]), local_cells=local[:counts[1]].copy(), send_ptr=sp, send_global=sg[:counts[2]].copy(),
+                recv_ptr=rp, recv_global=rg[:counts[3]].copy())
+
+
+def halo_exchange_local(sims):
+    """ep_halo_exchange_local: pack, exchange and unpack the halos of all parts of one sharding living in this process."""
+    arr = (_vp * len(sims))(*[s._h for s in sims])
+    _chk(lib().ep_halo_exchange_local(arr, len(sims)))
+
+
 class Sim:
     """One simulation handle (ep_sim*).  Method names follow the C-ABI calls.  cells [n,4]: tetrahedra (ep_mesh_create);
     cells [n,3]: a triangulated surface (ep_mesh_create_tri)."""
@@ -179,6 +208,41 @@ class Sim:
         self.n_tets = int(lib().ep_n_cells(self._h))
         self.n_nodes = int(lib().ep_n_nodes(self._h))
         self.n_states = 0
+
+    @classmethod
+    def shard(cls, xyz, tets, part, n_parts, fibre=None, sigma_scale=None, sigma_l=1.3, sigma_t=0.18, chi=1400.0, Cm=1.0):
+        """ep_shard_create: part `part` of an n_parts-way sharding of the GLOBAL mesh.  The handle is numbered locally;
+        self.global_ids[k] is the global id of local cell k, the first self.n_owned are the owned ones."""
+        xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+        tets = np.ascontiguousarray(tets, dtype=np.int32)
+        fibre = None if fibre is None else np.ascontiguousarray(fibre, dtype=np.float64)
+        sigma_scale = None if sigma_scale is None else np.ascontiguousarray(sigma_scale, dtype=np.float64)
+        s = cls.__new__(cls)
+        s._h = _vp()
+        _chk(lib().ep_shard_create(C.byref(s._h), xyz.shape[0], _p(xyz), tets.shape[0], _p(tets, C.c_int32), _p(fibre),
+                                   _p(sigma_scale), sigma_l, sigma_t, chi, Cm, int(part), int(n_parts)))
+        s.n_tets = int(lib().ep_n_cells(s._h))
+        s.n_nodes = int(lib().ep_n_nodes(s._h))
+        s.n_states = 0
+        no, nl = C.c_int64(), C.c_int64()
+        s.global_ids = np.empty(s.n_tets, np.int64)
+        s.send_ptr = np.empty(n_parts + 1, np.int64); s.recv_ptr = np.empty(n_parts + 1, np.int64)
+        _chk(lib().ep_shard_info(s._h, C.byref(no), C.byref(nl), _p(s.global_ids, C.c_int64), _p(s.send_ptr, C.c_int64),
+                                 _p(s.recv_ptr, C.c_int64)))
+        s.n_owned = int(no.value)
+        return s
+
+    def shard_buffers(self):
+        """Device pointers (ints) of the send and receive buffers."""
+        a, b = _vp(), _vp()
+        _chk(lib().ep_shard_buffers(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def halo_pack(self):
+        _chk(lib().ep_halo_pack(self._h))
+
+    def halo_unpack(self):
+        _chk(lib().ep_halo_unpack(self._h))
 
     @classmethod
     def from_problem(cls, prob):

@@ -81,6 +81,12 @@ struct ep_sim {
     int bd_restart = 30, bd_max_cycles = 200, bd_check = 5;
     double bd_tol = 1e-10;
     bool vext_valid = false;
+    // shard of a larger mesh (ep_shard_create): local cell k <-> global cell id, exchange lists as device positions
+    int n_parts = 1, part = 0;
+    int64_t n_owned = 0;
+    std::vector<int64_t> shard_global, send_ptr, recv_ptr;
+    int32_t *d_send_idx = nullptr, *d_recv_idx = nullptr;
+    double *d_send = nullptr, *d_recv = nullptr;
     // second-order time stepping (ep_set_time_order): history rows and whether they hold t^{n-1} of the current state
     int order = 1;
     double* d_hist = nullptr;
@@ -136,7 +142,8 @@ int64_t step_index(double t, double dt) { return (int64_t)std::ceil(t / dt - 1e-
 void free_all(ep_sim* s) {
     void* ptrs[] = {s->d_cidx, s->d_nidx, s->d_perm, s->d_inv, s->d_ccoef, s->d_nw, s->d_slice_ptr, s->d_vm[0],
                     s->d_vm[1], s->d_y, s->d_vn, s->d_tact, s->d_tmp, s->d_tmp2, s->d_red, s->d_ctype, s->d_smask,
-                    s->d_vol, s->d_tmask, s->d_trig_fire, s->d_trig_par, s->d_ccoef_ie, s->d_vext, s->d_src, s->d_b, s->d_hist};
+                    s->d_vol, s->d_tmask, s->d_trig_fire, s->d_trig_par, s->d_ccoef_ie, s->d_vext, s->d_src, s->d_b, s->d_hist, s->d_send_idx, s->d_recv_idx,
+                    s->d_send, s->d_recv};
     epk::gmres_free(s->gm);
     for (void* p : ptrs) if (p) cudaFree(p);
     for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
@@ -355,7 +362,7 @@ int ep_host_stencil(int64_t n_nodes, const double* xyz, int64_t n_tets, const in
 // ext_l, ext_t > 0: bidomain; (sigma_l, sigma_t) are then the intracellular conductivities
 static int mesh_create_impl(ep_sim** out, int dim, int64_t n_nodes, const double* xyz, int64_t n_tets, const int32_t* tets,
                             const double* fibre, const double* sigma_scale, double sigma_l, double sigma_t, double chi,
-                            double Cm, double ext_l = 0.0, double ext_t = 0.0) {
+                            double Cm, double ext_l = 0.0, double ext_t = 0.0, int64_t n_owned = -1) {
     if (!out) return fail(EP_ERR_ARG, "out is NULL");
     *out = nullptr;
     ep_sim* s = nullptr;
@@ -371,10 +378,11 @@ static int mesh_create_impl(ep_sim** out, int dim, int64_t n_nodes, const double
         int rc = dim == 3 ? ep::build_stencil(n_nodes, xyz, n_tets, tets, fibre, sigma_scale, sigma_l, sigma_t, chi, Cm, st, err)
                           : ep::build_stencil_tri(n_nodes, xyz, n_tets, tets, fibre, sigma_scale, sigma_l, sigma_t, chi, Cm, st, err);
         if (rc) return fail(rc, err);
-        rc = ep::pack(st, xyz, pk, err);
+        rc = ep::pack(st, xyz, pk, err, n_owned);
         if (rc) return fail(rc, err);
         s = new ep_sim();
         s->dim = dim;
+        s->n_owned = (n_owned >= 0 && n_owned < n_tets) ? n_owned : n_tets;
         cudaGetDevice(&s->device);
         s->pdl = (std::getenv("EP_NO_PDL") == nullptr);
         s->nc = pk.nc; s->nn = pk.nn; s->nc_pad = pk.nc_pad; s->chi = chi; s->Cm = Cm;
@@ -411,6 +419,7 @@ static int mesh_create_impl(ep_sim** out, int dim, int64_t n_nodes, const double
         cudaMemset(s->d_trig_fire, 0xff, sizeof(long long) * epk::MAX_TRIGGERS);
         cudaMemset(s->d_trig_par, 0, sizeof(epk::TrigPar) * epk::MAX_TRIGGERS);
         s->dm.nc = s->nc; s->dm.nn = s->nn; s->dm.nc_pad = s->nc_pad; s->dm.n_slices = pk.n_slices;
+        s->dm.nc_active = s->n_owned;
         s->dm.cidx = s->d_cidx; s->dm.ccoef = s->d_ccoef; s->dm.slice_ptr = s->d_slice_ptr;
         s->dm.nidx = s->d_nidx; s->dm.nw = s->d_nw;
         if (ext_l > 0.0 || ext_t > 0.0) {
@@ -419,7 +428,7 @@ static int mesh_create_impl(ep_sim** out, int dim, int64_t n_nodes, const double
             ep::Packed pk2;
             rc = ep::build_stencil(n_nodes, xyz, n_tets, tets, fibre, sigma_scale, sigma_l + ext_l, sigma_t + ext_t, chi, Cm, st2, err);
             if (rc) return bail(fail(rc, err));
-            rc = ep::pack(st2, xyz, pk2, err);
+            rc = ep::pack(st2, xyz, pk2, err, n_owned);
             if (rc) return bail(fail(rc, err));
             if (pk2.cidx != pk.cidx) return bail(fail(EP_ERR_MESH, "internal: index tables of the two operators differ"));
             if ((rc = upload(s, &s->d_ccoef_ie, pk2.ccoef)) || (rc = dev_alloc(s, &s->d_vext, s->nc_pad)) ||
@@ -490,6 +499,137 @@ int ep_mesh_create_bidomain(ep_sim** out, int64_t n_nodes, const double* xyz, in
     if (!(sigma_ext_l > 0.0) || !(sigma_ext_t > 0.0)) return fail(EP_ERR_ARG, "extracellular conductivities must be positive");
     return mesh_create_impl(out, 3, n_nodes, xyz, n_tets, tets, fibre, sigma_scale, sigma_int_l, sigma_int_t, chi, Cm,
                             sigma_ext_l, sigma_ext_t);
+}
+
+int ep_shard_plan(int64_t n_nodes, const double* xyz, int64_t n_tets, const int32_t* tets, int part, int n_parts,
+                  int64_t* counts, int64_t* local_cells, int64_t* send_ptr, int64_t* send_global, int64_t* recv_ptr,
+                  int64_t* recv_global) {
+    if (!counts) return fail(EP_ERR_ARG, "counts is NULL");
+    try {
+        ep::ShardPlan pl;
+        std::string err;
+        int rc = ep::shard_plan(n_nodes, xyz, n_tets, tets, part, n_parts, pl, err);
+        if (rc) return fail(rc, err);
+        counts[0] = pl.n_owned; counts[1] = (int64_t)pl.local_cells.size();
+        counts[2] = (int64_t)pl.send_cells.size(); counts[3] = (int64_t)pl.recv_cells.size();
+        if (local_cells) std::memcpy(local_cells, pl.local_cells.data(), sizeof(int64_t) * pl.local_cells.size());
+        if (send_ptr) std::memcpy(send_ptr, pl.send_ptr.data(), sizeof(int64_t) * pl.send_ptr.size());
+        if (recv_ptr) std::memcpy(recv_ptr, pl.recv_ptr.data(), sizeof(int64_t) * pl.recv_ptr.size());
+        if (send_global) for (size_t k = 0; k < pl.send_cells.size(); ++k) send_global[k] = pl.local_cells[pl.send_cells[k]];
+        if (recv_global) for (size_t k = 0; k < pl.recv_cells.size(); ++k) recv_global[k] = pl.local_cells[pl.recv_cells[k]];
+        return EP_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(EP_ERR_NOMEM, "host allocation failed");
+    } catch (...) {
+        return fail(EP_ERR_ARG, "unexpected exception in the partitioner");
+    }
+}
+
+int ep_shard_create(ep_sim** out, int64_t n_nodes, const double* xyz, int64_t n_tets, const int32_t* tets,
+                    const double* fibre, const double* sigma_scale, double sigma_l, double sigma_t, double chi, double Cm,
+                    int part, int n_parts) {
+    if (!out) return fail(EP_ERR_ARG, "out is NULL");
+    *out = nullptr;
+    try {
+        ep::ShardPlan pl;
+        std::string err;
+        int rc = ep::shard_plan(n_nodes, xyz, n_tets, tets, part, n_parts, pl, err);
+        if (rc) return fail(rc, err);
+        const int64_t nl = (int64_t)pl.local_cells.size(), nln = (int64_t)pl.local_nodes.size();
+        std::vector<double> lxyz(3 * nln), lfib, lscale;
+        for (int64_t k = 0; k < nln; ++k)
+            for (int d = 0; d < 3; ++d) lxyz[3 * k + d] = xyz[3 * pl.local_nodes[k] + d];
+        if (fibre) {
+            lfib.resize(3 * nl);
+            for (int64_t k = 0; k < nl; ++k)
+                for (int d = 0; d < 3; ++d) lfib[3 * k + d] = fibre[3 * pl.local_cells[k] + d];
+        }
+        if (sigma_scale) {
+            lscale.resize(nl);
+            for (int64_t k = 0; k < nl; ++k) lscale[k] = sigma_scale[pl.local_cells[k]];
+        }
+        ep_sim* s = nullptr;
+        rc = mesh_create_impl(&s, 3, nln, lxyz.data(), nl, pl.local_tets.data(), fibre ? lfib.data() : nullptr,
+                              sigma_scale ? lscale.data() : nullptr, sigma_l, sigma_t, chi, Cm, 0.0, 0.0, pl.n_owned);
+        if (rc) return rc;
+        s->n_parts = n_parts; s->part = part;
+        s->shard_global = pl.local_cells;
+        s->send_ptr = pl.send_ptr; s->recv_ptr = pl.recv_ptr;
+        std::vector<int32_t> si(pl.send_cells.size()), ri(pl.recv_cells.size());
+        for (size_t k = 0; k < si.size(); ++k) si[k] = s->inv_c[pl.send_cells[k]];
+        for (size_t k = 0; k < ri.size(); ++k) ri[k] = s->inv_c[pl.recv_cells[k]];
+        if ((rc = upload(s, &s->d_send_idx, si)) || (rc = upload(s, &s->d_recv_idx, ri)) ||
+            (rc = dev_alloc(s, &s->d_send, (int64_t)si.size())) || (rc = dev_alloc(s, &s->d_recv, (int64_t)ri.size()))) {
+            free_all(s); delete s;
+            return rc;
+        }
+        *out = s;
+        return EP_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(EP_ERR_NOMEM, "host allocation failed");
+    } catch (...) {
+        return fail(EP_ERR_ARG, "unexpected exception");
+    }
+}
+
+int ep_shard_info(ep_sim* s, int64_t* n_owned, int64_t* n_local, int64_t* global_ids, int64_t* send_ptr, int64_t* recv_ptr) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    if (s->shard_global.empty()) return fail(EP_ERR_STATE, "not a shard (ep_shard_create)");
+    if (n_owned) *n_owned = s->n_owned;
+    if (n_local) *n_local = s->nc;
+    if (global_ids) std::memcpy(global_ids, s->shard_global.data(), sizeof(int64_t) * s->shard_global.size());
+    if (send_ptr) std::memcpy(send_ptr, s->send_ptr.data(), sizeof(int64_t) * s->send_ptr.size());
+    if (recv_ptr) std::memcpy(recv_ptr, s->recv_ptr.data(), sizeof(int64_t) * s->recv_ptr.size());
+    return EP_OK;
+}
+
+int ep_shard_buffers(ep_sim* s, void** send_dptr, void** recv_dptr) {
+    if (!s) return fail(EP_ERR_ARG, "null sim handle");
+    if (s->shard_global.empty()) return fail(EP_ERR_STATE, "not a shard (ep_shard_create)");
+    if (send_dptr) *send_dptr = s->d_send;
+    if (recv_dptr) *recv_dptr = s->d_recv;
+    return EP_OK;
+}
+
+int ep_halo_pack(ep_sim* s) {
+    int rc = check_sim(s);
+    if (rc) return rc;
+    if (s->shard_global.empty()) return fail(EP_ERR_STATE, "not a shard (ep_shard_create)");
+    const int64_t n = s->send_ptr.back();
+    if (n > 0) { epk::launch_gather_f64(n, s->d_vm[s->cur], s->d_send_idx, s->d_send, s->stream); s->launches++; }
+    EP_CUDA(s, cudaGetLastError());
+    return EP_OK;
+}
+
+int ep_halo_unpack(ep_sim* s) {
+    int rc = check_sim(s);
+    if (rc) return rc;
+    if (s->shard_global.empty()) return fail(EP_ERR_STATE, "not a shard (ep_shard_create)");
+    const int64_t n = s->recv_ptr.back();
+    if (n > 0) { epk::launch_scatter_f64(n, s->d_recv, s->d_recv_idx, s->d_vm[s->cur], s->stream); s->launches++; }
+    EP_CUDA(s, cudaGetLastError());
+    return EP_OK;
+}
+
+int ep_halo_exchange_local(ep_sim** sims, int n) {
+    if (!sims || n < 1) return fail(EP_ERR_ARG, "bad shard list");
+    for (int p = 0; p < n; ++p) {
+        if (!sims[p] || sims[p]->shard_global.empty() || sims[p]->n_parts != n || sims[p]->part != p)
+            return fail(EP_ERR_ARG, "sims[p] must be part p of an n-part sharding");
+    }
+    int rc;
+    for (int p = 0; p < n; ++p) if ((rc = ep_halo_pack(sims[p]))) return rc;
+    for (int p = 0; p < n; ++p) EP_CUDA(sims[p], cudaStreamSynchronize(sims[p]->stream));
+    for (int p = 0; p < n; ++p)          // p receives from q what q sends to p: same cells, same order
+        for (int q = 0; q < n; ++q) {
+            const int64_t cnt = sims[p]->recv_ptr[q + 1] - sims[p]->recv_ptr[q];
+            if (cnt != sims[q]->send_ptr[p + 1] - sims[q]->send_ptr[p]) return fail(EP_ERR_STATE, "exchange lists do not match");
+            if (cnt == 0) continue;
+            EP_CUDA(sims[p], cudaMemcpyAsync(sims[p]->d_recv + sims[p]->recv_ptr[q], sims[q]->d_send + sims[q]->send_ptr[p],
+                                             sizeof(double) * cnt, cudaMemcpyDeviceToDevice, sims[p]->stream));
+        }
+    for (int p = 0; p < n; ++p) if ((rc = ep_halo_unpack(sims[p]))) return rc;
+    return EP_OK;
 }
 
 void ep_destroy(ep_sim* s) {

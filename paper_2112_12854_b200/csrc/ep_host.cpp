@@ -422,11 +422,13 @@ int build_stencil_tri(int64_t nn, const double* xyz, int64_t nc, const int32_t* 
     return 0;
 }
 
-int pack(const Stencil& st, const double* xyz, Packed& out, std::string& err) {
+int pack(const Stencil& st, const double* xyz, Packed& out, std::string& err, int64_t n_owned) {
     (void)err;
     const int64_t nc = st.nc, nn = st.nn;
     out.nc = nc; out.nn = nn;
     morton_order(st.centroid.data(), nc, out.perm_c);
+    if (n_owned >= 0 && n_owned < nc)   // shard: owned cells first; each group keeps its Morton order
+        std::stable_partition(out.perm_c.begin(), out.perm_c.end(), [&](int32_t c) { return (int64_t)c < n_owned; });
     morton_order(xyz, nn, out.perm_n);
     out.inv_c.resize(nc);
     for (int64_t i = 0; i < nc; ++i) out.inv_c[out.perm_c[i]] = (int32_t)i;
@@ -438,10 +440,11 @@ int pack(const Stencil& st, const double* xyz, Packed& out, std::string& err) {
     out.ccoef.assign(12 * out.nc_pad, 0.0);
     out.vol.assign(out.nc_pad, 0.0);
     out.vol_total = 0.0;
-    for (int64_t c = 0; c < nc; ++c) out.vol_total += st.vol[c];
+    const int64_t n_weighted = (n_owned >= 0 && n_owned < nc) ? n_owned : nc;
+    for (int64_t c = 0; c < n_weighted; ++c) out.vol_total += st.vol[c];
     for (int64_t i = 0; i < nc; ++i) {
         const int64_t c = out.perm_c[i];
-        out.vol[i] = st.vol[c];
+        out.vol[i] = c < n_weighted ? st.vol[c] : 0.0;
         for (int m = 0; m < 8; ++m) {
             out.cidx[tile_index(i, m, 12)] = inv_n[st.node[8 * c + m]];
             out.ccoef[tile_index(i, m, 12)] = st.a[8 * c + m];
@@ -478,6 +481,83 @@ int pack(const Stencil& st, const double* xyz, Packed& out, std::string& err) {
             if (k < (int64_t)tmp.size()) { out.nidx[at] = tmp[k].first; out.nw[at] = tmp[k].second; }
             else { out.nidx[at] = tmp.empty() ? 0 : tmp[0].first; out.nw[at] = 0.0; }
         }
+    }
+    return 0;
+}
+
+
+int shard_plan(int64_t nn, const double* xyz, int64_t nc, const int32_t* tets, int part, int n_parts, ShardPlan& out,
+               std::string& err) {
+    if (nn <= 0 || nc <= 0 || !xyz || !tets) { err = "null pointer or non-positive mesh size"; return ERR_ARG; }
+    if (n_parts < 1 || n_parts > 64 || part < 0 || part >= n_parts) { err = "need 0 <= part < n_parts <= 64"; return ERR_ARG; }
+    if (nc < n_parts) { err = "fewer cells than parts"; return ERR_ARG; }
+    for (int64_t i = 0; i < 4 * nc; ++i)
+        if (tets[i] < 0 || tets[i] >= nn) { err = "tet node index out of range"; return ERR_MESH; }
+    // ownership: contiguous ranges of the Morton curve through the cell centroids
+    std::vector<double> cen(3 * nc);
+    for (int64_t c = 0; c < nc; ++c)
+        for (int d = 0; d < 3; ++d) {
+            double a = 0.0;
+            for (int k = 0; k < 4; ++k) a += xyz[3 * (int64_t)tets[4 * c + k] + d];
+            cen[3 * c + d] = 0.25 * a;
+        }
+    std::vector<int32_t> perm;
+    morton_order(cen.data(), nc, perm);
+    std::vector<uint8_t> owner(nc);
+    for (int64_t i = 0; i < nc; ++i) owner[perm[i]] = (uint8_t)((i * n_parts) / nc);
+    // node stars
+    std::vector<int64_t> ptr(nn + 1, 0);
+    for (int64_t i = 0; i < 4 * nc; ++i) ptr[tets[i] + 1]++;
+    for (int64_t n = 0; n < nn; ++n) ptr[n + 1] += ptr[n];
+    std::vector<int32_t> star(4 * nc);
+    {
+        std::vector<int64_t> fill(ptr.begin(), ptr.end() - 1);
+        for (int64_t c = 0; c < nc; ++c)
+            for (int k = 0; k < 4; ++k) star[fill[tets[4 * c + k]]++] = (int32_t)c;
+    }
+    // ring1[c]: parts owning a cell that shares a node with c; ring2[c]: the same one node-ring further
+    std::vector<uint64_t> node_mask(nn, 0), ring1(nc, 0), ring2(nc, 0);
+    for (int64_t c = 0; c < nc; ++c)
+        for (int k = 0; k < 4; ++k) node_mask[tets[4 * c + k]] |= 1ULL << owner[c];
+    for (int64_t c = 0; c < nc; ++c)
+        for (int k = 0; k < 4; ++k) ring1[c] |= node_mask[tets[4 * c + k]];
+    std::fill(node_mask.begin(), node_mask.end(), 0);
+    for (int64_t c = 0; c < nc; ++c)
+        for (int k = 0; k < 4; ++k) node_mask[tets[4 * c + k]] |= ring1[c];
+    for (int64_t c = 0; c < nc; ++c)
+        for (int k = 0; k < 4; ++k) ring2[c] |= node_mask[tets[4 * c + k]];
+    // local cells: owned (ascending), then halo (ascending)
+    out = ShardPlan();
+    out.part = part; out.n_parts = n_parts;
+    const uint64_t me = 1ULL << part;
+    for (int64_t c = 0; c < nc; ++c) if (owner[c] == part) out.local_cells.push_back(c);
+    out.n_owned = (int64_t)out.local_cells.size();
+    if (out.n_owned == 0) { err = "a part owns no cells"; return ERR_ARG; }
+    for (int64_t c = 0; c < nc; ++c) if (owner[c] != part && (ring2[c] & me)) out.local_cells.push_back(c);
+    const int64_t nl = (int64_t)out.local_cells.size();
+    std::vector<int32_t> cell_local(nc, -1);
+    for (int64_t k = 0; k < nl; ++k) cell_local[out.local_cells[k]] = (int32_t)k;
+    // local nodes
+    std::vector<int32_t> node_local(nn, -1);
+    for (int64_t k = 0; k < nl; ++k)
+        for (int j = 0; j < 4; ++j) node_local[tets[4 * out.local_cells[k] + j]] = 0;
+    for (int64_t n = 0; n < nn; ++n)
+        if (node_local[n] == 0) { node_local[n] = (int32_t)out.local_nodes.size(); out.local_nodes.push_back(n); }
+    out.local_tets.resize(4 * nl);
+    for (int64_t k = 0; k < nl; ++k)
+        for (int j = 0; j < 4; ++j) out.local_tets[4 * k + j] = node_local[tets[4 * out.local_cells[k] + j]];
+    // exchange lists: what I receive from q = my halo cells owned by q; what I send to q = my owned cells in q's halo
+    out.send_ptr.assign(n_parts + 1, 0); out.recv_ptr.assign(n_parts + 1, 0);
+    for (int q = 0; q < n_parts; ++q) {
+        if (q != part) {
+            for (int64_t k = out.n_owned; k < nl; ++k)
+                if (owner[out.local_cells[k]] == q) out.recv_cells.push_back(k);
+            const uint64_t qb = 1ULL << q;
+            for (int64_t k = 0; k < out.n_owned; ++k)
+                if (ring2[out.local_cells[k]] & qb) out.send_cells.push_back(k);
+        }
+        out.send_ptr[q + 1] = (int64_t)out.send_cells.size();
+        out.recv_ptr[q + 1] = (int64_t)out.recv_cells.size();
     }
     return 0;
 }

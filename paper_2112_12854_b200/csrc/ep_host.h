@@ -61,6 +61,26 @@ int build_stencil(int64_t nn, const double* xyz, int64_t nc, const int32_t* tets
 int build_stencil_tri(int64_t nn, const double* xyz, int64_t nc, const int32_t* tris, const double* fibre,
                       const double* scale, double sigma_l, double sigma_t, double chi, double Cm, Stencil& out,
                       std::string& err);
-int pack(const Stencil& st, const double* xyz, Packed& out, std::string& err);
+// n_owned < nc: the first n_owned cells (caller numbering) are put first on the device (Morton order among themselves, then
+// the rest in Morton order) and only they carry volume weights -- the layout of a shard (owned cells, then halo cells).
+int pack(const Stencil& st, const double* xyz, Packed& out, std::string& err, int64_t n_owned = -1);
+
+// Intra-mesh sharding: the cells are cut into n_parts contiguous ranges of the Morton curve through their
+// centroids; part p owns one range and keeps, as halo, every other cell within two node-rings of an owned cell (the reach of
+// the stencil: the nodes of a cell and of its face neighbours, and the stars of those nodes).  Per step each
+// part needs the new Vm of its halo cells from their owners: one neighbour exchange, no global reduction.
+struct ShardPlan {
+    int part = 0, n_parts = 1;
+    int64_t n_owned = 0;
+    std::vector<int64_t> local_cells;   // global cell id of local cell k: owned first (ascending global id), then halo (ascending)
+    std::vector<int64_t> local_nodes;   // global node id of local node k (ascending)
+    std::vector<int32_t> local_tets;    // [n_local*4], local node ids
+    std::vector<int64_t> send_ptr, recv_ptr;     // [n_parts+1]: segment of peer q in send_cells / recv_cells
+    std::vector<int64_t> send_cells, recv_cells; // LOCAL cell ids; within a segment ascending global id, so that the segment
+                                                 // part p sends to q lists the same cells, in the same order, as q's
+                                                 // receive segment from p
+};
+int shard_plan(int64_t nn, const double* xyz, int64_t nc, const int32_t* tets, int part, int n_parts, ShardPlan& out,
+               std::string& err);
 
 }  // namespace ep

@@ -243,6 +243,11 @@ __global__ void gather_f64_kernel(int64_t n, const double* __restrict__ src, con
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) dst[i] = src[idx[i]];
 }
+__global__ void scatter_f64_kernel(int64_t n, const double* __restrict__ src, const int32_t* __restrict__ idx,
+                                   double* __restrict__ dst) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[idx[i]] = src[i];
+}
 // state row k (tile-major, S rows) <-> a linear array in another numbering: dst[c] = y[(idx[c], k)] / y[(i, k)] = src[idx[i]]
 __global__ void state_row_get_kernel(int64_t n, const double* __restrict__ y, int S, int k,
                                      const int32_t* __restrict__ idx, double* __restrict__ dst) {
@@ -378,11 +383,12 @@ void launch_node_gather(const DeviceMesh& m, const double* vm, double* vn, cudaS
 }
 
 void launch_cell_step(const DeviceMesh& m, int model, const StepArgs& a, cudaStream_t s, bool pdl) {
-    const unsigned grid = blocks_for(m.nc, CELL_THREADS);
-    if (model == 0 && a.hist) launch_pdl(cell_step_kernel<0, 2>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
-    else if (model == 0) launch_pdl(cell_step_kernel<0>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
-    else if (model == 1) launch_pdl(cell_step_kernel<1>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
-    else launch_pdl(cell_step_kernel<2>, grid, CELL_THREADS, s, pdl, m.nc, m.cidx, m.ccoef, a);
+    const int64_t nact = m.nc_active > 0 ? m.nc_active : m.nc;
+    const unsigned grid = blocks_for(nact, CELL_THREADS);
+    if (model == 0 && a.hist) launch_pdl(cell_step_kernel<0, 2>, grid, CELL_THREADS, s, pdl, nact, m.cidx, m.ccoef, a);
+    else if (model == 0) launch_pdl(cell_step_kernel<0>, grid, CELL_THREADS, s, pdl, nact, m.cidx, m.ccoef, a);
+    else if (model == 1) launch_pdl(cell_step_kernel<1>, grid, CELL_THREADS, s, pdl, nact, m.cidx, m.ccoef, a);
+    else launch_pdl(cell_step_kernel<2>, grid, CELL_THREADS, s, pdl, nact, m.cidx, m.ccoef, a);
 }
 
 void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* vn, double* out, cudaStream_t s,
@@ -397,6 +403,9 @@ void launch_state_fill(int model, int64_t nc, int64_t nc_pad, const uint8_t* cty
                                                               tact);
 }
 
+void launch_scatter_f64(int64_t n, const double* src, const int32_t* idx, double* dst, cudaStream_t s) {
+    if (n > 0) scatter_f64_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, src, idx, dst);
+}
 void launch_gather_f64(int64_t n, const double* src, const int32_t* idx, double* dst, cudaStream_t s) {
     gather_f64_kernel<<<blocks_for(n, 256), 256, 0, s>>>(n, src, idx, dst);
 }

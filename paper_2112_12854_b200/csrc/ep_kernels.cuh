@@ -8,6 +8,7 @@ namespace epk {
 
 struct DeviceMesh {
     int64_t nc = 0, nn = 0, nc_pad = 0, n_slices = 0;
+    int64_t nc_active = 0;              // cells the step kernel advances: nc, or the owned cells of a shard (they come first)
     const int32_t* cidx = nullptr;      // tile-major [nc_pad/128][12][128]
     const double* ccoef = nullptr;      // tile-major [nc_pad/128][12][128]
     const int64_t* slice_ptr = nullptr; // [n_slices+1]
@@ -64,6 +65,8 @@ void launch_diffusion_only(const DeviceMesh& m, const double* vm, const double* 
 // fill y rows with one state vector per cell type; y0 is a DEVICE pointer [n_types*S]; NULL = built-in rest state
 void launch_state_fill(int model, int64_t nc, int64_t nc_pad, const uint8_t* ctype, const double* y0_dev, double* y,
                        double* vm, double* tact, cudaStream_t s);
+// dst[idx[i]] = src[i] (halo unpack)
+void launch_scatter_f64(int64_t n, const double* src, const int32_t* idx, double* dst, cudaStream_t s);
 // permutation helpers: dst[i] = src[idx[i]]
 void launch_gather_f64(int64_t n, const double* src, const int32_t* idx, double* dst, cudaStream_t s);
 // state row k of the tile-major state array: dst[c] = y(inv[c], k)   /   y(i, k) = src[perm[i]]
