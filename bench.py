@@ -93,9 +93,13 @@ def _run_dt(prob) -> float:
 
 def _oracle_leg(prob, budget_s: float, threads: int):
     """Time the oracle, as it stands, on this host: whole mesh, as many steps as fit the budget (at least 1)."""
-    from oracle import ep_oracle as O
-    O.set_threads(threads)
-    o = O.OracleSim.from_problem(prob)
+    if hasattr(prob.mesh, "tris"):          # 2D medium: the triangle / Stewart oracle (OpenMP, all cores)
+        from oracle import ep_oracle2d as O2
+        o = O2.OracleSim2D.from_problem(prob)
+    else:
+        from oracle import ep_oracle as O
+        O.set_threads(threads)
+        o = O.OracleSim.from_problem(prob)
     t0 = time.perf_counter()
     o.step(1, _run_dt(prob))
     t1 = time.perf_counter() - t0
@@ -188,6 +192,8 @@ def run_ours(args):
     sim = ep.Sim.from_problem(prob)
     stream = torch.cuda.Stream()
     sim.set_stream(stream.cuda_stream)
+    if args.order == 2:
+        sim.set_time_order(2)     # PAPER.md:232 variant (TP06 only); not the headline configuration
     S = sim.n_states
     # explicit stability (reading S): config 2 runs at dt = nominal/4; ep_stable_dt confirms the choice
     dt_max = sim.stable_dt()
@@ -312,6 +318,7 @@ def run_ours(args):
                    "dt_divisor": dt_k, "dt_stable_max_ms": dt_max,
                    "time_steps_per_step": inner, "states": "config initial condition (rest + stimulus at t=0), window starts after warm-up",
                    "l2": "inputs larger than L2 (%.0f MB touched per time step)" % (sim.step_bytes / 1e6),
+                   "time_order": args.order,
                    "parallelism": "replicas" if world > 1 else "single"},
         "simulated_ms_per_wall_s": dt * inner * args.steps / (ms_max * 1e-3),
         "us_per_time_step": 1e3 * ms_max / (inner * args.steps),
@@ -334,10 +341,12 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference", "disttest"])
-    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5; 6/7/8 = the paper's Table-1 slab at dx 0.5/0.2/0.1 mm")
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5; 6/7/8 = the paper's Table-1 slab at dx 0.5/0.2/0.1 mm; 9/10 = Purkinje strip / sheet (2D, Stewart)")
     ap.add_argument("--inner", type=int, default=100, help="explicit time steps per bench step")
     ap.add_argument("--ref-inner", type=int, default=1, help="oracle time steps per bench step (--impl reference)")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--order", type=int, default=1, choices=[1, 2],
+                    help="time-stepping order: 1 = the paper's Rush-Larsen + forward Euler (headline), 2 = AB2 + second-order Rush-Larsen")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")
     args = ap.parse_args()

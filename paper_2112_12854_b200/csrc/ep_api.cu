@@ -76,7 +76,8 @@ struct ep_sim {
     int dim = 3;                                // 3: tetrahedra, 2: triangulated surface
     // bidomain (ep_mesh_create_bidomain): the mesh's own tables hold M_int; second coefficient table for M_int + M_ext
     bool bidomain = false;
-    double *d_ccoef_ie = nullptr, *d_vext = nullptr, *d_src = nullptr, *d_b = nullptr;
+    double *d_ccoef_ie = nullptr, *d_vext = nullptr, *d_src = nullptr, *d_b = nullptr, *d_vext_prev = nullptr;
+    int vext_hist = 0;                          // consecutive solutions held in d_vext / d_vext_prev (0, 1, 2)
     epk::Gmres gm;
     int bd_restart = 30, bd_max_cycles = 200, bd_check = 5;
     double bd_tol = 1e-10;
@@ -143,7 +144,7 @@ void free_all(ep_sim* s) {
     void* ptrs[] = {s->d_cidx, s->d_nidx, s->d_perm, s->d_inv, s->d_ccoef, s->d_nw, s->d_slice_ptr, s->d_vm[0],
                     s->d_vm[1], s->d_y, s->d_vn, s->d_tact, s->d_tmp, s->d_tmp2, s->d_red, s->d_ctype, s->d_smask,
                     s->d_vol, s->d_tmask, s->d_trig_fire, s->d_trig_par, s->d_ccoef_ie, s->d_vext, s->d_src, s->d_b, s->d_hist, s->d_send_idx, s->d_recv_idx,
-                    s->d_send, s->d_recv};
+                    s->d_send, s->d_recv, s->d_vext_prev};
     epk::gmres_free(s->gm);
     for (void* p : ptrs) if (p) cudaFree(p);
     for (cudaEvent_t e : s->ev) cudaEventDestroy(e);
@@ -294,6 +295,10 @@ int bidomain_solve(ep_sim* s) {
         epk::launch_node_gather(s->dm, x, s->d_vn, st);
         epk::launch_diffusion_only(s->dm, x, s->d_vn, out, st, s->d_ccoef_ie, s->d_vol, 1.0);      // V A_ie x
     };
+    // first estimate: the paper uses v_ext^n; with two previous solutions at hand their linear extrapolation
+    // 2 v_ext^n - v_ext^{n-1} starts one order in dt closer (the gauge is preserved: both have zero weighted mean)
+    epk::launch_extrapolate(s->nc, s->d_vext, s->d_vext_prev, s->vext_hist >= 2 ? 1 : 0, s->stream);
+    s->launches++;
     double rel = 0.0;
     // reading E3: besides the relative criterion the solve stops at a residual density of rel_tol * 0.1 mV/ms (1e-11 mV/ms at
     // the default), the level at which the coupling term is exact for the purposes of the Vm update; a right-hand side that
@@ -317,6 +322,7 @@ int bidomain_solve(ep_sim* s) {
     epk::launch_diffusion_only(s->dm, s->d_vext, s->d_vn, s->d_src, s->stream);                  // A_i v_ext/(chi Cm), mV/ms
     s->launches += 5;
     s->vext_valid = true;
+    if (s->vext_hist < 2) s->vext_hist++;
     return EP_OK;
 }
 
@@ -432,7 +438,8 @@ static int mesh_create_impl(ep_sim** out, int dim, int64_t n_nodes, const double
             if (rc) return bail(fail(rc, err));
             if (pk2.cidx != pk.cidx) return bail(fail(EP_ERR_MESH, "internal: index tables of the two operators differ"));
             if ((rc = upload(s, &s->d_ccoef_ie, pk2.ccoef)) || (rc = dev_alloc(s, &s->d_vext, s->nc_pad)) ||
-                (rc = dev_alloc(s, &s->d_src, s->nc_pad)) || (rc = dev_alloc(s, &s->d_b, s->nc_pad)))
+                (rc = dev_alloc(s, &s->d_src, s->nc_pad)) || (rc = dev_alloc(s, &s->d_b, s->nc_pad)) ||
+                (rc = dev_alloc(s, &s->d_vext_prev, s->nc_pad)))
                 return bail(rc);
             cudaMemset(s->d_vext, 0, sizeof(double) * s->nc_pad);
             cudaMemset(s->d_src, 0, sizeof(double) * s->nc_pad);
@@ -684,6 +691,7 @@ int ep_state_init(ep_sim* s, int model, const uint8_t* cell_type, const double* 
     if (s->order == 2 && model != EP_MODEL_TP06) s->order = 1;   // the second-order scheme exists for TP06 only
     if (s->bidomain) {
         s->vext_valid = false;
+        s->vext_hist = 0;
         EP_CUDA(s, cudaMemsetAsync(s->d_vext, 0, sizeof(double) * s->nc_pad, s->stream));
         EP_CUDA(s, cudaMemsetAsync(s->d_src, 0, sizeof(double) * s->nc_pad, s->stream));
     }
@@ -852,7 +860,7 @@ int ep_write_state(ep_sim* s, int var, const double* in) {
     if (var == 0) epk::launch_gather_f64(s->nc, s->d_tmp, s->d_perm, s->d_vm[s->cur], s->stream);
     else epk::launch_state_row_put(s->nc, s->d_tmp, s->d_perm, s->S, var, s->d_y, s->stream);
     s->launches++;
-    if (var == 0) s->vext_valid = false;
+    if (var == 0) { s->vext_valid = false; s->vext_hist = 0; }
     s->o2_have = false;      // a rewritten state has no history
     EP_CUDA(s, cudaStreamSynchronize(s->stream));
     return EP_OK;
@@ -933,6 +941,7 @@ int ep_write_states(ep_sim* s, const double* in) {
         EP_CUDA(s, cudaEventRecord(s->io_consumed[b], s->stream));
     }
     s->vext_valid = false;
+    s->vext_hist = 0;
     s->o2_have = false;
     EP_CUDA(s, cudaStreamSynchronize(s->stream));
     return EP_OK;
@@ -1249,7 +1258,8 @@ int64_t ep_kernel_bytes(const ep_sim* s, int kernel) {
     if (!s) return 0;
     const int64_t S = s->S > 0 ? s->S : 19;
     if (kernel == 0) return s->star_entries * 12 + s->nn * 8;                 // node table + v_n written
-    if (kernel == 1) return s->nc * (2 * 8 * S + 12 * 12 + 2) + s->nn * 8;    // states r+w, cell tables, masks, v_n read
+    const int64_t hist = (s->order == 2) ? 2 * 8 * epk::O2_ROWS : 0;           // second order: 8 history rows read + written
+    if (kernel == 1) return s->n_owned * (2 * 8 * S + 12 * 12 + 2 + hist) + s->nn * 8;   // states r+w, cell tables, masks, v_n read
     return 0;
 }
 
@@ -1258,7 +1268,8 @@ int64_t ep_step_bytes(const ep_sim* s) {
     const int64_t S = s->S > 0 ? s->S : 19;
     // state read + write, cell tables (12 f64 + 12 i32), node table (f64 + i32 per star entry),
     // node values written once and read once, cell type + stimulus mask.  Gathers are assumed cache hits.
-    return s->nc * (2 * 8 * S + 12 * 12 + 2) + s->star_entries * 12 + s->nn * 16;
+    const int64_t hist = (s->order == 2) ? 2 * 8 * epk::O2_ROWS : 0;
+    return s->n_owned * (2 * 8 * S + 12 * 12 + 2 + hist) + s->star_entries * 12 + s->nn * 16;
 }
 
 }  // extern "C"

@@ -144,6 +144,15 @@ __global__ void __launch_bounds__(256) shift_kernel(int64_t n, double* __restric
     if (i < n) x[i] -= wsum[0] * inv_total;
 }
 
+// first estimate by linear extrapolation in time: x <- 2 x - x_prev, x_prev <- x (the old one)
+__global__ void __launch_bounds__(256) extrapolate_kernel(int64_t n, double* __restrict__ x, double* __restrict__ xprev, int have) {
+    const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (i >= n) return;
+    const double xo = x[i];
+    if (have) x[i] = fma(2.0, xo, -xprev[i]);
+    xprev[i] = xo;
+}
+
 inline unsigned blocks256(int64_t n) { return (unsigned)((n + 255) / 256); }
 
 }  // namespace
@@ -249,6 +258,10 @@ void launch_remove_mean(const Gmres& G, double* x, cudaStream_t s) {
     multi_dot_partial_kernel<<<dim3(NB, 1), 256, 0, s>>>(G.n, x, nullptr, G.stride, -1, G.partial);
     multi_dot_final_kernel<<<1, 256, 0, s>>>(G.partial, G.scal + 2, 0);
     shift_kernel<<<blocks256(G.n), 256, 0, s>>>(G.n, x, G.scal + 2, 1.0 / (double)G.n);
+}
+
+void launch_extrapolate(int64_t n, double* x, double* xprev, int have, cudaStream_t s) {
+    extrapolate_kernel<<<blocks256(n), 256, 0, s>>>(n, x, xprev, have);
 }
 
 void launch_remove_weighted_mean(const Gmres& G, double* x, const double* weight, double total, cudaStream_t s) {

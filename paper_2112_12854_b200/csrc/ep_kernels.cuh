@@ -108,6 +108,8 @@ void gmres_free(Gmres& G);
 // Also stops when the residual estimate <= abs_tol (a right-hand side that is round-off noise has no meaningful relative scale).
 int gmres_solve(Gmres& G, const GmresOp& apply, const double* b, double* x, double rel_tol, double abs_tol, int max_cycles,
                 int check_every, cudaStream_t s, double* rel_res_out, int64_t* launches);
+// x <- 2 x - xprev (if have), xprev <- old x: linear extrapolation of the first estimate from the two previous solutions
+void launch_extrapolate(int64_t n, double* x, double* xprev, int have, cudaStream_t s);
 // x -= (sum_i x[i]) / n
 void launch_remove_mean(const Gmres& G, double* x, cudaStream_t s);
 // x -= (sum_i weight[i] x[i]) / total
