@@ -76,7 +76,7 @@ def test_elliptic_equation_compatibility_and_gauge():
 def test_table2_bidomain_is_not_a_relabelled_monodomain():
     """Unequal anisotropy ratios (sigma_i 1.7/0.19, sigma_e 6.2/2.4 mS/cm): no single lambda exists; the bidomain front runs
     close to -- but not on -- the monodomain front with the harmonic-mean conductivities 1.334 / 0.176 mS/cm."""
-    m = _slab(nx=24, ny=6, nz=2, h=0.25)
+    m = _slab(nx=20, ny=5, nz=2, h=0.25)
     cen = m.centroids()
     ids = np.nonzero(cen[:, 0] < 0.5)[0].astype(np.int64)
     si, se = (1.7, 0.19), (6.2, 2.4)
@@ -87,12 +87,12 @@ def test_table2_bidomain_is_not_a_relabelled_monodomain():
     mono = O.OracleSim(m.xyz, m.tets, m.fibre, None, hm[0], hm[1])
     mono.state_init(0, m.cell_type)
     mono.stimulus_set(0, ids, -52.0, 0.0, 1.0)
-    bd.step(750, 0.02); mono.step(750, 0.02)
+    bd.step(650, 0.02); mono.step(650, 0.02)
     ta_b, ta_m = bd.activation_times(), mono.activation_times()
-    far = cen[:, 0] > 4.0
+    far = cen[:, 0] > 3.5
     assert (ta_b[far] >= 0).all() and (ta_m[far] >= 0).all()
     band = lambda x0: np.abs(cen[:, 0] - x0) < 0.25
-    cv_b = 3.0 / (ta_b[band(4.5)].mean() - ta_b[band(1.5)].mean())
-    cv_m = 3.0 / (ta_m[band(4.5)].mean() - ta_m[band(1.5)].mean())
+    cv_b = 2.5 / (ta_b[band(4.0)].mean() - ta_b[band(1.5)].mean())
+    cv_m = 2.5 / (ta_m[band(4.0)].mean() - ta_m[band(1.5)].mean())
     assert cv_b == pytest.approx(cv_m, rel=0.05) and 0.3 < cv_b < 0.8       # m/s, plane wave along the fibres
     assert np.abs(bd.read_vm() - mono.read_vm()).max() > 1e-3               # but it is a different solution
