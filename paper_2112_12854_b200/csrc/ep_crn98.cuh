@@ -66,38 +66,6 @@ __device__ __forceinline__ double phi(double x, double ex) {
 }
 }  // namespace crn
 
-// y_g <- inf_g + (y_g - inf_g) exp(arg_g) for the ten gates of the rolled loop, written to their state rows.
-template <int BLOCK>
-__device__ __forceinline__ void crn_rush_larsen_slots(double* col, double* ycol, int64_t stride) {
-    using namespace crn;
-    // software-pipelined like ep_exp2_slots (ep_math.cuh): next trip's exponents and this trip's steady states / old gate
-    // values are read before the polynomials run.  Slots B_INF0 + 10, 11 and G_OLD0 + 10, 11 are read but not used.
-    double e[EXP_W];
-#pragma unroll
-    for (int j = 0; j < EXP_W; ++j) e[j] = col[j * BLOCK];
-#pragma unroll 1
-    for (int g = 0; g < N_EXPB; g += EXP_W) {
-        const int gn = (g + EXP_W < N_EXPB) ? g + EXP_W : g;
-        double ne[EXP_W], yi[EXP_W], yo[EXP_W];
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) {
-            ne[j] = col[(gn + j) * BLOCK];
-            yi[j] = col[(B_INF0 + g + j) * BLOCK];
-            yo[j] = col[(G_OLD0 + g + j) * BLOCK];
-        }
-        ep_exp2_wide<EXP_W>(e);
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) {
-            if (g + j < N_RLB) {
-                const int row = (g + j < 8) ? C_OA + g + j : C_VG + (g + j - 8);
-                ycol[row * stride] = fma(yo[j] - yi[j], e[j], yi[j]);
-            }
-        }
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) e[j] = ne[j];
-    }
-}
-
 // One step of one cell (same contract as tp06_step).  Returns Vm^{n+1}.
 template <int BLOCK, class Stim, class Issue, class Finish>
 __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t stride, double dt, Stim stimulus,
@@ -126,54 +94,74 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
     const bool hi = (v >= -40.0);   // reading B7
 
     // ---- batch 2: voltage-dependent exponentials (+ the two constant Rush-Larsen factors of fCa and u)
+    // (arguments in registers, only the results go to the slot array: see tp06_step)
+#ifdef EP_CRN_BATCH1_DIRECT
+    double a1[N_EXPA];
+#define ARG(k) a1[k]
+#else
+#define ARG(k) col[(k) * BLOCK]
+#endif
     const double x1 = fma(vg, -0.1, CK(-0.1 * 47.13));
     const double xb = fma(vg, CK(1.0 / 5.1237), CK(-3.3328 / 5.1237));
     const double xd = fma(vg, CK(1.0 / 9.0), CK(-19.9 / 9.0));
     const double dx = fma(vg, CK(-1.0 / 6.24), CK(-10.0 / 6.24));
-    col[A_E17 * BLOCK] = vg * CK(L2E / 17.0);
-    col[A_W * BLOCK] = vg * CK(0.05 * FRT * L2E);
-    col[A_X1 * BLOCK] = x1 * CK(L2E);
-    col[A_BM * BLOCK] = vg * CK(-L2E / 11.0);
-    col[A_K1 * BLOCK] = fma(vg, CK(0.07 * L2E), CK(0.07 * 80.0 * L2E));
-    col[A_OA1 * BLOCK] = fma(vg, CK(-L2E / 8.5), CK(-10.0 * L2E / 8.5));
-    col[A_OA2 * BLOCK] = fma(vg, CK(-L2E / 59.0), CK(30.0 * L2E / 59.0));
-    col[A_OAI * BLOCK] = fma(vg, CK(-L2E / 17.54), CK(-20.47 * L2E / 17.54));
-    col[A_UAI * BLOCK] = fma(vg, CK(-L2E / 9.6), CK(-30.3 * L2E / 9.6));
-    col[A_OI1 * BLOCK] = fma(vg, CK(L2E / 10.95), CK(113.7 * L2E / 10.95));
-    col[A_OI2 * BLOCK] = fma(vg, CK(-L2E / 7.44), CK(-1.26 * L2E / 7.44));
-    col[A_OII * BLOCK] = fma(vg, CK(L2E / 5.3), CK(43.1 * L2E / 5.3));
-    col[A_UI1 * BLOCK] = fma(vg, CK(-L2E / 28.0), CK(185.0 * L2E / 28.0));
-    col[A_UI2 * BLOCK] = fma(vg, CK(L2E / 16.0), CK(-158.0 * L2E / 16.0));
-    col[A_UII * BLOCK] = fma(vg, CK(L2E / 27.48), CK(-99.45 * L2E / 27.48));
-    col[A_KUR * BLOCK] = fma(vg, CK(-L2E / 13.0), CK(15.0 * L2E / 13.0));
-    col[A_KR * BLOCK] = fma(vg, CK(L2E / 22.4), CK(15.0 * L2E / 22.4));
-    col[A_E5M * BLOCK] = vg * CK(-0.2 * L2E);
-    col[A_XB * BLOCK] = xb * CK(L2E);
-    col[A_XRI * BLOCK] = fma(vg, CK(-L2E / 6.5), CK(-14.1 * L2E / 6.5));
-    col[A_XD * BLOCK] = xd * CK(L2E);
-    col[A_XSI * BLOCK] = fma(vg, CK(-L2E / 12.7), CK(19.9 * L2E / 12.7));
-    col[A_DX * BLOCK] = dx * CK(L2E);
-    col[A_DI * BLOCK] = fma(vg, CK(-0.125 * L2E), CK(-1.25 * L2E));
-    col[A_FG * BLOCK] = (vg + 10.0) * (vg + 10.0) * CK(-0.0337 * 0.0337 * L2E);
-    col[A_FI * BLOCK] = fma(vg, CK(L2E / 6.9), CK(28.0 * L2E / 6.9));
+    ARG(A_E17) = vg * CK(L2E / 17.0);
+    ARG(A_W) = vg * CK(0.05 * FRT * L2E);
+    ARG(A_X1) = x1 * CK(L2E);
+    ARG(A_BM) = vg * CK(-L2E / 11.0);
+    ARG(A_K1) = fma(vg, CK(0.07 * L2E), CK(0.07 * 80.0 * L2E));
+    ARG(A_OA1) = fma(vg, CK(-L2E / 8.5), CK(-10.0 * L2E / 8.5));
+    ARG(A_OA2) = fma(vg, CK(-L2E / 59.0), CK(30.0 * L2E / 59.0));
+    ARG(A_OAI) = fma(vg, CK(-L2E / 17.54), CK(-20.47 * L2E / 17.54));
+    ARG(A_UAI) = fma(vg, CK(-L2E / 9.6), CK(-30.3 * L2E / 9.6));
+    ARG(A_OI1) = fma(vg, CK(L2E / 10.95), CK(113.7 * L2E / 10.95));
+    ARG(A_OI2) = fma(vg, CK(-L2E / 7.44), CK(-1.26 * L2E / 7.44));
+    ARG(A_OII) = fma(vg, CK(L2E / 5.3), CK(43.1 * L2E / 5.3));
+    ARG(A_UI1) = fma(vg, CK(-L2E / 28.0), CK(185.0 * L2E / 28.0));
+    ARG(A_UI2) = fma(vg, CK(L2E / 16.0), CK(-158.0 * L2E / 16.0));
+    ARG(A_UII) = fma(vg, CK(L2E / 27.48), CK(-99.45 * L2E / 27.48));
+    ARG(A_KUR) = fma(vg, CK(-L2E / 13.0), CK(15.0 * L2E / 13.0));
+    ARG(A_KR) = fma(vg, CK(L2E / 22.4), CK(15.0 * L2E / 22.4));
+    ARG(A_E5M) = vg * CK(-0.2 * L2E);
+    ARG(A_XB) = xb * CK(L2E);
+    ARG(A_XRI) = fma(vg, CK(-L2E / 6.5), CK(-14.1 * L2E / 6.5));
+    ARG(A_XD) = xd * CK(L2E);
+    ARG(A_XSI) = fma(vg, CK(-L2E / 12.7), CK(19.9 * L2E / 12.7));
+    ARG(A_DX) = dx * CK(L2E);
+    ARG(A_DI) = fma(vg, CK(-0.125 * L2E), CK(-1.25 * L2E));
+    ARG(A_FG) = (vg + 10.0) * (vg + 10.0) * CK(-0.0337 * 0.0337 * L2E);
+    ARG(A_FI) = fma(vg, CK(L2E / 6.9), CK(28.0 * L2E / 6.9));
     if (hi) {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
-        col[(A_HJ0 + 1) * BLOCK] = vg * CK(-2.535e-7 * L2E);
+        ARG((A_HJ0 + 0)) = fma(vg, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
+        ARG((A_HJ0 + 1)) = vg * CK(-2.535e-7 * L2E);
 #pragma unroll
-        for (int k = 2; k < 8; ++k) col[(A_HJ0 + k) * BLOCK] = 0.0;
+        for (int k = 2; k < 8; ++k) ARG((A_HJ0 + k)) = 0.0;
     } else {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));
-        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.079 * L2E);
-        col[(A_HJ0 + 2) * BLOCK] = vg * CK(0.35 * L2E);
-        col[(A_HJ0 + 3) * BLOCK] = vg * CK(0.2444 * L2E);
-        col[(A_HJ0 + 4) * BLOCK] = vg * CK(-0.04391 * L2E);
-        col[(A_HJ0 + 5) * BLOCK] = fma(vg, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
-        col[(A_HJ0 + 6) * BLOCK] = vg * CK(-0.01052 * L2E);
-        col[(A_HJ0 + 7) * BLOCK] = fma(vg, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
+        ARG((A_HJ0 + 0)) = fma(vg, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));
+        ARG((A_HJ0 + 1)) = vg * CK(0.079 * L2E);
+        ARG((A_HJ0 + 2)) = vg * CK(0.35 * L2E);
+        ARG((A_HJ0 + 3)) = vg * CK(0.2444 * L2E);
+        ARG((A_HJ0 + 4)) = vg * CK(-0.04391 * L2E);
+        ARG((A_HJ0 + 5)) = fma(vg, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
+        ARG((A_HJ0 + 6)) = vg * CK(-0.01052 * L2E);
+        ARG((A_HJ0 + 7)) = fma(vg, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
     }
-    col[A_TFCA * BLOCK] = dtl * -0.5;     // tau_fCa = 2 ms
-    col[A_TU * BLOCK] = dtl * -0.125;     // tau_u = 8 ms
+    ARG(A_TFCA) = dtl * -0.5;     // tau_fCa = 2 ms
+    ARG(A_TU) = dtl * -0.125;     // tau_u = 8 ms
+#ifdef EP_CRN_BATCH1_DIRECT
+#pragma unroll
+    for (int s0 = 0; s0 < N_EXPA; s0 += EXP_W) {
+        double x[EXP_W];
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) x[j] = a1[s0 + j];
+        ep_exp2_wide<EXP_W>(x);
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) col[(s0 + j) * BLOCK] = x[j];
+    }
+#else
     ep_exp2_slots<N_EXPA, BLOCK, EXP_W>(col);
+#endif
+#undef ARG
     const double dv_diff = finish_gather();   // the gathers have landed during the batch: 12 values -> 1
     const double istim = stimulus();          // late on purpose: see tp06_step
     ep_cp_async_wait();                       // so have the gate values: products for the currents
@@ -333,14 +321,27 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
         inf[9] = CK(E40_17) * ep_rcp(e17 + CK(E40_17));
         rate[9] = CK(1.0 / 1.2) * phi(xw, ex) * fma(CK(0.3), ex, 1.0);
     }
+    // Rush-Larsen of the ten gates of this list: exponents and steady states in registers (three unrolled groups), only the
+    // parked gate values come from shared memory (see tp06_step)
 #pragma unroll
-    for (int g = 0; g < N_RLB; ++g) {
-        col[g * BLOCK] = fmax(-dtl * rate[g], -1000.0);
-        col[(B_INF0 + g) * BLOCK] = inf[g];
+    for (int g0 = 0; g0 < N_EXPB; g0 += EXP_W) {
+        double e[EXP_W], yo[EXP_W];
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) {
+            const int g = g0 + j;
+            e[j] = (g < N_RLB) ? fmax(-dtl * rate[g], -1000.0) : 0.0;
+            yo[j] = col[(G_OLD0 + g) * BLOCK];        // slots G_OLD0 + 10, 11 are pads: read, not used
+        }
+        ep_exp2_wide<EXP_W>(e);
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) {
+            const int g = g0 + j;
+            if (g < N_RLB) {
+                const int row = (g < 8) ? C_OA + g : C_VG + (g - 8);
+                ycol[row * stride] = fma(yo[j] - inf[g], e[j], inf[g]);
+            }
+        }
     }
-    col[10 * BLOCK] = 0.0;
-    col[11 * BLOCK] = 0.0;
-    crn_rush_larsen_slots<BLOCK>(col, ycol, stride);
     return v_new;
 }
 

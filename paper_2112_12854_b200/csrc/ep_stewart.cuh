@@ -53,43 +53,13 @@ constexpr int A_B600 = 0, A_E14 = 1, A_M = 2, A_H = 3, A_XR1 = 4, A_D = 5, A_PK 
 constexpr int N_EXPA_HI = 20;
 constexpr int EXP_W = 4;
 constexpr int N_RLB = 12;    // Rush-Larsen gates whose rate depends on batch 2: y xr1 xr2 xs m h j d f f2 (rows 1..10), s r (12, 13)
-constexpr int N_EXPB = 12;
-constexpr int B_INF0 = 12;   // steady states, slots 12..23
+constexpr int N_EXPB = 12;   // their Rush-Larsen exponentials, evaluated in registers
 constexpr int G_OLD0 = 24;   // the 12 gate values at t^n, slots 24..35
 constexpr int N_SLOTS = 36;
-static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && N_EXPA <= G_OLD0 && B_INF0 + N_RLB <= G_OLD0 &&
-              G_OLD0 + N_RLB <= N_SLOTS, "slot layout");
+static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && N_RLB == N_EXPB && N_EXPA <= G_OLD0 && G_OLD0 + N_RLB <= N_SLOTS,
+              "slot layout");
 __device__ __forceinline__ constexpr int rl_row(int g) { return g < 10 ? 1 + g : 2 + g; }   // skips fCass (row 11)
 }  // namespace stw
-
-template <int BLOCK>
-__device__ __forceinline__ void stw_rush_larsen_slots(double* col, double* ycol, int64_t stride) {
-    using namespace stw;
-    double e[EXP_W];
-#pragma unroll
-    for (int j = 0; j < EXP_W; ++j) e[j] = col[j * BLOCK];
-#pragma unroll 1
-    for (int g = 0; g < N_EXPB; g += EXP_W) {
-        const int gn = (g + EXP_W < N_EXPB) ? g + EXP_W : g;
-        double ne[EXP_W], yi[EXP_W], yo[EXP_W];
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) {
-            ne[j] = col[(gn + j) * BLOCK];
-            yi[j] = col[(B_INF0 + g + j) * BLOCK];
-            yo[j] = col[(G_OLD0 + g + j) * BLOCK];
-        }
-        ep_exp2_wide<EXP_W>(e);
-        // rows 1..4, 5..8, then 9, 10, 12, 13
-        double* dst = ycol + (int64_t)(1 + g) * stride;
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) {
-            const int64_t off = (g == 8 && j >= 2) ? (int64_t)(j + 1) * stride : (int64_t)j * stride;
-            dst[off] = fma(yo[j] - yi[j], e[j], yi[j]);
-        }
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) e[j] = ne[j];
-    }
-}
 
 // One step of one cell (same contract as tp06_step, without cell types).  Returns Vm^{n+1}.
 template <int BLOCK, class Stim, class Issue, class Finish>
@@ -115,45 +85,62 @@ __device__ __forceinline__ double stw_step(double v, double* ycol, int64_t strid
     const double u = v - EK;
     const bool hi = (v >= -40.0);   // reading B7
 
-    // ---- batch 2: voltage-dependent exponentials that are not integer powers of another one
-    col[A_B600 * BLOCK] = vg * CK(L2E / 600.0);
-    col[A_E14 * BLOCK] = vg * CK(L2E / 14.0);
-    col[A_M * BLOCK] = fma(vg, CK(-L2E / 9.03), CK(-56.86 * L2E / 9.03));
-    col[A_H * BLOCK] = fma(vg, CK(L2E / 7.43), CK(71.55 * L2E / 7.43));
-    col[A_XR1 * BLOCK] = fma(vg, CK(L2E / 11.5), CK(30.0 * L2E / 11.5));
-    col[A_D * BLOCK] = fma(vg, CK(-L2E / 13.0), CK(-35.0 * L2E / 13.0));
-    col[A_PK * BLOCK] = fma(vg, CK(-L2E / 5.98), CK(25.0 * L2E / 5.98));
-    col[A_W * BLOCK] = vg * CK(0.05 * FRT * L2E);
-    col[A_GR * BLOCK] = (vg + 40.0) * (vg + 40.0) * CK(-L2E / 1800.0);
-    col[A_GS * BLOCK] = (vg + 25.0) * (vg + 25.0) * CK(-L2E / 320.0);
-    col[A_G27 * BLOCK] = (vg + 27.0) * (vg + 27.0) * CK(-L2E / 3600.0);
+    // ---- batch 2: voltage-dependent exponentials that are not integer powers of another one (arguments in registers, only the
+    // results go to the slot array: see tp06_step)
+    double a1[N_EXPA];
+#define ARG(k) a1[k]
+    ARG(A_B600) = vg * CK(L2E / 600.0);
+    ARG(A_E14) = vg * CK(L2E / 14.0);
+    ARG(A_M) = fma(vg, CK(-L2E / 9.03), CK(-56.86 * L2E / 9.03));
+    ARG(A_H) = fma(vg, CK(L2E / 7.43), CK(71.55 * L2E / 7.43));
+    ARG(A_XR1) = fma(vg, CK(L2E / 11.5), CK(30.0 * L2E / 11.5));
+    ARG(A_D) = fma(vg, CK(-L2E / 13.0), CK(-35.0 * L2E / 13.0));
+    ARG(A_PK) = fma(vg, CK(-L2E / 5.98), CK(25.0 * L2E / 5.98));
+    ARG(A_W) = vg * CK(0.05 * FRT * L2E);
+    ARG(A_GR) = (vg + 40.0) * (vg + 40.0) * CK(-L2E / 1800.0);
+    ARG(A_GS) = (vg + 25.0) * (vg + 25.0) * CK(-L2E / 320.0);
+    ARG(A_G27) = (vg + 27.0) * (vg + 27.0) * CK(-L2E / 3600.0);
     const double xcal = (vg - 15.0) * CK(2.0 * FRT);
-    col[A_CAL * BLOCK] = fma(vg, CK(2.0 * FRT * L2E), CK(-30.0 * FRT * L2E));
-    col[A_Y * BLOCK] = fma(vg, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));      // e^{-(v+80)/6.8}: y_inf, and alpha_h below -40 mV
-    col[A_SUS * BLOCK] = vg * CK(-L2E / 17.0);                             // e^{-v/17}: I_sus
+    ARG(A_CAL) = fma(vg, CK(2.0 * FRT * L2E), CK(-30.0 * FRT * L2E));
+    ARG(A_Y) = fma(vg, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));      // e^{-(v+80)/6.8}: y_inf, and alpha_h below -40 mV
+    ARG(A_SUS) = vg * CK(-L2E / 17.0);                             // e^{-v/17}: I_sus
     if (hi) {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vg, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
-        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.057 * L2E);
+        ARG((A_HJ0 + 0)) = fma(vg, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
+        ARG((A_HJ0 + 1)) = vg * CK(0.057 * L2E);
 #pragma unroll
-        for (int k = 0; k < 6; ++k) col[(A_HJ2 + k) * BLOCK] = 0.0;
+        for (int k = 0; k < 6; ++k) ARG((A_HJ2 + k)) = 0.0;
     } else {
-        col[(A_HJ0 + 0) * BLOCK] = 0.0;
-        col[(A_HJ0 + 1) * BLOCK] = vg * CK(0.079 * L2E);
-        col[(A_HJ2 + 0) * BLOCK] = vg * CK(0.3485 * L2E);
-        col[(A_HJ2 + 1) * BLOCK] = vg * CK(0.2444 * L2E);
-        col[(A_HJ2 + 2) * BLOCK] = vg * CK(-0.04391 * L2E);
-        col[(A_HJ2 + 3) * BLOCK] = fma(vg, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
-        col[(A_HJ2 + 4) * BLOCK] = vg * CK(-0.01052 * L2E);
-        col[(A_HJ2 + 5) * BLOCK] = fma(vg, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
+        ARG((A_HJ0 + 0)) = 0.0;
+        ARG((A_HJ0 + 1)) = vg * CK(0.079 * L2E);
+        ARG((A_HJ2 + 0)) = vg * CK(0.3485 * L2E);
+        ARG((A_HJ2 + 1)) = vg * CK(0.2444 * L2E);
+        ARG((A_HJ2 + 2)) = vg * CK(-0.04391 * L2E);
+        ARG((A_HJ2 + 3)) = fma(vg, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
+        ARG((A_HJ2 + 4)) = vg * CK(-0.01052 * L2E);
+        ARG((A_HJ2 + 5)) = fma(vg, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
     }
     // fCass: its Rush-Larsen rate needs no exponential, so exp(-dt/tau) rides in this batch
     const double c2 = CaSR * CaSR, css2 = CaSS * CaSS, ci2 = Cai * Cai;
     const double kcasr = fma(-(maxsr - minsr) * c2, ep_rcp(c2 + EC * EC), maxsr);
     const double qf = ep_rcp(fma(400.0, css2, 1.0));
     const double fCass_inf = fma(CK(0.6), qf, CK(0.4));
-    col[A_RLF * BLOCK] = -dtl * ep_rcp(fma(80.0, qf, 2.0));
-    col[(A_RLF + 1) * BLOCK] = 0.0;
-    ep_exp2_slots<N_EXPA, BLOCK, EXP_W>(col, __all_sync(__activemask(), hi) ? N_EXPA_HI : N_EXPA);
+    ARG(A_RLF) = -dtl * ep_rcp(fma(80.0, qf, 2.0));
+    ARG((A_RLF + 1)) = 0.0;
+    {
+        const int n1 = __all_sync(__activemask(), hi) ? N_EXPA_HI : N_EXPA;
+#pragma unroll
+        for (int s0 = 0; s0 < N_EXPA; s0 += EXP_W) {
+            if (s0 < n1) {
+                double x[EXP_W];
+#pragma unroll
+                for (int j = 0; j < EXP_W; ++j) x[j] = a1[s0 + j];
+                ep_exp2_wide<EXP_W>(x);
+#pragma unroll
+                for (int j = 0; j < EXP_W; ++j) col[(s0 + j) * BLOCK] = x[j];
+            }
+        }
+    }
+#undef ARG
     const double dv_diff = finish_gather();
     const double istim = stimulus();          // late on purpose: see tp06_step
     ep_cp_async_wait();
@@ -304,15 +291,25 @@ __device__ __forceinline__ double stw_step(double v, double* ycol, int64_t strid
         inf[11] = ep_rcp(fma(CK(E55_13), D13, 1.0));                       // 1/(1 + e^{(20-v)/13})
         rate[11] = ep_rcp(fma(10.45, col[A_GR * BLOCK], CK(7.3)));
     }
-    // ---- batch 3: Rush-Larsen
+    // ---- batch 3: Rush-Larsen, exponents and steady states in registers (three unrolled groups)
 #pragma unroll
-    for (int g = 0; g < N_RLB; ++g) {
-        // m, h, j, xr1 can be faster than 700/dt inside the clamp range (see the note in tp06_step), and so can y: its rate
-        // reaches 3e7 per ms at +200 mV (2 per ms at +50 mV).  2^-1000 stands for the oracle's underflow to 0.
-        col[g * BLOCK] = (g <= 1 || (g >= 4 && g <= 6)) ? fmax(-dtl * rate[g], -1000.0) : -dtl * rate[g];
-        col[(B_INF0 + g) * BLOCK] = inf[g];
+    for (int g0 = 0; g0 < N_EXPB; g0 += EXP_W) {
+        double e[EXP_W], yo[EXP_W];
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) {
+            const int g = g0 + j;
+            // m, h, j, xr1 can be faster than 700/dt inside the clamp range (see the note in tp06_step), and so can y: its rate
+            // reaches 3e7 per ms at +200 mV (2 per ms at +50 mV).  2^-1000 stands for the oracle's underflow to 0.
+            e[j] = (g <= 1 || (g >= 4 && g <= 6)) ? fmax(-dtl * rate[g], -1000.0) : -dtl * rate[g];
+            yo[j] = col[(G_OLD0 + g) * BLOCK];
+        }
+        ep_exp2_wide<EXP_W>(e);
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) {
+            const int g = g0 + j;
+            ycol[rl_row(g) * stride] = fma(yo[j] - inf[g], e[j], inf[g]);
+        }
     }
-    stw_rush_larsen_slots<BLOCK>(col, ycol, stride);
     return v_new;
 }
 

@@ -77,66 +77,19 @@ constexpr double E3 = 20.085536923187668;         // e^(3)
 constexpr double E5C = 148.4131591025766;         // e^(5)
 constexpr double EM1 = 0.36787944117144233;       // e^(-1)
 
-// shared-memory slots of the two exponential batches
+// shared-memory slots: results of the first exponential batch (0..23), parked gate values (24..35)
 constexpr int A_B600 = 0, A_E14 = 1, A_M = 2, A_H = 3, A_XR1 = 4, A_D = 5, A_PK = 6, A_W = 7, A_GR = 8, A_GS = 9, A_G27 = 10,
               A_CAL = 11, A_K1Q = 12, A_K1Q2 = 13, A_HJ0 = 14, A_RLF = 16, A_RLR = 17, A_HJ2 = 18, N_EXPA = 24;
 constexpr int N_EXPA_HI = 20;   // a warp whose cells are all above -40 mV needs no h/j slot beyond the first two
 constexpr int EXP_W = 4;     // exponentials evaluated side by side in the batch loops
 constexpr int N_RLB = 11;    // Rush-Larsen variables whose rate depends on batch 2: m h j xr1 xr2 xs r s d f f2
-constexpr int N_EXPB = 12;   // their arguments + 1 pad, slots 0..11 (fCass and Rbar ride in batch 2: rates need no exp)
-constexpr int B_INF0 = 12;   // 11 steady states, slots 12..22 (written after batch 2 has been consumed)
+constexpr int N_EXPB = 12;   // their Rush-Larsen exponentials + 1 pad, evaluated in registers (fCass and Rbar ride in the first batch)
 constexpr int G_OLD0 = 24;   // 11 gate values at t^n, parked from the first load to the Rush-Larsen update, slots 24..34
 constexpr int G_RBAR = 35;   // Rbar at t^n
 constexpr int N_SLOTS = 36;
-static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && N_EXPA <= G_OLD0 && B_INF0 + N_RLB <= G_OLD0 &&
-              G_OLD0 + N_RLB <= G_RBAR && G_RBAR < N_SLOTS, "slot layout");
+static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && N_EXPA <= G_OLD0 && G_OLD0 + N_RLB <= G_RBAR && G_RBAR < N_SLOTS,
+              "slot layout");
 }  // namespace tp06
-
-// Batch 3: y_g <- inf_g + (y_g - inf_g) exp(arg_g) for the 11 voltage-driven Rush-Larsen variables,
-// written straight to their state rows 1..11.  Rolled, EXP_W gates per trip.
-template <int BLOCK>
-__device__ __forceinline__ void tp06_rush_larsen_slots(double* col, double* ycol, int64_t stride) {
-    using namespace tp06;
-#ifdef EP_SLOTS_UNPIPELINED
-#pragma unroll 1
-    for (int g = 0; g < N_EXPB; g += EXP_W) {
-        double e[EXP_W];
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) e[j] = col[(g + j) * BLOCK];
-        ep_exp2_wide<EXP_W>(e);
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) {
-            if (g + j < N_RLB) {
-                const double yi = col[(B_INF0 + g + j) * BLOCK], yo = col[(G_OLD0 + g + j) * BLOCK];
-                ycol[(1 + g + j) * stride] = fma(yo - yi, e[j], yi);
-            }
-        }
-    }
-#else
-    // software-pipelined like ep_exp2_slots: next trip's exponents, and this trip's steady states / old gate values, are
-    // read before the polynomials run
-    double e[EXP_W];
-#pragma unroll
-    for (int j = 0; j < EXP_W; ++j) e[j] = col[j * BLOCK];
-#pragma unroll 1
-    for (int g = 0; g < N_EXPB; g += EXP_W) {
-        const int gn = (g + EXP_W < N_EXPB) ? g + EXP_W : g;
-        double ne[EXP_W], yi[EXP_W], yo[EXP_W];
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) {
-            ne[j] = col[(gn + j) * BLOCK];
-            yi[j] = col[(B_INF0 + g + j) * BLOCK];      // slot B_INF0 + 11 is the (unused) pad of the last trip
-            yo[j] = col[(G_OLD0 + g + j) * BLOCK];      // slot G_OLD0 + 11 = G_RBAR: read, not used
-        }
-        ep_exp2_wide<EXP_W>(e);
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j)
-            if (g + j < N_RLB) ycol[(1 + g + j) * stride] = fma(yo[j] - yi[j], e[j], yi[j]);
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) e[j] = ne[j];
-    }
-#endif
-}
 
 // One step of one cell, everything on the right-hand side at t^n.  v = Vm^n of this cell, ycol = &y[0][cell] (state
 // row k at ycol[k*stride]; rows 1..18 are read and overwritten), type: 0 endo, 1 mid, 2 epi, stimulus() returns
@@ -201,36 +154,41 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const bool hi = (vs >= -40.0);   // reading B7 (on the gates' own argument)
 
     // ---- batch 2: every voltage-dependent exponential that is not an integer power of another one
-    col[A_B600 * BLOCK] = vgs * CK(L2E / 600.0);
-    col[A_E14 * BLOCK] = vgs * CK(L2E / 14.0);
-    col[A_M * BLOCK] = fma(vgs, CK(-L2E / 9.03), CK(-56.86 * L2E / 9.03));
-    col[A_H * BLOCK] = fma(vgs, CK(L2E / 7.43), CK(71.55 * L2E / 7.43));
-    col[A_XR1 * BLOCK] = fma(vgs, CK(L2E / 11.5), CK(30.0 * L2E / 11.5));
-    col[A_D * BLOCK] = fma(vgs, CK(-L2E / 13.0), CK(-35.0 * L2E / 13.0));
-    col[A_PK * BLOCK] = fma(vg, CK(-L2E / 5.98), CK(25.0 * L2E / 5.98));
-    col[A_W * BLOCK] = vg * CK(0.05 * FRT * L2E);
-    col[A_GR * BLOCK] = (vgs + 40.0) * (vgs + 40.0) * CK(-L2E / 1800.0);
-    col[A_GS * BLOCK] = (type == 0) ? (vgs + 67.0) * (vgs + 67.0) * CK(-L2E / 1000.0)
+    // The arguments stay in registers: each group of EXP_W is evaluated as soon as the loop below reaches it and only its
+    // RESULTS go to the slot array (an argument round trip through shared memory was 18 % of the kernel's LSU wavefronts;
+    // profiles/r02_cell_kernel.md).
+    double a1[N_EXPA];
+#define ARG(k) a1[k]
+    ARG(A_B600) = vgs * CK(L2E / 600.0);
+    ARG(A_E14) = vgs * CK(L2E / 14.0);
+    ARG(A_M) = fma(vgs, CK(-L2E / 9.03), CK(-56.86 * L2E / 9.03));
+    ARG(A_H) = fma(vgs, CK(L2E / 7.43), CK(71.55 * L2E / 7.43));
+    ARG(A_XR1) = fma(vgs, CK(L2E / 11.5), CK(30.0 * L2E / 11.5));
+    ARG(A_D) = fma(vgs, CK(-L2E / 13.0), CK(-35.0 * L2E / 13.0));
+    ARG(A_PK) = fma(vg, CK(-L2E / 5.98), CK(25.0 * L2E / 5.98));
+    ARG(A_W) = vg * CK(0.05 * FRT * L2E);
+    ARG(A_GR) = (vgs + 40.0) * (vgs + 40.0) * CK(-L2E / 1800.0);
+    ARG(A_GS) = (type == 0) ? (vgs + 67.0) * (vgs + 67.0) * CK(-L2E / 1000.0)
                                     : (vgs + 45.0) * (vgs + 45.0) * CK(-L2E / 320.0);
-    col[A_G27 * BLOCK] = (vgs + 27.0) * (vgs + 27.0) * CK(-L2E / 3600.0);
+    ARG(A_G27) = (vgs + 27.0) * (vgs + 27.0) * CK(-L2E / 3600.0);
     const double xcal = (vg - 15.0) * CK(2.0 * FRT);
-    col[A_CAL * BLOCK] = fma(vg, CK(2.0 * FRT * L2E), CK(-30.0 * FRT * L2E));   // xcal in base-2 units
-    col[A_K1Q * BLOCK] = fma(ug, CK(0.0002 * L2E), CK(0.02 * L2E));   // 0.0002 (u + 100)
-    col[A_K1Q2 * BLOCK] = ug * CK(0.02 * L2E);
+    ARG(A_CAL) = fma(vg, CK(2.0 * FRT * L2E), CK(-30.0 * FRT * L2E));   // xcal in base-2 units
+    ARG(A_K1Q) = fma(ug, CK(0.0002 * L2E), CK(0.02 * L2E));   // 0.0002 (u + 100)
+    ARG(A_K1Q2) = ug * CK(0.02 * L2E);
     if (hi) {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vgs, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
-        col[(A_HJ0 + 1) * BLOCK] = vgs * CK(0.057 * L2E);
+        ARG((A_HJ0 + 0)) = fma(vgs, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
+        ARG((A_HJ0 + 1)) = vgs * CK(0.057 * L2E);
 #pragma unroll
-        for (int k = 0; k < 6; ++k) col[(A_HJ2 + k) * BLOCK] = 0.0;
+        for (int k = 0; k < 6; ++k) ARG(A_HJ2 + k) = 0.0;
     } else {
-        col[(A_HJ0 + 0) * BLOCK] = fma(vgs, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));
-        col[(A_HJ0 + 1) * BLOCK] = vgs * CK(0.079 * L2E);
-        col[(A_HJ2 + 0) * BLOCK] = vgs * CK(0.3485 * L2E);
-        col[(A_HJ2 + 1) * BLOCK] = vgs * CK(0.2444 * L2E);
-        col[(A_HJ2 + 2) * BLOCK] = vgs * CK(-0.04391 * L2E);
-        col[(A_HJ2 + 3) * BLOCK] = fma(vgs, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
-        col[(A_HJ2 + 4) * BLOCK] = vgs * CK(-0.01052 * L2E);
-        col[(A_HJ2 + 5) * BLOCK] = fma(vgs, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
+        ARG((A_HJ0 + 0)) = fma(vgs, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));
+        ARG((A_HJ0 + 1)) = vgs * CK(0.079 * L2E);
+        ARG((A_HJ2 + 0)) = vgs * CK(0.3485 * L2E);
+        ARG((A_HJ2 + 1)) = vgs * CK(0.2444 * L2E);
+        ARG((A_HJ2 + 2)) = vgs * CK(-0.04391 * L2E);
+        ARG((A_HJ2 + 3)) = fma(vgs, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
+        ARG((A_HJ2 + 4)) = vgs * CK(-0.01052 * L2E);
+        ARG((A_HJ2 + 5)) = fma(vgs, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
     }
     // fCass and Rbar: their Rush-Larsen rates need no exponential, so exp(-dt/tau) rides in this batch
     const double c2 = CaSR * CaSR, css2 = CaSS * CaSS, ci2 = Cai * Cai;
@@ -245,10 +203,24 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double fCass_inf = fma(CK(0.6), qf, CK(0.4));
     const double Rbar_rate = fma(CK(k2p) * kcasr_s, CaSSs, CK(k4));   // dR/dt = k4 (1 - R) - k2 CaSS R (reading B1)
     const double Rbar_inf = CK(k4) * ep_rcp(Rbar_rate);
-    col[A_RLF * BLOCK] = -dtl * ep_rcp(fma(80.0, qf, 2.0));         // tau_fCass >= 2 ms
-    col[A_RLR * BLOCK] = fmax(-dtl * Rbar_rate, -1000.0);           // rate grows with Ca_SS: keep the clamp
+    ARG(A_RLF) = -dtl * ep_rcp(fma(80.0, qf, 2.0));         // tau_fCass >= 2 ms
+    ARG(A_RLR) = fmax(-dtl * Rbar_rate, -1000.0);           // rate grows with Ca_SS: keep the clamp
     // warp-uniform trip count: during the plateau (every cell of the warp above -40 mV) the last trip is skipped
-    ep_exp2_slots<N_EXPA, BLOCK, EXP_W>(col, __all_sync(__activemask(), hi) ? N_EXPA_HI : N_EXPA);
+    {
+        const int n1 = __all_sync(__activemask(), hi) ? N_EXPA_HI : N_EXPA;
+#pragma unroll
+        for (int s0 = 0; s0 < N_EXPA; s0 += EXP_W) {
+            if (s0 < n1) {
+                double x[EXP_W];
+#pragma unroll
+                for (int j = 0; j < EXP_W; ++j) x[j] = a1[s0 + j];
+                ep_exp2_wide<EXP_W>(x);
+#pragma unroll
+                for (int j = 0; j < EXP_W; ++j) col[(s0 + j) * BLOCK] = x[j];
+            }
+        }
+    }
+#undef ARG
     const double dv_diff = finish_gather();   // the gathers have landed during the batch: 12 values -> 1
     // I_s/C_m of this cell and step.  Evaluated here, not before the loads above: its first instruction waits for the
     // cell's stimulus mask, and a wait at the top of the kernel would delay the issue of every other load by one DRAM
@@ -427,14 +399,24 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
         inf[10] = fma(CK(0.67), ep_rcp(fma(CK(E5C), E7, 1.0)), CK(0.33));
         rate[10] = Qc * Qb * ep_rcp(fma(562.0 * Gf2, Qc * Qb, fma(31.0 * E10, Qb, 80.0 * Qc)));
     }
-    // ---- batch 3: Rush-Larsen (every value of batch 2 has been consumed above, so its slots are free)
+    // ---- batch 3: Rush-Larsen
+    // exponents and steady states stay in registers: three unrolled groups, only the parked gate values come from shared memory
 #pragma unroll
-    for (int g = 0; g < N_RLB; ++g) {
-        col[g * BLOCK] = (g <= 3) ? fmax(-dtl * rate[g], -1000.0) : -dtl * rate[g];   // m, h, j, xr1: see the clamp note above
-        col[(B_INF0 + g) * BLOCK] = inf[g];
+    for (int g0 = 0; g0 < N_EXPB; g0 += EXP_W) {
+        double e[EXP_W], yo[EXP_W];
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) {
+            const int g = g0 + j;
+            e[j] = (g < N_RLB) ? ((g <= 3) ? fmax(-dtl * rate[g], -1000.0) : -dtl * rate[g]) : 0.0;
+            yo[j] = col[(G_OLD0 + g) * BLOCK];
+        }
+        ep_exp2_wide<EXP_W>(e);
+#pragma unroll
+        for (int j = 0; j < EXP_W; ++j) {
+            const int g = g0 + j;
+            if (g < N_RLB) ycol[(1 + g) * stride] = fma(yo[j] - inf[g], e[j], inf[g]);
+        }
     }
-    col[N_RLB * BLOCK] = 0.0;
-    tp06_rush_larsen_slots<BLOCK>(col, ycol, stride);
     return v_new;
 }
 
