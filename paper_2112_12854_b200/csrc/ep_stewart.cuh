@@ -8,8 +8,8 @@
 //
 // Production form, same rearrangements as ep_tp06.cuh: exponentials with commensurate slopes are integer
 // powers of one exponential (v/600 -> 1/200, 1/25 (I_f), 1/24, 1/20, 1/15, 1/10, 1/7.5, 1/6, 1/5 and 0.11 (I_f);
-// -(v+35)/13 serves tau_d, r_inf and s_inf), every sigmoid product is one rational function with a single reciprocal, the rest
-// is evaluated in shared-memory batches.  Units: mV, ms, mM, currents uA/uF.
+// -(v+35)/13 serves tau_d, r_inf and s_inf), every sigmoid product is one rational function with a single reciprocal, the
+// exponentials are evaluated four at a time right before their consumers (streaming form, see ep_tp06.cuh).  Units: mV, ms, mM, currents uA/uF.
 #pragma once
 #include "ep_tp06.cuh"   // CK(), the shared TP06 constants (tp06::), ep_math.cuh
 
@@ -47,17 +47,11 @@ constexpr double EM8_13 = 0.5404329964865341;      // e^(-8/13)
 constexpr double EM8 = 0.00033546262790251185;     // e^(-8)
 constexpr double E5_17 = 1.3419417698828804;       // e^(5/17)
 
-// shared-memory slots of the two exponential batches
-constexpr int A_B600 = 0, A_E14 = 1, A_M = 2, A_H = 3, A_XR1 = 4, A_D = 5, A_PK = 6, A_W = 7, A_GR = 8, A_GS = 9, A_G27 = 10,
-              A_CAL = 11, A_Y = 12, A_SUS = 13, A_HJ0 = 14, A_RLF = 16, A_HJ2 = 18, N_EXPA = 24;   // slot 17: pad
-constexpr int N_EXPA_HI = 20;
-constexpr int EXP_W = 4;
-constexpr int N_RLB = 12;    // Rush-Larsen gates whose rate depends on batch 2: y xr1 xr2 xs m h j d f f2 (rows 1..10), s r (12, 13)
-constexpr int N_EXPB = 12;   // their Rush-Larsen exponentials, evaluated in registers
-constexpr int G_OLD0 = 24;   // the 12 gate values at t^n, slots 24..35
-constexpr int N_SLOTS = 36;
-static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && N_RLB == N_EXPB && N_EXPA <= G_OLD0 && G_OLD0 + N_RLB <= N_SLOTS,
-              "slot layout");
+// shared-memory slots (one column of BLOCK doubles per thread): the 12 voltage-driven gate values at t^n, parked by asynchronous copies
+constexpr int EXP_W = 4;     // exponentials evaluated side by side
+constexpr int N_RLB = 12;    // Rush-Larsen list: 0 y, 1 xr1, 2 xr2, 3 xs, 4 m, 5 h, 6 j, 7 d, 8 f, 9 f2 (rows 1..10), 10 s, 11 r (rows 12, 13)
+constexpr int G_OLD0 = 0;
+constexpr int N_SLOTS = 12;
 __device__ __forceinline__ constexpr int rl_row(int g) { return g < 10 ? 1 + g : 2 + g; }   // skips fCass (row 11)
 }  // namespace stw
 
@@ -85,62 +79,21 @@ __device__ __forceinline__ double stw_step(double v, double* ycol, int64_t strid
     const double u = v - EK;
     const bool hi = (v >= -40.0);   // reading B7
 
-    // ---- batch 2: voltage-dependent exponentials that are not integer powers of another one (arguments in registers, only the
-    // results go to the slot array: see tp06_step)
-    double a1[N_EXPA];
-#define ARG(k) a1[k]
-    ARG(A_B600) = vg * CK(L2E / 600.0);
-    ARG(A_E14) = vg * CK(L2E / 14.0);
-    ARG(A_M) = fma(vg, CK(-L2E / 9.03), CK(-56.86 * L2E / 9.03));
-    ARG(A_H) = fma(vg, CK(L2E / 7.43), CK(71.55 * L2E / 7.43));
-    ARG(A_XR1) = fma(vg, CK(L2E / 11.5), CK(30.0 * L2E / 11.5));
-    ARG(A_D) = fma(vg, CK(-L2E / 13.0), CK(-35.0 * L2E / 13.0));
-    ARG(A_PK) = fma(vg, CK(-L2E / 5.98), CK(25.0 * L2E / 5.98));
-    ARG(A_W) = vg * CK(0.05 * FRT * L2E);
-    ARG(A_GR) = (vg + 40.0) * (vg + 40.0) * CK(-L2E / 1800.0);
-    ARG(A_GS) = (vg + 25.0) * (vg + 25.0) * CK(-L2E / 320.0);
-    ARG(A_G27) = (vg + 27.0) * (vg + 27.0) * CK(-L2E / 3600.0);
-    const double xcal = (vg - 15.0) * CK(2.0 * FRT);
-    ARG(A_CAL) = fma(vg, CK(2.0 * FRT * L2E), CK(-30.0 * FRT * L2E));
-    ARG(A_Y) = fma(vg, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));      // e^{-(v+80)/6.8}: y_inf, and alpha_h below -40 mV
-    ARG(A_SUS) = vg * CK(-L2E / 17.0);                             // e^{-v/17}: I_sus
-    if (hi) {
-        ARG((A_HJ0 + 0)) = fma(vg, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
-        ARG((A_HJ0 + 1)) = vg * CK(0.057 * L2E);
-#pragma unroll
-        for (int k = 0; k < 6; ++k) ARG((A_HJ2 + k)) = 0.0;
-    } else {
-        ARG((A_HJ0 + 0)) = 0.0;
-        ARG((A_HJ0 + 1)) = vg * CK(0.079 * L2E);
-        ARG((A_HJ2 + 0)) = vg * CK(0.3485 * L2E);
-        ARG((A_HJ2 + 1)) = vg * CK(0.2444 * L2E);
-        ARG((A_HJ2 + 2)) = vg * CK(-0.04391 * L2E);
-        ARG((A_HJ2 + 3)) = fma(vg, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
-        ARG((A_HJ2 + 4)) = vg * CK(-0.01052 * L2E);
-        ARG((A_HJ2 + 5)) = fma(vg, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
-    }
-    // fCass: its Rush-Larsen rate needs no exponential, so exp(-dt/tau) rides in this batch
+    // ---- streaming form (see tp06_step): nine groups of EXP_W exponentials, each evaluated right before its consumers, so that
+    // arguments and results stay in registers; the slot array only parks the 12 gate values at t^n and the stencil coefficients
     const double c2 = CaSR * CaSR, css2 = CaSS * CaSS, ci2 = Cai * Cai;
     const double kcasr = fma(-(maxsr - minsr) * c2, ep_rcp(c2 + EC * EC), maxsr);
     const double qf = ep_rcp(fma(400.0, css2, 1.0));
     const double fCass_inf = fma(CK(0.6), qf, CK(0.4));
-    ARG(A_RLF) = -dtl * ep_rcp(fma(80.0, qf, 2.0));
-    ARG((A_RLF + 1)) = 0.0;
-    {
-        const int n1 = __all_sync(__activemask(), hi) ? N_EXPA_HI : N_EXPA;
-#pragma unroll
-        for (int s0 = 0; s0 < N_EXPA; s0 += EXP_W) {
-            if (s0 < n1) {
-                double x[EXP_W];
-#pragma unroll
-                for (int j = 0; j < EXP_W; ++j) x[j] = a1[s0 + j];
-                ep_exp2_wide<EXP_W>(x);
-#pragma unroll
-                for (int j = 0; j < EXP_W; ++j) col[(s0 + j) * BLOCK] = x[j];
-            }
-        }
-    }
-#undef ARG
+    // group 0: the two shared gate exponentials and the two current exponentials that are raised to powers
+    double x0[EXP_W] = {vg * CK(L2E / 600.0), vg * CK(L2E / 14.0), vg * CK(0.05 * FRT * L2E),
+                        fma(vg, CK(2.0 * FRT * L2E), CK(-30.0 * FRT * L2E))};
+    const double xcal = (vg - 15.0) * CK(2.0 * FRT);
+    ep_exp2_wide<EXP_W>(x0);
+    // group 1: I_pK, the Gaussian of tau_f / tau_f2, e^{-(v+80)/6.8} (y_inf, alpha_h below -40 mV), e^{-v/17} (I_sus)
+    double x1[EXP_W] = {fma(vg, CK(-L2E / 5.98), CK(25.0 * L2E / 5.98)), (vg + 27.0) * (vg + 27.0) * CK(-L2E / 3600.0),
+                        fma(vg, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8)), vg * CK(-L2E / 17.0)};
+    ep_exp2_wide<EXP_W>(x1);
     const double dv_diff = finish_gather();
     const double istim = stimulus();          // late on purpose: see tp06_step
     ep_cp_async_wait();
@@ -157,39 +110,36 @@ __device__ __forceinline__ double stw_step(double v, double* ycol, int64_t strid
         gCaL = (g[7] * g[8]) * (g[9] * fCass);
         gto = g[10] * g[11];
     }
-    ycol[W_FCASS * stride] = fma(fCass - fCass_inf, col[A_RLF * BLOCK], fCass_inf);   // Rush-Larsen
-
     // ---- integer powers
     double E200, E24, E20, E15, E10, E7p5, E6, E5, B24, B90;
     {
-        const double B = col[A_B600 * BLOCK];
+        const double B = x0[0];
         const double B2 = B * B, B3 = B2 * B, B5 = B2 * B3, B10 = B5 * B5, B20 = B10 * B10, B40 = B20 * B20;
         const double B30 = B20 * B10, B60 = B30 * B30;
         E200 = B3; E24 = B20 * B5; E20 = B30; E15 = B40; E10 = B60; E7p5 = B40 * B40; E6 = B60 * B40; E5 = B60 * B60;
         B24 = B20 * (B3 * B);      // e^{0.04 v}
         B90 = B60 * B30;           // e^{0.15 v}
     }
-    const double E14 = col[A_E14 * BLOCK], E7 = E14 * E14;
+    const double E14 = x0[1], E7 = E14 * E14;
     double W13, W18, W20;
     {
-        const double W = col[A_W * BLOCK];
+        const double W = x0[2];
         const double W2 = W * W, W4 = W2 * W2, W8 = W4 * W4, W16 = W8 * W8;
         W13 = W8 * W4 * W; W18 = W16 * W2; W20 = W18 * W2;
     }
     double Gf, Gf2;
     {
-        const double b = col[A_G27 * BLOCK];
+        const double b = x1[1];
         const double b2 = b * b, b4 = b2 * b2, b8 = b4 * b4;
         Gf = b8 * b8; Gf2 = (b8 * b4) * (b2 * b);
     }
-    const double D13 = col[A_D * BLOCK];     // e^{-(v+35)/13}
-    const double Y68 = col[A_Y * BLOCK];     // e^{-(v+80)/6.8}
+    const double Y68 = x1[2];     // e^{-(v+80)/6.8}
 
     // ---- membrane currents
     const double INa = CK(GNas) * gNa * (v - ENa);
     double ICaL;
     {
-        const double ex = col[A_CAL * BLOCK];
+        const double ex = x0[3];
         const double xo = (fabs(xcal) < 1e-7) ? fma(-0.5, xcal, 1.0) : xcal * ep_rcp(ex - 1.0);   // reading B6
         ICaL = CK(GCaL * 2.0 * F) * gCaL * xo * fma(0.25 * CaSS, ex, -Cao);
     }
@@ -199,14 +149,14 @@ __device__ __forceinline__ double stw_step(double v, double* ycol, int64_t strid
     const double IKr = CK(GKrs) * gKr * u;     // sqrt(Ko/5.4) = 1
     const double IKs = CK(GKss) * gKs * (v - EKs);
     const double IK1 = CK(GK1s) * (u - 8.0) * ep_rcp(fma(CK(E7544), E10, 1.0));     // 1/(1 + e^{0.1 (v + 75.44)})
-    const double Isus = CK(Gsus) * u * ep_rcp(fma(CK(E5_17), col[A_SUS * BLOCK], 1.0));   // 1/(1 + e^{(5 - v)/17})
+    const double Isus = CK(Gsus) * u * ep_rcp(fma(CK(E5_17), x1[3], 1.0));   // 1/(1 + e^{(5 - v)/17})
     const double Nai3 = Nai * Nai * Nai;
     const double INaCa = CK(kNaCa / ((KmNai * KmNai * KmNai + Nao * Nao * Nao) * (KmCa + Cao)))
                          * fma(W20, Nai3 * Cao, CK(-(Nao * Nao * Nao * alpha)) * Cai) * ep_rcp(W13 + CK(ksat));
     const double INaK = CK(PNaK * Ko / (Ko + KmK)) * Nai * W20
                         * ep_rcp((Nai + KmNa) * fma(CK(0.1245), W18, W20 + CK(0.0353)));
     const double IpCa = CK(GpCa) * Cai * ep_rcp(CK(KpCa) + Cai);
-    const double IpK = CK(GpK) * u * ep_rcp(1.0 + col[A_PK * BLOCK]);
+    const double IpK = CK(GpK) * u * ep_rcp(1.0 + x1[0]);
     const double IbNa = CK(GbNa) * (v - ENa);
     const double IbCa = CK(GbCa) * (v - ECa);
     const double iion = IK1 + Ito + Isus + IKr + IKs + ICaL + INaK + INa + IbNa + INaCa + IbCa + IpK + IpCa + IfNa + IfK;
@@ -236,79 +186,111 @@ __device__ __forceinline__ double stw_step(double v, double* ycol, int64_t strid
     ycol[W_NAI * stride] = fma(dt, dNai, Nai);
     ycol[W_KI * stride] = fma(dt, dKi, Ki);
 
-    // ---- gates: steady states and rates 1/tau, each as one rational function
-    double inf[N_RLB], rate[N_RLB];
-    {   // y: inf = 1/(1 + e^{(v+80.6)/6.8}), tau = 4000/(e^{-2.9-0.04v} + e^{3.6+0.11v})
-        inf[0] = Y68 * ep_rcp(Y68 + CK(E06_68));
-        rate[0] = fma(CK(E36), B90, CK(EM29)) * ep_rcp(4000.0 * B24);
-    }
-    {   // xr1, xr2, xs (as TP06)
-        inf[1] = E7 * ep_rcp(E7 + CK(EM26_7));
-        rate[1] = (E10 + CK(EM45)) * (1.0 + col[A_XR1 * BLOCK]) * ep_rcp(2700.0 * E10);
-        inf[2] = ep_rcp(fma(CK(E88_24), E24, 1.0));
-        rate[2] = (E20 + CK(EM3)) * fma(CK(EM3), E20, 1.0) * ep_rcp(CK(3.36) * E20);
-        inf[3] = E14 * ep_rcp(E14 + CK(EM5_14));
-        const double t = ep_rsqrt((E6 + CK(E5_6)) * E6) * E6;
-        const double P15 = fma(CK(EM35_15), E15, 1.0);
-        rate[3] = P15 * ep_rcp(fma(1400.0, t, 80.0 * P15));
-    }
-    {   // m
-        const double sm = ep_rcp(1.0 + col[A_M * BLOCK]);
-        inf[4] = sm * sm;
-        const double P = fma(CK(E7C), E5, 1.0), Q = fma(CK(EM025), E200, 1.0);
-        rate[4] = (E5 + CK(EM12)) * P * Q * ep_rcp(CK(0.1) * E5 * (P + Q));
-    }
-    {   // h, j
-        const double sh = ep_rcp(1.0 + col[A_H * BLOCK]);
-        inf[5] = inf[6] = sh * sh;
-        const double s0 = col[(A_HJ0 + 0) * BLOCK], s1 = col[(A_HJ0 + 1) * BLOCK];
-        if (hi) {
-            rate[5] = CK(0.77 / 0.13) * ep_rcp(1.0 + s0);
-            rate[6] = CK(0.6) * s1 * E10 * ep_rcp(E10 + CK(EM32));
-        } else {
-            const double s2 = col[(A_HJ2 + 0) * BLOCK], s3 = col[(A_HJ2 + 1) * BLOCK], s4 = col[(A_HJ2 + 2) * BLOCK],
-                         s5 = col[(A_HJ2 + 3) * BLOCK], s6 = col[(A_HJ2 + 4) * BLOCK], s7 = col[(A_HJ2 + 5) * BLOCK];
-            rate[5] = fma(CK(0.057), Y68, fma(CK(2.7), s1, 3.1e5 * s2));
-            const double N1 = fma(-2.5428e4, s3, CK(-6.948e-6) * s4) * (vg + CK(37.78)), D1 = 1.0 + s5;
-            const double N2 = CK(0.02424) * s6, D2 = 1.0 + s7;
-            rate[6] = fma(N1, D2, N2 * D1) * ep_rcp(D1 * D2);
-        }
-    }
-    {   // d, f, f2 (as TP06)
-        inf[7] = E7p5 * ep_rcp(E7p5 + CK(EM8_75));
-        const double D = 1.0 + D13, P5 = fma(CK(E1), E5, 1.0), Q20 = E20 + CK(E25);
-        rate[7] = D * P5 * Q20 * ep_rcp(fma(fma(0.25, D, CK(1.4)) * CK(1.4), Q20, E20 * D * P5));
-        const double Qa = E10 + CK(E13), Qb = fma(CK(E3), E10, 1.0), Qc = E10 + CK(E25);
-        inf[8] = ep_rcp(fma(CK(E20_7), E7, 1.0));
-        rate[8] = Qa * Qb * ep_rcp(fma(fma(1102.5, Gf, 20.0), Qa * Qb, fma(200.0 * E10, Qb, 180.0 * Qa)));
-        inf[9] = fma(CK(0.67), ep_rcp(fma(CK(E5C), E7, 1.0)), CK(0.33));
-        rate[9] = Qc * Qb * ep_rcp(fma(562.0 * Gf2, Qc * Qb, fma(31.0 * E10, Qb, 80.0 * Qc)));
-    }
-    {   // s, r of the Purkinje transient outward current
-        inf[10] = D13 * ep_rcp(D13 + CK(EM8_13));                          // 1/(1 + e^{(v+27)/13})
-        const double P = fma(CK(EM8), E5, 1.0);                            // 1 + e^{(v-40)/5}
-        rate[10] = P * ep_rcp(fma(fma(85.0, col[A_GS * BLOCK], 42.0), P, 5.0));
-        inf[11] = ep_rcp(fma(CK(E55_13), D13, 1.0));                       // 1/(1 + e^{(20-v)/13})
-        rate[11] = ep_rcp(fma(10.45, col[A_GR * BLOCK], CK(7.3)));
-    }
-    // ---- batch 3: Rush-Larsen, exponents and steady states in registers (three unrolled groups)
+    // one Rush-Larsen group: y <- inf + (y_old - inf) 2^e for four gates (g = position in the Rush-Larsen list)
+    auto rush_larsen4 = [&](double (&e)[EXP_W], const double (&in)[EXP_W], int g0, int g1, int g2, int g3) {
+        const int gi[EXP_W] = {g0, g1, g2, g3};
+        double yo[EXP_W];
 #pragma unroll
-    for (int g0 = 0; g0 < N_EXPB; g0 += EXP_W) {
-        double e[EXP_W], yo[EXP_W];
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) {
-            const int g = g0 + j;
-            // m, h, j, xr1 can be faster than 700/dt inside the clamp range (see the note in tp06_step), and so can y: its rate
-            // reaches 3e7 per ms at +200 mV (2 per ms at +50 mV).  2^-1000 stands for the oracle's underflow to 0.
-            e[j] = (g <= 1 || (g >= 4 && g <= 6)) ? fmax(-dtl * rate[g], -1000.0) : -dtl * rate[g];
-            yo[j] = col[(G_OLD0 + g) * BLOCK];
-        }
+        for (int j = 0; j < EXP_W; ++j) yo[j] = col[(G_OLD0 + gi[j]) * BLOCK];
         ep_exp2_wide<EXP_W>(e);
 #pragma unroll
-        for (int j = 0; j < EXP_W; ++j) {
-            const int g = g0 + j;
-            ycol[rl_row(g) * stride] = fma(yo[j] - inf[g], e[j], inf[g]);
+        for (int j = 0; j < EXP_W; ++j) ycol[rl_row(gi[j]) * stride] = fma(yo[j] - in[j], e[j], in[j]);
+    };
+    // m, h, j, xr1 can be faster than 700/dt inside the clamp range (see the note in tp06_step), and so can y: its rate reaches
+    // 3e7 per ms at +200 mV (2 per ms at +50 mV).  Their exponents are clamped to -1000: 2^-1000 stands for the oracle's 0.
+    double D13, h_exp;
+    // ---- group 2: m, h_inf, xr1, tau_d / r_inf / s_inf; gates y, xr1, m, d
+    {
+        double x2[EXP_W] = {fma(vg, CK(-L2E / 9.03), CK(-56.86 * L2E / 9.03)), fma(vg, CK(L2E / 7.43), CK(71.55 * L2E / 7.43)),
+                            fma(vg, CK(L2E / 11.5), CK(30.0 * L2E / 11.5)), fma(vg, CK(-L2E / 13.0), CK(-35.0 * L2E / 13.0))};
+        ep_exp2_wide<EXP_W>(x2);
+        h_exp = x2[1];
+        D13 = x2[3];                                                       // e^{-(v+35)/13}
+        double in[EXP_W], e[EXP_W];
+        in[0] = Y68 * ep_rcp(Y68 + CK(E06_68));                            // y: 1/(1 + e^{(v+80.6)/6.8})
+        e[0] = fmax(-dtl * (fma(CK(E36), B90, CK(EM29)) * ep_rcp(4000.0 * B24)), -1000.0);   // tau = 4000/(e^{-2.9-0.04v} + e^{3.6+0.11v})
+        in[1] = E7 * ep_rcp(E7 + CK(EM26_7));                              // xr1
+        e[1] = fmax(-dtl * ((E10 + CK(EM45)) * (1.0 + x2[2]) * ep_rcp(2700.0 * E10)), -1000.0);
+        {   // m
+            const double sm = ep_rcp(1.0 + x2[0]);
+            in[2] = sm * sm;
+            const double P = fma(CK(E7C), E5, 1.0), Q = fma(CK(EM025), E200, 1.0);
+            e[2] = fmax(-dtl * ((E5 + CK(EM12)) * P * Q * ep_rcp(CK(0.1) * E5 * (P + Q))), -1000.0);
         }
+        {   // d
+            in[3] = E7p5 * ep_rcp(E7p5 + CK(EM8_75));
+            const double D = 1.0 + D13, P5 = fma(CK(E1), E5, 1.0), Q20 = E20 + CK(E25);
+            e[3] = -dtl * (D * P5 * Q20 * ep_rcp(fma(fma(0.25, D, CK(1.4)) * CK(1.4), Q20, E20 * D * P5)));
+        }
+        rush_larsen4(e, in, 0, 1, 4, 7);
+    }
+    // ---- group 3: the Gaussians of tau_r and tau_s, exp(-dt/tau) of fCass; gates xr2, xs, s, r
+    {
+        double x3[EXP_W] = {(vg + 40.0) * (vg + 40.0) * CK(-L2E / 1800.0), (vg + 25.0) * (vg + 25.0) * CK(-L2E / 320.0),
+                            -dtl * ep_rcp(fma(80.0, qf, 2.0)), 0.0};
+        ep_exp2_wide<EXP_W>(x3);
+        ycol[W_FCASS * stride] = fma(fCass - fCass_inf, x3[2], fCass_inf);   // Rush-Larsen
+        double in[EXP_W], e[EXP_W];
+        in[0] = ep_rcp(fma(CK(E88_24), E24, 1.0));                                                     // xr2
+        e[0] = -dtl * ((E20 + CK(EM3)) * fma(CK(EM3), E20, 1.0) * ep_rcp(CK(3.36) * E20));
+        {   // xs
+            in[1] = E14 * ep_rcp(E14 + CK(EM5_14));
+            const double t = ep_rsqrt((E6 + CK(E5_6)) * E6) * E6;
+            const double P15 = fma(CK(EM35_15), E15, 1.0);
+            e[1] = -dtl * (P15 * ep_rcp(fma(1400.0, t, 80.0 * P15)));
+        }
+        {   // s, r of the Purkinje transient outward current
+            in[2] = D13 * ep_rcp(D13 + CK(EM8_13));                        // 1/(1 + e^{(v+27)/13})
+            const double P = fma(CK(EM8), E5, 1.0);                        // 1 + e^{(v-40)/5}
+            e[2] = -dtl * (P * ep_rcp(fma(fma(85.0, x3[1], 42.0), P, 5.0)));
+            in[3] = ep_rcp(fma(CK(E55_13), D13, 1.0));                     // 1/(1 + e^{(20-v)/13})
+            e[3] = -dtl * ep_rcp(fma(10.45, x3[0], CK(7.3)));
+        }
+        rush_larsen4(e, in, 2, 3, 10, 11);
+    }
+    // ---- groups 4, 5: the h / j rate exponentials (the second group is skipped when every cell of the warp is above -40 mV);
+    // gates h, j, f, f2
+    {
+        double x4[EXP_W], x5[EXP_W] = {1.0, 1.0, 1.0, 1.0};
+        const bool all_hi = __all_sync(__activemask(), hi);
+        if (hi) {
+            x4[0] = fma(vg, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
+            x4[1] = vg * CK(0.057 * L2E);
+            x4[2] = 0.0; x4[3] = 0.0;
+        } else {
+            x4[0] = vg * CK(0.079 * L2E);
+            x4[1] = vg * CK(0.3485 * L2E);
+            x4[2] = vg * CK(0.2444 * L2E);
+            x4[3] = vg * CK(-0.04391 * L2E);
+        }
+        ep_exp2_wide<EXP_W>(x4);
+        if (!all_hi) {
+            x5[0] = fma(vg, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
+            x5[1] = vg * CK(-0.01052 * L2E);
+            x5[2] = fma(vg, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
+            x5[3] = 0.0;
+            ep_exp2_wide<EXP_W>(x5);
+        }
+        double in[EXP_W], e[EXP_W];
+        const double sh = ep_rcp(1.0 + h_exp);
+        in[0] = in[1] = sh * sh;
+        if (hi) {
+            e[0] = fmax(-dtl * (CK(0.77 / 0.13) * ep_rcp(1.0 + x4[0])), -1000.0);
+            e[1] = fmax(-dtl * (CK(0.6) * x4[1] * E10 * ep_rcp(E10 + CK(EM32))), -1000.0);
+        } else {
+            e[0] = fmax(-dtl * fma(CK(0.057), Y68, fma(CK(2.7), x4[0], 3.1e5 * x4[1])), -1000.0);
+            const double N1 = fma(-2.5428e4, x4[2], CK(-6.948e-6) * x4[3]) * (vg + CK(37.78)), D1 = 1.0 + x5[0];
+            const double N2 = CK(0.02424) * x5[1], D2 = 1.0 + x5[2];
+            e[1] = fmax(-dtl * (fma(N1, D2, N2 * D1) * ep_rcp(D1 * D2)), -1000.0);
+        }
+        {   // f, f2 (as TP06)
+            const double Qa = E10 + CK(E13), Qb = fma(CK(E3), E10, 1.0), Qc = E10 + CK(E25);
+            in[2] = ep_rcp(fma(CK(E20_7), E7, 1.0));
+            e[2] = -dtl * (Qa * Qb * ep_rcp(fma(fma(1102.5, Gf, 20.0), Qa * Qb, fma(200.0 * E10, Qb, 180.0 * Qa))));
+            in[3] = fma(CK(0.67), ep_rcp(fma(CK(E5C), E7, 1.0)), CK(0.33));
+            e[3] = -dtl * (Qc * Qb * ep_rcp(fma(562.0 * Gf2, Qc * Qb, fma(31.0 * E10, Qb, 80.0 * Qc))));
+        }
+        rush_larsen4(e, in, 5, 6, 8, 9);
     }
     return v_new;
 }

@@ -10,8 +10,9 @@
 // (DESIGN.md section 7): exponentials with commensurate slopes are integer powers of one exponential
 // (v/600 -> slopes 1/200, 1/24, 1/20, 1/15, 1/10, 1/7.5, 1/6, 1/5; v/14 -> 1/14, 1/7; vF/20RT -> 0.1, 0.65, 0.9, 1 vF/RT;
 // 0.02(v-E_K) -> 0.06, 0.1, 0.5; (v+27)^2/3600 -> /240, /225), every sigmoid product is written as one rational function
-// with a single reciprocal, and the remaining exponentials / logarithms are evaluated in shared-memory batches
-// (ep_math.cuh).  Relative differences from the literal formulas are <= ~2e-14 (120-fold powers of a 1-ulp value),
+// with a single reciprocal, and the remaining 35 exponentials are evaluated four at a time (interleaved dependency chains,
+// ep_math.cuh) in nine groups, each right before the quantities that consume it, so that arguments and results stay in
+// registers; shared memory only parks the gate values at t^n and the stencil coefficients.  Relative differences from the literal formulas are <= ~2e-14 (120-fold powers of a 1-ulp value),
 // three orders of magnitude inside the 1e-11 one-step tolerance.  (The literal transcription was the first kernel of
 // this repo -- profiles/r01a_baseline_direct_kernel.md -- and lives on only in the CPU oracle.)
 //
@@ -77,18 +78,13 @@ constexpr double E3 = 20.085536923187668;         // e^(3)
 constexpr double E5C = 148.4131591025766;         // e^(5)
 constexpr double EM1 = 0.36787944117144233;       // e^(-1)
 
-// shared-memory slots: results of the first exponential batch (0..23), parked gate values (24..35)
-constexpr int A_B600 = 0, A_E14 = 1, A_M = 2, A_H = 3, A_XR1 = 4, A_D = 5, A_PK = 6, A_W = 7, A_GR = 8, A_GS = 9, A_G27 = 10,
-              A_CAL = 11, A_K1Q = 12, A_K1Q2 = 13, A_HJ0 = 14, A_RLF = 16, A_RLR = 17, A_HJ2 = 18, N_EXPA = 24;
-constexpr int N_EXPA_HI = 20;   // a warp whose cells are all above -40 mV needs no h/j slot beyond the first two
-constexpr int EXP_W = 4;     // exponentials evaluated side by side in the batch loops
-constexpr int N_RLB = 11;    // Rush-Larsen variables whose rate depends on batch 2: m h j xr1 xr2 xs r s d f f2
-constexpr int N_EXPB = 12;   // their Rush-Larsen exponentials + 1 pad, evaluated in registers (fCass and Rbar ride in the first batch)
-constexpr int G_OLD0 = 24;   // 11 gate values at t^n, parked from the first load to the Rush-Larsen update, slots 24..34
-constexpr int G_RBAR = 35;   // Rbar at t^n
-constexpr int N_SLOTS = 36;
-static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && N_EXPA <= G_OLD0 && G_OLD0 + N_RLB <= G_RBAR && G_RBAR < N_SLOTS,
-              "slot layout");
+// shared-memory slots (one column of BLOCK doubles per thread): the gate values at t^n, parked by asynchronous copies
+constexpr int EXP_W = 4;     // exponentials evaluated side by side (four interleaved dependency chains)
+constexpr int N_RLB = 11;    // Rush-Larsen variables with voltage-driven rates: m h j xr1 xr2 xs r s d f f2 (fCass and Rbar: rates need no exp)
+constexpr int G_OLD0 = 0;    // 11 gate values at t^n, parked from the first load to the Rush-Larsen update, slots 0..10
+constexpr int G_RBAR = 11;   // Rbar at t^n
+constexpr int N_SLOTS = 12;
+static_assert(G_OLD0 + N_RLB <= G_RBAR && G_RBAR < N_SLOTS, "slot layout");
 }  // namespace tp06
 
 // One step of one cell, everything on the right-hand side at t^n.  v = Vm^n of this cell, ycol = &y[0][cell] (state
@@ -153,43 +149,11 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double ug = ep_clamp(u, -150.0, 300.0);
     const bool hi = (vs >= -40.0);   // reading B7 (on the gates' own argument)
 
-    // ---- batch 2: every voltage-dependent exponential that is not an integer power of another one
-    // The arguments stay in registers: each group of EXP_W is evaluated as soon as the loop below reaches it and only its
-    // RESULTS go to the slot array (an argument round trip through shared memory was 18 % of the kernel's LSU wavefronts;
-    // profiles/r02_cell_kernel.md).
-    double a1[N_EXPA];
-#define ARG(k) a1[k]
-    ARG(A_B600) = vgs * CK(L2E / 600.0);
-    ARG(A_E14) = vgs * CK(L2E / 14.0);
-    ARG(A_M) = fma(vgs, CK(-L2E / 9.03), CK(-56.86 * L2E / 9.03));
-    ARG(A_H) = fma(vgs, CK(L2E / 7.43), CK(71.55 * L2E / 7.43));
-    ARG(A_XR1) = fma(vgs, CK(L2E / 11.5), CK(30.0 * L2E / 11.5));
-    ARG(A_D) = fma(vgs, CK(-L2E / 13.0), CK(-35.0 * L2E / 13.0));
-    ARG(A_PK) = fma(vg, CK(-L2E / 5.98), CK(25.0 * L2E / 5.98));
-    ARG(A_W) = vg * CK(0.05 * FRT * L2E);
-    ARG(A_GR) = (vgs + 40.0) * (vgs + 40.0) * CK(-L2E / 1800.0);
-    ARG(A_GS) = (type == 0) ? (vgs + 67.0) * (vgs + 67.0) * CK(-L2E / 1000.0)
-                                    : (vgs + 45.0) * (vgs + 45.0) * CK(-L2E / 320.0);
-    ARG(A_G27) = (vgs + 27.0) * (vgs + 27.0) * CK(-L2E / 3600.0);
-    const double xcal = (vg - 15.0) * CK(2.0 * FRT);
-    ARG(A_CAL) = fma(vg, CK(2.0 * FRT * L2E), CK(-30.0 * FRT * L2E));   // xcal in base-2 units
-    ARG(A_K1Q) = fma(ug, CK(0.0002 * L2E), CK(0.02 * L2E));   // 0.0002 (u + 100)
-    ARG(A_K1Q2) = ug * CK(0.02 * L2E);
-    if (hi) {
-        ARG((A_HJ0 + 0)) = fma(vgs, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
-        ARG((A_HJ0 + 1)) = vgs * CK(0.057 * L2E);
-#pragma unroll
-        for (int k = 0; k < 6; ++k) ARG(A_HJ2 + k) = 0.0;
-    } else {
-        ARG((A_HJ0 + 0)) = fma(vgs, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));
-        ARG((A_HJ0 + 1)) = vgs * CK(0.079 * L2E);
-        ARG((A_HJ2 + 0)) = vgs * CK(0.3485 * L2E);
-        ARG((A_HJ2 + 1)) = vgs * CK(0.2444 * L2E);
-        ARG((A_HJ2 + 2)) = vgs * CK(-0.04391 * L2E);
-        ARG((A_HJ2 + 3)) = fma(vgs, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
-        ARG((A_HJ2 + 4)) = vgs * CK(-0.01052 * L2E);
-        ARG((A_HJ2 + 5)) = fma(vgs, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
-    }
+    double h_exp;   // e^{(v+71.55)/7.43}: evaluated with group 2, used for h_inf = j_inf with the last group
+    // ---- streaming form: the exponentials are evaluated in nine groups of EXP_W, each group right before the quantities that
+    // consume it, so that their arguments AND results stay in registers; the slot array only parks the gate values at t^n and
+    // the stencil coefficients (profiles/r02_cell_kernel.md: shared-memory traffic, not the fp64 pipe, was what the batch form
+    // of this kernel ran into).
     // fCass and Rbar: their Rush-Larsen rates need no exponential, so exp(-dt/tau) rides in this batch
     const double c2 = CaSR * CaSR, css2 = CaSS * CaSS, ci2 = Cai * Cai;
     const double kcasr = fma(-(maxsr - minsr) * c2, ep_rcp(c2 + EC * EC), maxsr);
@@ -203,31 +167,18 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double fCass_inf = fma(CK(0.6), qf, CK(0.4));
     const double Rbar_rate = fma(CK(k2p) * kcasr_s, CaSSs, CK(k4));   // dR/dt = k4 (1 - R) - k2 CaSS R (reading B1)
     const double Rbar_inf = CK(k4) * ep_rcp(Rbar_rate);
-    ARG(A_RLF) = -dtl * ep_rcp(fma(80.0, qf, 2.0));         // tau_fCass >= 2 ms
-    ARG(A_RLR) = fmax(-dtl * Rbar_rate, -1000.0);           // rate grows with Ca_SS: keep the clamp
-    // warp-uniform trip count: during the plateau (every cell of the warp above -40 mV) the last trip is skipped
-    {
-        const int n1 = __all_sync(__activemask(), hi) ? N_EXPA_HI : N_EXPA;
-#pragma unroll
-        for (int s0 = 0; s0 < N_EXPA; s0 += EXP_W) {
-            if (s0 < n1) {
-                double x[EXP_W];
-#pragma unroll
-                for (int j = 0; j < EXP_W; ++j) x[j] = a1[s0 + j];
-                ep_exp2_wide<EXP_W>(x);
-#pragma unroll
-                for (int j = 0; j < EXP_W; ++j) col[(s0 + j) * BLOCK] = x[j];
-            }
-        }
-    }
-#undef ARG
-    const double dv_diff = finish_gather();   // the gathers have landed during the batch: 12 values -> 1
-    // I_s/C_m of this cell and step.  Evaluated here, not before the loads above: its first instruction waits for the
-    // cell's stimulus mask, and a wait at the top of the kernel would delay the issue of every other load by one DRAM
-    // round trip (profiles/r02a: two serialised long-scoreboard waits in the prologue, 12 % of all stall samples).
-    const double istim = stimulus();
-    // gate values have landed too (finish_gather waited for this thread's asynchronous copies): products for the currents
-    ep_cp_async_wait();
+    // group 0: the two shared gate exponentials and the two current exponentials that are raised to powers
+    double x0[EXP_W] = {vgs * CK(L2E / 600.0), vgs * CK(L2E / 14.0), vg * CK(0.05 * FRT * L2E),
+                        fma(vg, CK(2.0 * FRT * L2E), CK(-30.0 * FRT * L2E))};
+    const double xcal = (vg - 15.0) * CK(2.0 * FRT);
+    ep_exp2_wide<EXP_W>(x0);
+    // group 1: I_pK, the two I_K1 exponentials, the Gaussian of tau_f / tau_f2
+    double x1[EXP_W] = {fma(vg, CK(-L2E / 5.98), CK(25.0 * L2E / 5.98)), fma(ug, CK(0.0002 * L2E), CK(0.02 * L2E)),
+                        ug * CK(0.02 * L2E), (vgs + 27.0) * (vgs + 27.0) * CK(-L2E / 3600.0)};
+    ep_exp2_wide<EXP_W>(x1);
+    const double dv_diff = finish_gather();   // the gathers have landed by now: 12 values -> 1
+    const double istim = stimulus();          // late on purpose: its first instruction waits for the cell's stimulus mask
+    ep_cp_async_wait();                       // the parked gate values have landed too
     double gNa, gCaL, gto, gKr, gKs;
     const double Rbar = col[G_RBAR * BLOCK];
     {
@@ -240,27 +191,24 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
         gKr = g[Y_XR1 - 1] * g[Y_XR2 - 1];
         gKs = g[Y_XS - 1] * g[Y_XS - 1];
     }
-    ycol[Y_FCASS * stride] = fma(fCass - fCass_inf, col[A_RLF * BLOCK], fCass_inf);   // Rush-Larsen
-    ycol[Y_RBAR * stride] = fma(Rbar - Rbar_inf, col[A_RLR * BLOCK], Rbar_inf);
-
     // ---- integer powers
     double E200, E24, E20, E15, E10, E7p5, E6, E5;
     {
-        const double B = col[A_B600 * BLOCK];
+        const double B = x0[0];
         const double B2 = B * B, B3 = B2 * B, B5 = B2 * B3, B10 = B5 * B5, B20 = B10 * B10, B40 = B20 * B20;
         const double B30 = B20 * B10, B60 = B30 * B30;
         E200 = B3; E24 = B20 * B5; E20 = B30; E15 = B40; E10 = B60; E7p5 = B40 * B40; E6 = B60 * B40; E5 = B60 * B60;
     }
-    const double E14 = col[A_E14 * BLOCK], E7 = E14 * E14;
+    const double E14 = x0[1], E7 = E14 * E14;
     double W13, W18, W20;
     {
-        const double W = col[A_W * BLOCK];
+        const double W = x0[2];
         const double W2 = W * W, W4 = W2 * W2, W8 = W4 * W4, W16 = W8 * W8;
         W13 = W8 * W4 * W; W18 = W16 * W2; W20 = W18 * W2;
     }
     double Gf, Gf2;   // exp(-(v+27)^2/225), exp(-(v+27)^2/240)
     {
-        const double b = col[A_G27 * BLOCK];
+        const double b = x1[3];
         const double b2 = b * b, b4 = b2 * b2, b8 = b4 * b4;
         Gf = b8 * b8; Gf2 = (b8 * b4) * (b2 * b);
     }
@@ -269,7 +217,7 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double INa = CK(GNa) * gNa * (v - ENa);
     double ICaL;
     {
-        const double ex = col[A_CAL * BLOCK];
+        const double ex = x0[3];
         // x/(e^x - 1), with the series 1 - x/2 inside |x| < 1e-7 (reading B6)
         const double xo = (fabs(xcal) < 1e-7) ? fma(-0.5, xcal, 1.0) : xcal * ep_rcp(ex - 1.0);
         ICaL = CK(GCaL * 2.0 * F) * gCaL * xo * fma(0.25 * CaSS, ex, -Cao);
@@ -281,7 +229,7 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double IKs = GKs * gKs * (v - EKs);
     double IK1;
     {
-        const double q = col[A_K1Q * BLOCK], Q = col[A_K1Q2 * BLOCK];
+        const double q = x1[1], Q = x1[2];
         const double Q2 = Q * Q, Q3 = Q2 * Q, Q5 = Q2 * Q3, Q10 = Q5 * Q5, Q25 = Q10 * Q10 * Q5;
         const double t1 = fma(CK(0.1), Q25, CK(0.1));                                       // 0.1 (1 + e^{-0.5u}) Q^25
         const double t2 = fma(CK(EM1), Q5, 3.0 * q) * fma(CK(EM12), Q3, 1.0) * Q25;         // (3q + e^{0.1(u-10)})(1 + e^{0.06(u-200)}) Q^25
@@ -293,7 +241,7 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     const double INaK = CK(PNaK * Ko / (Ko + KmK)) * Nai * W20
                         * ep_rcp((Nai + KmNa) * fma(CK(0.1245), W18, W20 + CK(0.0353)));
     const double IpCa = CK(GpCa) * Cai * ep_rcp(CK(KpCa) + Cai);
-    const double IpK = CK(GpK) * u * ep_rcp(1.0 + col[A_PK * BLOCK]);
+    const double IpK = CK(GpK) * u * ep_rcp(1.0 + x1[0]);
     const double IbNa = CK(GbNa) * (v - ENa);
     const double IbCa = CK(GbCa) * (v - ECa);
     const double iion = INa + ICaL + Ito + IKr + IKs + IK1 + INaCa + INaK + IpCa + IpK + IbNa + IbCa;
@@ -342,80 +290,117 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
         ycol[Y_KI * stride] = fma(dt, w[5] - istim * CK(Cap / (Vc * F)), Ki);      // reading B8
     }
 
-    // ---- gates: steady states and rates 1/tau, each as one rational function
-    double inf[N_RLB], rate[N_RLB];   // index g = state index - 1
-    {   // m: tau = s(-60-v;5) [0.1 s(v+35;5) + 0.1 s(v-50;200)],  s(z) = 1/(1+e^z)
-        const double sm = ep_rcp(1.0 + col[A_M * BLOCK]);
-        inf[0] = sm * sm;
-        const double P = fma(CK(E7C), E5, 1.0), Q = fma(CK(EM025), E200, 1.0);
-        rate[0] = (E5 + CK(EM12)) * P * Q * ep_rcp(CK(0.1) * E5 * (P + Q));
-    }
-    {   // h, j share the steady state
-        const double sh = ep_rcp(1.0 + col[A_H * BLOCK]);
-        inf[1] = inf[2] = sh * sh;
-        const double s0 = col[(A_HJ0 + 0) * BLOCK], s1 = col[(A_HJ0 + 1) * BLOCK];
-        if (hi) {
-            rate[1] = CK(0.77 / 0.13) * ep_rcp(1.0 + s0);
-            rate[2] = CK(0.6) * s1 * E10 * ep_rcp(E10 + CK(EM32));
-        } else {
-            const double s2 = col[(A_HJ2 + 0) * BLOCK], s3 = col[(A_HJ2 + 1) * BLOCK], s4 = col[(A_HJ2 + 2) * BLOCK],
-                         s5 = col[(A_HJ2 + 3) * BLOCK], s6 = col[(A_HJ2 + 4) * BLOCK], s7 = col[(A_HJ2 + 5) * BLOCK];
-            rate[1] = fma(CK(0.057), s0, fma(CK(2.7), s1, 3.1e5 * s2));
-            const double N1 = fma(-2.5428e4, s3, CK(-6.948e-6) * s4) * (vgs + CK(37.78)), D1 = 1.0 + s5;
-            const double N2 = CK(0.02424) * s6, D2 = 1.0 + s7;
-            rate[2] = fma(N1, D2, N2 * D1) * ep_rcp(D1 * D2);
-        }
-    }
-    {   // xr1, xr2, xs
-        inf[3] = E7 * ep_rcp(E7 + CK(EM26_7));
-        rate[3] = (E10 + CK(EM45)) * (1.0 + col[A_XR1 * BLOCK]) * ep_rcp(2700.0 * E10);
-        inf[4] = ep_rcp(fma(CK(E88_24), E24, 1.0));
-        rate[4] = (E20 + CK(EM3)) * fma(CK(EM3), E20, 1.0) * ep_rcp(CK(3.36) * E20);
-        inf[5] = E14 * ep_rcp(E14 + CK(EM5_14));
-        const double t = ep_rsqrt((E6 + CK(E5_6)) * E6) * E6;          // 1/sqrt(1 + e^{(5-v)/6})
-        const double P15 = fma(CK(EM35_15), E15, 1.0);
-        rate[5] = P15 * ep_rcp(fma(1400.0, t, 80.0 * P15));
-    }
-    {   // r, s (reading B5: endo has its own s curves)
-        inf[6] = E6 * ep_rcp(E6 + CK(E20_6));
-        rate[6] = ep_rcp(fma(9.5, col[A_GR * BLOCK], CK(0.8)));
-        const double Gs = col[A_GS * BLOCK];
-        if (type == 0) {
-            inf[7] = ep_rcp(fma(CK(E56), E5, 1.0));
-            rate[7] = ep_rcp(fma(1000.0, Gs, 8.0));
-        } else {
-            inf[7] = ep_rcp(fma(CK(E4), E5, 1.0));
-            const double P = fma(CK(EM4), E5, 1.0);
-            rate[7] = P * ep_rcp(fma(fma(85.0, Gs, 3.0), P, 5.0));
-        }
-    }
-    {   // d, f, f2
-        inf[8] = E7p5 * ep_rcp(E7p5 + CK(EM8_75));
-        const double D = 1.0 + col[A_D * BLOCK], P5 = fma(CK(E1), E5, 1.0), Q20 = E20 + CK(E25);
-        rate[8] = D * P5 * Q20 * ep_rcp(fma(fma(0.25, D, CK(1.4)) * CK(1.4), Q20, E20 * D * P5));
-        const double Qa = E10 + CK(E13), Qb = fma(CK(E3), E10, 1.0), Qc = E10 + CK(E25);
-        inf[9] = ep_rcp(fma(CK(E20_7), E7, 1.0));
-        rate[9] = Qa * Qb * ep_rcp(fma(fma(1102.5, Gf, 20.0), Qa * Qb, fma(200.0 * E10, Qb, 180.0 * Qa)));
-        inf[10] = fma(CK(0.67), ep_rcp(fma(CK(E5C), E7, 1.0)), CK(0.33));
-        rate[10] = Qc * Qb * ep_rcp(fma(562.0 * Gf2, Qc * Qb, fma(31.0 * E10, Qb, 80.0 * Qc)));
-    }
-    // ---- batch 3: Rush-Larsen
-    // exponents and steady states stay in registers: three unrolled groups, only the parked gate values come from shared memory
+    // one Rush-Larsen group: y <- inf + (y_old - inf) 2^e for four gates (gate index g = state row - 1; g < 0: pad)
+    auto rush_larsen4 = [&](double (&e)[EXP_W], const double (&in)[EXP_W], int g0, int g1, int g2, int g3) {
+        const int gi[EXP_W] = {g0, g1, g2, g3};
+        double yo[EXP_W];
 #pragma unroll
-    for (int g0 = 0; g0 < N_EXPB; g0 += EXP_W) {
-        double e[EXP_W], yo[EXP_W];
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) {
-            const int g = g0 + j;
-            e[j] = (g < N_RLB) ? ((g <= 3) ? fmax(-dtl * rate[g], -1000.0) : -dtl * rate[g]) : 0.0;
-            yo[j] = col[(G_OLD0 + g) * BLOCK];
-        }
+        for (int j = 0; j < EXP_W; ++j) yo[j] = col[(G_OLD0 + (gi[j] < 0 ? 0 : gi[j])) * BLOCK];
         ep_exp2_wide<EXP_W>(e);
 #pragma unroll
-        for (int j = 0; j < EXP_W; ++j) {
-            const int g = g0 + j;
-            if (g < N_RLB) ycol[(1 + g) * stride] = fma(yo[j] - inf[g], e[j], inf[g]);
+        for (int j = 0; j < EXP_W; ++j)
+            if (gi[j] >= 0) ycol[(1 + gi[j]) * stride] = fma(yo[j] - in[j], e[j], in[j]);
+    };
+    // ---- group 2: m, h_inf, xr1, d; gates m, xr1, xr2, d
+    {
+        double x2[EXP_W] = {fma(vgs, CK(-L2E / 9.03), CK(-56.86 * L2E / 9.03)), fma(vgs, CK(L2E / 7.43), CK(71.55 * L2E / 7.43)),
+                            fma(vgs, CK(L2E / 11.5), CK(30.0 * L2E / 11.5)), fma(vgs, CK(-L2E / 13.0), CK(-35.0 * L2E / 13.0))};
+        ep_exp2_wide<EXP_W>(x2);
+        double in[EXP_W], e[EXP_W];
+        {   // m: tau = s(-60-v;5) [0.1 s(v+35;5) + 0.1 s(v-50;200)],  s(z) = 1/(1+e^z)
+            const double sm = ep_rcp(1.0 + x2[0]);
+            in[0] = sm * sm;
+            const double P = fma(CK(E7C), E5, 1.0), Q = fma(CK(EM025), E200, 1.0);
+            e[0] = fmax(-dtl * ((E5 + CK(EM12)) * P * Q * ep_rcp(CK(0.1) * E5 * (P + Q))), -1000.0);
         }
+        in[1] = E7 * ep_rcp(E7 + CK(EM26_7));                                                          // xr1
+        e[1] = fmax(-dtl * ((E10 + CK(EM45)) * (1.0 + x2[2]) * ep_rcp(2700.0 * E10)), -1000.0);
+        in[2] = ep_rcp(fma(CK(E88_24), E24, 1.0));                                                     // xr2
+        e[2] = -dtl * ((E20 + CK(EM3)) * fma(CK(EM3), E20, 1.0) * ep_rcp(CK(3.36) * E20));
+        {   // d
+            in[3] = E7p5 * ep_rcp(E7p5 + CK(EM8_75));
+            const double D = 1.0 + x2[3], P5 = fma(CK(E1), E5, 1.0), Q20 = E20 + CK(E25);
+            e[3] = -dtl * (D * P5 * Q20 * ep_rcp(fma(fma(0.25, D, CK(1.4)) * CK(1.4), Q20, E20 * D * P5)));
+        }
+        h_exp = x2[1];
+        rush_larsen4(e, in, Y_M - 1, Y_XR1 - 1, Y_XR2 - 1, Y_D - 1);
+    }
+    // ---- group 3: the Gaussians of tau_r and tau_s, exp(-dt/tau) of fCass and Rbar; gates xs, r, s, f
+    {
+        double x3[EXP_W] = {(vgs + 40.0) * (vgs + 40.0) * CK(-L2E / 1800.0),
+                            (type == 0) ? (vgs + 67.0) * (vgs + 67.0) * CK(-L2E / 1000.0)
+                                        : (vgs + 45.0) * (vgs + 45.0) * CK(-L2E / 320.0),
+                            -dtl * ep_rcp(fma(80.0, qf, 2.0)),              // tau_fCass >= 2 ms
+                            fmax(-dtl * Rbar_rate, -1000.0)};               // rate grows with Ca_SS: keep the clamp
+        ep_exp2_wide<EXP_W>(x3);
+        ycol[Y_FCASS * stride] = fma(fCass - fCass_inf, x3[2], fCass_inf);   // Rush-Larsen
+        ycol[Y_RBAR * stride] = fma(Rbar - Rbar_inf, x3[3], Rbar_inf);
+        double in[EXP_W], e[EXP_W];
+        {   // xs
+            in[0] = E14 * ep_rcp(E14 + CK(EM5_14));
+            const double t = ep_rsqrt((E6 + CK(E5_6)) * E6) * E6;          // 1/sqrt(1 + e^{(5-v)/6})
+            const double P15 = fma(CK(EM35_15), E15, 1.0);
+            e[0] = -dtl * (P15 * ep_rcp(fma(1400.0, t, 80.0 * P15)));
+        }
+        in[1] = E6 * ep_rcp(E6 + CK(E20_6));                                // r
+        e[1] = -dtl * ep_rcp(fma(9.5, x3[0], CK(0.8)));
+        if (type == 0) {                                                    // s (reading B5: endo has its own curves)
+            in[2] = ep_rcp(fma(CK(E56), E5, 1.0));
+            e[2] = -dtl * ep_rcp(fma(1000.0, x3[1], 8.0));
+        } else {
+            in[2] = ep_rcp(fma(CK(E4), E5, 1.0));
+            const double P = fma(CK(EM4), E5, 1.0);
+            e[2] = -dtl * (P * ep_rcp(fma(fma(85.0, x3[1], 3.0), P, 5.0)));
+        }
+        {   // f
+            const double Qa = E10 + CK(E13), Qb = fma(CK(E3), E10, 1.0);
+            in[3] = ep_rcp(fma(CK(E20_7), E7, 1.0));
+            e[3] = -dtl * (Qa * Qb * ep_rcp(fma(fma(1102.5, Gf, 20.0), Qa * Qb, fma(200.0 * E10, Qb, 180.0 * Qa))));
+        }
+        rush_larsen4(e, in, Y_XS - 1, Y_R - 1, Y_S - 1, Y_F - 1);
+    }
+    // ---- groups 4, 5: the h / j rate exponentials (the four that only the low-voltage branch needs are skipped when every
+    // cell of the warp is above -40 mV: warp-uniform); gates h, j, f2
+    {
+        double x4[EXP_W], x5[EXP_W] = {1.0, 1.0, 1.0, 1.0};
+        const bool all_hi = __all_sync(__activemask(), hi);
+        if (hi) {
+            x4[0] = fma(vgs, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
+            x4[1] = vgs * CK(0.057 * L2E);
+            x4[2] = 0.0; x4[3] = 0.0;
+        } else {
+            x4[0] = fma(vgs, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));
+            x4[1] = vgs * CK(0.079 * L2E);
+            x4[2] = vgs * CK(0.3485 * L2E);
+            x4[3] = vgs * CK(0.2444 * L2E);
+        }
+        ep_exp2_wide<EXP_W>(x4);
+        if (!all_hi) {
+            x5[0] = vgs * CK(-0.04391 * L2E);
+            x5[1] = fma(vgs, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
+            x5[2] = vgs * CK(-0.01052 * L2E);
+            x5[3] = fma(vgs, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
+            ep_exp2_wide<EXP_W>(x5);
+        }
+        double in[EXP_W], e[EXP_W];
+        const double sh = ep_rcp(1.0 + h_exp);
+        in[0] = in[1] = sh * sh;                                            // h, j share the steady state
+        if (hi) {
+            e[0] = fmax(-dtl * (CK(0.77 / 0.13) * ep_rcp(1.0 + x4[0])), -1000.0);
+            e[1] = fmax(-dtl * (CK(0.6) * x4[1] * E10 * ep_rcp(E10 + CK(EM32))), -1000.0);
+        } else {
+            e[0] = fmax(-dtl * fma(CK(0.057), x4[0], fma(CK(2.7), x4[1], 3.1e5 * x4[2])), -1000.0);
+            const double N1 = fma(-2.5428e4, x4[3], CK(-6.948e-6) * x5[0]) * (vgs + CK(37.78)), D1 = 1.0 + x5[1];
+            const double N2 = CK(0.02424) * x5[2], D2 = 1.0 + x5[3];
+            e[1] = fmax(-dtl * (fma(N1, D2, N2 * D1) * ep_rcp(D1 * D2)), -1000.0);
+        }
+        {   // f2
+            const double Qb = fma(CK(E3), E10, 1.0), Qc = E10 + CK(E25);
+            in[2] = fma(CK(0.67), ep_rcp(fma(CK(E5C), E7, 1.0)), CK(0.33));
+            e[2] = -dtl * (Qc * Qb * ep_rcp(fma(562.0 * Gf2, Qc * Qb, fma(31.0 * E10, Qb, 80.0 * Qc))));
+        }
+        in[3] = 0.0; e[3] = 0.0;
+        rush_larsen4(e, in, Y_H - 1, Y_J - 1, Y_F2 - 1, -1);
     }
     return v_new;
 }
