@@ -46,18 +46,11 @@ constexpr double E1513 = 4.540331377371345;        // e^(1.513) = e^(-0.1 (32 - 
 constexpr double SIGMA = 1.0009103049457282;       // (e^(Nao/67.3) - 1)/7
 constexpr double EM200 = 1.3838965267367376e-87;   // e^(-200) = e^(-(3.4175e-13 - 6.835e-14)/13.67e-16)
 
-// shared-memory slots
-constexpr int A_E17 = 0, A_W = 1, A_X1 = 2, A_BM = 3, A_K1 = 4, A_OA1 = 5, A_OA2 = 6, A_OAI = 7, A_UAI = 8, A_OI1 = 9,
-              A_OI2 = 10, A_OII = 11, A_UI1 = 12, A_UI2 = 13, A_UII = 14, A_KUR = 15, A_KR = 16, A_E5M = 17, A_XB = 18,
-              A_XRI = 19, A_XD = 20, A_XSI = 21, A_DX = 22, A_DI = 23, A_FG = 24, A_FI = 25, A_HJ0 = 26, A_TFCA = 34,
-              A_TU = 35, N_EXPA = 36;
-constexpr int EXP_W = 4;
-constexpr int N_RLB = 10;    // gates of the rolled Rush-Larsen loop: oa oi ua ui xr xs d f (rows 4..11), v w (rows 14, 15)
-constexpr int N_EXPB = 12;   // their arguments + 2 pads, slots 0..11
-constexpr int B_INF0 = 12;   // steady states, slots 12..21
-constexpr int G_OLD0 = 36;   // gate values at t^n of those ten, slots 36..45
-constexpr int N_SLOTS = 48;   // 46, 47: pads read (not used) by the last trip of the Rush-Larsen loop
-static_assert(N_EXPA % EXP_W == 0 && N_EXPB % EXP_W == 0 && B_INF0 + N_RLB <= G_OLD0 && N_EXPA <= G_OLD0, "slot layout");
+// shared-memory slots (one column of BLOCK doubles per thread): the ten gate values at t^n of the Rush-Larsen list
+// 0 oa, 1 oi, 2 ua, 3 ui, 4 xr, 5 xs, 6 d, 7 f (rows C_OA + g), 8 v, 9 w, parked by asynchronous copies
+constexpr int EXP_W = 4;     // exponentials evaluated side by side
+constexpr int G_OLD0 = 0;
+constexpr int N_SLOTS = 10;
 
 // phi(x) = x/(e^x - 1) given e^x (reading B11)
 __device__ __forceinline__ double phi(double x, double ex) {
@@ -75,8 +68,8 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
     const double dtl = dt * L2E;                    // Rush-Larsen exponents in base-2 units (the primitive is 2^x)
     const double Nai = ycol[C_NAI * stride], Ki = ycol[C_KI * stride], Cai = ycol[C_CAI * stride],
                  Caup = ycol[C_CAUP * stride], Carel = ycol[C_CAREL * stride];
-    // The ten gates of the rolled Rush-Larsen loop are copied into shared memory asynchronously (no registers held); they
-    // and m h j fCa u are first touched after the first exponential batch, which hides their latency.
+    // The ten gates of the Rush-Larsen list are copied into shared memory asynchronously (no registers held); they and
+    // m h j fCa u are first touched after the first two exponential groups, which hides their latency.
 #pragma unroll
     for (int k = 0; k < 8; ++k) ep_cp_async8(col + (G_OLD0 + k) * BLOCK, ycol + (C_OA + k) * stride);
     ep_cp_async8(col + (G_OLD0 + 8) * BLOCK, ycol + C_VG * stride);
@@ -93,76 +86,21 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
     const double ECa = CK(0.5 * RTF) * (CK(LN_CAO) - lg[2]);
     const bool hi = (v >= -40.0);   // reading B7
 
-    // ---- batch 2: voltage-dependent exponentials (+ the two constant Rush-Larsen factors of fCa and u)
-    // (arguments in registers, only the results go to the slot array: see tp06_step)
-#ifdef EP_CRN_BATCH1_DIRECT
-    double a1[N_EXPA];
-#define ARG(k) a1[k]
-#else
-#define ARG(k) col[(k) * BLOCK]
-#endif
+    // ---- streaming form (see tp06_step): the 36 voltage-driven exponentials are evaluated in nine groups of EXP_W, each right
+    // before the quantities that consume it, so that arguments and results stay in registers; the slot array only parks the ten
+    // gate values of the Rush-Larsen list below (the stencil coefficients of this model stay in registers)
     const double x1 = fma(vg, -0.1, CK(-0.1 * 47.13));
     const double xb = fma(vg, CK(1.0 / 5.1237), CK(-3.3328 / 5.1237));
     const double xd = fma(vg, CK(1.0 / 9.0), CK(-19.9 / 9.0));
     const double dx = fma(vg, CK(-1.0 / 6.24), CK(-10.0 / 6.24));
-    ARG(A_E17) = vg * CK(L2E / 17.0);
-    ARG(A_W) = vg * CK(0.05 * FRT * L2E);
-    ARG(A_X1) = x1 * CK(L2E);
-    ARG(A_BM) = vg * CK(-L2E / 11.0);
-    ARG(A_K1) = fma(vg, CK(0.07 * L2E), CK(0.07 * 80.0 * L2E));
-    ARG(A_OA1) = fma(vg, CK(-L2E / 8.5), CK(-10.0 * L2E / 8.5));
-    ARG(A_OA2) = fma(vg, CK(-L2E / 59.0), CK(30.0 * L2E / 59.0));
-    ARG(A_OAI) = fma(vg, CK(-L2E / 17.54), CK(-20.47 * L2E / 17.54));
-    ARG(A_UAI) = fma(vg, CK(-L2E / 9.6), CK(-30.3 * L2E / 9.6));
-    ARG(A_OI1) = fma(vg, CK(L2E / 10.95), CK(113.7 * L2E / 10.95));
-    ARG(A_OI2) = fma(vg, CK(-L2E / 7.44), CK(-1.26 * L2E / 7.44));
-    ARG(A_OII) = fma(vg, CK(L2E / 5.3), CK(43.1 * L2E / 5.3));
-    ARG(A_UI1) = fma(vg, CK(-L2E / 28.0), CK(185.0 * L2E / 28.0));
-    ARG(A_UI2) = fma(vg, CK(L2E / 16.0), CK(-158.0 * L2E / 16.0));
-    ARG(A_UII) = fma(vg, CK(L2E / 27.48), CK(-99.45 * L2E / 27.48));
-    ARG(A_KUR) = fma(vg, CK(-L2E / 13.0), CK(15.0 * L2E / 13.0));
-    ARG(A_KR) = fma(vg, CK(L2E / 22.4), CK(15.0 * L2E / 22.4));
-    ARG(A_E5M) = vg * CK(-0.2 * L2E);
-    ARG(A_XB) = xb * CK(L2E);
-    ARG(A_XRI) = fma(vg, CK(-L2E / 6.5), CK(-14.1 * L2E / 6.5));
-    ARG(A_XD) = xd * CK(L2E);
-    ARG(A_XSI) = fma(vg, CK(-L2E / 12.7), CK(19.9 * L2E / 12.7));
-    ARG(A_DX) = dx * CK(L2E);
-    ARG(A_DI) = fma(vg, CK(-0.125 * L2E), CK(-1.25 * L2E));
-    ARG(A_FG) = (vg + 10.0) * (vg + 10.0) * CK(-0.0337 * 0.0337 * L2E);
-    ARG(A_FI) = fma(vg, CK(L2E / 6.9), CK(28.0 * L2E / 6.9));
-    if (hi) {
-        ARG((A_HJ0 + 0)) = fma(vg, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
-        ARG((A_HJ0 + 1)) = vg * CK(-2.535e-7 * L2E);
-#pragma unroll
-        for (int k = 2; k < 8; ++k) ARG((A_HJ0 + k)) = 0.0;
-    } else {
-        ARG((A_HJ0 + 0)) = fma(vg, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));
-        ARG((A_HJ0 + 1)) = vg * CK(0.079 * L2E);
-        ARG((A_HJ0 + 2)) = vg * CK(0.35 * L2E);
-        ARG((A_HJ0 + 3)) = vg * CK(0.2444 * L2E);
-        ARG((A_HJ0 + 4)) = vg * CK(-0.04391 * L2E);
-        ARG((A_HJ0 + 5)) = fma(vg, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
-        ARG((A_HJ0 + 6)) = vg * CK(-0.01052 * L2E);
-        ARG((A_HJ0 + 7)) = fma(vg, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
-    }
-    ARG(A_TFCA) = dtl * -0.5;     // tau_fCa = 2 ms
-    ARG(A_TU) = dtl * -0.125;     // tau_u = 8 ms
-#ifdef EP_CRN_BATCH1_DIRECT
-#pragma unroll
-    for (int s0 = 0; s0 < N_EXPA; s0 += EXP_W) {
-        double x[EXP_W];
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) x[j] = a1[s0 + j];
-        ep_exp2_wide<EXP_W>(x);
-#pragma unroll
-        for (int j = 0; j < EXP_W; ++j) col[(s0 + j) * BLOCK] = x[j];
-    }
-#else
-    ep_exp2_slots<N_EXPA, BLOCK, EXP_W>(col);
-#endif
-#undef ARG
-    const double dv_diff = finish_gather();   // the gathers have landed during the batch: 12 values -> 1
+    // group 0: e^{V/17}, e^{VF/20RT}, e^{-V/5}, e^{-0.1(V+47.13)}: shared by several gates / raised to powers
+    double x0[EXP_W] = {vg * CK(L2E / 17.0), vg * CK(0.05 * FRT * L2E), vg * CK(-0.2 * L2E), x1 * CK(L2E)};
+    ep_exp2_wide<EXP_W>(x0);
+    // group 1: I_K1, I_Kur, I_Kr rectifiers and beta_m
+    double xg1[EXP_W] = {fma(vg, CK(0.07 * L2E), CK(0.07 * 80.0 * L2E)), fma(vg, CK(-L2E / 13.0), CK(15.0 * L2E / 13.0)),
+                         fma(vg, CK(L2E / 22.4), CK(15.0 * L2E / 22.4)), vg * CK(-L2E / 11.0)};
+    ep_exp2_wide<EXP_W>(xg1);
+    const double dv_diff = finish_gather();   // the gathers have landed by now: 12 values -> 1
     const double istim = stimulus();          // late on purpose: see tp06_step
     ep_cp_async_wait();                       // so have the gate values: products for the currents
     double gto3, gkur3, xr, xs2, gcal, uvw;
@@ -178,10 +116,10 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
         uvw = (u * u) * g[8] * g[9];                 // u^2 v w
     }
 
-    const double e17 = col[A_E17 * BLOCK], e5m = col[A_E5M * BLOCK], e1 = col[A_X1 * BLOCK];
+    const double e17 = x0[0], e5m = x0[2], e1 = x0[3];
     double W13, W18, W20;
     {
-        const double W = col[A_W * BLOCK];
+        const double W = x0[1];
         const double W2 = W * W, W4 = W2 * W2, W8 = W4 * W4, W16 = W8 * W8;
         W13 = W8 * W4 * W; W18 = W16 * W2; W20 = W18 * W2;
     }
@@ -189,10 +127,10 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
     // ---- membrane currents
     const double uK = v - EK;
     const double INa = CK(gNa) * (m * m * m) * h * j * (v - ENa);
-    const double IK1 = CK(gK1) * uK * ep_rcp(1.0 + col[A_K1 * BLOCK]);
+    const double IK1 = CK(gK1) * uK * ep_rcp(1.0 + xg1[0]);
     const double Ito = CK(gto) * gto3 * uK;
-    const double IKur = fma(0.05, ep_rcp(1.0 + col[A_KUR * BLOCK]), 0.005) * gkur3 * uK;
-    const double IKr = CK(gKr) * xr * uK * ep_rcp(1.0 + col[A_KR * BLOCK]);
+    const double IKur = fma(0.05, ep_rcp(1.0 + xg1[1]), 0.005) * gkur3 * uK;
+    const double IKr = CK(gKr) * xr * uK * ep_rcp(1.0 + xg1[2]);
     const double IKs = CK(gKs) * xs2 * uK;
     const double ICaL = CK(gCaL) * gcal * (v - 65.0);
     const double rna = CK(KmNai) * ep_rcp(Nai);
@@ -231,27 +169,44 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
     }
     const double v_new = fma(dt, dv_diff - iion - istim, v);   // eq. (7)
 
-    // ---- Rush-Larsen group 1 (registers): E1 of the release gates rides with m, h, j in one 4-wide exp
-    double m_inf, h_inf, j_inf;
+    // ---- groups 2, 3: the h / j rate exponentials (the second group is skipped when every cell of the warp is above -40 mV);
+    // m, h, j and the release-gate exponential E1 = exp(-(Fn - 3.4175e-13)/13.67e-16) share one Rush-Larsen group
     double e4[4];
     {
+        double x2[EXP_W], x3[EXP_W] = {1.0, 1.0, 1.0, 1.0};
+        const bool all_hi = __all_sync(__activemask(), hi);
+        if (hi) {
+            x2[0] = fma(vg, CK(-L2E / 11.1), CK(-10.66 * L2E / 11.1));
+            x2[1] = vg * CK(-2.535e-7 * L2E);
+            x2[2] = 0.0; x2[3] = 0.0;
+        } else {
+            x2[0] = fma(vg, CK(-L2E / 6.8), CK(-80.0 * L2E / 6.8));
+            x2[1] = vg * CK(0.079 * L2E);
+            x2[2] = vg * CK(0.35 * L2E);
+            x2[3] = vg * CK(0.2444 * L2E);
+        }
+        ep_exp2_wide<EXP_W>(x2);
+        if (!all_hi) {
+            x3[0] = vg * CK(-0.04391 * L2E);
+            x3[1] = fma(vg, CK(0.311 * L2E), CK(0.311 * 79.23 * L2E));
+            x3[2] = vg * CK(-0.01052 * L2E);
+            x3[3] = fma(vg, CK(-0.1378 * L2E), CK(-0.1378 * 40.14 * L2E));
+            ep_exp2_wide<EXP_W>(x3);
+        }
         const double am = 3.2 * phi(x1, e1);                            // 0.32 (V+47.13)/(1 - exp(-0.1 (V+47.13)))
-        const double rm = fma(CK(0.08), col[A_BM * BLOCK], am);
-        m_inf = am * ep_rcp(rm);
-        double rh, rj;
-        const double s0 = col[(A_HJ0 + 0) * BLOCK], s1 = col[(A_HJ0 + 1) * BLOCK];
+        const double rm = fma(CK(0.08), xg1[3], am);
+        const double m_inf = am * ep_rcp(rm);
+        double rh, rj, h_inf, j_inf;
         if (hi) {
             h_inf = 0.0; j_inf = 0.0;
-            rh = ep_rcp(0.13 * (1.0 + s0));
-            rj = CK(0.3) * s1 * ep_rcp(fma(CK(E1513), e1, 1.0));        // exp(-0.1 (V+32)) = e^{1.513} e^{x1}
+            rh = ep_rcp(0.13 * (1.0 + x2[0]));
+            rj = CK(0.3) * x2[1] * ep_rcp(fma(CK(E1513), e1, 1.0));     // exp(-0.1 (V+32)) = e^{1.513} e^{x1}
         } else {
-            const double s2 = col[(A_HJ0 + 2) * BLOCK], s3 = col[(A_HJ0 + 3) * BLOCK], s4 = col[(A_HJ0 + 4) * BLOCK],
-                         s5 = col[(A_HJ0 + 5) * BLOCK], s6 = col[(A_HJ0 + 6) * BLOCK], s7 = col[(A_HJ0 + 7) * BLOCK];
-            const double ah = CK(0.135) * s0;
-            rh = ah + fma(CK(3.56), s1, 3.1e5 * s2);
+            const double ah = CK(0.135) * x2[0];
+            rh = ah + fma(CK(3.56), x2[1], 3.1e5 * x2[2]);
             h_inf = ah * ep_rcp(rh);
-            const double N1 = fma(-127140.0, s3, CK(-3.474e-5) * s4) * (vg + CK(37.78)), D1 = 1.0 + s5;
-            const double N2 = CK(0.1212) * s6, D2 = 1.0 + s7;
+            const double N1 = fma(-127140.0, x2[3], CK(-3.474e-5) * x3[0]) * (vg + CK(37.78)), D1 = 1.0 + x3[1];
+            const double N2 = CK(0.1212) * x3[2], D2 = 1.0 + x3[3];
             const double num = fma(N1, D2, N2 * D1);
             rj = num * ep_rcp(D1 * D2);
             j_inf = N1 * D2 * ep_rcp(num);
@@ -261,86 +216,107 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
         e4[1] = fmax(-dtl * rm, -1000.0);
         e4[2] = fmax(-dtl * rh, -1000.0);
         e4[3] = fmax(-dtl * rj, -1000.0);
+        ep_exp2_wide<4>(e4);
+        ycol[C_M * stride] = fma(m - m_inf, e4[1], m_inf);              // Rush-Larsen
+        ycol[C_H * stride] = fma(h - h_inf, e4[2], h_inf);
+        ycol[C_J * stride] = fma(j - j_inf, e4[3], j_inf);
     }
-    ep_exp2_wide<4>(e4);
-    ycol[C_M * stride] = fma(m - m_inf, e4[1], m_inf);
-    ycol[C_H * stride] = fma(h - h_inf, e4[2], h_inf);
-    ycol[C_J * stride] = fma(j - j_inf, e4[3], j_inf);
-    {   // fCa (tau = 2 ms) and u (tau = 8 ms): constant Rush-Larsen factors from batch 2
-        const double fCa_inf = CK(0.00035) * ep_rcp(CK(0.00035) + Cai);
-        ycol[C_FCA * stride] = fma(fCa - fCa_inf, col[A_TFCA * BLOCK], fCa_inf);
-        const double u_inf = ep_rcp(1.0 + e4[0]);
-        ycol[C_U * stride] = fma(u - u_inf, col[A_TU * BLOCK], u_inf);
-    }
-
-    // ---- Rush-Larsen group 2 (rolled loop): oa oi ua ui xr xs d f v w
-    double inf[N_RLB], rate[N_RLB];
-    {   // oa, ua share alpha + beta; K_Q10 = 3 multiplies the rates
-        const double A = col[A_OA1 * BLOCK] + col[A_OA2 * BLOCK], Bq = fma(CK(E82_17), e17, 2.5);
-        const double r = 1.95 * (A + Bq) * ep_rcp(A * Bq);
-        inf[0] = ep_rcp(1.0 + col[A_OAI * BLOCK]); rate[0] = r;
-        inf[2] = ep_rcp(1.0 + col[A_UAI * BLOCK]); rate[2] = r;
-    }
-    {   // oi
-        const double P = CK(18.53) + col[A_OI1 * BLOCK], Q = CK(35.56) + col[A_OI2 * BLOCK];
-        inf[1] = ep_rcp(1.0 + col[A_OII * BLOCK]); rate[1] = 3.0 * (P + Q) * ep_rcp(P * Q);
-    }
-    {   // ui
-        const double P = 21.0 + col[A_UI1 * BLOCK];
-        inf[3] = ep_rcp(1.0 + col[A_UII * BLOCK]); rate[3] = 3.0 * fma(col[A_UI2 * BLOCK], P, 1.0) * ep_rcp(P);
-    }
-    {   // xr: alpha = 0.0015 phi(-(V+14.1)/5), beta = 7.3898e-5 * 5.1237 phi((V-3.3328)/5.1237)
-        const double xa = fma(vg, CK(-0.2), CK(-14.1 / 5.0));
-        inf[4] = ep_rcp(1.0 + col[A_XRI * BLOCK]);
-        rate[4] = fma(CK(0.0015), phi(xa, CK(EM141_5) * e5m), CK(7.3898e-5 * 5.1237) * phi(xb, col[A_XB * BLOCK]));
-    }
-    {   // xs: alpha = 6.8e-4 phi(-(V-19.9)/17), beta = 3.15e-4 phi((V-19.9)/9); tau = 0.5/(alpha+beta)
-        const double xc = fma(vg, CK(-1.0 / 17.0), CK(19.9 / 17.0));
-        const double series = fma(xc, fma(xc, 1.0 / 12.0, -0.5), 1.0);
-        const double pa = (fabs(xc) < 1e-4) ? series : xc * e17 * ep_rcp(CK(E199_17) - e17);   // e^{xc} = e^{19.9/17}/e17
-        inf[5] = ep_rsqrt(1.0 + col[A_XSI * BLOCK]);
-        rate[5] = 2.0 * fma(CK(6.8e-4), pa, CK(3.15e-4) * phi(xd, col[A_XD * BLOCK]));
-    }
-    {   // d: tau = 1/(0.035 * 6.24 phi(x)(1 + e^x)), x = -(V+10)/6.24
-        const double ex = col[A_DX * BLOCK];
-        inf[6] = ep_rcp(1.0 + col[A_DI * BLOCK]);
-        rate[6] = CK(0.035 * 6.24) * phi(dx, ex) * (1.0 + ex);
-    }
-    {   // f: tau = 9/(0.0197 G + 0.02)
-        inf[7] = ep_rcp(1.0 + col[A_FI * BLOCK]);
-        rate[7] = fma(CK(0.0197 / 9.0), col[A_FG * BLOCK], CK(0.02 / 9.0));
-    }
-    {   // v: inf = 1 - 1/(1+E2), tau = 1.91 + 2.09/(1+E1), E2 = E1 e^{-200}
-        const double E2 = e4[0] * CK(EM200);
-        inf[8] = E2 * ep_rcp(1.0 + E2);
-        rate[8] = ep_rcp(fma(CK(2.09), ep_rcp(1.0 + e4[0]), CK(1.91)));
-    }
-    {   // w: tau = 1.2/(phi(x)(1 + 0.3 e^x)), x = -(V-7.9)/5; inf = 1 - 1/(1 + e^{-(V-40)/17})
-        const double xw = fma(vg, CK(-0.2), CK(7.9 / 5.0));
-        const double ex = CK(E79_5) * e5m;
-        inf[9] = CK(E40_17) * ep_rcp(e17 + CK(E40_17));
-        rate[9] = CK(1.0 / 1.2) * phi(xw, ex) * fma(CK(0.3), ex, 1.0);
-    }
-    // Rush-Larsen of the ten gates of this list: exponents and steady states in registers (three unrolled groups), only the
-    // parked gate values come from shared memory (see tp06_step)
+    // one Rush-Larsen group of the parked list (0 oa, 1 oi, 2 ua, 3 ui, 4 xr, 5 xs, 6 d, 7 f -> rows C_OA + g; 8 v, 9 w; < 0: pad)
+    auto rush_larsen4 = [&](double (&e)[EXP_W], const double (&in)[EXP_W], int g0, int g1, int g2, int g3) {
+        const int gi[EXP_W] = {g0, g1, g2, g3};
+        double yo[EXP_W];
 #pragma unroll
-    for (int g0 = 0; g0 < N_EXPB; g0 += EXP_W) {
-        double e[EXP_W], yo[EXP_W];
+        for (int k = 0; k < EXP_W; ++k) yo[k] = col[(G_OLD0 + (gi[k] < 0 ? 0 : gi[k])) * BLOCK];
 #pragma unroll
-        for (int j = 0; j < EXP_W; ++j) {
-            const int g = g0 + j;
-            e[j] = (g < N_RLB) ? fmax(-dtl * rate[g], -1000.0) : 0.0;
-            yo[j] = col[(G_OLD0 + g) * BLOCK];        // slots G_OLD0 + 10, 11 are pads: read, not used
-        }
+        for (int k = 0; k < EXP_W; ++k) e[k] = fmax(-dtl * e[k], -1000.0);      // e comes in as the rate 1/tau
         ep_exp2_wide<EXP_W>(e);
 #pragma unroll
-        for (int j = 0; j < EXP_W; ++j) {
-            const int g = g0 + j;
-            if (g < N_RLB) {
-                const int row = (g < 8) ? C_OA + g : C_VG + (g - 8);
-                ycol[row * stride] = fma(yo[j] - inf[g], e[j], inf[g]);
-            }
+        for (int k = 0; k < EXP_W; ++k)
+            if (gi[k] >= 0) ycol[((gi[k] < 8) ? C_OA + gi[k] : C_VG + (gi[k] - 8)) * stride] = fma(yo[k] - in[k], e[k], in[k]);
+    };
+    // ---- group 4: the constant Rush-Larsen factors of fCa (tau = 2 ms) and u (tau = 8 ms), alpha of oa / ua
+    double oaA;
+    {
+        double x4[EXP_W] = {dtl * -0.5, dtl * -0.125, fma(vg, CK(-L2E / 8.5), CK(-10.0 * L2E / 8.5)),
+                            fma(vg, CK(-L2E / 59.0), CK(30.0 * L2E / 59.0))};
+        ep_exp2_wide<EXP_W>(x4);
+        const double fCa_inf = CK(0.00035) * ep_rcp(CK(0.00035) + Cai);
+        ycol[C_FCA * stride] = fma(fCa - fCa_inf, x4[0], fCa_inf);
+        const double u_inf = ep_rcp(1.0 + e4[0]);
+        ycol[C_U * stride] = fma(u - u_inf, x4[1], u_inf);
+        oaA = x4[2] + x4[3];
+    }
+    // ---- groups 5, 6: oa, ua, oi, ui (K_Q10 = 3 multiplies the rates)
+    {
+        double x5[EXP_W] = {fma(vg, CK(-L2E / 17.54), CK(-20.47 * L2E / 17.54)), fma(vg, CK(-L2E / 9.6), CK(-30.3 * L2E / 9.6)),
+                            fma(vg, CK(L2E / 10.95), CK(113.7 * L2E / 10.95)), fma(vg, CK(-L2E / 7.44), CK(-1.26 * L2E / 7.44))};
+        ep_exp2_wide<EXP_W>(x5);
+        double x6[EXP_W] = {fma(vg, CK(L2E / 5.3), CK(43.1 * L2E / 5.3)), fma(vg, CK(-L2E / 28.0), CK(185.0 * L2E / 28.0)),
+                            fma(vg, CK(L2E / 16.0), CK(-158.0 * L2E / 16.0)), fma(vg, CK(L2E / 27.48), CK(-99.45 * L2E / 27.48))};
+        ep_exp2_wide<EXP_W>(x6);
+        double in[EXP_W], r[EXP_W];
+        {   // oa, ua share alpha + beta
+            const double Bq = fma(CK(E82_17), e17, 2.5);
+            const double rr = 1.95 * (oaA + Bq) * ep_rcp(oaA * Bq);
+            in[0] = ep_rcp(1.0 + x5[0]); r[0] = rr;
+            in[2] = ep_rcp(1.0 + x5[1]); r[2] = rr;
         }
+        {   // oi
+            const double P = CK(18.53) + x5[2], Q = CK(35.56) + x5[3];
+            in[1] = ep_rcp(1.0 + x6[0]); r[1] = 3.0 * (P + Q) * ep_rcp(P * Q);
+        }
+        {   // ui
+            const double P = 21.0 + x6[1];
+            in[3] = ep_rcp(1.0 + x6[3]); r[3] = 3.0 * fma(x6[2], P, 1.0) * ep_rcp(P);
+        }
+        rush_larsen4(r, in, 0, 1, 2, 3);
+    }
+    // ---- groups 7, 8: xr, xs, d, f
+    {
+        double x7[EXP_W] = {fma(vg, CK(-L2E / 6.5), CK(-14.1 * L2E / 6.5)), xb * CK(L2E),
+                            fma(vg, CK(-L2E / 12.7), CK(19.9 * L2E / 12.7)), xd * CK(L2E)};
+        ep_exp2_wide<EXP_W>(x7);
+        double x8[EXP_W] = {dx * CK(L2E), fma(vg, CK(-0.125 * L2E), CK(-1.25 * L2E)),
+                            (vg + 10.0) * (vg + 10.0) * CK(-0.0337 * 0.0337 * L2E), fma(vg, CK(L2E / 6.9), CK(28.0 * L2E / 6.9))};
+        ep_exp2_wide<EXP_W>(x8);
+        double in[EXP_W], r[EXP_W];
+        {   // xr: alpha = 0.0015 phi(-(V+14.1)/5), beta = 7.3898e-5 * 5.1237 phi((V-3.3328)/5.1237)
+            const double xa = fma(vg, CK(-0.2), CK(-14.1 / 5.0));
+            in[0] = ep_rcp(1.0 + x7[0]);
+            r[0] = fma(CK(0.0015), phi(xa, CK(EM141_5) * e5m), CK(7.3898e-5 * 5.1237) * phi(xb, x7[1]));
+        }
+        {   // xs: alpha = 6.8e-4 phi(-(V-19.9)/17), beta = 3.15e-4 phi((V-19.9)/9); tau = 0.5/(alpha+beta)
+            const double xc = fma(vg, CK(-1.0 / 17.0), CK(19.9 / 17.0));
+            const double series = fma(xc, fma(xc, 1.0 / 12.0, -0.5), 1.0);
+            const double pa = (fabs(xc) < 1e-4) ? series : xc * e17 * ep_rcp(CK(E199_17) - e17);   // e^{xc} = e^{19.9/17}/e17
+            in[1] = ep_rsqrt(1.0 + x7[2]);
+            r[1] = 2.0 * fma(CK(6.8e-4), pa, CK(3.15e-4) * phi(xd, x7[3]));
+        }
+        {   // d: tau = 1/(0.035 * 6.24 phi(x)(1 + e^x)), x = -(V+10)/6.24
+            in[2] = ep_rcp(1.0 + x8[1]);
+            r[2] = CK(0.035 * 6.24) * phi(dx, x8[0]) * (1.0 + x8[0]);
+        }
+        {   // f: tau = 9/(0.0197 G + 0.02)
+            in[3] = ep_rcp(1.0 + x8[3]);
+            r[3] = fma(CK(0.0197 / 9.0), x8[2], CK(0.02 / 9.0));
+        }
+        rush_larsen4(r, in, 4, 5, 6, 7);
+    }
+    // ---- v, w: no further voltage exponentials
+    {
+        double in[EXP_W] = {0.0, 0.0, 0.0, 0.0}, r[EXP_W] = {0.0, 0.0, 0.0, 0.0};
+        {   // v: inf = 1 - 1/(1+E2), tau = 1.91 + 2.09/(1+E1), E2 = E1 e^{-200}
+            const double E2 = e4[0] * CK(EM200);
+            in[0] = E2 * ep_rcp(1.0 + E2);
+            r[0] = ep_rcp(fma(CK(2.09), ep_rcp(1.0 + e4[0]), CK(1.91)));
+        }
+        {   // w: tau = 1.2/(phi(x)(1 + 0.3 e^x)), x = -(V-7.9)/5; inf = 1 - 1/(1 + e^{-(V-40)/17})
+            const double xw = fma(vg, CK(-0.2), CK(7.9 / 5.0));
+            const double ex = CK(E79_5) * e5m;
+            in[1] = CK(E40_17) * ep_rcp(e17 + CK(E40_17));
+            r[1] = CK(1.0 / 1.2) * phi(xw, ex) * fma(CK(0.3), ex, 1.0);
+        }
+        rush_larsen4(r, in, 8, 9, -1, -1);
     }
     return v_new;
 }
