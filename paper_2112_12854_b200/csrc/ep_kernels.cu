@@ -116,9 +116,9 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
                                                                                      const int32_t* __restrict__ cidx,
                                                                                      const double* __restrict__ ccoef,
                                                                                      StepArgs a) {
-    // per-thread columns of the transcendental batches (ep_math.cuh): slot s of thread t at xs[s][t]
-    // TP06 also keeps its 12 stencil coefficients there (copied in asynchronously: no registers held until they are used)
-    constexpr bool CF_SMEM = (MODEL != 1);
+    // per-thread columns of the slot array (parked gate values of the cell models): slot s of thread t at xs[s][t]
+    constexpr bool CF_SMEM = false;   // stencil coefficients in registers: with the streaming cell models shared-memory traffic costs
+                                      // more than the 24 registers do (178.0 vs 179.6 us on config 3; the opposite held in round 1)
     constexpr int MSLOTS = (MODEL == 0) ? tp06::N_SLOTS : (MODEL == 1 ? crn::N_SLOTS : stw::N_SLOTS);
     constexpr int NSLOTS = MSLOTS + (CF_SMEM ? 12 : 0);
     __shared__ double xs[NSLOTS][CELL_THREADS];

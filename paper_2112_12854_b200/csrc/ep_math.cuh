@@ -5,10 +5,11 @@
 // (profiles/r1a_*.md) showed three things this file is built around:
 //   * 64-bit literals cost two extra issue slots each (UMOV pairs) unless they come from the constant bank through
 //     LDCU.128 into uniform registers  ->  polynomial coefficients live in __constant__ arrays;
-//   * 60 inlined exponentials made the kernel 86 KB of SASS, far beyond the 32 KB instruction cache (top stall:
-//     no_instruction)  ->  exponentials and logarithms are evaluated in BATCHES: a thread writes its arguments into
-//     its own column of a shared-memory slot array and one rolled loop (two arguments per trip for ILP) replaces
-//     them by their exponentials; the loop body exists once in the kernel and its constants stay in uniform registers;
+//   * 60 inlined exponentials of ~70 instructions each made the first kernel 86 KB of SASS (top stall: no_instruction).
+//     Round 1 answered with rolled loops over arguments parked in shared memory; round 2 found that traffic to be the next
+//     limiter and went back to inline evaluation, but of 35 shared exponentials of ~14 fp64 instructions each, FOUR AT A TIME
+//     (ep_exp2_wide<4>: four interleaved dependency chains, coefficients in uniform registers), each group placed right
+//     before its consumers (ep_tp06.cuh); the kernel is 43 KB of SASS and no_instruction stalls stay below 1 %;
 //   * IEEE division is ~10 fp64 instructions plus a slow-path call  ->  ep_rcp: MUFU.RCP64H seed + one third-order
 //     step (3 DFMA), arguments are finite, normal and far from the ends of the exponent range at every call site.
 //   * every exponential of the cell models has an argument of the form (compile-time constant) x (run-time value), so the
@@ -120,43 +121,6 @@ __device__ __forceinline__ void ep_exp2_wide(double (&x)[W]) {
     for (int j = 0; j < W; ++j) q[j] = fma(r[j], q[j], 1.0);
 #pragma unroll
     for (int j = 0; j < W; ++j) x[j] = __hiloint2double(__double2hiint(q[j]) + k[j] * 1048576, __double2loint(q[j]));
-}
-
-// Batched evaluation over a thread's own column of a shared-memory slot array xs[slot][BLOCK]; col = &xs[0][tid].
-// N must be a multiple of W.  The loops stay rolled on purpose (instruction-cache footprint).
-// n <= N (a multiple of W, the same for every lane of the warp) lets a caller skip trailing slots it does not need.
-template <int N, int BLOCK, int W>
-__device__ __forceinline__ void ep_exp2_slots(double* col, int n = N) {
-    static_assert(N % W == 0, "pad the slot list to a multiple of W");
-#ifdef EP_SLOTS_UNPIPELINED
-#pragma unroll 1
-    for (int s = 0; s < n; s += W) {
-        double x[W];
-#pragma unroll
-        for (int j = 0; j < W; ++j) x[j] = col[(s + j) * BLOCK];
-        ep_exp2_wide<W>(x);
-#pragma unroll
-        for (int j = 0; j < W; ++j) col[(s + j) * BLOCK] = x[j];
-    }
-#else
-    // software-pipelined: the arguments of the next trip are read from shared memory before this trip's polynomials are
-    // evaluated, so no trip starts by waiting for its own loads (the last trip prefetches itself: values unused)
-    double x[W];
-#pragma unroll
-    for (int j = 0; j < W; ++j) x[j] = col[j * BLOCK];
-#pragma unroll 1
-    for (int s = 0; s < n; s += W) {
-        const int sn = (s + W < n) ? s + W : s;
-        double nx[W];
-#pragma unroll
-        for (int j = 0; j < W; ++j) nx[j] = col[(sn + j) * BLOCK];
-        ep_exp2_wide<W>(x);
-#pragma unroll
-        for (int j = 0; j < W; ++j) col[(s + j) * BLOCK] = x[j];
-#pragma unroll
-        for (int j = 0; j < W; ++j) x[j] = nx[j];
-    }
-#endif
 }
 
 // W logarithms at once, stage by stage (same arithmetic as ep_log_core); arguments positive and normal.
