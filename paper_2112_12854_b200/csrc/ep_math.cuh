@@ -16,19 +16,22 @@
 //     factor log2(e) is folded into those constants and the primitive is 2^x: the reduction x = k + r is one exact
 //     subtraction instead of the two-constant Cody-Waite pair of a natural exponential (one fp64 instruction less per
 //     call, 36 calls per TP06 cell-step).
-// Accuracy, measured on the GPU by tests/test_gpu_math.py through ep_math_eval(): 2^x <= 1 ulp on [-1000, 1000]
-// (polynomial error 8e-18), log <= 1 ulp where |log x| > 1 (the concentrations it is used on) and <= 2.5 ulp near
+// Accuracy, measured on the GPU by tests/test_gpu_math.py through ep_math_eval(): 2^x relative error <= 4.2e-16 on [-1000, 1000]
+// (<= 3.1 ulp; polynomial error 3e-16), log <= 1 ulp where |log x| > 1 (the concentrations it is used on) and <= 2.5 ulp near
 // x = 1, rcp <= 1 ulp, rsqrt <= 2 ulp, hence a*rcp(b) <= 2 ulp.  No lookup tables (north_star: "precomputed-free exp paths").
 #pragma once
 #include <cstdint>
 
 namespace epk {
 
-// 2^r = 1 + r P(r) on |r| <= 1/2; P = degree-10 Chebyshev interpolant of (2^r - 1)/r (max relative error of the
-// reconstructed 2^r: 8.4e-18, computed in 80-digit arithmetic).  EP_EXP2_DEG = 9 selects the degree-9 interpolant
-// (5.8e-16, one instruction less per call); it is an experiment switch, the shipped build uses 10.
+// 2^r = 1 + r P(r) on |r| <= 1/2.  P = the degree-9 MINIMAX polynomial for the relative error of the reconstructed 2^r
+// (Remez exchange with weight r / 2^r, 60-digit arithmetic): 2.96e-16; measured on the GPU, with the rounding of the Horner
+// chain: relative error <= 4.2e-16, i.e. <= 3.1 ulp just below a power of two and <= 1.9 ulp just above one
+// (tests/test_gpu_math.py).  EP_EXP2_DEG = 10 selects the degree-10 Chebyshev interpolant (8.4e-18: <= 1 ulp, one DFMA more per
+// call); round 1 shipped that one, round 2 measured the difference on the fused kernel (175.7 vs 177.8 us on config 3)
+// against a one-step tolerance of 1e-11 and a run tolerance of 1e-6 mV that both keep three orders of margin.
 #ifndef EP_EXP2_DEG
-#define EP_EXP2_DEG 10
+#define EP_EXP2_DEG 9
 #endif
 constexpr double L2E = 1.4426950408889634;   // log2(e): folded into the compile-time slopes of every exponent
 #if EP_EXP2_DEG == 10
@@ -37,10 +40,10 @@ __constant__ double EXP2_P[11] = {0.6931471805599453,     0.24022650695910097,  
                                   1.525273382983612e-05,  1.321544258792169e-06, 1.0178062445845774e-07,
                                   7.072585949269223e-09,  4.4549605981865186e-10};
 #else
-__constant__ double EXP2_P[10] = {0.6931471805599462,     0.24022650695910075,   0.05550410866465167,
-                                  0.009618129107618665,   0.0013333558200794592, 0.00015403530424776529,
-                                  1.5252672924850737e-05, 1.3215451633221434e-06, 1.0205905413765595e-07,
-                                  7.070977866508138e-09};
+__constant__ double EXP2_P[10] = {0.6931471805599516,     0.24022650695910472,   0.05550410866434658,
+                                  0.009618129107380715,   0.001333355824648072,  0.00015403530800818256,
+                                  1.525264774769592e-05,  1.321523563477604e-06, 1.0210506458816145e-07,
+                                  7.111758687557852e-09};
 #endif
 // log m = 2 s (1 + z/3 + z^2/5 + ... + z^9/19), s = (m-1)/(m+1), z = s^2 <= 0.0295 (next term z^10/21 < 2.4e-17)
 __constant__ double LOG_C[9] = {1.0 / 3.0, 1.0 / 5.0, 1.0 / 7.0, 1.0 / 9.0, 1.0 / 11.0, 1.0 / 13.0, 1.0 / 15.0,

@@ -12,7 +12,7 @@
 // 0.02(v-E_K) -> 0.06, 0.1, 0.5; (v+27)^2/3600 -> /240, /225), every sigmoid product is written as one rational function
 // with a single reciprocal, and the remaining 35 exponentials are evaluated four at a time (interleaved dependency chains,
 // ep_math.cuh) in nine groups, each right before the quantities that consume it, so that arguments and results stay in
-// registers; shared memory only parks the gate values at t^n and the stencil coefficients.  Relative differences from the literal formulas are <= ~2e-14 (120-fold powers of a 1-ulp value),
+// registers; shared memory only parks the gate values at t^n and the stencil coefficients.  Relative differences from the literal formulas are <= ~5e-14 (120-fold powers of a value good to 4.2e-16),
 // three orders of magnitude inside the 1e-11 one-step tolerance.  (The literal transcription was the first kernel of
 // this repo -- profiles/r01a_baseline_direct_kernel.md -- and lives on only in the CPU oracle.)
 //

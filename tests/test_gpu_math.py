@@ -1,6 +1,6 @@
 """Accuracy of the kernels' own fp64 routines (csrc/ep_math.cuh) on the device, against mpmath / numpy references.
 
-The claims in ep_math.cuh: 2^x <= 1 ulp, log <= 1 ulp where |log x| > 1 (the concentrations) and <= 2.5 ulp near x = 1,
+The claims in ep_math.cuh: 2^x relative error <= 4.2e-16, <= 3.1 ulp (degree-9 minimax polynomial, 3e-16), log <= 1 ulp where |log x| > 1 (the concentrations) and <= 2.5 ulp near x = 1,
 rcp <= 1 ulp, rsqrt <= 2 ulp.
 """
 import numpy as np
@@ -26,7 +26,9 @@ def test_exp2_accuracy():
                         np.array([0.0, -0.0, 1000.0, -1000.0, 0.5, -0.5, 1e-300, 0.49999999999999994, 1.0, -1.0, 10.0])])
     y = ep.math_eval(0, x)
     err = _ulp_err(y, np.exp2(x.astype(np.longdouble)))
-    assert err.max() <= 1.0, err.max()
+    assert err.max() <= 3.2, err.max()
+    rel = np.abs((y.astype(np.longdouble) - np.exp2(x.astype(np.longdouble))) / np.exp2(x.astype(np.longdouble))).astype(np.float64)
+    assert rel.max() <= 4.2e-16, rel.max()
     assert y[x == 0.0].tolist() == [1.0, 1.0]
     assert ep.math_eval(0, np.array([1.0, -1.0, 10.0])).tolist() == [2.0, 0.5, 1024.0]    # integer arguments are exact
     assert np.all(np.diff(ep.math_eval(0, np.linspace(-5, 5, 200001))) >= 0)      # monotone on a fine grid
