@@ -122,7 +122,13 @@ def run_reference(args):
     cores = os.cpu_count() or 1
     O.set_threads(cores)
     o = O.OracleSim.from_problem(prob)
-    per = max(1, args.ref_inner)
+    # one bench step = the same `--inner` explicit time steps as the GPU arm's bench step when the whole run (warm-up included)
+    # fits in about four minutes of oracle time on this host; otherwise as many as fit (at least one).  --ref-inner overrides.
+    t0 = time.perf_counter()
+    o.step(1, _run_dt(prob))
+    t1 = max(time.perf_counter() - t0, 1e-6)
+    fit = int(240.0 / (t1 * (args.steps + args.warmup)))
+    per = args.ref_inner if args.ref_inner > 0 else max(1, min(args.inner, fit))
     for _ in range(args.warmup):
         o.step(per, _run_dt(prob))
     t0 = time.perf_counter()
@@ -136,7 +142,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": prob.name, "cells": prob.mesh.n_tets, "dt_ms": _run_dt(prob), "time_steps_per_step": per},
+        "config": {"workload": prob.name, "cells": prob.mesh.n_tets, "nodes": prob.mesh.n_nodes, "dt_ms": _run_dt(prob),
+                   "dt_nominal_ms": prob.dt, "time_steps_per_step": per, "time_order": 1},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
@@ -343,7 +350,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference", "disttest"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number 1..5; 6/7/8 = the paper's Table-1 slab at dx 0.5/0.2/0.1 mm; 9/10 = Purkinje strip / sheet (2D, Stewart)")
     ap.add_argument("--inner", type=int, default=100, help="explicit time steps per bench step")
-    ap.add_argument("--ref-inner", type=int, default=1, help="oracle time steps per bench step (--impl reference)")
+    ap.add_argument("--ref-inner", type=int, default=0,
+                    help="oracle time steps per bench step (--impl reference); 0 = --inner if the run fits in ~4 minutes, else fewer")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--order", type=int, default=1, choices=[1, 2],
                     help="time-stepping order: 1 = the paper's Rush-Larsen + forward Euler (headline), 2 = AB2 + second-order Rush-Larsen")

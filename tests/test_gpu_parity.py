@@ -31,7 +31,7 @@ def ep():
 
 def _pair(ep, oracle, prob, threads=0):
     import os
-    oracle.set_threads(threads or max(1, (os.cpu_count() or 2) // 2))
+    oracle.set_threads(threads or (os.cpu_count() or 1))
     g = ep.Sim.from_problem(prob)
     o = oracle.OracleSim.from_problem(prob)
     return g, o
