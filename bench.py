@@ -112,7 +112,7 @@ def _oracle_leg(prob, budget_s: float, threads: int):
 
 
 def run_reference(args):
-    """--impl reference: the oracle on the host cores; each bench step = one oracle time step on the full mesh."""
+    """--impl reference: the oracle on the host cores; each bench step = --inner oracle time steps on the full mesh (fewer if they do not fit)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
