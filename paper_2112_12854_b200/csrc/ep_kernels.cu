@@ -58,13 +58,27 @@ __global__ void __launch_bounds__(NODE_THREADS) node_gather_kernel(int64_t nn, i
     if (slice < n_slices) {
         int64_t q = beg + 32 * p + lane;
         const int64_t step = 32 * NODE_PARTS;
-        for (; q + step < end; q += 2 * step) {   // two independent gathers in flight per trip
-            const int32_t i0 = __ldg(nidx + q), i1 = __ldg(nidx + q + step);
-            const double w0 = __ldg(nw + q), w1 = __ldg(nw + q + step);
-            acc0 = fma(w0, vm[i0], acc0);
-            acc1 = fma(w1, vm[i1], acc1);
+#ifndef EP_NODE_INFLIGHT
+#define EP_NODE_INFLIGHT 6
+#endif
+        constexpr int NF = EP_NODE_INFLIGHT;      // rows of this warp in flight per trip: NF table loads, then NF dependent gathers
+        for (; q < end; q += NF * step) {
+            int32_t ii[NF];
+            double ww[NF], vv[NF];
+#pragma unroll
+            for (int r = 0; r < NF; ++r) {
+                const bool on = q + r * step < end;
+                ii[r] = 0; ww[r] = 0.0;
+                if (on) { ii[r] = ep_ldg_stream(nidx + q + r * step); ww[r] = ep_ldg_stream(nw + q + r * step); }
+            }
+#pragma unroll
+            for (int r = 0; r < NF; ++r) vv[r] = vm[ii[r]];   // padded rows: weight 0 times vm[0]
+#pragma unroll
+            for (int r = 0; r < NF; ++r) {
+                if (r & 1) acc1 = fma(ww[r], vv[r], acc1);
+                else acc0 = fma(ww[r], vv[r], acc0);
+            }
         }
-        if (q < end) acc0 = fma(__ldg(nw + q), vm[__ldg(nidx + q)], acc0);
     }
     part[sl][p][lane] = acc0 + acc1;
     __syncthreads();
@@ -138,9 +152,9 @@ __global__ void __launch_bounds__(CELL_THREADS, EP_CELL_MIN_BLOCKS) cell_step_ke
     double cf[12];
 #pragma unroll
     for (int m = 0; m < 12; ++m) {
-        id[m] = __ldg(tidx + m * CELL_THREADS);
+        id[m] = ep_ldg_stream(tidx + m * CELL_THREADS);
         if constexpr (CF_SMEM) ep_cp_async8(&xs[MSLOTS + m][threadIdx.x], tcoef + m * CELL_THREADS);
-        else cf[m] = __ldg(tcoef + m * CELL_THREADS);
+        else cf[m] = ep_ldg_stream(tcoef + m * CELL_THREADS);
     }
     double gv[12];
     auto issue_gather = [&]() {

@@ -171,6 +171,39 @@ __device__ __forceinline__ void ep_cp_async_wait() {
     asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
 }
 
+// Streaming loads: data that is read once per step (stencil tables, state rows, the node table) does not allocate in L1,
+// which then keeps the gather targets (node values, neighbour potentials) that neighbouring cells share.
+#ifndef EP_STREAM_LOADS
+#define EP_STREAM_LOADS 1
+#endif
+__device__ __forceinline__ double ep_ldg_stream(const double* q) {   // read-only for the lifetime of the kernel
+#if EP_STREAM_LOADS
+    double v;
+    asm("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(q));
+    return v;
+#else
+    return __ldg(q);
+#endif
+}
+__device__ __forceinline__ int32_t ep_ldg_stream(const int32_t* q) {
+#if EP_STREAM_LOADS
+    int32_t v;
+    asm("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(v) : "l"(q));
+    return v;
+#else
+    return __ldg(q);
+#endif
+}
+__device__ __forceinline__ double ep_ld_stream(const double* q) {    // state rows: read here, overwritten later by the same thread
+#if EP_STREAM_LOADS
+    double v;
+    asm volatile("ld.global.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(q) : "memory");
+    return v;
+#else
+    return *q;
+#endif
+}
+
 __device__ __forceinline__ double ep_clamp(double x, double lo, double hi) { return fmin(fmax(x, lo), hi); }
 
 }  // namespace epk

@@ -115,8 +115,9 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     // their base-2 exponents are clamped to -1000 below (2^-1000 = 1e-301 stands for the oracle's underflow to 0).
     const double vg = ep_clamp(v, -200.0, 200.0);
     const double dtl = dt * L2E;   // Rush-Larsen exponents -dt/tau in base-2 units (the exponential primitive is 2^x)
-    const double Cai = ycol[Y_CAI * stride], CaSR = ycol[Y_CASR * stride], CaSS = ycol[Y_CASS * stride],
-                 Nai = ycol[Y_NAI * stride], Ki = ycol[Y_KI * stride];
+    const double Cai = ep_ld_stream(ycol + Y_CAI * stride), CaSR = ep_ld_stream(ycol + Y_CASR * stride),
+                 CaSS = ep_ld_stream(ycol + Y_CASS * stride), Nai = ep_ld_stream(ycol + Y_NAI * stride),
+                 Ki = ep_ld_stream(ycol + Y_KI * stride);
     // arguments of the gate functions: the values at t^n (first order) or extrapolated to t^{n+1/2} (second order)
     double vs = v, vgs = vg, CaSSs = CaSS, CaSRs = CaSR;
     double fprev[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
@@ -135,7 +136,7 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
 #pragma unroll
     for (int k = 0; k < N_RLB; ++k) ep_cp_async8(col + (G_OLD0 + k) * BLOCK, ycol + (1 + k) * stride);
     ep_cp_async8(col + G_RBAR * BLOCK, ycol + Y_RBAR * stride);
-    const double fCass = ycol[Y_FCASS * stride];
+    const double fCass = ep_ld_stream(ycol + Y_FCASS * stride);
 
     // ---- batch 1: the four logarithms of the reversal potentials, side by side in registers
     double lg[4] = {Ki, Nai, fma(CK(pKNa), Nai, Ki), Cai};
