@@ -66,16 +66,18 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
     using namespace crn;
     const double vg = ep_clamp(v, -250.0, 250.0);   // argument of every transcendental
     const double dtl = dt * L2E;                    // Rush-Larsen exponents in base-2 units (the primitive is 2^x)
-    const double Nai = ycol[C_NAI * stride], Ki = ycol[C_KI * stride], Cai = ycol[C_CAI * stride],
-                 Caup = ycol[C_CAUP * stride], Carel = ycol[C_CAREL * stride];
+    const double Nai = ep_ld_stream(ycol + C_NAI * stride), Ki = ep_ld_stream(ycol + C_KI * stride),
+                 Cai = ep_ld_stream(ycol + C_CAI * stride), Caup = ep_ld_stream(ycol + C_CAUP * stride),
+                 Carel = ep_ld_stream(ycol + C_CAREL * stride);
     // The ten gates of the Rush-Larsen list are copied into shared memory asynchronously (no registers held); they and
     // m h j fCa u are first touched after the first two exponential groups, which hides their latency.
 #pragma unroll
     for (int k = 0; k < 8; ++k) ep_cp_async8(col + (G_OLD0 + k) * BLOCK, ycol + (C_OA + k) * stride);
     ep_cp_async8(col + (G_OLD0 + 8) * BLOCK, ycol + C_VG * stride);
     ep_cp_async8(col + (G_OLD0 + 9) * BLOCK, ycol + C_W * stride);
-    const double m = ycol[C_M * stride], h = ycol[C_H * stride], j = ycol[C_J * stride], fCa = ycol[C_FCA * stride],
-                 u = ycol[C_U * stride];
+    const double m = ep_ld_stream(ycol + C_M * stride), h = ep_ld_stream(ycol + C_H * stride),
+                 j = ep_ld_stream(ycol + C_J * stride), fCa = ep_ld_stream(ycol + C_FCA * stride),
+                 u = ep_ld_stream(ycol + C_U * stride);
 
     // ---- batch 1: logarithms of the reversal potentials
     double lg[3] = {Nai, Ki, Cai};
@@ -161,11 +163,11 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
         const double dCaup = Iup - Iupleak - Itr * CK(Vrel / Vup);
         const double tq = (Carel + CK(KmCsqn)) * (Carel + CK(KmCsqn));
         const double dCarel = (Itr - Irel) * tq * ep_rcp(tq + CK(Csqnmax * KmCsqn));
-        ycol[C_NAI * stride] = fma(dt, dNai, Nai);
-        ycol[C_KI * stride] = fma(dt, dKi, Ki);
-        ycol[C_CAI * stride] = fma(dt, B1 * invB2, Cai);
-        ycol[C_CAUP * stride] = fma(dt, dCaup, Caup);
-        ycol[C_CAREL * stride] = fma(dt, dCarel, Carel);
+        ep_st_stream(ycol + C_NAI * stride, fma(dt, dNai, Nai));
+        ep_st_stream(ycol + C_KI * stride, fma(dt, dKi, Ki));
+        ep_st_stream(ycol + C_CAI * stride, fma(dt, B1 * invB2, Cai));
+        ep_st_stream(ycol + C_CAUP * stride, fma(dt, dCaup, Caup));
+        ep_st_stream(ycol + C_CAREL * stride, fma(dt, dCarel, Carel));
     }
     const double v_new = fma(dt, dv_diff - iion - istim, v);   // eq. (7)
 
@@ -217,9 +219,9 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
         e4[2] = fmax(-dtl * rh, -1000.0);
         e4[3] = fmax(-dtl * rj, -1000.0);
         ep_exp2_wide<4>(e4);
-        ycol[C_M * stride] = fma(m - m_inf, e4[1], m_inf);              // Rush-Larsen
-        ycol[C_H * stride] = fma(h - h_inf, e4[2], h_inf);
-        ycol[C_J * stride] = fma(j - j_inf, e4[3], j_inf);
+        ep_st_stream(ycol + C_M * stride, fma(m - m_inf, e4[1], m_inf));              // Rush-Larsen
+        ep_st_stream(ycol + C_H * stride, fma(h - h_inf, e4[2], h_inf));
+        ep_st_stream(ycol + C_J * stride, fma(j - j_inf, e4[3], j_inf));
     }
     // one Rush-Larsen group of the parked list (0 oa, 1 oi, 2 ua, 3 ui, 4 xr, 5 xs, 6 d, 7 f -> rows C_OA + g; 8 v, 9 w; < 0: pad)
     auto rush_larsen4 = [&](double (&e)[EXP_W], const double (&in)[EXP_W], int g0, int g1, int g2, int g3) {
@@ -232,7 +234,8 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
         ep_exp2_wide<EXP_W>(e);
 #pragma unroll
         for (int k = 0; k < EXP_W; ++k)
-            if (gi[k] >= 0) ycol[((gi[k] < 8) ? C_OA + gi[k] : C_VG + (gi[k] - 8)) * stride] = fma(yo[k] - in[k], e[k], in[k]);
+            if (gi[k] >= 0)
+                ep_st_stream(ycol + ((gi[k] < 8) ? C_OA + gi[k] : C_VG + (gi[k] - 8)) * stride, fma(yo[k] - in[k], e[k], in[k]));
     };
     // ---- group 4: the constant Rush-Larsen factors of fCa (tau = 2 ms) and u (tau = 8 ms), alpha of oa / ua
     double oaA;
@@ -241,9 +244,9 @@ __device__ __forceinline__ double crn_step(double v, double* ycol, int64_t strid
                             fma(vg, CK(-L2E / 59.0), CK(30.0 * L2E / 59.0))};
         ep_exp2_wide<EXP_W>(x4);
         const double fCa_inf = CK(0.00035) * ep_rcp(CK(0.00035) + Cai);
-        ycol[C_FCA * stride] = fma(fCa - fCa_inf, x4[0], fCa_inf);
+        ep_st_stream(ycol + C_FCA * stride, fma(fCa - fCa_inf, x4[0], fCa_inf));
         const double u_inf = ep_rcp(1.0 + e4[0]);
-        ycol[C_U * stride] = fma(u - u_inf, x4[1], u_inf);
+        ep_st_stream(ycol + C_U * stride, fma(u - u_inf, x4[1], u_inf));
         oaA = x4[2] + x4[3];
     }
     // ---- groups 5, 6: oa, ua, oi, ui (K_Q10 = 3 multiplies the rates)

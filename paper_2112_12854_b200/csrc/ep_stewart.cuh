@@ -62,11 +62,12 @@ __device__ __forceinline__ double stw_step(double v, double* ycol, int64_t strid
     using namespace stw;
     const double vg = ep_clamp(v, -200.0, 200.0);   // argument of every transcendental (reading T2, as TP06)
     const double dtl = dt * L2E;
-    const double Cai = ycol[W_CAI * stride], CaSR = ycol[W_CASR * stride], CaSS = ycol[W_CASS * stride],
-                 Nai = ycol[W_NAI * stride], Ki = ycol[W_KI * stride];
+    const double Cai = ep_ld_stream(ycol + W_CAI * stride), CaSR = ep_ld_stream(ycol + W_CASR * stride),
+                 CaSS = ep_ld_stream(ycol + W_CASS * stride),
+                 Nai = ep_ld_stream(ycol + W_NAI * stride), Ki = ep_ld_stream(ycol + W_KI * stride);
 #pragma unroll
     for (int k = 0; k < N_RLB; ++k) ep_cp_async8(col + (G_OLD0 + k) * BLOCK, ycol + rl_row(k) * stride);
-    const double fCass = ycol[W_FCASS * stride], Rp = ycol[W_RP * stride];
+    const double fCass = ep_ld_stream(ycol + W_FCASS * stride), Rp = ep_ld_stream(ycol + W_RP * stride);
 
     // ---- batch 1: logarithms of the reversal potentials
     double lg[4] = {Ki, Nai, fma(CK(pKNa), Nai, Ki), Cai};
@@ -179,12 +180,12 @@ __device__ __forceinline__ double stw_step(double v, double* ycol, int64_t strid
     const double dKi = -(IK1 + Ito + IfK + Isus + IKr + IKs + IpK + istim - 2.0 * INaK) * CK(Cap / (Vc * F));
     const double dRp = fma(-CK(k2p) * kcasr * CaSS, Rp, CK(k4) * (1.0 - Rp));     // reading B12: forward Euler
     const double v_new = fma(dt, dv_diff - iion - istim, v);   // eq. (7)
-    ycol[W_RP * stride] = fma(dt, dRp, Rp);
-    ycol[W_CAI * stride] = fma(dt, dCai, Cai);
-    ycol[W_CASR * stride] = fma(dt, dCaSR, CaSR);
-    ycol[W_CASS * stride] = fma(dt, dCaSS, CaSS);
-    ycol[W_NAI * stride] = fma(dt, dNai, Nai);
-    ycol[W_KI * stride] = fma(dt, dKi, Ki);
+    ep_st_stream(ycol + W_RP * stride, fma(dt, dRp, Rp));
+    ep_st_stream(ycol + W_CAI * stride, fma(dt, dCai, Cai));
+    ep_st_stream(ycol + W_CASR * stride, fma(dt, dCaSR, CaSR));
+    ep_st_stream(ycol + W_CASS * stride, fma(dt, dCaSS, CaSS));
+    ep_st_stream(ycol + W_NAI * stride, fma(dt, dNai, Nai));
+    ep_st_stream(ycol + W_KI * stride, fma(dt, dKi, Ki));
 
     // one Rush-Larsen group: y <- inf + (y_old - inf) 2^e for four gates (g = position in the Rush-Larsen list)
     auto rush_larsen4 = [&](double (&e)[EXP_W], const double (&in)[EXP_W], int g0, int g1, int g2, int g3) {
@@ -194,7 +195,7 @@ __device__ __forceinline__ double stw_step(double v, double* ycol, int64_t strid
         for (int j = 0; j < EXP_W; ++j) yo[j] = col[(G_OLD0 + gi[j]) * BLOCK];
         ep_exp2_wide<EXP_W>(e);
 #pragma unroll
-        for (int j = 0; j < EXP_W; ++j) ycol[rl_row(gi[j]) * stride] = fma(yo[j] - in[j], e[j], in[j]);
+        for (int j = 0; j < EXP_W; ++j) ep_st_stream(ycol + rl_row(gi[j]) * stride, fma(yo[j] - in[j], e[j], in[j]));
     };
     // m, h, j, xr1 can be faster than 700/dt inside the clamp range (see the note in tp06_step), and so can y: its rate reaches
     // 3e7 per ms at +200 mV (2 per ms at +50 mV).  Their exponents are clamped to -1000: 2^-1000 stands for the oracle's 0.
@@ -229,7 +230,7 @@ __device__ __forceinline__ double stw_step(double v, double* ycol, int64_t strid
         double x3[EXP_W] = {(vg + 40.0) * (vg + 40.0) * CK(-L2E / 1800.0), (vg + 25.0) * (vg + 25.0) * CK(-L2E / 320.0),
                             -dtl * ep_rcp(fma(80.0, qf, 2.0)), 0.0};
         ep_exp2_wide<EXP_W>(x3);
-        ycol[W_FCASS * stride] = fma(fCass - fCass_inf, x3[2], fCass_inf);   // Rush-Larsen
+        ep_st_stream(ycol + W_FCASS * stride, fma(fCass - fCass_inf, x3[2], fCass_inf));   // Rush-Larsen
         double in[EXP_W], e[EXP_W];
         in[0] = ep_rcp(fma(CK(E88_24), E24, 1.0));                                                     // xr2
         e[0] = -dtl * ((E20 + CK(EM3)) * fma(CK(EM3), E20, 1.0) * ep_rcp(CK(3.36) * E20));

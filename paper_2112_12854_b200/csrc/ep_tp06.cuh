@@ -266,11 +266,11 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
     if constexpr (ORDER == 1) {
         const double dKi = -(IK1 + Ito + IKr + IKs - 2.0 * INaK + IpK + istim) * CK(Cap / (Vc * F));   // reading B8
         v_new = fma(dt, dv_diff - iion - istim, v);            // eq. (7); explicit increment :172
-        ycol[Y_CAI * stride] = fma(dt, dCai, Cai);             // forward Euler
-        ycol[Y_CASR * stride] = fma(dt, dCaSR, CaSR);
-        ycol[Y_CASS * stride] = fma(dt, dCaSS, CaSS);
-        ycol[Y_NAI * stride] = fma(dt, dNai, Nai);
-        ycol[Y_KI * stride] = fma(dt, dKi, Ki);
+        ep_st_stream(ycol + Y_CAI * stride, fma(dt, dCai, Cai));             // forward Euler
+        ep_st_stream(ycol + Y_CASR * stride, fma(dt, dCaSR, CaSR));
+        ep_st_stream(ycol + Y_CASS * stride, fma(dt, dCaSS, CaSS));
+        ep_st_stream(ycol + Y_NAI * stride, fma(dt, dNai, Nai));
+        ep_st_stream(ycol + Y_KI * stride, fma(dt, dKi, Ki));
     } else {
         // right-hand sides without the stimulus; AB2 where there is a history, the stimulus added as its exact integral
         const double f[6] = {dv_diff - iion, dCai, dCaSR, dCaSS, dNai,
@@ -284,11 +284,11 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
         hist.hcol[6 * hist.stride] = CaSS;
         hist.hcol[7 * hist.stride] = CaSR;
         v_new = fma(dt, w[0] - istim, v);
-        ycol[Y_CAI * stride] = fma(dt, w[1], Cai);
-        ycol[Y_CASR * stride] = fma(dt, w[2], CaSR);
-        ycol[Y_CASS * stride] = fma(dt, w[3], CaSS);
-        ycol[Y_NAI * stride] = fma(dt, w[4], Nai);
-        ycol[Y_KI * stride] = fma(dt, w[5] - istim * CK(Cap / (Vc * F)), Ki);      // reading B8
+        ep_st_stream(ycol + Y_CAI * stride, fma(dt, w[1], Cai));
+        ep_st_stream(ycol + Y_CASR * stride, fma(dt, w[2], CaSR));
+        ep_st_stream(ycol + Y_CASS * stride, fma(dt, w[3], CaSS));
+        ep_st_stream(ycol + Y_NAI * stride, fma(dt, w[4], Nai));
+        ep_st_stream(ycol + Y_KI * stride, fma(dt, w[5] - istim * CK(Cap / (Vc * F)), Ki));      // reading B8
     }
 
     // one Rush-Larsen group: y <- inf + (y_old - inf) 2^e for four gates (gate index g = state row - 1; g < 0: pad)
@@ -300,7 +300,7 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
         ep_exp2_wide<EXP_W>(e);
 #pragma unroll
         for (int j = 0; j < EXP_W; ++j)
-            if (gi[j] >= 0) ycol[(1 + gi[j]) * stride] = fma(yo[j] - in[j], e[j], in[j]);
+            if (gi[j] >= 0) ep_st_stream(ycol + (1 + gi[j]) * stride, fma(yo[j] - in[j], e[j], in[j]));
     };
     // ---- group 2: m, h_inf, xr1, d; gates m, xr1, xr2, d
     {
@@ -334,8 +334,8 @@ __device__ __forceinline__ double tp06_step(double v, double* ycol, int64_t stri
                             -dtl * ep_rcp(fma(80.0, qf, 2.0)),              // tau_fCass >= 2 ms
                             fmax(-dtl * Rbar_rate, -1000.0)};               // rate grows with Ca_SS: keep the clamp
         ep_exp2_wide<EXP_W>(x3);
-        ycol[Y_FCASS * stride] = fma(fCass - fCass_inf, x3[2], fCass_inf);   // Rush-Larsen
-        ycol[Y_RBAR * stride] = fma(Rbar - Rbar_inf, x3[3], Rbar_inf);
+        ep_st_stream(ycol + Y_FCASS * stride, fma(fCass - fCass_inf, x3[2], fCass_inf));   // Rush-Larsen
+        ep_st_stream(ycol + Y_RBAR * stride, fma(Rbar - Rbar_inf, x3[3], Rbar_inf));
         double in[EXP_W], e[EXP_W];
         {   // xs
             in[0] = E14 * ep_rcp(E14 + CK(EM5_14));
