@@ -240,6 +240,26 @@ int ep_math_eval(int fn, int64_t n, const double *x, double *y);
  * counted number of fp64 warp instructions per 32 cells (t_roof = max(bytes/BW_HBM, I_alg/R_fp64)). */
 int ep_fp64_rate(double *warp_dfma_per_s);
 
+/* The one call that allocates nothing -- for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight
+ * serving loops, harnesses that forbid it); every other call works on a handle whose buffers ep_mesh_create allocated.
+ * Weighted mean of a caller-owned DEVICE array: out_dev[0] = sum_i w_i v_i / sum_i w_i, out_dev[1] = sum_i w_i; with
+ * v = the potentials of ep_device_vm() and w = the cell volumes in the same order this is the volume-averaged potential
+ * v_bar of PAPER.md:216 / :230 that ep_mean_vm returns (a variant of its deterministic two-pass reduction; the summation
+ * order differs, so the two agree to rounding, ~1e-13 relative, not bit for bit).
+ *   v_dev, w_dev  DEVICE pointers, double[n], read only          out_dev  DEVICE pointer, double[2], written
+ *   cuda_stream   cudaStream_t the two kernels are launched on (NULL: the default stream).  The call does NOT synchronise:
+ *                 out_dev is valid once the stream has reached this point.
+ * Scratch: a file-scope device array of 128 KB (one partial sum of w v and of w per 4,096 elements) that every GPU which
+ * loads the library holds until the process exits; hence n <= EP_NOALLOC_MAX_N, larger n is refused with EP_ERR_ARG and a
+ * message that names the limit.  No cudaMalloc / cudaFree / allocating library routine is called; the first call on each
+ * device resolves the array's device address (cudaGetSymbolAddress, no allocation; make that call before capturing).
+ * All calls share the array and it keeps the last call's contents (nothing in it needs to start at zero: each call reads
+ * only the slots it has just written).  Calls that OVERLAP on the GPU -- different streams, concurrent graph replays --
+ * race on it; calls ordered on one stream do not.  Runs on the current device; the pointers must belong to it.
+ * Errors: EP_ERR_ARG (NULL pointer, n <= 0, n > EP_NOALLOC_MAX_N), EP_ERR_CUDA. */
+#define EP_NOALLOC_MAX_N 33554432LL /* 8,192 blocks x 4,096 elements */
+int ep_weighted_mean_noalloc(const double *v_dev, const double *w_dev, int64_t n, double *out_dev, void *cuda_stream);
+
 /* Host-only preprocessor output for tests (no CUDA call is made).  Returns the factored stencil in the CALLER's
  * numbering: for cell c,  dv_diff[c] = sum_{m<8} a[c*8+m] * v_node[node[c*8+m]] + sum_{j<4} b[c*4+j] * (v[nbr[c*4+j]] - v[c])
  * in mV/ms (= D_c/(chi Cm)), where v_node[n] = sum_{k<node_deg[n]} w[node_ptr[n]+k] * v[node_cell[node_ptr[n]+k]].

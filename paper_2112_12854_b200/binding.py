@@ -70,6 +70,7 @@ SIGNATURES = {
     "ep_profile_read": (C.c_int, [_vp, _dp]),
     "ep_math_eval": (C.c_int, [C.c_int, C.c_int64, _dp, _dp]),
     "ep_fp64_rate": (C.c_int, [_dp]),
+    "ep_weighted_mean_noalloc": (C.c_int, [_vp, _vp, C.c_int64, _vp, _vp]),
     "ep_destroy": (None, [_vp]),
     "ep_last_error": (C.c_char_p, []),
     "ep_host_stencil": (C.c_int, [C.c_int64, _dp, C.c_int64, _i32p, _dp, _dp, C.c_double, C.c_double, C.c_double,
@@ -124,6 +125,15 @@ def fp64_rate() -> float:
     r = C.c_double(0.0)
     _chk(lib().ep_fp64_rate(C.byref(r)))
     return float(r.value)
+
+
+NOALLOC_MAX_N = 33554432   # EP_NOALLOC_MAX_N of include/ep.h
+
+
+def weighted_mean_noalloc(v_dptr: int, w_dptr: int, n: int, out_dptr: int, stream=None) -> None:
+    """ep_weighted_mean_noalloc: out[0] = sum(w v) / sum(w), out[1] = sum(w) of DEVICE arrays (raw pointers, double[n] /
+    double[2]); allocates nothing, asynchronous on `stream` (a cudaStream_t as int, None: the default stream)."""
+    _chk(lib().ep_weighted_mean_noalloc(_vp(v_dptr), _vp(w_dptr), int(n), _vp(out_dptr), _vp(stream) if stream else None))
 
 
 def model_n_states(model: int) -> int:

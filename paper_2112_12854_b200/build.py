@@ -15,7 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libep.so")
-SOURCES = ["ep_api.cu", "ep_kernels.cu", "ep_elliptic.cu", "ep_host.cpp"]
+SOURCES = ["ep_api.cu", "ep_kernels.cu", "ep_elliptic.cu", "ep_noalloc.cu", "ep_host.cpp"]
 HEADERS = ["ep_host.h", "ep_kernels.cuh", "ep_math.cuh", "ep_tp06.cuh", "ep_crn98.cuh", "ep_stewart.cuh", os.path.join("..", "..", "include", "ep.h")]
 
 

@@ -328,6 +328,11 @@ int bidomain_solve(ep_sim* s) {
 
 }  // namespace
 
+namespace ep {
+// for the other translation units of the library (ep_noalloc.cu): record the message ep_last_error() returns
+int set_error(int code, const char* msg) { return fail(code, msg ? msg : ""); }
+}  // namespace ep
+
 extern "C" {
 
 const char* ep_last_error(void) { return g_err.c_str(); }

@@ -79,3 +79,22 @@ def test_mesh_create_without_gpu_fails_loudly():
     with pytest.raises(ep.EpError) as e:
         ep.Sim(xyz, np.array([[0, 1, 2, 3]], dtype=np.int32))
     assert e.value.code == -4 and "no CPU fallback" in str(e.value)
+
+
+def test_noalloc_entry_point_refuses_bad_sizes_without_a_gpu():
+    """ep_weighted_mean_noalloc checks its arguments before any CUDA call: the size limit of its fixed scratch is an error
+    that names the limit (include/ep.h: EP_NOALLOC_MAX_N)."""
+    import paper_2112_12854_b200 as ep
+    txt = open(os.path.join(ROOT, "include", "ep.h")).read()
+    assert int(re.search(r"#define EP_NOALLOC_MAX_N (\d+)LL", txt).group(1)) == ep.NOALLOC_MAX_N == 8192 * 4096
+    with pytest.raises(ep.EpError) as e:
+        ep.weighted_mean_noalloc(8, 8, ep.NOALLOC_MAX_N + 1, 8)
+    assert e.value.code == -1 and "EP_NOALLOC_MAX_N" in str(e.value) and str(ep.NOALLOC_MAX_N) in str(e.value)
+    for args in ((0, 8, 8, 8), (8, 0, 8, 8), (8, 8, 8, 0), (8, 8, 0, 8), (8, 8, -3, 8)):
+        with pytest.raises(ep.EpError) as e:
+            ep.weighted_mean_noalloc(*args)
+        assert e.value.code == -1
+    src = open(os.path.join(ROOT, "paper_2112_12854_b200", "csrc", "ep_noalloc.cu")).read()
+    code = re.sub(r"//.*", "", src)
+    assert "cudaMalloc" not in code and "cudaFree" not in code and "cudaGetSymbolAddress" in code
+
