@@ -38,9 +38,14 @@ constexpr int NODE_THREADS = 256;
 // takes rows k = p, p + NODE_PARTS, ... (each row read is 32 consecutive entries: fully coalesced) and the partial sums
 // meet in shared memory.  Four times the threads of a warp-per-slice mapping; the kernel is a dependent gather (index,
 // then value) that runs at 64 % of the HBM peak (profiles/r01b_to_r01e_cell_kernel.md, node kernel section).
+// Resident blocks per SM the node kernel is compiled for: 6 (40 registers, 48 warps).  Measured on config 3 with six table rows
+// in flight per warp: 67 registers 43.0 us, 59 registers 36.7 us, 40 registers 31.7 us, 32 registers (8 blocks) 34.3 us.
+#ifndef EP_NODE_MIN_BLOCKS
+#define EP_NODE_MIN_BLOCKS 6
+#endif
 constexpr int NODE_PARTS = 4;
 constexpr int NODE_SLICES_PER_BLOCK = NODE_THREADS / 32 / NODE_PARTS;
-__global__ void __launch_bounds__(NODE_THREADS) node_gather_kernel(int64_t nn, int64_t n_slices,
+__global__ void __launch_bounds__(NODE_THREADS, EP_NODE_MIN_BLOCKS) node_gather_kernel(int64_t nn, int64_t n_slices,
                                                                     const int64_t* __restrict__ slice_ptr,
                                                                     const int32_t* __restrict__ nidx,
                                                                     const double* __restrict__ nw,
