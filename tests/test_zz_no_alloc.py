@@ -71,7 +71,7 @@ def test_no_alloc_mean_matches_mean_vm_on_calls_in_a_row(ep, capsys):
     ep.weighted_mean_noalloc(vm_ptr, vol.data_ptr(), n, out.data_ptr(), stream)
     ep.weighted_mean_noalloc(vm_ptr, vol.data_ptr(), n, out2.data_ptr(), stream)
     torch.cuda.synchronize()
-    assert torch.cuda.mem_get_info()[0] == free_before
+    assert torch.cuda.mem_get_info()[0] >= free_before          # no device memory was taken
     got3, got4 = out.cpu().numpy().copy(), out2.cpu().numpy().copy()
     ref3 = g.mean_vm()
     assert abs(got3[0] - ref3) <= TOL_MV, (got3[0], ref3)
