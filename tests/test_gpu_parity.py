@@ -617,6 +617,45 @@ def test_device_view_streams_and_two_sims(ep):
     a.close(); b.close(); ref.close()
 
 
+def test_jobs_double_buffered_over_two_handles(ep):
+    """The end-to-end pattern of bench.py: self-contained jobs (state, clock and activation times written from the host, n
+    steps, result read back) alternate between two handles so that the copies of one job overlap the kernels of the other.
+    Every job must return exactly what the same job returns on a handle used alone."""
+    prob = make(3, coarsen=2.0)
+    n, dt, nc = 96, prob.dt, prob.mesh.n_tets
+    ref = ep.Sim.from_problem(prob)
+    S = ref.n_states
+    y0 = np.empty((S, nc))
+    ref.read_states(y0)
+    rng = np.random.default_rng(11)
+    jobs = []
+    for k in range(4):                                  # four different jobs: the initial Vm of a random tenth of the cells raised
+        y = y0.copy()
+        y[0, rng.random(nc) < 0.1] += 40.0 + 5.0 * k
+        jobs.append(y)
+    none = np.full(nc, -1.0)
+
+    def submit(h, y):
+        h.write_states(y); h.set_step_count(0, dt); h.write_activation_times(none)
+        h.step(n, dt)
+
+    want = []
+    for y in jobs:
+        submit(ref, y)
+        want.append((ref.read_vm(), ref.activation_times()))
+    pair = (ep.Sim.from_problem(prob), ep.Sim.from_problem(prob))
+    got = []
+    submit(pair[0], jobs[0])
+    for k in range(len(jobs)):
+        if k + 1 < len(jobs):
+            submit(pair[(k + 1) % 2], jobs[k + 1])       # uploads and starts job k + 1 while job k is still running
+        got.append((pair[k % 2].read_vm(), pair[k % 2].activation_times()))
+    for k, ((v, t), (vw, tw)) in enumerate(zip(got, want)):
+        assert np.array_equal(v, vw) and np.array_equal(t, tw), k
+    assert (want[0][1] >= 0).sum() > 0 and not np.array_equal(want[0][0], want[3][0])
+    ref.close(); pair[0].close(); pair[1].close()
+
+
 def _window(ep, oracle, prob, n_steps, dt, frac, t_span, capsys, label, chunks=4):
     """Window parity from a seeded 'wave in progress' state (tests/wavestate.py): same painted state into both sides, n_steps
     explicit steps, compared at `chunks` checkpoints; returns the oracle's final Vm and both activation-time arrays."""
